@@ -1,0 +1,133 @@
+"""Parameters and the homomorphic hot path on arbitrary-precision integers (test infrastructure).
+
+The paper names the operations (`mult_pairwise_into` = ciphertext product followed by
+relinearisation; `rescaleBy_pairwise_into`) and the ring
+(Z_Q[X]/(X^N+1), Q = 2^logQ for CKKS) but prints no formula for key switching
+or rounding; the readings used here are the ones listed in DESIGN.md section 3.
+
+Ciphertext ct = (c0, c1), decryption c0 + c1*s mod Q.  Tensor triple (d0, d1, d2) decrypts as
+d0 + d1*s + d2*s^2.  Every polynomial is a list of N Python ints in [0, modulus).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+from .ring import pm, add
+
+
+def make_modulus(log: int, t: int) -> int:
+    """t == 0: 2^log (CKKS).  t > 0: the least odd integer > 2^log that is 1 (mod t) (BGV)."""
+    if t == 0:
+        return 1 << log
+    q = (1 << log) + 1
+    while not (q % 2 == 1 and q % t == 1):
+        q += 1
+    return q
+
+
+@dataclass(frozen=True)
+class Params:
+    N: int
+    logQ: int
+    logP: int
+    t: int = 0          # 0 = CKKS, odd t > 0 = BGV plaintext modulus
+
+    @property
+    def Q(self) -> int:
+        return make_modulus(self.logQ, self.t)
+
+    @property
+    def P(self) -> int:
+        return make_modulus(self.logP, self.t)
+
+    @property
+    def PQ(self) -> int:
+        return self.P * self.Q
+
+    @property
+    def L(self) -> int:
+        return ((self.Q - 1).bit_length() + 31) // 32
+
+    @property
+    def L_PQ(self) -> int:
+        return ((self.PQ - 1).bit_length() + 31) // 32
+
+    @property
+    def is_ckks(self) -> bool:
+        return self.t == 0
+
+
+def polymul(prm: Params, a, b) -> list:
+    """c = a * b in Z_Q[X]/(X^N+1)."""
+    return pm(a, b, prm.Q)
+
+
+def he_mult(prm: Params, ct1, ct2):
+    """Tensor product (north_star item 4):
+    d0 = c0*c0', d1 = c0*c1' + c1*c0', d2 = c1*c1'   (all mod Q)."""
+    Q = prm.Q
+    c0, c1 = ct1
+    e0, e1 = ct2
+    d0 = pm(c0, e0, Q)
+    d1 = add(pm(c0, e1, Q), pm(c1, e0, Q), Q)
+    d2 = pm(c1, e1, Q)
+    return d0, d1, d2
+
+
+def round_shift(x: int, k: int) -> int:
+    """floor((x + 2^(k-1)) / 2^k): round half up on the canonical representative (DESIGN 3, A3)."""
+    return (x + (1 << (k - 1))) >> k
+
+
+def relinearize_ckks(prm: Params, d, evk):
+    """CKKS key switch with one big auxiliary modulus P = 2^logP (DESIGN 3, A2-A4):
+    x_b = d2*b' mod PQ, x_a = d2*a' mod PQ as canonical values in [0, PQ);
+    k = ((x + P/2) >> logP) mod Q;  out = (d0 + k_b, d1 + k_a) mod Q."""
+    assert prm.is_ckks
+    Q, PQ = prm.Q, prm.PQ
+    d0, d1, d2 = d
+    evk_b, evk_a = evk
+    xb = pm(d2, evk_b, PQ)
+    xa = pm(d2, evk_a, PQ)
+    kb = [round_shift(x, prm.logP) % Q for x in xb]
+    ka = [round_shift(x, prm.logP) % Q for x in xa]
+    return add(d0, kb, Q), add(d1, ka, Q)
+
+
+def _div_p_bgv(x: int, P: int, Q: int, t: int, Pinv_t: int) -> int:
+    """One coefficient of the BGV divide-by-P (DESIGN 3, A10 / SURVEY 8c step 6)."""
+    r = x % P
+    if r > P // 2:                 # recentre to (-P/2, P/2); P odd, no tie
+        r -= P
+    k = (-r * Pinv_t) % t
+    if k > t // 2:                 # recentre to (-t/2, t/2); t odd, no tie
+        k -= t
+    assert (x - r) % P == 0
+    return ((x - r) // P - k) % Q
+
+
+def relinearize_bgv(prm: Params, d, evk):
+    """BGV key switch, P and Q odd, P = 1 (mod t): nearest multiple of P removed, then the
+    mod-t correction k so that the removed quantity r + P*k is 0 (mod t)."""
+    assert not prm.is_ckks
+    Q, P, PQ, t = prm.Q, prm.P, prm.PQ, prm.t
+    Pinv_t = pow(P % t, -1, t)
+    d0, d1, d2 = d
+    evk_b, evk_a = evk
+    xb = pm(d2, evk_b, PQ)
+    xa = pm(d2, evk_a, PQ)
+    kb = [_div_p_bgv(x, P, Q, t, Pinv_t) for x in xb]
+    ka = [_div_p_bgv(x, P, Q, t, Pinv_t) for x in xa]
+    return add(d0, kb, Q), add(d1, ka, Q)
+
+
+def relinearize(prm: Params, d, evk):
+    return relinearize_ckks(prm, d, evk) if prm.is_ckks else relinearize_bgv(prm, d, evk)
+
+
+def rescale(prm: Params, ct, p: int):
+    """CKKS rescale by 2^p (DESIGN 3, A3):
+    c' = ((c + 2^(p-1)) >> p) mod 2^(logQ - p) on canonical c in [0, Q), both components."""
+    assert prm.is_ckks and 1 <= p < prm.logQ
+    Q2 = 1 << (prm.logQ - p)
+    return tuple([round_shift(int(c), p) % Q2 for c in comp] for comp in ct)

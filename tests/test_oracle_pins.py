@@ -1,0 +1,321 @@
+"""Pins for the CPU oracle: each check ties an oracle function to something other than itself
+(hand brute force, closed forms, a library big-int multiply, algebraic laws, decryption
+invariants).  CPU only.  Citations: PAPER.md line numbers; DESIGN.md section 3 for readings."""
+import os
+import random
+
+import numpy as np
+import pytest
+
+import synth
+from oracle import harness, ntt, ring, scheme
+from oracle.limbs import from_limbs, to_limbs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _read_golden(name):
+    out = {}
+    with open(os.path.join(GOLD, name)) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            k, *v = line.split()
+            out[k] = [int(x) for x in v]
+    return out
+
+
+def _naive_negacyclic(a, b):
+    """Eq. 5-6 expanded term by term into a dict of exponents (test-local)."""
+    N = len(a)
+    tilde = {}
+    for i, x in enumerate(a):
+        for j, y in enumerate(b):
+            tilde[i + j] = tilde.get(i + j, 0) + x * y
+    return [tilde.get(i, 0) - tilde.get(N + i, 0) for i in range(N)]
+
+
+# ---- P2: hand brute force, tiny case -------------------------------------------------------
+def test_p2_golden_n4():
+    g = _read_golden("negacyclic_n4.txt")
+    a, b = g["a"], g["b"]
+    big = 1 << 64
+    got = ring.pm_schoolbook(a, b, big)
+    assert [ring.centre(v, big) for v in got] == g["integers"]
+    assert ring.pm_schoolbook(a, b, 256) == g["mod256"]
+    assert ring.pm_schoolbook(a, b, 97) == g["mod97"]
+    assert ring.pm_ntt(a, b, 256) == g["mod256"]
+    assert ring.pm_ntt(a, b, 97) == g["mod97"]
+
+
+# ---- P1: definition on random small inputs ---------------------------------------------------
+@pytest.mark.parametrize("N,bits", [(8, 5), (8, 70), (16, 128), (32, 33)])
+def test_p1_definition_small(N, bits):
+    rnd = random.Random(N * 1000 + bits)
+    M = (1 << bits) - rnd.randrange(0, 3)
+    a = [rnd.randrange(M) for _ in range(N)]
+    b = [rnd.randrange(M) for _ in range(N)]
+    want = [v % M for v in _naive_negacyclic(a, b)]
+    assert ring.pm_schoolbook(a, b, M) == want
+    assert ring.pm_ntt(a, b, M) == want
+    for k in (0, 1, N - 1):
+        assert ring.pm_coeff(a, b, k, M) == want[k]
+
+
+# ---- P3: monomials ---------------------------------------------------------------------------
+@pytest.mark.parametrize("route", [ring.pm_schoolbook, ring.pm_ntt])
+def test_p3_monomials(route):
+    N, Q = 64, 1 << 100
+    rnd = random.Random(3)
+    a = [rnd.randrange(Q) for _ in range(N)]
+    one = [1] + [0] * (N - 1)
+    assert route(a, one, Q) == a                                  # a * 1 = a
+    x = [0, 1] + [0] * (N - 2)
+    xn1 = [0] * (N - 1) + [1]
+    assert route(x, xn1, Q) == [Q - 1] + [0] * (N - 1)           # X * X^(N-1) = -1
+    for k in (1, 5, N - 1):
+        xk = [0] * N
+        xk[k] = 1
+        want = [(-a[i - k + N]) % Q if i < k else a[i - k] for i in range(N)]   # signed rotation
+        assert route(a, xk, Q) == want
+
+
+# ---- P4: ring laws ---------------------------------------------------------------------------
+def test_p4_ring_laws():
+    N, Q = 32, (1 << 90) + 7
+    rnd = random.Random(4)
+    a, b, c = ([rnd.randrange(Q) for _ in range(N)] for _ in range(3))
+    pm = ring.pm_ntt
+    assert pm(a, b, Q) == pm(b, a, Q)
+    assert pm(a, ring.add(b, c, Q), Q) == ring.add(pm(a, b, Q), pm(a, c, Q), Q)
+    assert pm(pm(a, b, Q), c, Q) == pm(a, pm(b, c, Q), Q)
+
+
+# ---- P5: closed form at the extreme of the bound -------------------------------------------------
+@pytest.mark.parametrize("N,logQ", [(16, 64), (256, 128), (2048, 218)])
+def test_p5_all_qm1_closed_form(N, logQ):
+    """a = b = (Q-1, ..., Q-1): c_k = (Q-1)^2 ((k+1) - (N-1-k)) = 2k + 2 - N (mod Q).
+    The raw values reach +N(Q-1)^2 and -(N-2)(Q-1)^2, i.e. both ends of the CRT range."""
+    Q = 1 << logQ
+    a = [Q - 1] * N
+    want = [(2 * k + 2 - N) % Q for k in range(N)]
+    assert ring.pm(a, a, Q) == want
+    if N <= 256:
+        assert ring.pm_schoolbook(a, a, Q) == want
+    assert ring.pm_ntt(a, a, Q) == want
+
+
+# ---- P6: reduction to one library big-int multiply (Kronecker substitution) ----------------------
+def _kronecker(a, b, M):
+    N = len(a)
+    w = 2 * max(max(a), max(b), 1).bit_length() + N.bit_length() + 1
+    A = sum(int(v) << (w * i) for i, v in enumerate(a))
+    B = sum(int(v) << (w * i) for i, v in enumerate(b))
+    C = A * B
+    mask = (1 << w) - 1
+    ct = [(C >> (w * i)) & mask for i in range(2 * N)]
+    return [(ct[i] - ct[N + i]) % M for i in range(N)]
+
+
+@pytest.mark.parametrize("N,logQ", [(64, 128), (1024, 128), (4096, 218)])
+def test_p6_kronecker(N, logQ):
+    g = synth.rng(60 + N)
+    Q = 1 << logQ
+    a = synth.uniform_big(g, N, logQ)
+    b = synth.uniform_big(g, N, logQ)
+    want = _kronecker(a, b, Q)
+    assert ring.pm_ntt(a, b, Q) == want
+    if N <= 1024:
+        assert ring.pm_schoolbook(a, b, Q) == want       # schoolbook vs its NTT at N <= 2^10
+    for k in (0, N // 2, N - 1):
+        assert ring.pm_coeff(a, b, k, Q) == want[k]
+
+
+# ---- P7: transforms and CRT ------------------------------------------------------------------
+@pytest.mark.parametrize("N", [8, 64])
+def test_p7_ntt_matches_eq8_and_inverts(N):
+    q = ntt.oracle_primes(N, 1 << 40)[1]
+    assert q % (2 * N) == 1 and ntt.is_prime(q)
+    psi = ntt.primitive_2n_root(q, N)
+    assert pow(psi, N, q) == q - 1 and pow(psi, 2 * N, q) == 1
+    rnd = random.Random(N)
+    a = np.array([rnd.randrange(q) for _ in range(N)], dtype=np.uint64)
+    fa = ntt.ntt_forward(a, q, psi)
+    assert [int(v) for v in fa] == ntt.ntt_forward_direct(a, q, psi)          # Eq. 8 literally
+    assert np.array_equal(ntt.ntt_inverse(fa, q, psi), a)                      # Eq. 9 inverts Eq. 8
+
+
+def test_p7_ntt_roundtrip_large_and_convolution():
+    N = 4096
+    q = ntt.oracle_primes(N, 1)[0]
+    psi = ntt.primitive_2n_root(q, N)
+    g = synth.rng(7)
+    a = g.integers(0, q, size=N, dtype=np.uint64)
+    b = g.integers(0, q, size=N, dtype=np.uint64)
+    assert np.array_equal(ntt.ntt_inverse(ntt.ntt_forward(a, q, psi), q, psi), a)
+    c = ntt.ntt_inverse(ntt.ntt_forward(a, q, psi) * ntt.ntt_forward(b, q, psi) % np.uint64(q), q, psi)
+    for k in (0, 17, N - 1):                                                   # Eq. 7 against Eq. 5-6
+        assert int(c[k]) == ring.pm_coeff(a.tolist(), b.tolist(), k, q)
+
+
+def test_p7_crt_roundtrip():
+    primes = ntt.oracle_primes(64, 1 << 200)
+    Mp = 1
+    for q in primes:
+        Mp *= q
+    rnd = random.Random(9)
+    xs = [rnd.randrange(Mp) for _ in range(5)] + [0, 1, Mp - 1]
+    res = [np.array([x % q for x in xs], dtype=np.uint64) for q in primes]
+    got, Mp2 = ring.crt_direct(res, primes)
+    assert Mp2 == Mp and got == xs
+
+
+def test_miller_rabin_small():
+    sieve = [n for n in range(2, 2000) if all(n % d for d in range(2, int(n ** 0.5) + 1))]
+    assert [n for n in range(2, 2000) if ntt.is_prime(n)] == sieve
+    assert not ntt.is_prime(3215031751) and ntt.is_prime(2147483647)          # strong pseudoprime to 2,3,5,7
+
+
+# ---- limbs -----------------------------------------------------------------------------------
+def test_limb_packing():
+    rnd = random.Random(1)
+    xs = [rnd.randrange(1 << 218) for _ in range(16)] + [0, (1 << 218) - 1]
+    arr = to_limbs(xs, 7)
+    assert arr.shape == (7, 18) and arr.dtype == np.uint32
+    assert from_limbs(arr) == xs
+    assert int(arr[0, -1]) == 0xFFFFFFFF and int(arr[6, -1]) == (1 << (218 - 192)) - 1
+    g = synth.rng(5)
+    u = synth.uniform_limbs(g, (2,), 8, 218)
+    assert u.shape == (2, 7, 8) and int(u[:, 6].max()) < (1 << 26)
+
+
+# ---- moduli ----------------------------------------------------------------------------------
+def test_bgv_modulus_c4():
+    g = _read_golden("moduli.txt")
+    t, lg, off = g["t"][0], g["log"][0], g["offset"][0]
+    Q = scheme.make_modulus(lg, t)
+    assert Q == (1 << lg) + off and Q % 2 == 1 and Q % t == 1
+    assert all(not (c % 2 == 1 and c % t == 1) for c in range((1 << lg) + 1, Q))
+    prm = scheme.Params(1 << 14, 437, 437, t)
+    assert prm.P == prm.Q and prm.L == 14 and prm.L_PQ == 28
+    assert scheme.Params(1 << 16, 1240, 1240).L == 39 and scheme.Params(1 << 16, 1240, 1240).L_PQ == 78
+
+
+# ---- R1: rescale rounding interval -----------------------------------------------------------------
+def test_r1_rescale_interval():
+    prm = scheme.Params(16, 128, 128)
+    g = synth.rng(11)
+    ct = (synth.uniform_big(g, 16, 128), synth.uniform_big(g, 16, 128))
+    ct[0][0] = 0
+    ct[0][1] = (1 << 128) - 1
+    ct[0][2] = 1 << 39
+    ct[0][3] = (1 << 39) - 1
+    for p in (1, 40, 127):
+        out = scheme.rescale(prm, ct, p)
+        Q2 = 1 << (128 - p)
+        for comp_in, comp_out in zip(ct, out):
+            for c, cp in zip(comp_in, comp_out):
+                assert 0 <= cp < Q2
+                # cp = round(c / 2^p) mod Q2 with ties up: 2^p cp - c in (-2^(p-1), 2^(p-1)] mod 2^logQ
+                diff = ring.centre((cp << p) - c, 1 << 128)
+                assert -(1 << (p - 1)) < diff <= (1 << (p - 1))
+    assert scheme.rescale(prm, ([1 << 39] + [0] * 15, [0] * 16), 40)[0][0] == 1      # tie rounds up
+    assert scheme.rescale(prm, ([(1 << 39) - 1] + [0] * 15, [0] * 16), 40)[0][0] == 0
+
+
+# ---- harness: encode / decode ------------------------------------------------------------------
+def test_encode_decode_roundtrip_and_homomorphism():
+    N, D = 256, float(1 << 40)
+    g = synth.rng(21)
+    z1, z2 = synth.unit_disk(g, N // 2), synth.unit_disk(g, N // 2)
+    assert np.abs(z1).max() <= 1.0
+    m1, m2 = harness.encode(z1, N, D), harness.encode(z2, N, D)
+    assert np.abs(harness.decode(m1, N, D) - z1).max() < 1e-9
+    # direct evaluation of m(zeta_j) for one slot (kernel of Eq. 10)
+    j = 5
+    zeta = np.exp(1j * np.pi * (2 * j + 1) / N)
+    direct = sum(int(m1[k]) * zeta ** k for k in range(N)) / D
+    assert abs(direct - z1[j]) < 1e-9
+    big = 1 << 200
+    prod = [ring.centre(v, big) for v in ring.pm_schoolbook(m1, m2, big)]
+    assert np.abs(harness.decode(prod, N, D * D) - z1 * z2).max() < 1e-8
+
+
+def test_pm_sparse_matches_definition():
+    N, Q = 64, 1 << 77
+    g = synth.rng(31)
+    a = synth.uniform_big(g, N, 77)
+    s = [int(v) for v in synth.ternary_hwt(g, N, 9)]
+    assert harness.pm_sparse(a, s, Q) == ring.pm_schoolbook(a, [v % Q for v in s], Q)
+    assert sum(1 for v in s if v) == 9 and set(s) <= {-1, 0, 1}
+
+
+# ---- R2/R3/R5: CKKS ----------------------------------------------------------------------------
+def _ckks_setup(N, logQ, logP, seed, hwt):
+    prm = scheme.Params(N, logQ, logP)
+    g = synth.rng(seed)
+    s, evk = harness.keygen(prm, g, hwt=hwt)
+    D = float(1 << 40)
+    z1, z2 = synth.unit_disk(g, N // 2), synth.unit_disk(g, N // 2)
+    ct1 = harness.encrypt(prm, g, s, harness.encode(z1, N, D))
+    ct2 = harness.encrypt(prm, g, s, harness.encode(z2, N, D))
+    return prm, s, evk, z1, z2, ct1, ct2, D
+
+
+def test_r3_ckks_end_to_end_config1():
+    """BASELINE.json configs[0]: N=2^10, Q=P=2^128, Delta=2^40, HWT 64, sigma 3.2, seed 0."""
+    N = 1 << 10
+    prm, s, evk, z1, z2, ct1, ct2, D = _ckks_setup(N, 128, 128, 0, 64)
+    assert np.abs(harness.decode(harness.decrypt(ct1, s, prm.Q), N, D) - z1).max() < 1e-6
+    d = scheme.he_mult(prm, ct1, ct2)
+    # tensor triple decrypts to the product of the two decryptions (exact ring identity)
+    mu1 = harness.decrypt(ct1, s, prm.Q)
+    mu2 = harness.decrypt(ct2, s, prm.Q)
+    assert harness.decrypt3(d, s, prm.Q) == [ring.centre(v, prm.Q) for v in ring.pm(mu1, mu2, prm.Q)]
+    r = scheme.relinearize(prm, d, evk)
+    # R2: relinearisation changes the decryption only by a small error
+    err = [ring.centre(x - y, prm.Q) for x, y in zip(harness.decrypt(r, s, prm.Q), harness.decrypt3(d, s, prm.Q))]
+    assert max(abs(e) for e in err) < (1 << 20)
+    out = scheme.rescale(prm, r, 40)
+    got = harness.decode(harness.decrypt(out, s, prm.Q >> 40), N, D)
+    assert np.abs(got - z1 * z2).max() <= 2.0 ** -20                         # north_star bound
+
+
+def test_r5_degenerate_relin_ckks():
+    N = 64
+    prm = scheme.Params(N, 96, 96)
+    g = synth.rng(55)
+    d0, d1, d2 = (synth.uniform_big(g, N, 96) for _ in range(3))
+    s = [int(v) for v in synth.ternary_hwt(g, N, 8)]
+    zero = [0] * N
+    evk_rand = (synth.uniform_big(g, N, 192), synth.uniform_big(g, N, 192))
+    assert scheme.relinearize(prm, (d0, d1, zero), evk_rand) == (d0, d1)      # d2 = 0
+    s2 = ring.pm([v % prm.PQ for v in s], [v % prm.PQ for v in s], prm.PQ)
+    evk0 = ([(prm.P * v) % prm.PQ for v in s2], zero)                         # e' = 0, a' = 0
+    o0, o1 = scheme.relinearize(prm, (d0, d1, d2), evk0)
+    d2s2 = ring.pm(d2, [v % prm.Q for v in s2], prm.Q)
+    assert o0 == ring.add(d0, d2s2, prm.Q) and o1 == d1                       # k_b = d2 s^2 exactly
+
+
+# ---- R4/R5: BGV --------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,logQ,t,hwt", [(64, 80, 257, 16), (256, 120, 65537, None)])
+def test_r4_bgv_exact(N, logQ, t, hwt):
+    prm = scheme.Params(N, logQ, logQ, t)
+    assert prm.Q % t == 1 and prm.Q % 2 == 1 and prm.P == prm.Q
+    g = synth.rng(77 + N)
+    s, evk = harness.keygen(prm, g, hwt=hwt)
+    m1 = [int(v) for v in synth.uniform_mod(g, N, t)]
+    m2 = [int(v) for v in synth.uniform_mod(g, N, t)]
+    ct1, ct2 = harness.encrypt(prm, g, s, m1), harness.encrypt(prm, g, s, m2)
+    assert harness.decrypt_bgv(ct1, s, prm) == m1
+    d = scheme.he_mult(prm, ct1, ct2)
+    want = ring.pm(m1, m2, t)
+    assert [v % t for v in harness.decrypt3(d, s, prm.Q)] == want
+    r = scheme.relinearize(prm, d, evk)
+    assert harness.decrypt_bgv(r, s, prm) == want                             # exact mod t
+    # R2: the switch error is a multiple of t and small
+    err = [ring.centre(x - y, prm.Q) for x, y in zip(harness.decrypt(r, s, prm.Q), harness.decrypt3(d, s, prm.Q))]
+    assert all(e % t == 0 for e in err) and max(abs(e) for e in err) < t * N * 64
+    zero = [0] * N
+    assert scheme.relinearize(prm, (d[0], d[1], zero), evk) == (d[0], d[1])
