@@ -1,0 +1,148 @@
+/* fhe.h -- C ABI of the B200-native non-RNS CKKS/BGV hot path (arxiv/paper_2607_05920, "LibFHE").
+ *
+ * One thing is exported: exact negacyclic multiplication of polynomials with multi-limb coefficients in
+ * Z_Q[X]/(X^N+1) (Eq. 5-6) through the paper's limb -> RNS -> NTT -> pointwise -> iNTT ->
+ * CRT -> limb pipeline, wrapped as the homomorphic hot path
+ * mult (tensor product + relinearisation) and rescale.
+ * Readings of everything the paper leaves open are listed in DESIGN.md section 3.
+ *
+ * Conventions (all entry points)
+ *   - "d_" pointers are DEVICE memory owned by the caller, 16-byte aligned, contiguous.  "h_" pointers are HOST memory.
+ *   - A polynomial is a uint32 array [L][N]: limb index before coefficient index, limb 0 least significant
+ *     (radix representation X = sum_i x_i 2^(32 i), Eq. 22-23).  L = ceil(bits(Q)/32).
+ *   - A ciphertext is [2][L][N] = (c0, c1) with decryption c0 + c1*s; a tensor triple is [3][L][N] = (d0, d1, d2)
+ *     with decryption d0 + d1*s + d2*s^2.  A batch is the outermost dimension (the paper's `cnum`).
+ *   - Outputs are canonical representatives in [0, Q) with unused top-limb bits zero.  CKKS inputs are taken
+ *     mod 2^logQ (bits above logQ are ignored).  BGV inputs must already be < Q (precondition, not checked).
+ *   - Hot-path calls allocate nothing, enqueue on the caller's stream (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream), never synchronise and never touch host copies of data.  Outputs must not alias
+ *     inputs or the workspace.  The workspace is caller-supplied device memory of at least
+ *     fhe_workspace_bytes(ctx, op, batch) bytes, 256-byte aligned.
+ *   - Errors are return codes only: no exceptions, no abort, nothing printed.  Argument errors are detected
+ *     before anything is launched.  fhe_last_error(ctx) returns a static or ctx-owned string for the last failure.
+ *   - A context is not thread-safe; use one per host thread / stream.
+ */
+#ifndef FHE_H_
+#define FHE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fhe_ctx fhe_ctx; /* opaque: owns prime/twiddle/CRT tables (device) and the transformed evk */
+
+typedef enum {
+  FHE_OK = 0,
+  FHE_ERR_ARG = 1,         /* NULL pointer, misaligned pointer, bad size, batch == 0 handled as OK no-op */
+  FHE_ERR_UNSUPPORTED = 2, /* parameter combination the library does not implement */
+  FHE_ERR_STATE = 3,       /* e.g. fhe_relinearize before fhe_set_evk */
+  FHE_ERR_CUDA = 4,        /* a CUDA runtime call failed; text in fhe_last_error */
+  FHE_ERR_NOMEM = 5        /* host or device allocation failed, or workspace too small */
+} fhe_status;
+
+typedef enum {            /* `op` argument of fhe_workspace_bytes */
+  FHE_OP_POLYMUL = 0,
+  FHE_OP_HE_MULT = 1,
+  FHE_OP_RELINEARIZE = 2,
+  FHE_OP_RESCALE = 3,     /* needs no workspace: returns 0 */
+  FHE_OP_MULT_RELIN_RESCALE = 4,
+  FHE_OP_SET_EVK = 5
+} fhe_op;
+
+typedef struct {
+  uint32_t N;        /* ring degree */
+  uint32_t logQ;     /* as given to fhe_ctx_create */
+  uint32_t logP;
+  uint64_t t;        /* 0 = CKKS, else BGV plaintext modulus */
+  uint32_t bitsQ;    /* bit length of Q-1 (CKKS: logQ; BGV: logQ+1) */
+  uint32_t bitsPQ;   /* bit length of P*Q-1 */
+  uint32_t L;        /* uint32 limbs per coefficient mod Q */
+  uint32_t L_PQ;     /* uint32 limbs per coefficient mod P*Q (the evk) */
+  uint32_t K_pm;     /* NTT primes used by fhe_polymul   (product > 4*N*Q^2, see DESIGN.md 3-A5) */
+  uint32_t K1;       /* NTT primes used by fhe_he_mult   (product > 8*N*Q^2) */
+  uint32_t K2;       /* NTT primes used by fhe_relinearize (product > 4*N*Q*PQ) */
+  uint32_t n_sm;     /* SM count of the device the context lives on */
+} fhe_info;
+
+/* Create a context on the current CUDA device.
+ *   t == 0 : CKKS, Q = 2^logQ, P = 2^logP
+ *   t  > 0 : BGV, t odd and < 2^31; Q = least odd integer > 2^logQ with Q = 1 (mod t), P likewise from logP
+ *            (so logP == logQ gives P == Q)                                 (DESIGN.md 3-A10, A11)
+ *   N a power of two, 2^8 <= N <= 2^16; 32 <= logQ; logQ, logP <= 2560.
+ * Precomputes on the host and uploads: the NTT primes (31-bit, = 1 mod 2^17), psi/psi^-1 power
+ * tables with Shoup companions, 2^(26 d) mod q_j and the CRT constants
+ * (this build uses the direct form of Eq. 1).  Synchronises. */
+fhe_status fhe_ctx_create(fhe_ctx** out, uint32_t N, uint32_t logQ, uint32_t logP, uint64_t t);
+void fhe_ctx_destroy(fhe_ctx* ctx);
+fhe_status fhe_ctx_info(const fhe_ctx* ctx, fhe_info* out);
+const char* fhe_last_error(const fhe_ctx* ctx); /* ctx may be NULL: returns the last create-time error */
+
+/* Copy Q (which = 0) or P (1) or P*Q (2) to h_limbs as little-endian uint32 limbs; n_limbs must be >= the
+ * limb count of the value (L, L_P, L_PQ+1 suffices).  Extra limbs are zeroed.  Host-only helper for callers. */
+fhe_status fhe_get_modulus(const fhe_ctx* ctx, int which, uint32_t* h_limbs, uint32_t n_limbs);
+
+/* Bytes of device workspace the op needs for `batch` items (0 if none). */
+size_t fhe_workspace_bytes(const fhe_ctx* ctx, int op, uint32_t batch);
+
+/* Install the relinearisation key evk = (b', a') mod P*Q, d_evk = [2][L_PQ][N] (DESIGN.md 3-A2: b' = -a's + e'
+ * + P s^2, resp. + t e' for BGV).  Decomposes it into the K2 relin primes and stores its forward NTT
+ * ("evk-hat", [2][K2][N]) inside the context (device allocation on first call).  Once per key; enqueued on
+ * `stream`; d_evk may be freed after the stream reaches this point.  d_ws: FHE_OP_SET_EVK bytes. */
+fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t ws_bytes, void* stream);
+
+/* out[i] = a[i] * b[i] in Z_Q[X]/(X^N+1), i < batch.  d_out, d_a, d_b: [batch][L][N]. */
+fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,
+                       void* d_ws, size_t ws_bytes, void* stream);
+
+/* Tensor product (north_star item 4): d0 = c0 c0', d1 = c0 c1' + c1 c0', d2 = c1 c1' (mod Q).
+ * d_out3: [batch][3][L][N]; d_ct1, d_ct2: [batch][2][L][N]. */
+fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, const uint32_t* d_ct2,
+                       uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Relinearisation (formulas DESIGN.md 3-A2..A4, A10): with x_b = d2*b', x_a = d2*a' in [0, PQ),
+ *   CKKS: k = ((x + 2^(logP-1)) >> logP) mod Q
+ *   BGV : r = x mod P centred, kk = (-r P^-1) mod t centred, k = ((x - r)/P - kk) mod Q
+ * out = ((d0 + k_b) mod Q, (d1 + k_a) mod Q).  d_out2: [batch][2][L][N]; d_in3: [batch][3][L][N].
+ * FHE_ERR_STATE if no evk is installed. */
+fhe_status fhe_relinearize(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in3, uint32_t batch, void* d_ws,
+                           size_t ws_bytes, void* stream);
+
+/* CKKS rescale by 2^p (DESIGN.md 3-A3): c' = ((c + 2^(p-1)) >> p) mod 2^(logQ-p) on the
+ * canonical c, every component.  d_out2, d_in2: [batch][2][L][N] (same L-limb stride; top bits zero).
+ * 1 <= p_bits < logQ.  FHE_ERR_UNSUPPORTED on a BGV context.  In-place (d_out2 == d_in2) is allowed here. */
+fhe_status fhe_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uint32_t p_bits, uint32_t batch,
+                       void* stream);
+
+/* Convenience for the headline metric: he_mult -> relinearize -> rescale (p_bits == 0: no rescale; BGV requires 0)
+ * without materialising d0/d1/d2 for the caller.  Result identical to the three calls in sequence. */
+fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct1, const uint32_t* d_ct2,
+                                  uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
+
+/* Same computation as fhe_mult_relin_rescale with HOST buffers (pageable or pinned): copies the inputs to the
+ * device, runs, copies the result back and synchronises `stream`.  d_ws must additionally hold the device copies:
+ * fhe_workspace_bytes(op) + 3 ciphertext batches.  Used for the end-to-end ("e2e") measurement. */
+fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uint32_t* h_ct1, const uint32_t* h_ct2,
+                                       uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
+
+/* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
+
+/* Host copies of the first `count` NTT primes and the primitive 2N-th roots psi_j the tables were built from. */
+fhe_status fhe_debug_primes(const fhe_ctx* ctx, uint32_t* h_q, uint32_t* h_psi, uint32_t count);
+/* S1: d_res [npoly][K][N] = residues of d_limbs [npoly][Lin][N] mod the first K primes.
+ * mask_bits > 0: the input is first reduced mod 2^mask_bits (CKKS load masking). */
+fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_limbs, uint32_t npoly, uint32_t Lin,
+                               uint32_t K, uint32_t mask_bits, void* stream);
+/* S2 / S4 (Eq. 8-9) in place on d_res [npoly][K][N].  Forward output is in bit-reversed index
+ * order: res[bitrev(i)] = sum_j a_j psi^((2i+1) j).  inverse != 0: expects that order, returns natural order,
+ * scaled by N^-1 only (no CRT constant folded in). */
+fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream);
+/* Number of kernel launches the context has enqueued so far (for bench.py's gpu_launches). */
+uint64_t fhe_debug_launch_count(const fhe_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FHE_H_ */

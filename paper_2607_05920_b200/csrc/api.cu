@@ -1,0 +1,229 @@
+// api.cu -- the hot-path entry points: argument checks, then kernel launches on the caller's stream.  No allocation,
+// no synchronisation, no host copies (except the explicit *_host end-to-end variant).
+#include "fhe_internal.cuh"
+
+using namespace fhe;
+
+namespace {
+
+inline Context* C(fhe_ctx* p) { return reinterpret_cast<Context*>(p); }
+inline const Context* C(const fhe_ctx* p) { return reinterpret_cast<const Context*>(p); }
+inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) != 0; }
+
+fhe_status err(Context* c, fhe_status st, const char* msg) { c->err = msg; return st; }
+fhe_status cuda_fail(Context* c, cudaError_t e, const char* where) {
+  c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return FHE_ERR_CUDA;
+}
+#define CK(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, where); } while (0)
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+size_t ws_polymul(const Context* c, uint32_t b) { return align256((size_t)b * 2 * c->K_pm * c->N * 4); }
+size_t ws_tensor(const Context* c, uint32_t b) { return align256((size_t)b * 4 * c->K1 * c->N * 4); }
+size_t ws_relin(const Context* c, uint32_t b) { return align256((size_t)b * 2 * c->K2 * c->N * 4); }
+size_t ws_d3(const Context* c, uint32_t b) { return align256((size_t)b * 3 * c->L * c->N * 4); }
+size_t ws_evk(const Context* c) { return 0; }   // evk-hat is transformed in place inside the context
+
+// he_mult core: ct1, ct2 [B][2][L][N] -> out3 [B][3][L][N]; ws: [B][4][K1][N]
+fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const uint32_t* d_ct2, uint32_t B,
+                      uint32_t* ws, cudaStream_t s) {
+  const uint32_t N = c->N, L = c->L, K = c->K1;
+  const size_t rp = (size_t)K * N;           // residue poly stride
+  const uint32_t mask = c->t == 0 ? c->logQ : 0;
+  // slots (a0, a1, b0, b1) per batch item: ct1 polys go to slots 0,1 ; ct2 polys to slots 2,3
+  for (uint32_t comp = 0; comp < 2; ++comp) {
+    // all batch items of component `comp`: input poly stride 2*L*N, output stride 4*rp
+    CK(launch_decompose(c, ws + comp * rp, 4 * rp, d_ct1 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
+    CK(launch_decompose(c, ws + (2 + comp) * rp, 4 * rp, d_ct2 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
+  }
+  CK(launch_ntt(c, ws, B * 4, K, false, nullptr, s), "ntt fwd");
+  CK(launch_pw_tensor(c, ws, B, K, s), "pointwise tensor");
+  // inverse on slots 0..2 of every item: items are 4 slots apart -> run per item group via npoly = B*4 would waste 25%;
+  // slots 0..2 of item b are contiguous [3][K][N], so launch per item
+  for (uint32_t b = 0; b < B; ++b)
+    CK(launch_ntt(c, ws + (size_t)b * 4 * rp, 3, K, true, c->tgt_tensor.d_scale, s), "ntt inv");
+  for (uint32_t b = 0; b < B; ++b)
+    CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3 + (size_t)b * 3 * L * N, (size_t)L * N,
+                  ws + (size_t)b * 4 * rp, rp, nullptr, 0, 3, s), "crt");
+  return FHE_OK;
+}
+
+// relin core: in3 [B][3][L][N] -> out2 [B][2][L][N]; ws: [B][2][K2][N]; rescale_bits fused into the CRT epilogue
+fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_t B, uint32_t* ws, uint32_t rescale_bits,
+                    cudaStream_t s) {
+  const uint32_t N = c->N, L = c->L, K = c->K2;
+  const size_t rp = (size_t)K * N;
+  const uint32_t mask = c->t == 0 ? c->logQ : 0;
+  CK(launch_decompose(c, ws, 2 * rp, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, B, L, K, mask, s), "decompose d2");
+  for (uint32_t b = 0; b < B; ++b)
+    CK(launch_ntt(c, ws + (size_t)b * 2 * rp, 1, K, false, nullptr, s), "ntt fwd d2");
+  CK(launch_pw_relin(c, ws, c->d_evk_hat, B, K, s), "pointwise relin");
+  CK(launch_ntt(c, ws, B * 2, K, true, c->tgt_relin.d_scale, s), "ntt inv relin");
+  PostParams pp = c->post_relin;
+  pp.rescale_bits = rescale_bits;
+  for (uint32_t b = 0; b < B; ++b)
+    CK(launch_crt(c, c->tgt_relin, pp, d_out2 + (size_t)b * 2 * L * N, (size_t)L * N, ws + (size_t)b * 2 * rp, rp,
+                  d_in3 + (size_t)b * 3 * L * N, (size_t)L * N, 2, s), "crt relin");
+  return FHE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t fhe_workspace_bytes(const fhe_ctx* ctx, int op, uint32_t batch) {
+  if (!ctx) return 0;
+  const Context* c = C(ctx);
+  switch (op) {
+    case FHE_OP_POLYMUL: return ws_polymul(c, batch);
+    case FHE_OP_HE_MULT: return ws_tensor(c, batch);
+    case FHE_OP_RELINEARIZE: return ws_relin(c, batch);
+    case FHE_OP_RESCALE: return 0;
+    case FHE_OP_MULT_RELIN_RESCALE: {
+      size_t a = ws_tensor(c, batch), b = ws_relin(c, batch);
+      return (a > b ? a : b) + ws_d3(c, batch);
+    }
+    case FHE_OP_SET_EVK: return ws_evk(c);
+    default: return 0;
+  }
+}
+
+fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  (void)d_ws; (void)ws_bytes;
+  if (!d_evk || misaligned(d_evk, 16)) return err(c, FHE_ERR_ARG, "d_evk NULL or misaligned");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t bytes = (size_t)2 * c->K2 * c->N * 4;
+  if (!c->d_evk_hat) {
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return err(c, FHE_ERR_NOMEM, "evk-hat allocation failed"); }
+    c->d_evk_hat = (uint32_t*)p;
+  }
+  c->have_evk = false;
+  const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
+  CK(launch_decompose(c, c->d_evk_hat, (size_t)c->K2 * c->N, d_evk, (size_t)c->L_PQ * c->N, 2, c->L_PQ, c->K2, mask, s), "decompose evk");
+  CK(launch_ntt(c, c->d_evk_hat, 2, c->K2, false, nullptr, s), "ntt evk");
+  c->have_evk = true;
+  return FHE_OK;
+}
+
+fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,
+                       void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out || !d_a || !d_b || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out, 16) || misaligned(d_a, 16) || misaligned(d_b, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (ws_bytes < ws_polymul(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  cudaStream_t s = (cudaStream_t)stream;
+  const uint32_t N = c->N, L = c->L, K = c->K_pm;
+  const size_t rp = (size_t)K * N;
+  uint32_t* ra = (uint32_t*)d_ws;
+  uint32_t* rb = ra + (size_t)batch * rp;
+  const uint32_t mask = c->t == 0 ? c->logQ : 0;
+  CK(launch_decompose(c, ra, rp, d_a, (size_t)L * N, batch, L, K, mask, s), "decompose a");
+  CK(launch_decompose(c, rb, rp, d_b, (size_t)L * N, batch, L, K, mask, s), "decompose b");
+  CK(launch_ntt(c, ra, 2 * batch, K, false, nullptr, s), "ntt fwd");
+  CK(launch_pw_polymul(c, ra, rb, batch, K, s), "pointwise");
+  CK(launch_ntt(c, ra, batch, K, true, c->tgt_pm.d_scale, s), "ntt inv");
+  CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, (size_t)L * N, ra, rp, nullptr, 0, batch, s), "crt");
+  return FHE_OK;
+}
+
+fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, const uint32_t* d_ct2, uint32_t batch,
+                       void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out3 || !d_ct1 || !d_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out3, 16) || misaligned(d_ct1, 16) || misaligned(d_ct2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (ws_bytes < ws_tensor(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  return do_he_mult(c, d_out3, d_ct1, d_ct2, batch, (uint32_t*)d_ws, (cudaStream_t)stream);
+}
+
+fhe_status fhe_relinearize(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in3, uint32_t batch, void* d_ws,
+                           size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_in3 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_in3, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (!c->have_evk) return err(c, FHE_ERR_STATE, "no evk installed (call fhe_set_evk first)");
+  if (ws_bytes < ws_relin(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  return do_relin(c, d_out2, d_in3, batch, (uint32_t*)d_ws, 0, (cudaStream_t)stream);
+}
+
+fhe_status fhe_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uint32_t p_bits, uint32_t batch,
+                       void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (c->t != 0) return err(c, FHE_ERR_UNSUPPORTED, "rescale is CKKS-only");
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_in2) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_in2, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (p_bits < 1 || p_bits >= c->logQ) return err(c, FHE_ERR_ARG, "p_bits out of range");
+  CK(launch_rescale(c, d_out2, d_in2, batch * 2, p_bits, (cudaStream_t)stream), "rescale");
+  return FHE_OK;
+}
+
+fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct1, const uint32_t* d_ct2,
+                                  uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_ct1 || !d_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_ct1, 16) || misaligned(d_ct2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (!c->have_evk) return err(c, FHE_ERR_STATE, "no evk installed (call fhe_set_evk first)");
+  if (c->t != 0 && p_bits != 0) return err(c, FHE_ERR_UNSUPPORTED, "rescale is CKKS-only");
+  if (p_bits >= c->logQ) return err(c, FHE_ERR_ARG, "p_bits out of range");
+  if (ws_bytes < fhe_workspace_bytes(ctx, FHE_OP_MULT_RELIN_RESCALE, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  cudaStream_t s = (cudaStream_t)stream;
+  uint32_t* d3 = (uint32_t*)d_ws;
+  uint32_t* ws = (uint32_t*)((char*)d_ws + ws_d3(c, batch));
+  fhe_status st = do_he_mult(c, d3, d_ct1, d_ct2, batch, ws, s);
+  if (st != FHE_OK) return st;
+  return do_relin(c, d_out2, d3, batch, ws, p_bits, s);
+}
+
+fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uint32_t* h_ct1, const uint32_t* h_ct2,
+                                       uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!h_out2 || !h_ct1 || !h_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  const size_t ctb = align256((size_t)batch * 2 * c->L * c->N * 4);
+  const size_t inner = fhe_workspace_bytes(ctx, FHE_OP_MULT_RELIN_RESCALE, batch);
+  if (ws_bytes < inner + 3 * ctb) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  cudaStream_t s = (cudaStream_t)stream;
+  char* base = (char*)d_ws + inner;
+  uint32_t* d1 = (uint32_t*)base; uint32_t* d2 = (uint32_t*)(base + ctb); uint32_t* d_o = (uint32_t*)(base + 2 * ctb);
+  const size_t bytes = (size_t)batch * 2 * c->L * c->N * 4;
+  CK(cudaMemcpyAsync(d1, h_ct1, bytes, cudaMemcpyHostToDevice, s), "H2D ct1");
+  CK(cudaMemcpyAsync(d2, h_ct2, bytes, cudaMemcpyHostToDevice, s), "H2D ct2");
+  fhe_status st = fhe_mult_relin_rescale(ctx, d_o, d1, d2, p_bits, batch, d_ws, inner, stream);
+  if (st != FHE_OK) return st;
+  CK(cudaMemcpyAsync(h_out2, d_o, bytes, cudaMemcpyDeviceToHost, s), "D2H out");
+  CK(cudaStreamSynchronize(s), "sync");
+  return FHE_OK;
+}
+
+fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_limbs, uint32_t npoly, uint32_t Lin,
+                               uint32_t K, uint32_t mask_bits, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (!d_res || !d_limbs || K == 0 || K > c->Kmax || Lin == 0 || Lin > MAX_LIMBS_IN) return err(c, FHE_ERR_ARG, "bad argument");
+  CK(launch_decompose(c, d_res, (size_t)K * c->N, d_limbs, (size_t)Lin * c->N, npoly, Lin, K, mask_bits, (cudaStream_t)stream), "decompose");
+  return FHE_OK;
+}
+
+fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (!d_res || K == 0 || K > c->Kmax) return err(c, FHE_ERR_ARG, "bad argument");
+  CK(launch_ntt(c, d_res, npoly, K, inverse != 0, c->d_scale_plain, (cudaStream_t)stream), "ntt");
+  return FHE_OK;
+}
+
+}  // extern "C"

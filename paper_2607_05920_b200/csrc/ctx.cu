@@ -1,0 +1,349 @@
+// ctx.cu -- fhe_ctx_create: host precomputation of every table the kernels read (section 5.2),
+// uploaded once.  Nothing here runs on the hot path.
+#include <cstring>
+#include <new>
+
+#include "bigu.hpp"
+#include "fhe_internal.cuh"
+
+namespace fhe {
+
+static std::string g_create_err;
+
+// ---- word-sized number theory ------------------------------------------------------------------------------------
+static inline uint32_t mulmod(uint32_t a, uint32_t b, uint32_t m) { return (uint32_t)((uint64_t)a * b % m); }
+static uint32_t powmod(uint32_t a, uint64_t e, uint32_t m) {
+  uint32_t r = 1 % m;
+  a %= m;
+  while (e) {
+    if (e & 1) r = mulmod(r, a, m);
+    a = mulmod(a, a, m);
+    e >>= 1;
+  }
+  return r;
+}
+static bool is_prime32(uint32_t n) {   // deterministic Miller-Rabin for n < 2^32 (bases 2, 7, 61)
+  if (n < 2) return false;
+  for (uint32_t p : {2u, 3u, 5u, 7u, 11u, 13u, 17u, 19u, 23u, 29u, 31u, 37u}) {
+    if (n % p == 0) return n == p;
+  }
+  uint32_t d = n - 1, r = 0;
+  while ((d & 1) == 0) { d >>= 1; ++r; }
+  for (uint32_t a : {2u, 7u, 61u}) {
+    uint32_t x = powmod(a, d, n);
+    if (x == 1 || x == n - 1) continue;
+    bool comp = true;
+    for (uint32_t i = 1; i < r; ++i) {
+      x = mulmod(x, x, n);
+      if (x == n - 1) { comp = false; break; }
+    }
+    if (comp) return false;
+  }
+  return true;
+}
+static uint32_t bitrev(uint32_t x, uint32_t bits) {
+  uint32_t r = 0;
+  for (uint32_t i = 0; i < bits; ++i) r |= ((x >> i) & 1u) << (bits - 1 - i);
+  return r;
+}
+static inline uint32_t shoup(uint32_t w, uint32_t q) { return (uint32_t)(((uint64_t)w << 32) / q); }
+
+template <class T>
+static cudaError_t upload(Context* c, T** dptr, const std::vector<T>& h) {
+  void* p = nullptr;
+  size_t bytes = h.size() * sizeof(T);
+  cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
+  if (e != cudaSuccess) return e;
+  c->allocs.push_back(p);
+  *dptr = (T*)p;
+  if (bytes) e = cudaMemcpy(p, h.data(), bytes, cudaMemcpyHostToDevice);
+  return e;
+}
+
+// modulus 2^log (t == 0) or the least odd integer > 2^log that is 1 mod t
+static BigU make_modulus(uint32_t log, uint64_t t) {
+  BigU m = BigU::pow2(log);
+  if (t == 0) return m;
+  uint32_t tt = (uint32_t)t;
+  uint32_t two = powmod(2, log, tt);
+  uint32_t c0 = (uint32_t)(((uint64_t)1 + tt - two) % tt);   // (1 - 2^log) mod t
+  uint64_t c = c0 == 0 ? tt : c0;
+  if ((c & 1) == 0) c += tt;                                  // t odd: flips parity
+  m.add(BigU(c));
+  return m;
+}
+
+// smallest K such that the product of the first K primes exceeds bound; extends the prime list on demand
+static uint32_t primes_for(std::vector<uint32_t>& primes, const BigU& bound) {
+  BigU M((uint64_t)1);
+  uint32_t K = 0;
+  uint32_t cand = primes.empty() ? 0x80000001u - (1u << 17) : primes.back() - (1u << 17);
+  while (BigU::cmp(M, bound) <= 0) {
+    if (K == primes.size()) {
+      while (!is_prime32(cand)) cand -= (1u << 17);
+      primes.push_back(cand);
+      cand -= (1u << 17);
+    }
+    M.mul_small(primes[K]);
+    ++K;
+  }
+  return K;
+}
+
+static void digits_of(const BigU& x, uint32_t wbits, uint32_t D, uint32_t* out) {
+  for (uint32_t d = 0; d < D; ++d) {
+    uint32_t bit = d * wbits, w = bit >> 5, sh = bit & 31;
+    uint64_t v = (uint64_t)x.limb(w) | ((uint64_t)x.limb(w + 1) << 32);
+    out[d] = (uint32_t)((v >> sh) & ((1ull << wbits) - 1ull));
+  }
+}
+
+// T_kind: 0 -> T = 2^(wbits D) covering `width_bits`; 1 -> T = the odd modulus `Tmod`
+static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2, uint32_t width_bits,
+                                const BigU& Tmod) {
+  tg.K = K;
+  tg.wbits = (K + 1 <= 127) ? 26 : (K + 1 <= 255) ? 25 : 24;
+  uint32_t clogK = 0;
+  while ((1u << clogK) < K + 1) ++clogK;
+  uint32_t vbits = pow2 ? width_bits : (Tmod.bits() + 31 + clogK + 1);
+  tg.D = (vbits + tg.wbits - 1) / tg.wbits;
+  tg.Dpad = (tg.D + 7) / 8 * 8;
+  tg.Lraw = (tg.D * tg.wbits + 31) / 32;
+  BigU T = pow2 ? BigU::pow2(tg.wbits * tg.D) : Tmod;
+  BigU M((uint64_t)1);
+  for (uint32_t i = 0; i < K; ++i) M.mul_small(c->h_q[i]);
+  std::vector<uint32_t> W((size_t)(K + 1) * tg.Dpad, 0u);
+  std::vector<uint2> scale(K);
+  for (uint32_t i = 0; i < K; ++i) {
+    const uint32_t q = c->h_q[i];
+    BigU Mi = M;
+    uint32_t rem = Mi.divmod_small(q);
+    if (rem != 0) return cudaErrorUnknown;
+    uint32_t inv = powmod(Mi.mod_small(q), q - 2, q);              // (M/q_i)^-1 mod q_i
+    BigU Wi = pow2 ? Mi.low_bits(tg.wbits * tg.D) : BigU::mod(Mi, T);
+    digits_of(Wi, tg.wbits, tg.D, &W[(size_t)i * tg.Dpad]);
+    uint32_t ninv = powmod(c->N % q, q - 2, q);
+    uint32_t r32 = (uint32_t)((1ull << 32) % q);
+    uint32_t sc = mulmod(mulmod(ninv, inv, q), r32, q);
+    scale[i] = make_uint2(sc, shoup(sc, q));
+  }
+  {  // row K: (-M) mod T
+    BigU Mt = pow2 ? M.low_bits(tg.wbits * tg.D) : BigU::mod(M, T);
+    BigU neg;
+    if (!Mt.is_zero()) { neg = T; neg.sub(Mt); }
+    digits_of(neg, tg.wbits, tg.D, &W[(size_t)K * tg.Dpad]);
+  }
+  cudaError_t e = upload(c, &tg.d_W, W);
+  if (e != cudaSuccess) return e;
+  return upload(c, &tg.d_scale, scale);
+}
+
+static uint64_t mu1_of(const BigU& m) {   // floor(2^(bits(m)+62) / m), in (2^62, 2^63]
+  BigU q, r;
+  BigU::divmod(BigU::pow2(m.bits() + 62), m, q, r);
+  return (uint64_t)q.limb(0) | ((uint64_t)q.limb(1) << 32);
+}
+
+static fhe_status fail(Context* c, fhe_status st, const std::string& msg) {
+  if (c) c->err = msg;
+  g_create_err = msg;
+  return st;
+}
+
+static void destroy(Context* c) {
+  if (!c) return;
+  for (void* p : c->allocs) cudaFree(p);
+  if (c->d_evk_hat) cudaFree(c->d_evk_hat);
+  delete c;
+}
+
+static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP, uint64_t t) {
+  if (!out) return fail(nullptr, FHE_ERR_ARG, "out is NULL");
+  *out = nullptr;
+  if (N < 256 || N > 65536 || (N & (N - 1))) return fail(nullptr, FHE_ERR_UNSUPPORTED, "N must be a power of two in [2^8, 2^16]");
+  if (logQ < 32 || logQ > 2560 || logP < 1 || logP > 2560) return fail(nullptr, FHE_ERR_UNSUPPORTED, "logQ in [32,2560], logP in [1,2560]");
+  if (logQ + logP + 2 > 3328) return fail(nullptr, FHE_ERR_UNSUPPORTED, "logQ + logP too large (evk wider than 3326 bits)");
+  if (t != 0 && ((t & 1) == 0 || t < 3 || t >= (1ull << 31))) return fail(nullptr, FHE_ERR_UNSUPPORTED, "BGV t must be odd, 3 <= t < 2^31");
+  Context* c = new (std::nothrow) Context();
+  if (!c) return fail(nullptr, FHE_ERR_NOMEM, "host allocation failed");
+  c->N = N; c->logQ = logQ; c->logP = logP; c->t = t;
+  while ((1u << c->logN) < N) ++c->logN;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "no CUDA device: " + m); }
+
+  const BigU Q = make_modulus(logQ, t), P = make_modulus(logP, t);
+  const BigU PQ = BigU::mul(P, Q);
+  auto bits_m1 = [](const BigU& m) { BigU x = m; x.sub(BigU((uint64_t)1)); return x.bits(); };
+  c->bitsQ = bits_m1(Q); c->bitsP = bits_m1(P); c->bitsPQ = bits_m1(PQ);
+  c->L = (c->bitsQ + 31) / 32; c->L_P = (c->bitsP + 31) / 32; c->L_PQ = (c->bitsPQ + 31) / 32;
+  c->h_Q.assign(c->L + 2, 0); Q.to_limbs(c->h_Q.data(), c->L + 2);
+  c->h_P.assign(c->L_P + 2, 0); P.to_limbs(c->h_P.data(), c->L_P + 2);
+  c->h_PQ.assign(c->L_PQ + 2, 0); PQ.to_limbs(c->h_PQ.data(), c->L_PQ + 2);
+
+  // ---- primes: 31-bit, = 1 (mod 2^17), descending from 2^31; bounds DESIGN.md 3-A5 ------------
+  {
+    BigU NQ2 = BigU::mul(Q, Q); NQ2.mul_small(N);
+    BigU b_pm = NQ2; b_pm.mul_small(4);
+    BigU b_t = NQ2; b_t.mul_small(8);
+    BigU b_r = BigU::mul(Q, PQ); b_r.mul_small(N); b_r.mul_small(4);
+    c->K_pm = primes_for(c->h_q, b_pm);
+    c->K1 = primes_for(c->h_q, b_t);
+    c->K2 = primes_for(c->h_q, b_r);
+    c->Kmax = (uint32_t)c->h_q.size();
+  }
+  const uint32_t Kmax = c->Kmax;
+
+  // ---- per-prime constants and twiddle tables ---------------------------------------------------------------------
+  std::vector<uint32_t> qn(Kmax), f62(Kmax);
+  std::vector<uint64_t> mu64(Kmax);
+  std::vector<uint2> scale_plain(Kmax);
+  std::vector<uint4> cdec((size_t)((Kmax + 3) / 4) * MAX_DIGITS_IN, make_uint4(0, 0, 0, 0));
+  c->h_psi.resize(Kmax);
+  std::vector<uint2> twf((size_t)Kmax * N), twi((size_t)Kmax * N);
+  std::vector<uint32_t> pw(N), ipw(N);
+  for (uint32_t j = 0; j < Kmax; ++j) {
+    const uint32_t q = c->h_q[j];
+    uint32_t inv = 1;                                  // q^-1 mod 2^32 by Newton iteration
+    for (int it = 0; it < 5; ++it) inv *= 2u - q * inv;
+    qn[j] = 0u - inv;
+    mu64[j] = ~0ull / q;                               // floor((2^64 - 1)/q) = floor(2^64/q): q is odd, never divides 2^64
+    f62[j] = (uint32_t)((1ull << 62) / q);
+    uint32_t psi = 0;
+    for (uint32_t g = 2; g < 2000 && !psi; ++g) {
+      uint32_t cand = powmod(g, (q - 1) / (2 * N), q);
+      if (powmod(cand, N, q) == q - 1) psi = cand;     // order exactly 2N
+    }
+    if (!psi) { destroy(c); return fail(nullptr, FHE_ERR_UNSUPPORTED, "no primitive root found"); }
+    c->h_psi[j] = psi;
+    const uint32_t ipsi = powmod(psi, q - 2, q);
+    pw[0] = ipw[0] = 1;
+    for (uint32_t k = 1; k < N; ++k) { pw[k] = mulmod(pw[k - 1], psi, q); ipw[k] = mulmod(ipw[k - 1], ipsi, q); }
+    for (uint32_t k = 0; k < N; ++k) {
+      uint32_t r = bitrev(k, c->logN);
+      twf[(size_t)j * N + k] = make_uint2(pw[r], shoup(pw[r], q));
+      twi[(size_t)j * N + k] = make_uint2(ipw[r], shoup(ipw[r], q));
+    }
+    uint32_t ninv = powmod(N % q, q - 2, q);
+    scale_plain[j] = make_uint2(ninv, shoup(ninv, q));
+    uint32_t p26 = (uint32_t)((1ull << DIGIT_BITS) % q), cur = 1;
+    for (int d = 0; d < MAX_DIGITS_IN; ++d) {
+      uint4& slot = cdec[(size_t)(j / 4) * MAX_DIGITS_IN + d];
+      (&slot.x)[j % 4] = cur;
+      cur = mulmod(cur, p26, q);
+    }
+  }
+#define UP(dst, vec)                                                                                   \
+  if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
+    std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
+  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_mu64, mu64) UP(d_f62, f62) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
+  UP(d_scale_plain, scale_plain) UP(d_cdec, cdec)
+
+  // ---- CRT targets -------------------------------------------------------------------------------------------------
+  const bool ckks = (t == 0);
+  if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q)) != cudaSuccess ||
+      (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q)) != cudaSuccess ||
+      (e = build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ)) != cudaSuccess) {
+    std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "CRT table build failed: " + m);
+  }
+
+  // ---- post-processing parameters -----------------------------------------------------------------------------------
+  PostParams pp;
+  memset(&pp, 0, sizeof(pp));
+  pp.L = c->L; pp.L_PQ = c->L_PQ; pp.L_P = c->L_P; pp.logQ = logQ; pp.logP = logP;
+  pp.bitsQ = Q.bits(); pp.bitsP = P.bits(); pp.bitsPQ = PQ.bits();   // significant bits of the moduli themselves
+  if (!ckks) {
+    std::vector<uint32_t> hQ(c->L + 2), hP(c->L_P + 2), hPQ(c->L_PQ + 2);
+    Q.to_limbs(hQ.data(), hQ.size()); P.to_limbs(hP.data(), hP.size()); PQ.to_limbs(hPQ.data(), hPQ.size());
+    UP(d_Qlimbs, hQ) UP(d_Plimbs, hP) UP(d_PQlimbs, hPQ)
+    BigU mu, r;
+    BigU::divmod(BigU::pow2(32 * c->L_PQ), P, mu, r);
+    std::vector<uint32_t> hmu(mu.v.size() + 1, 0u);
+    mu.to_limbs(hmu.data(), hmu.size());
+    UP(d_muP, hmu)
+    pp.muP_limbs = (uint32_t)mu.v.size();
+    pp.g_limbs = c->L_PQ - c->L_P;
+    if ((pp.g_limbs + 1) + pp.muP_limbs > c->K2 + 1) { destroy(c); return fail(nullptr, FHE_ERR_UNSUPPORTED, "BGV: logP too small relative to logQ for the division scratch"); }
+    const uint32_t tt = (uint32_t)t;
+    std::vector<uint32_t> p32(c->L_P + 2);
+    uint32_t cur = 1 % tt, b32 = (uint32_t)((1ull << 32) % tt);
+    for (uint32_t i = 0; i < c->L_P; ++i) { p32[i] = cur; cur = mulmod(cur, b32, tt); }
+    p32[c->L_P] = P.mod_small(tt);                       // slot L_P holds P mod t
+    UP(d_pow32_t, p32)
+    pp.d_Q = c->d_Qlimbs; pp.d_P = c->d_Plimbs; pp.d_PQ = c->d_PQlimbs; pp.d_muP = c->d_muP; pp.d_pow32_t = c->d_pow32_t;
+    pp.mu1_Q = mu1_of(Q); pp.mu1_PQ = mu1_of(PQ);
+    pp.t = tt; pp.Pinv_t = powmod(P.mod_small(tt), (uint64_t)tt - 2, tt);
+    // t need not be prime: fall back to a search-free extended Euclid if Fermat fails
+    if (mulmod(pp.Pinv_t, P.mod_small(tt), tt) != 1 % tt) {
+      int64_t a = P.mod_small(tt), b = tt, x0 = 1, x1 = 0;
+      while (b) { int64_t qq = a / b, tmp = a - qq * b; a = b; b = tmp; tmp = x0 - qq * x1; x0 = x1; x1 = tmp; }
+      if (a != 1) { destroy(c); return fail(nullptr, FHE_ERR_UNSUPPORTED, "gcd(P, t) != 1"); }
+      pp.Pinv_t = (uint32_t)((x0 % (int64_t)tt + tt) % tt);
+    }
+  }
+#undef UP
+  c->post_pm = pp;     c->post_pm.mode = ckks ? POST_CKKS_MASK : POST_BGV_MODQ;
+  c->post_tensor = c->post_pm;
+  c->post_relin = pp;  c->post_relin.mode = ckks ? POST_CKKS_RELIN : POST_BGV_RELIN;
+  e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, m); }
+  *out = c;
+  return FHE_OK;
+}
+
+}  // namespace fhe
+
+using namespace fhe;
+
+extern "C" {
+
+// fhe_ctx stays an incomplete type: an fhe_ctx* is a fhe::Context* in disguise.
+
+fhe_status fhe_ctx_create(fhe_ctx** out, uint32_t N, uint32_t logQ, uint32_t logP, uint64_t t) {
+  try {
+    return create(reinterpret_cast<Context**>(out), N, logQ, logP, t);
+  } catch (const std::bad_alloc&) {
+    g_create_err = "host allocation failed";
+    return FHE_ERR_NOMEM;
+  } catch (...) {
+    g_create_err = "unexpected host exception";
+    return FHE_ERR_ARG;
+  }
+}
+void fhe_ctx_destroy(fhe_ctx* ctx) { destroy(reinterpret_cast<Context*>(ctx)); }
+
+fhe_status fhe_ctx_info(const fhe_ctx* ctx, fhe_info* o) {
+  if (!ctx || !o) return FHE_ERR_ARG;
+  const Context* c = reinterpret_cast<const Context*>(ctx);
+  o->N = c->N; o->logQ = c->logQ; o->logP = c->logP; o->t = c->t; o->bitsQ = c->bitsQ; o->bitsPQ = c->bitsPQ;
+  o->L = c->L; o->L_PQ = c->L_PQ; o->K_pm = c->K_pm; o->K1 = c->K1; o->K2 = c->K2; o->n_sm = (uint32_t)c->n_sm;
+  return FHE_OK;
+}
+const char* fhe_last_error(const fhe_ctx* ctx) {
+  if (!ctx) return g_create_err.c_str();
+  return reinterpret_cast<const Context*>(ctx)->err.c_str();
+}
+fhe_status fhe_get_modulus(const fhe_ctx* ctx, int which, uint32_t* h, uint32_t n) {
+  if (!ctx || !h) return FHE_ERR_ARG;
+  const Context* c = reinterpret_cast<const Context*>(ctx);
+  const std::vector<uint32_t>& v = which == 0 ? c->h_Q : which == 1 ? c->h_P : c->h_PQ;
+  if (which < 0 || which > 2) return FHE_ERR_ARG;
+  size_t need = v.size();
+  while (need && v[need - 1] == 0) --need;
+  if (n < need) return FHE_ERR_ARG;
+  for (uint32_t i = 0; i < n; ++i) h[i] = i < v.size() ? v[i] : 0u;
+  return FHE_OK;
+}
+fhe_status fhe_debug_primes(const fhe_ctx* ctx, uint32_t* h_q, uint32_t* h_psi, uint32_t count) {
+  if (!ctx || !h_q || !h_psi) return FHE_ERR_ARG;
+  const Context* c = reinterpret_cast<const Context*>(ctx);
+  if (count > c->Kmax) return FHE_ERR_ARG;
+  for (uint32_t i = 0; i < count; ++i) { h_q[i] = c->h_q[i]; h_psi[i] = c->h_psi[i]; }
+  return FHE_OK;
+}
+uint64_t fhe_debug_launch_count(const fhe_ctx* ctx) {
+  return ctx ? reinterpret_cast<const Context*>(ctx)->launches : 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,133 @@
+// fhe_internal.cuh -- context layout, launch declarations and device arithmetic shared by the kernels.
+// Product code: nothing here is shared with oracle/ (tests only).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/fhe.h"
+
+namespace fhe {
+
+constexpr int DIGIT_BITS = 26;                 // decompose / CRT digit width: digit * 31-bit constant < 2^57,
+constexpr uint32_t DIGIT_MASK = (1u << DIGIT_BITS) - 1u;  // so up to 128 products fit a uint64 accumulator
+constexpr int MAX_DIGITS_IN = 128;             // decompose input: <= 8 chunks of 16 digits (13 limbs each)
+constexpr int MAX_LIMBS_IN = 104;
+
+// ---- CRT target: turns y_i = x_i * (M/q_i)^-1 mod q_i (i < K) into limbs of X = sum y_i (M/q_i) - alpha M ------------
+struct CrtTarget {
+  uint32_t K = 0;        // primes in the basis (prefix of the context's prime list)
+  uint32_t D = 0;        // 26-bit digits accumulated
+  uint32_t Dpad = 0;     // D rounded up to a multiple of 8 (table row stride)
+  uint32_t wbits = 26;   // digit width: 26 while K+1 <= 127 (uint64 accumulators cannot overflow), else 25 / 24
+  uint32_t Lraw = 0;     // 32-bit limbs of the raw accumulated value (ceil(wbits D / 32))
+  uint32_t* d_W = nullptr;   // [(K+1)][Dpad]: digits of W_i = (M/q_i) mod T, row K: (-M) mod T   (T: see ctx)
+  uint2* d_scale = nullptr;  // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
+};
+
+enum PostMode : int {
+  POST_CKKS_MASK = 0,    // out = X mod 2^logQ
+  POST_CKKS_RELIN = 1,   // out = (d + ((X mod 2^logPQ + P/2) >> logP)) mod 2^logQ  [then optional rescale]
+  POST_BGV_MODQ = 2,     // out = V mod Q
+  POST_BGV_RELIN = 3     // out = (d + round(V mod PQ / P) - kk) mod Q
+};
+
+struct PostParams {
+  int mode;
+  uint32_t L, L_PQ, logQ, logP, bitsQ, bitsP, bitsPQ;
+  uint32_t rescale_bits;       // POST_CKKS_RELIN only; 0 = none
+  // BGV constants (device pointers, little-endian limbs)
+  const uint32_t* d_Q;         // [L+1]
+  const uint32_t* d_P;         // [L_P+1]
+  const uint32_t* d_PQ;        // [L_PQ+1]
+  const uint32_t* d_muP;       // Barrett constant for division by P: floor(2^(32 (L_P + g)) / P), g = quotient limbs
+  uint32_t L_P, muP_limbs, g_limbs;
+  uint64_t mu1_Q, mu1_PQ;      // floor(2^(bits+62) / Q), floor(2^(bitsPQ+62) / PQ): one-word Barrett quotient estimates
+  uint32_t t, Pinv_t;          // plaintext modulus and P^-1 mod t
+  const uint32_t* d_pow32_t;   // [L_P+1]: 2^(32 i) mod t
+};
+
+struct Context {
+  // parameters
+  uint32_t N = 0, logN = 0, logQ = 0, logP = 0;
+  uint64_t t = 0;
+  uint32_t bitsQ = 0, bitsP = 0, bitsPQ = 0, L = 0, L_P = 0, L_PQ = 0;
+  uint32_t K_pm = 0, K1 = 0, K2 = 0, Kmax = 0;
+  int n_sm = 0;
+  std::vector<uint32_t> h_q, h_psi;
+  std::vector<uint32_t> h_Q, h_P, h_PQ;   // limbs
+  // device tables (all primes 0..Kmax-1)
+  uint32_t* d_q = nullptr;        // [Kmax]
+  uint32_t* d_qinv_neg = nullptr; // [Kmax] -q^-1 mod 2^32 (Montgomery)
+  uint64_t* d_mu64 = nullptr;     // [Kmax] floor(2^64 / q)  (reduction of 64-bit accumulators)
+  uint32_t* d_f62 = nullptr;      // [Kmax] floor(2^62 / q)  (alpha fixed point)
+  uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion
+  uint2* d_tw_inv = nullptr;      // [Kmax][N]: psi^-bitrev(k) and Shoup companion
+  uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
+  uint4* d_cdec = nullptr;        // [ceil(Kmax/4)][MAX_DIGITS_IN]: 2^(26 d) mod q_j for 4 primes j = 4g..4g+3
+  CrtTarget tgt_pm, tgt_tensor, tgt_relin;
+  PostParams post_pm, post_tensor, post_relin;
+  uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
+  // evk-hat
+  uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
+  bool have_evk = false;
+  // bookkeeping
+  mutable std::string err;
+  uint64_t launches = 0;
+  std::vector<void*> allocs;
+};
+
+// ---- launchers (kernels.cu) --------------------------------------------------------------------------------------
+// decompose: limbs [npoly][Lin][N] -> residues [npoly][K][N] (poly p of the input goes to out + out_poly_stride * p)
+cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_limbs,
+                             size_t limb_poly_stride, uint32_t npoly, uint32_t Lin, uint32_t K, uint32_t mask_bits,
+                             cudaStream_t s);
+// forward / inverse NTT in place on [npoly][K][N]; scale: per-prime final constant of the inverse ([K] uint2)
+cudaError_t launch_ntt(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, bool inverse, const uint2* d_scale,
+                       cudaStream_t s);
+// pointwise products (Montgomery: result carries a factor 2^-32 that the inverse scale removes)
+cudaError_t launch_pw_polymul(Context* c, uint32_t* d_a, const uint32_t* d_b, uint32_t batch, uint32_t K,
+                              cudaStream_t s);                      // a <- a*b, [batch][K][N]
+cudaError_t launch_pw_tensor(Context* c, uint32_t* d_r, uint32_t batch, uint32_t K, cudaStream_t s);
+// r: [batch][4][K][N] = (a0,a1,b0,b1)^ -> slots 0..2 = (d0,d1,d2)^
+cudaError_t launch_pw_relin(Context* c, uint32_t* d_r, const uint32_t* d_evk_hat, uint32_t batch, uint32_t K,
+                            cudaStream_t s);                        // r: [batch][2][K][N], slot0 = d2^ in
+// CRT + post: residues [npoly][K][N] (poly p at d_res + p*res_poly_stride) -> limbs out [npoly][L][N]
+// d_add: for the relin modes, the polynomial added at the end (same indexing as out), else nullptr
+cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_poly_stride,
+                       const uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_add, size_t add_poly_stride,
+                       uint32_t npoly, cudaStream_t s);
+cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
+                           cudaStream_t s);
+
+// ---- device arithmetic ------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t mulhi32(uint32_t a, uint32_t b) { return __umulhi(a, b); }
+
+// x in [0, 2q) -> [0, q)
+__device__ __forceinline__ uint32_t csub(uint32_t x, uint32_t q) { return min(x, x - q); }
+
+// Shoup multiplication by a constant w < q with companion w' = floor(w 2^32 / q): result in [0, 2q), any a < 2^32.
+__device__ __forceinline__ uint32_t mul_shoup_lazy(uint32_t a, uint32_t w, uint32_t wp, uint32_t q) {
+  uint32_t h = mulhi32(a, wp);
+  return a * w - h * q;
+}
+__device__ __forceinline__ uint32_t mul_shoup(uint32_t a, uint32_t w, uint32_t wp, uint32_t q) {
+  return csub(mul_shoup_lazy(a, w, wp, q), q);
+}
+// Montgomery reduction of t < 2^63 (t < 2 q^2 suffices): returns t 2^-32 mod q in [0, q).  qn = -q^-1 mod 2^32.
+__device__ __forceinline__ uint32_t mont_redc(uint64_t t, uint32_t q, uint32_t qn) {
+  uint32_t m = (uint32_t)t * qn;
+  uint64_t u = t + (uint64_t)m * q;   // < 2^64: t < 2^63, m q < 2^63
+  return csub((uint32_t)(u >> 32), q);
+}
+// reduce a 64-bit accumulator mod q with mu = floor(2^64 / q)
+__device__ __forceinline__ uint32_t barrett64(uint64_t x, uint32_t q, uint64_t mu) {
+  uint64_t h = __umul64hi(x, mu);
+  uint32_t r = (uint32_t)x - (uint32_t)h * q;   // x - h q in [0, 2q) fits 32 bits
+  return csub(r, q);
+}
+#endif
+
+}  // namespace fhe
