@@ -174,3 +174,177 @@ def test_rescale_shift_amounts(p_bits):
     for i in range(3):
         want = scheme.rescale(prm, (from_limbs(ct[i, 0]), from_limbs(ct[i, 1])), p_bits)
         assert got[i] == [list(w) for w in want]
+
+
+# ---- full-size configs: sampled coefficients from the definition ----------------------------------------------------
+def _sample_ks(N, seed, count=4):
+    rnd = np.random.default_rng(seed)
+    return [0, N - 1] + [int(v) for v in rnd.integers(1, N - 1, size=count)]
+
+
+def _check_he_mult_samples(out3, ct1, ct2, Q, ks):
+    """out3: uint32 [3][L][N]; ct1/ct2: uint32 [2][L][N]."""
+    c0, c1 = from_limbs(ct1[0]), from_limbs(ct1[1])
+    e0, e1 = from_limbs(ct2[0]), from_limbs(ct2[1])
+    for k in ks:
+        assert coeff_from_limbs(out3[0], k) == ring.pm_coeff(c0, e0, k, Q), ("d0", k)
+        assert coeff_from_limbs(out3[1], k) == (ring.pm_coeff(c0, e1, k, Q) + ring.pm_coeff(c1, e0, k, Q)) % Q, ("d1", k)
+        assert coeff_from_limbs(out3[2], k) == ring.pm_coeff(c1, e1, k, Q), ("d2", k)
+
+
+def _relin_coeff_ckks(prm, d3, evk_polys, k):
+    d2 = from_limbs(d3[2])
+    out = []
+    for comp in range(2):
+        x = ring.pm_coeff(d2, evk_polys[comp], k, prm.PQ)
+        kk = scheme.round_shift(x, prm.logP) % prm.Q
+        out.append((coeff_from_limbs(d3[comp], k) + kk) % prm.Q)
+    return out
+
+
+def _relin_coeff_bgv(prm, d3, evk_polys, k):
+    d2 = from_limbs(d3[2])
+    Pinv_t = pow(prm.P % prm.t, -1, prm.t)
+    out = []
+    for comp in range(2):
+        x = ring.pm_coeff(d2, evk_polys[comp], k, prm.PQ)
+        kk = scheme._div_p_bgv(x, prm.P, prm.Q, prm.t, Pinv_t)
+        out.append((coeff_from_limbs(d3[comp], k) + kk) % prm.Q)
+    return out
+
+
+@pytest.mark.parametrize("N,logQ,logP,B", [(1 << 15, 620, 620, 8), (1 << 16, 1240, 1240, 4)])
+def test_ckks_full_size_sampled(N, logQ, logP, B):
+    """configs[2] and configs[4]: uniform random ciphertexts and key of the configured shape (parity does not need
+    real encryptions); each call checked on sampled coefficients; the fused call must equal the three calls."""
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logP, 0)
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(N + logQ)
+    ct1 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    ct2 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    evk = synth.uniform_limbs(g, (2,), N, logQ + logP)
+    ct1[0, 0, :, 0] = 0xFFFFFFFF                     # a coefficient with every stored bit set (masked on load)
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk))
+    d1, d2 = limbs_np_to_tensor(ct1), limbs_np_to_tensor(ct2)
+    t3 = ctx.fhe_he_mult(d1, d2)
+    out3 = tensor_to_np(t3)
+    ct1m = ct1.copy()
+    ct1m[..., ctx.L - 1, :] &= np.uint32((1 << (logQ % 32)) - 1) if logQ % 32 else np.uint32(0xFFFFFFFF)
+    for b in (0, B - 1):
+        _check_he_mult_samples(out3[b], ct1m[b], ct2[b], prm.Q, _sample_ks(N, b, 2))
+    t2 = ctx.fhe_relinearize(t3)
+    out2 = tensor_to_np(t2)
+    evk_polys = [from_limbs(evk[0]), from_limbs(evk[1])]
+    for b in (0, B - 1):
+        for k in _sample_ks(N, 10 + b, 2):
+            want = _relin_coeff_ckks(prm, out3[b], evk_polys, k)
+            assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
+    tr = ctx.fhe_rescale(t2, 40)
+    outr = tensor_to_np(tr)
+    Q2 = 1 << (logQ - 40)
+    rnd = np.random.default_rng(3)
+    for b in range(B):
+        for comp in range(2):
+            for k in [int(v) for v in rnd.integers(0, N, size=16)]:
+                c = coeff_from_limbs(out2[b, comp], k)
+                assert coeff_from_limbs(outr[b, comp], k) == scheme.round_shift(c, 40) % Q2
+    fused = ctx.fhe_mult_relin_rescale(d1, d2, 40)
+    assert torch.equal(fused, tr)
+    # R1 (any size): 2^p c' - c in (-2^(p-1), 2^(p-1)] mod Q, checked on every coefficient of one component with numpy
+    lo_in = out2[0, 0, 0].astype(np.uint64) | (out2[0, 0, 1].astype(np.uint64) << np.uint64(32))
+    lo_out = outr[0, 0, 0].astype(np.uint64)
+    diff = ((lo_out << np.uint64(40)) - lo_in).astype(np.int64)     # low 64 bits suffice for the low-bit identity
+    low40 = (lo_in & np.uint64((1 << 40) - 1)).astype(np.int64)
+    expect = np.where(low40 >= (1 << 39), (1 << 40) - low40, -low40)
+    assert np.array_equal(diff & ((1 << 62) - 1), expect & ((1 << 62) - 1))
+
+
+def test_c3_ckks_decryption_bound_real_encryptions():
+    """configs[2] with real encryptions (one pair of the batch): CKKS decrypt(mult) within 2^-20 of the slot product."""
+    fhe = _lib()
+    N, logQ, logP = 1 << 15, 620, 620
+    prm, s, evk, cts1, cts2, zs = _ckks_setup(N, logQ, logP, 1, seed=0)
+    ctx = fhe.Context(N, logQ, logP)
+    ctx.fhe_set_evk(polys_to_tensor(list(evk), ctx.L_PQ))
+    out = ctx.fhe_mult_relin_rescale(polys_to_tensor(cts1, ctx.L), polys_to_tensor(cts2, ctx.L), 40)
+    got = tensor_to_polys(out)[0]
+    mu = harness.decrypt(tuple(got), s, 1 << (logQ - 40))
+    z = harness.decode(mu, N, 2.0 ** 40)
+    assert np.max(np.abs(z - zs[0][0] * zs[0][1])) <= 2.0 ** -20
+
+
+# ---- configs[3]: non-RNS BGV ---------------------------------------------------------------------------------------------
+def _bgv_setup(N, logQ, logP, t, B, seed):
+    prm = scheme.Params(N, logQ, logP, t)
+    g = synth.rng(seed)
+    s, evk = harness.keygen(prm, g, hwt=None)
+    cts1, cts2, ms = [], [], []
+    for _ in range(B):
+        m1 = [int(v) for v in synth.uniform_mod(g, N, t)]
+        m2 = [int(v) for v in synth.uniform_mod(g, N, t)]
+        cts1.append(harness.encrypt(prm, g, s, m1))
+        cts2.append(harness.encrypt(prm, g, s, m2))
+        ms.append((m1, m2))
+    return prm, s, evk, cts1, cts2, ms
+
+
+@pytest.mark.parametrize("N,logQ,logP,t", [(256, 100, 100, 257), (1024, 437, 437, 65537), (512, 150, 220, 65537)])
+def test_bgv_small_full(N, logQ, logP, t):
+    fhe = _lib()
+    prm, s, evk, cts1, cts2, ms = _bgv_setup(N, logQ, logP, t, 2, seed=N + t)
+    ctx = fhe.Context(N, logQ, logP, t)
+    assert ctx.modulus(0) == prm.Q and ctx.modulus(1) == prm.P and ctx.modulus(2) == prm.PQ
+    assert (ctx.L, ctx.L_PQ) == (prm.L, prm.L_PQ)
+    ctx.fhe_set_evk(polys_to_tensor(list(evk), ctx.L_PQ))
+    d1, d2 = polys_to_tensor(cts1, ctx.L), polys_to_tensor(cts2, ctx.L)
+    t3 = ctx.fhe_he_mult(d1, d2)
+    want3 = [scheme.he_mult(prm, cts1[i], cts2[i]) for i in range(2)]
+    assert tensor_to_polys(t3) == [[list(p) for p in w] for w in want3]
+    t2 = ctx.fhe_relinearize(t3)
+    want2 = [scheme.relinearize(prm, want3[i], evk) for i in range(2)]
+    got2 = tensor_to_polys(t2)
+    assert got2 == [[list(p) for p in w] for w in want2]
+    assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, 0), t2)
+    for i in range(2):   # R4: exact decryption mod t from the GPU ciphertext
+        assert harness.decrypt_bgv(tuple(got2[i]), s, prm) == ring.pm(ms[i][0], ms[i][1], t)
+    with pytest.raises(fhe.FheError):
+        ctx.fhe_rescale(t2, 8)
+
+
+def test_c4_bgv_full_size():
+    """configs[3]: N = 2^14, t = 65537, Q = P = least odd > 2^437 that is 1 mod t; batch of 16.  Pair 0 is a real
+    encryption checked in full (and decrypted exactly mod t); the rest of the batch is uniform below Q, sampled."""
+    fhe = _lib()
+    N, logQ, logP, t, B = 1 << 14, 437, 437, 65537, 16
+    prm, s, evk, cts1, cts2, ms = _bgv_setup(N, logQ, logP, t, 1, seed=4)
+    ctx = fhe.Context(N, logQ, logP, t)
+    assert ctx.modulus(0) == (1 << 437) + 33 and (ctx.L, ctx.L_PQ) == (14, 28)
+    g = synth.rng(44)
+    r1 = synth.uniform_limbs(g, (B, 2), N, 437)          # < 2^437 < Q
+    r2 = synth.uniform_limbs(g, (B, 2), N, 437)
+    r1 = np.concatenate([r1, np.zeros((B, 2, ctx.L - r1.shape[2], N), np.uint32)], axis=2) if r1.shape[2] < ctx.L else r1
+    r2 = np.concatenate([r2, np.zeros((B, 2, ctx.L - r2.shape[2], N), np.uint32)], axis=2) if r2.shape[2] < ctx.L else r2
+    r1[0] = np.stack([to_limbs(p, ctx.L) for p in cts1[0]])
+    r2[0] = np.stack([to_limbs(p, ctx.L) for p in cts2[0]])
+    r1[1, 0] = to_limbs([prm.Q - 1] * N, ctx.L)            # extreme inputs: every coefficient Q - 1
+    r2[1, 0] = to_limbs([prm.Q - 1] * N, ctx.L)
+    ctx.fhe_set_evk(polys_to_tensor(list(evk), ctx.L_PQ))
+    d1, d2 = limbs_np_to_tensor(r1), limbs_np_to_tensor(r2)
+    t3 = ctx.fhe_he_mult(d1, d2)
+    out3 = tensor_to_np(t3)
+    want3 = scheme.he_mult(prm, cts1[0], cts2[0])
+    assert [from_limbs(out3[0, i]) for i in range(3)] == [list(p) for p in want3]
+    for b in (1, 7, B - 1):
+        _check_he_mult_samples(out3[b], r1[b], r2[b], prm.Q, _sample_ks(N, b, 2))
+    t2 = ctx.fhe_relinearize(t3)
+    out2 = tensor_to_np(t2)
+    want2 = scheme.relinearize(prm, want3, evk)
+    got0 = [from_limbs(out2[0, i]) for i in range(2)]
+    assert got0 == [list(p) for p in want2]
+    assert harness.decrypt_bgv(tuple(got0), s, prm) == ring.pm(ms[0][0], ms[0][1], t)
+    for b in (1, B - 1):
+        for k in _sample_ks(N, 20 + b, 2):
+            want = _relin_coeff_bgv(prm, out3[b], list(evk), k)
+            assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
+    assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, 0), t2)
