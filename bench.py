@@ -1,0 +1,388 @@
+#!/usr/bin/env python
+"""bench.py -- CKKS HE-mult + relinearise + rescale throughput at N = 2^16, logQ = 1240 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (decompose, forward NTT, tensor pointwise,
+inverse NTT, CRT + mod Q, relinearise with evk mod PQ + divide by P, rescale by 2^40) over one batch of 4
+synthetic ciphertext pairs per GPU (BASELINE.json configs[4]).  Prints ONE JSON line (rank 0).
+Multi-GPU: the batch dimension shards with no data-path collective -> weak scaling, evk replicated.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "CKKS HE-mult+relin+rescale ops/s at N=2^16 logQ=1240"
+UNIT = "ops/s"
+WORKLOADS = {
+    # name: (N, logQ, logP, batch, rescale bits)
+    "c5": (1 << 16, 1240, 1240, 4, 40),      # BASELINE.json configs[4], the configuration the metric is quoted on
+    "c3": (1 << 15, 620, 620, 8, 40),
+    "c1": (1 << 10, 128, 128, 1, 40),
+}
+# one op at C5 on the oracle = 4 ring products mod Q + 2 mod PQ; a mod-PQ product costs 2.06x a mod-Q product
+# (measured once on the dev box: 61.7 s vs 29.9 s); used only to scale the timed CPU sample to ops/s.
+ORACLE_PRODUCTS_PER_OP = 4 + 2 * 2.06
+ALU_PEAK_TMULS = 64 * 148 * 1.965e9 / 1e12   # 32-bit IMAD: 16 lanes/clk/SMSP x 4 SMSP x 148 SMs x 1.965 GHz
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured"
+    except Exception:
+        return 6650.0, "fallback"
+
+
+# ---- algorithmic work model of the algorithm actually shipped ---------------------------------------------
+def work_model(N, logQ, logP, L, L_PQ, K1, K2, B):
+    """32x32-bit multiplies and compulsory HBM bytes per kernel class for one step (B ops)."""
+    import math
+    logN = N.bit_length() - 1
+    dq = math.ceil(logQ / 26)                 # 26-bit digits of an input coefficient
+    d_t = math.ceil(logQ / 26)                # CRT output digits, tensor
+    d_r = math.ceil((logQ + logP) / (26 if K2 + 1 <= 127 else 25))
+    bfly = N // 2 * logN                      # butterflies per transform, 3 multiplies each (Shoup)
+    mul = {
+        "decompose": B * N * (4 * K1 + K2) * (dq + 6),
+        "ntt_fwd": B * (4 * K1 + K2) * bfly * 3,
+        "ntt_inv": B * (3 * K1 + 2 * K2) * (bfly * 3 + N * 3),
+        "pointwise": B * N * (K1 * 4 * 3 + K2 * 2 * 3),
+        "crt": B * N * (3 * ((K1 + 1) * d_t + K1) + 2 * ((K2 + 1) * d_r + K2)),
+        "rescale": 0,
+    }
+    w = 4
+    byt = {   # bytes each class must move if every intermediate makes exactly one HBM round trip
+        "decompose": B * N * w * (4 * L + L + 4 * K1 + K2),
+        "ntt_fwd": B * N * w * 2 * 2 * (4 * K1 + K2),
+        "ntt_inv": B * N * w * 2 * 2 * (3 * K1 + 2 * K2),
+        "pointwise": B * N * w * (7 * K1 + 3 * K2) + N * w * 2 * K2,
+        "crt": B * N * w * (3 * K1 + 3 * L + 2 * K2 + 2 * L + 2 * L),
+        "rescale": 0,
+    }
+    compulsory = B * N * w * (4 * L + 2 * L) + N * w * 2 * K2      # read 2 cts, write 1, evk-hat once per batch
+    return mul, byt, compulsory
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+              "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=self.tmp, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+        try:
+            self.tmp.flush()
+            with open(self.tmp.name) as f:
+                rows = [r.strip().split(", ") for r in f if r.strip()]
+            os.unlink(self.tmp.name)
+            sm = sorted(float(r[1]) for r in rows if len(r) >= 9)
+            if sm:
+                out["sm_mhz"] = sm[len(sm) // 2]
+                out["sm_max_mhz"] = float(rows[0][2])
+                out["samples"] = len(sm)
+                names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+                seen = set()
+                for r in rows:
+                    for name, val in zip(names, r[5:9]):
+                        if val.strip().lower().startswith("active"):
+                            seen.add(name)
+                out["reasons"] = sorted(seen)
+        except Exception:
+            pass
+        return out
+
+
+# ---- distributed plumbing (also exercised on CPU with gloo in tests/test_bench_dist.py) ---------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def dist_init(backend: str):
+    import torch.distributed as dist
+    rank, _, world = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world
+
+
+def barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(x: float, world: int, device="cpu") -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def shard_units(per_gpu_batch: int, world: int):
+    """Weak scaling: every rank owns `per_gpu_batch` independent ciphertext pairs; total = world * per_gpu_batch."""
+    return per_gpu_batch, per_gpu_batch * world
+
+
+# ---- the CPU oracle arm ---------------------------------------------------------------------------------------------------
+def oracle_sample_product(N, logQ, seed=0):
+    """Time ONE ring product mod Q of the workload's shape on the oracle (its own NTT route). Returns seconds."""
+    import synth
+    from oracle import ring
+    from oracle.limbs import from_limbs
+    g = synth.rng(seed)
+    a = from_limbs(synth.uniform_limbs(g, (), N, logQ))
+    b = from_limbs(synth.uniform_limbs(g, (), N, logQ))
+    t0 = time.perf_counter()
+    ring.pm(a, b, 1 << logQ)
+    return time.perf_counter() - t0
+
+
+def oracle_sample_coeffs(N, logQ, logP, p_bits, count, seed=0):
+    """`count` output coefficients of one full op (he_mult -> relinearize -> rescale) straight from the definition
+    (oracle.ring.pm_coeff, Eq. 5-6) and the oracle's rounding rules.  Returns seconds."""
+    import numpy as np
+    import synth
+    from oracle import ring, scheme
+    from oracle.limbs import from_limbs
+    g = synth.rng(seed)
+    Q, PQ = 1 << logQ, 1 << (logQ + logP)
+    c = [from_limbs(synth.uniform_limbs(g, (), N, logQ)) for _ in range(4)]
+    evk = [from_limbs(synth.uniform_limbs(g, (), N, logQ + logP)) for _ in range(2)]
+    d2 = from_limbs(synth.uniform_limbs(g, (), N, logQ))   # stands in for the full d2 the relin product needs
+    ks = [int(v) for v in np.random.default_rng(seed).integers(0, N, size=count)]
+    t0 = time.perf_counter()
+    for k in ks:
+        d0 = ring.pm_coeff(c[0], c[2], k, Q)
+        d1 = (ring.pm_coeff(c[0], c[3], k, Q) + ring.pm_coeff(c[1], c[2], k, Q)) % Q
+        _ = ring.pm_coeff(c[1], c[3], k, Q)
+        out = []
+        for comp, d in ((0, d0), (1, d1)):
+            x = ring.pm_coeff(d2, evk[comp], k, PQ)
+            v = (d + scheme.round_shift(x, logP) % Q) % Q
+            out.append(scheme.round_shift(v, p_bits) % (1 << (logQ - p_bits)))
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    N, logQ, logP, B, p_bits = WORKLOADS[args.workload]
+    total_steps = args.steps + args.warmup
+    budget = max(0.5, min(20.0, 150.0 / max(1, total_steps)))      # seconds per step
+    t_probe = oracle_sample_coeffs(N, logQ, logP, p_bits, 1)
+    count = max(1, int(budget / max(t_probe, 1e-3)))
+    for _ in range(args.warmup):
+        oracle_sample_coeffs(N, logQ, logP, p_bits, count)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        oracle_sample_coeffs(N, logQ, logP, p_bits, count, seed=i)
+    dt = time.perf_counter() - t0
+    value = (args.steps * count / N) / dt          # ops/s: an op has N output coefficients (per component pair)
+    sample = f"{count} of {N} output coefficients of one op per step via the definition (oracle.ring.pm_coeff, Eq. 5-6), scaled by N/{count}"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int (python big integers)", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: CKKS N={N} logQ={logQ} logP={logP} batch={B} rescale={p_bits}"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---- the CUDA arm -----------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import numpy as np
+    import torch
+    import synth
+    import paper_2607_05920_b200 as fhe
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback on the product path)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist_init("nccl")
+    N, logQ, logP, B, p_bits = WORKLOADS[args.workload]
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(1000 + rank)
+
+    def dev_limbs(lead, bits):
+        a = synth.uniform_limbs(g, lead, N, bits)
+        return torch.from_numpy(a.view(np.int32)).to(dev)
+
+    ct1, ct2 = dev_limbs((B, 2), logQ), dev_limbs((B, 2), logQ)
+    ctx.fhe_set_evk(dev_limbs((2,), logQ + logP))
+    out = torch.empty((B, 2, ctx.L, N), dtype=torch.int32, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def step():
+        ctx.fhe_mult_relin_rescale(ct1, ct2, p_bits, out=out, stream=stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    # ---- timed region: K steps, device time on the launching stream, max over ranks ----
+    l0 = ctx.launch_count()
+    barrier(world)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    barrier(world)
+    ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    _, total_units = shard_units(B, world)
+    value = total_units * args.steps / (ms_total / 1e3)
+
+    # ---- per-kernel durations over an instrumented repeat of the region (event pair around every launch) ----
+    ctx.fhe_debug_timing(True)
+    torch.cuda.synchronize()
+    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s0.record(stream)
+    for _ in range(args.steps):
+        step()
+    s1.record(stream)
+    torch.cuda.synchronize()
+    per_class = ctx.fhe_debug_timing_read()
+    ms_instr = s0.elapsed_time(s1)
+    ctx.fhe_debug_timing(False)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    h1, h2 = ct1.cpu().pin_memory(), ct2.cpu().pin_memory()
+    hout = torch.empty((B, 2, ctx.L, N), dtype=torch.int32).pin_memory()
+    ctx.fhe_mult_relin_rescale_host(h1, h2, p_bits, h_out=hout, stream=stream)
+    same = bool(torch.equal(hout, out.cpu()))
+    barrier(world)
+    torch.cuda.synchronize()
+    e2e_steps = max(3, min(args.steps, 10))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.fhe_mult_relin_rescale_host(h1, h2, p_bits, h_out=hout, stream=stream)   # synchronises the stream itself
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3, world, dev)
+    e2e_value = total_units * e2e_steps / (e2e_ms / 1e3)
+    ct_bytes = B * 2 * ctx.L * N * 4
+
+    if rank != 0:
+        return 0
+    hbm_gbs, peak_kind = _peaks()
+    mul, byt, compulsory = work_model(N, logQ, logP, ctx.L, ctx.L_PQ, ctx.K1, ctx.K2, B)
+    kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps,
+                "share": v[0] / max(1e-9, sum(x[0] for x in per_class.values())),
+                "gmul_per_step": mul[k] / 1e9, "mb_per_step": byt[k] / 1e6} for k, v in per_class.items()}
+    top = max(per_class, key=lambda k: per_class[k][0])
+    n_launch_top = max(1, per_class[top][1])
+    avg_launch_s = per_class[top][0] / 1e3 / n_launch_top
+    mul_per_launch = mul[top] * args.steps / n_launch_top
+    t_alu = mul[top] / (ALU_PEAK_TMULS * 1e12)
+    t_hbm = byt[top] / (hbm_gbs * 1e9)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "kernel": top, "achieved": mul_per_launch / avg_launch_s / 1e12, "peak": ALU_PEAK_TMULS,
+                "unit": "Tmul32/s", "peak_kind": "derived: 64 IMAD/clk/SM x 148 SM x 1.965 GHz (DESIGN.md 7)"}
+    else:
+        roof = {"bound": "hbm", "kernel": top, "achieved": byt[top] * args.steps / n_launch_top / avg_launch_s / 1e9,
+                "peak": hbm_gbs, "unit": "GB/s", "peak_kind": peak_kind}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["avg_launch_ms"] = avg_launch_s * 1e3
+    # whole-path roofline (north_star): slower of all multiplies at the ALU peak and compulsory bytes at HBM peak
+    t_path_alu = sum(mul.values()) / (ALU_PEAK_TMULS * 1e12)
+    t_path_hbm = compulsory / (hbm_gbs * 1e9)
+    t_step = ms_total / args.steps / 1e3
+    path = {"t_alu_ms": t_path_alu * 1e3, "t_hbm_ms": t_path_hbm * 1e3, "t_measured_ms": t_step * 1e3,
+            "frac": max(t_path_alu, t_path_hbm) / t_step, "gmul_per_step": sum(mul.values()) / 1e9,
+            "compulsory_mb_per_step": compulsory / 1e6}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        t_prod = oracle_sample_product(N, logQ)
+        cpu = {"value": 1.0 / (t_prod * ORACLE_PRODUCTS_PER_OP), "unit": UNIT, "cores": 1, "kind": "oracle",
+               "host_cores": os.cpu_count(),
+               "sample": (f"1 ring product mod Q of 1 pair (oracle.ring.pm, own NTT route) = {t_prod:.1f} s; "
+                          f"an op = 4 products mod Q + 2 mod PQ = {ORACLE_PRODUCTS_PER_OP:.2f} such products")}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 (exact integer)", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: CKKS N={N} logQ={logQ} logP={logP} batch={B}/GPU rescale={p_bits} "
+                               f"(BASELINE.json configs[4])" if args.workload == "c5" else args.workload,
+                   "L": ctx.L, "K1": ctx.K1, "K2": ctx.K2, "global_batch": total_units, "parallelism": f"batch-sharded x{world}, no collective",
+                   "l2": "inputs + workspace per step (~0.9 GB) exceed the 126 MB L2; no explicit flush"},
+        "clocks": clocks, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 2 * ct_bytes, "d2h_bytes_per_step": ct_bytes,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps, "matches_device_result": same},
+        "roofline": roof, "path_roofline": path, "kernels": kern,
+        "instrumented_ms_per_step": ms_instr / args.steps,
+        "cpu_baseline": cpu,
+        "latency_us_per_op": ms_total / args.steps / B * 1e3,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

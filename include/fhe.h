@@ -141,6 +141,12 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
 fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream);
 /* Number of kernel launches the context has enqueued so far (for bench.py's gpu_launches). */
 uint64_t fhe_debug_launch_count(const fhe_ctx* ctx);
+/* Per-kernel device timing for the roofline report.  enable != 0: every later launch is bracketed by a CUDA event
+ * pair on its stream (the only case in which a hot-path call creates anything); enable == 0: off, events freed.
+ * fhe_debug_timing_read synchronises on the recorded events and returns the summed duration and launch count of one
+ * kernel class: 0 decompose, 1 forward NTT, 2 inverse NTT, 3 pointwise, 4 CRT(+post), 5 rescale. */
+fhe_status fhe_debug_timing(fhe_ctx* ctx, int enable);
+fhe_status fhe_debug_timing_read(fhe_ctx* ctx, int kernel_class, double* ms_total, uint64_t* launches);
 
 #ifdef __cplusplus
 }

@@ -23,7 +23,7 @@ EXPORTS = [
     "fhe_ctx_create", "fhe_ctx_destroy", "fhe_ctx_info", "fhe_last_error", "fhe_get_modulus", "fhe_workspace_bytes",
     "fhe_set_evk", "fhe_polymul", "fhe_he_mult", "fhe_relinearize", "fhe_rescale", "fhe_mult_relin_rescale",
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
-    "fhe_debug_launch_count",
+    "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read",
 ]
 
 
@@ -86,6 +86,10 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_debug_ntt.restype = c_int
     lib.fhe_debug_launch_count.argtypes = [vp]
     lib.fhe_debug_launch_count.restype = c_uint64
+    lib.fhe_debug_timing.argtypes = [vp, c_int]
+    lib.fhe_debug_timing.restype = c_int
+    lib.fhe_debug_timing_read.argtypes = [vp, c_int, POINTER(ctypes.c_double), POINTER(c_uint64)]
+    lib.fhe_debug_timing_read.restype = c_int
     _lib = lib
     return lib
 
@@ -178,6 +182,20 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.fhe_debug_launch_count(self._h))
+
+    KERNEL_CLASSES = ("decompose", "ntt_fwd", "ntt_inv", "pointwise", "crt", "rescale")
+
+    def fhe_debug_timing(self, enable: bool):
+        self._check(self._lib.fhe_debug_timing(self._h, 1 if enable else 0))
+
+    def fhe_debug_timing_read(self):
+        """{class name: (total ms, launches)} for the launches recorded since timing was enabled."""
+        out = {}
+        for i, name in enumerate(self.KERNEL_CLASSES):
+            ms, n = ctypes.c_double(), c_uint64()
+            self._check(self._lib.fhe_debug_timing_read(self._h, i, byref(ms), byref(n)))
+            out[name] = (ms.value, int(n.value))
+        return out
 
     def _empty(self, *shape):
         torch = _torch()

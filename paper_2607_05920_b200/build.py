@@ -36,7 +36,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     cmd = [
         _nvcc(), "-shared", "-Xcompiler", "-fPIC", "-std=c++17", "-O3", "-lineinfo",
-        "-gencode", "arch=compute_100a,code=sm_100a",
+        "-gencode", "arch=compute_100a,code=sm_100a", "-t", "4",
         "-o", LIB,
     ] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:

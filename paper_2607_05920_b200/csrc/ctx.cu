@@ -154,6 +154,7 @@ static void destroy(Context* c) {
   if (!c) return;
   for (void* p : c->allocs) cudaFree(p);
   if (c->d_evk_hat) cudaFree(c->d_evk_hat);
+  for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   delete c;
 }
 
@@ -344,6 +345,32 @@ fhe_status fhe_debug_primes(const fhe_ctx* ctx, uint32_t* h_q, uint32_t* h_psi, 
 }
 uint64_t fhe_debug_launch_count(const fhe_ctx* ctx) {
   return ctx ? reinterpret_cast<const Context*>(ctx)->launches : 0;
+}
+fhe_status fhe_debug_timing(fhe_ctx* ctx, int enable) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = reinterpret_cast<Context*>(ctx);
+  for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  c->events.clear();
+  c->timing = enable != 0;
+  return FHE_OK;
+}
+fhe_status fhe_debug_timing_read(fhe_ctx* ctx, int kernel_class, double* ms_total, uint64_t* launches) {
+  if (!ctx || !ms_total || !launches || kernel_class < 0 || kernel_class >= KC_COUNT) return FHE_ERR_ARG;
+  Context* c = reinterpret_cast<Context*>(ctx);
+  double tot = 0;
+  uint64_t n = 0;
+  for (auto& e : c->events) {
+    if (e.cls != kernel_class) continue;
+    cudaError_t st = cudaEventSynchronize(e.b);
+    float ms = 0;
+    if (st == cudaSuccess) st = cudaEventElapsedTime(&ms, e.a, e.b);
+    if (st != cudaSuccess) { c->err = cudaGetErrorString(st); return FHE_ERR_CUDA; }
+    tot += ms;
+    ++n;
+  }
+  *ms_total = tot;
+  *launches = n;
+  return FHE_OK;
 }
 
 }  // extern "C"

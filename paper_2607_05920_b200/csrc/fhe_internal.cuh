@@ -76,6 +76,27 @@ struct Context {
   mutable std::string err;
   uint64_t launches = 0;
   std::vector<void*> allocs;
+  // optional per-kernel timing (fhe_debug_timing): one CUDA event pair per launch, on the launch stream
+  bool timing = false;
+  struct Ev { int cls; cudaEvent_t a, b; };
+  std::vector<Ev> events;
+};
+
+enum KernelClass : int { KC_DECOMPOSE = 0, KC_NTT_FWD = 1, KC_NTT_INV = 2, KC_POINTWISE = 3, KC_CRT = 4, KC_RESCALE = 5, KC_COUNT = 6 };
+
+// brackets one kernel launch with events when timing is on (no-ops otherwise)
+struct LaunchTimer {
+  Context* c; cudaStream_t s; cudaEvent_t b = nullptr;
+  LaunchTimer(Context* c_, int cls, cudaStream_t s_) : c(c_), s(s_) {
+    c->launches++;
+    if (!c->timing) return;
+    Context::Ev e; e.cls = cls;
+    if (cudaEventCreate(&e.a) != cudaSuccess || cudaEventCreate(&e.b) != cudaSuccess) return;
+    cudaEventRecord(e.a, s);
+    b = e.b;
+    c->events.push_back(e);
+  }
+  ~LaunchTimer() { if (b) cudaEventRecord(b, s); }
 };
 
 // ---- launchers (kernels.cu) --------------------------------------------------------------------------------------

@@ -342,8 +342,8 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
     if (e != cudaSuccess) return e;
     configured = smem;
   }
+  LaunchTimer lt(c, KC_CRT, s);
   crt_kernel<<<(c->N / TC) * npoly, TC, smem, s>>>(a, pp);
-  c->launches++;
   return cudaGetLastError();
 }
 
@@ -389,8 +389,8 @@ rescale_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, uint
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s) {
   if (!npoly) return cudaSuccess;
+  LaunchTimer lt(c, KC_RESCALE, s);
   rescale_kernel<<<(c->N / 256) * npoly, 256, 0, s>>>(d_out, d_in, c->N, c->L, c->logQ, p_bits);
-  c->launches++;
   return cudaGetLastError();
 }
 

@@ -83,6 +83,7 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride
   uint32_t eff_limbs = Lin;
   if (mask_bits && (mask_bits + 31) / 32 < eff_limbs) eff_limbs = (mask_bits + 31) / 32;
   int nchunk = (eff_limbs + 12) / 13;
+  LaunchTimer lt(c, KC_DECOMPOSE, s);
 #define DEC_CASE(NC)                                                                                              \
   case NC:                                                                                                        \
     decompose_kernel<NC><<<grid, 128, 0, s>>>(d_res, res_poly_stride, d_limbs, limb_poly_stride, c->N, Lin, K,  \
@@ -93,7 +94,6 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride
     default: return cudaErrorInvalidValue;
   }
 #undef DEC_CASE
-  c->launches++;
   return cudaGetLastError();
 }
 
@@ -173,11 +173,11 @@ cudaError_t launch_ntt(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, 
   const uint32_t ntr = npoly * K;
   if (logN <= 13) {   // one kernel: the whole transform in shared memory
     size_t smem = (size_t)N * 4;
+    LaunchTimer lt(c, inverse ? KC_NTT_INV : KC_NTT_FWD, s);
     if (!inverse)
       ntt_tile_kernel<false, false><<<ntr, 256, smem, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, logN, 0, 0, 1, false);
     else
       ntt_tile_kernel<true, false><<<ntr, 256, smem, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, logN, 0, 0, 1, true);
-    c->launches++;
     return cudaGetLastError();
   }
   const uint32_t ln2 = 8, ln1 = logN - ln2, N1 = 1u << ln1, N2 = 1u << ln2;
@@ -185,13 +185,16 @@ cudaError_t launch_ntt(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, 
   const uint32_t col_tiles = N2 >> lTc, row_tiles = N1 >> lTr;
   const size_t smem_col = (size_t)N1 * (1u << lTc) * 4, smem_row = (size_t)N2 * (1u << lTr) * 4;
   if (!inverse) {
-    ntt_tile_kernel<false, true><<<ntr * col_tiles, 256, smem_col, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln1, lTc, N1, col_tiles, false);
-    ntt_tile_kernel<false, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false);
+    { LaunchTimer lt(c, KC_NTT_FWD, s);
+    ntt_tile_kernel<false, true><<<ntr * col_tiles, 256, smem_col, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln1, lTc, N1, col_tiles, false); }
+    { LaunchTimer lt(c, KC_NTT_FWD, s);
+    ntt_tile_kernel<false, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false); }
   } else {
-    ntt_tile_kernel<true, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false);
+    { LaunchTimer lt(c, KC_NTT_INV, s);
+    ntt_tile_kernel<true, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false); }
+    LaunchTimer lt(c, KC_NTT_INV, s);
     ntt_tile_kernel<true, true><<<ntr * col_tiles, 256, smem_col, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, ln1, lTc, N1, col_tiles, true);
   }
-  c->launches += 2;
   return cudaGetLastError();
 }
 
@@ -263,23 +266,23 @@ cudaError_t launch_pw_polymul(Context* c, uint32_t* d_a, const uint32_t* d_b, ui
                               cudaStream_t s) {
   if (!batch) return cudaSuccess;
   const uint32_t N4 = c->N / 4;
+  LaunchTimer lt(c, KC_POINTWISE, s);
   pw_polymul_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_a, d_b, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
-  c->launches++;
   return cudaGetLastError();
 }
 cudaError_t launch_pw_tensor(Context* c, uint32_t* d_r, uint32_t batch, uint32_t K, cudaStream_t s) {
   if (!batch) return cudaSuccess;
   const uint32_t N4 = c->N / 4;
+  LaunchTimer lt(c, KC_POINTWISE, s);
   pw_tensor_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_r, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
-  c->launches++;
   return cudaGetLastError();
 }
 cudaError_t launch_pw_relin(Context* c, uint32_t* d_r, const uint32_t* d_evk_hat, uint32_t batch, uint32_t K,
                             cudaStream_t s) {
   if (!batch) return cudaSuccess;
   const uint32_t N4 = c->N / 4;
+  LaunchTimer lt(c, KC_POINTWISE, s);
   pw_relin_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_r, d_evk_hat, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
-  c->launches++;
   return cudaGetLastError();
 }
 
