@@ -90,51 +90,75 @@ static uint32_t primes_for(std::vector<uint32_t>& primes, const BigU& bound) {
   return K;
 }
 
-static void digits_of(const BigU& x, uint32_t wbits, uint32_t D, uint32_t* out) {
-  for (uint32_t d = 0; d < D; ++d) {
-    uint32_t bit = d * wbits, w = bit >> 5, sh = bit & 31;
-    uint64_t v = (uint64_t)x.limb(w) | ((uint64_t)x.limb(w + 1) << 32);
-    out[d] = (uint32_t)((v >> sh) & ((1ull << wbits) - 1ull));
-  }
+// value as `n` little-endian bytes
+static std::vector<uint8_t> bytes_of(const BigU& x, size_t n) {
+  std::vector<uint8_t> o(n, 0);
+  for (size_t i = 0; i < n; ++i) o[i] = (uint8_t)(x.limb(i / 4) >> (8 * (i % 4)));
+  return o;
 }
 
-// T_kind: 0 -> T = 2^(wbits D) covering `width_bits`; 1 -> T = the odd modulus `Tmod`
+// Largest chunk width whose CRT kernel footprint (A image / limb columns + two constant buffers) still lets two CTAs
+// share an SM; 32 as the floor.
+static uint32_t pick_crt_nc(uint32_t KB, uint32_t ncols, uint32_t region_bytes) {
+  for (uint32_t nc : {128u, 64u}) {
+    if (nc / 2 >= ncols) continue;                       // do not pad a narrow target to a wide chunk
+    if ((size_t)region_bytes + 2 * (size_t)KB * nc + 1024 <= 112 * 1024) return nc;
+  }
+  return 32;
+}
+
+// CRT constants for the basis q_0..q_{K-1} and the target T (pow2: T = 2^(32 Lraw) with Lraw = ceil(width_bits/32);
+// else T = Tmod odd).  See fhe_internal.cuh (CrtTarget) and kernels_crt.cu for how the image is consumed.
 static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2, uint32_t width_bits,
-                                const BigU& Tmod) {
+                                const BigU& Tmod, uint32_t post_limbs) {
   tg.K = K;
-  tg.wbits = (K + 1 <= 127) ? 26 : (K + 1 <= 255) ? 25 : 24;
+  tg.KB = (4 * K + 31) / 32 * 32;
   uint32_t clogK = 0;
   while ((1u << clogK) < K + 1) ++clogK;
-  uint32_t vbits = pow2 ? width_bits : (Tmod.bits() + 31 + clogK + 1);
-  tg.D = (vbits + tg.wbits - 1) / tg.wbits;
-  tg.Dpad = (tg.D + 7) / 8 * 8;
-  tg.Lraw = (tg.D * tg.wbits + 31) / 32;
-  BigU T = pow2 ? BigU::pow2(tg.wbits * tg.D) : Tmod;
+  const uint32_t vbits = pow2 ? width_bits : (Tmod.bits() + 32 + clogK + 1);   // V < (K+1) 2^32 T
+  tg.Lraw = (vbits + 31) / 32;
+  const uint32_t nbytes = 4 * tg.Lraw;
+  const uint32_t ncols = CRT_ALPHA_COLS + nbytes;
+  tg.Lx = std::max(tg.Lraw + 1, post_limbs);
+  const uint32_t region = std::max(tg.KB * 128u, tg.Lx * 512u);
+  tg.NC = pick_crt_nc(tg.KB, ncols, region);
+  tg.nchunks = (ncols + tg.NC - 1) / tg.NC;
+  if (tg.nchunks * tg.NC > 512) return cudaErrorInvalidValue;
+  const BigU T = pow2 ? BigU::pow2(32 * tg.Lraw) : Tmod;
   BigU M((uint64_t)1);
   for (uint32_t i = 0; i < K; ++i) M.mul_small(c->h_q[i]);
-  std::vector<uint32_t> W((size_t)(K + 1) * tg.Dpad, 0u);
+  const size_t chunk_bytes = (size_t)tg.KB * tg.NC;
+  std::vector<uint8_t> img(chunk_bytes * tg.nchunks, 0);
+  auto put = [&](uint32_t kb, uint32_t col, uint8_t v) {
+    img[(size_t)(col / tg.NC) * chunk_bytes + (size_t)(kb / 16) * tg.NC * 16 + (size_t)(col % tg.NC) * 16 + kb % 16] = v;
+  };
   std::vector<uint2> scale(K);
   for (uint32_t i = 0; i < K; ++i) {
     const uint32_t q = c->h_q[i];
     BigU Mi = M;
-    uint32_t rem = Mi.divmod_small(q);
-    if (rem != 0) return cudaErrorUnknown;
-    uint32_t inv = powmod(Mi.mod_small(q), q - 2, q);              // (M/q_i)^-1 mod q_i
-    BigU Wi = pow2 ? Mi.low_bits(tg.wbits * tg.D) : BigU::mod(Mi, T);
-    digits_of(Wi, tg.wbits, tg.D, &W[(size_t)i * tg.Dpad]);
-    uint32_t ninv = powmod(c->N % q, q - 2, q);
-    uint32_t r32 = (uint32_t)((1ull << 32) % q);
-    uint32_t sc = mulmod(mulmod(ninv, inv, q), r32, q);
+    if (Mi.divmod_small(q) != 0) return cudaErrorUnknown;
+    const uint32_t inv = powmod(Mi.mod_small(q), q - 2, q);            // (M/q_i)^-1 mod q_i
+    const std::vector<uint8_t> W = bytes_of(pow2 ? Mi.low_bits(32 * tg.Lraw) : BigU::mod(Mi, T), nbytes);
+    const uint64_t F = (1ull << ALPHA_SHIFT) / q;                       // < 2^19: three bytes
+    for (uint32_t b = 0; b < 4; ++b) {                                  // byte b of y_i weighs 2^(8 b)
+      for (uint32_t e = b; e < nbytes; ++e) put(4 * i + b, CRT_ALPHA_COLS + e, W[e - b]);
+      for (uint32_t cc = 0; cc < 3; ++cc) put(4 * i + b, b + cc, (uint8_t)(F >> (8 * cc)));
+    }
+    const uint32_t ninv = powmod(c->N % q, q - 2, q);
+    const uint32_t r32 = (uint32_t)((1ull << 32) % q);
+    const uint32_t sc = mulmod(mulmod(ninv, inv, q), r32, q);
     scale[i] = make_uint2(sc, shoup(sc, q));
   }
-  {  // row K: (-M) mod T
-    BigU Mt = pow2 ? M.low_bits(tg.wbits * tg.D) : BigU::mod(M, T);
+  std::vector<uint32_t> negM(tg.Lraw, 0u);
+  {
+    BigU Mt = pow2 ? M.low_bits(32 * tg.Lraw) : BigU::mod(M, T);
     BigU neg;
     if (!Mt.is_zero()) { neg = T; neg.sub(Mt); }
-    digits_of(neg, tg.wbits, tg.D, &W[(size_t)K * tg.Dpad]);
+    neg.to_limbs(negM.data(), negM.size());
   }
-  cudaError_t e = upload(c, &tg.d_W, W);
+  cudaError_t e = upload(c, &tg.d_B, img);
   if (e != cudaSuccess) return e;
+  if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
   return upload(c, &tg.d_scale, scale);
 }
 
@@ -197,10 +221,13 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   const uint32_t Kmax = c->Kmax;
 
   // ---- per-prime constants and twiddle tables ---------------------------------------------------------------------
-  std::vector<uint32_t> qn(Kmax), f62(Kmax);
-  std::vector<uint64_t> mu64(Kmax);
+  std::vector<uint32_t> qn(Kmax);
+  std::vector<uint2> qmu(Kmax);
   std::vector<uint2> scale_plain(Kmax);
-  std::vector<uint4> cdec((size_t)((Kmax + 3) / 4) * MAX_DIGITS_IN, make_uint4(0, 0, 0, 0));
+  // decompose constants: widest input is the evk (L_PQ limbs) or what fhe_debug_decompose may pass (MAX_LIMBS_IN)
+  c->dec_KBimg = (4 * MAX_LIMBS_IN + 31) / 32 * 32;
+  const size_t dec_chunk = (size_t)c->dec_KBimg * DEC_NC;
+  std::vector<uint8_t> decB(dec_chunk * ((Kmax + 15) / 16), 0);
   c->h_psi.resize(Kmax);
   std::vector<uint2> twf((size_t)Kmax * N), twi((size_t)Kmax * N);
   std::vector<uint32_t> pw(N), ipw(N);
@@ -209,8 +236,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     uint32_t inv = 1;                                  // q^-1 mod 2^32 by Newton iteration
     for (int it = 0; it < 5; ++it) inv *= 2u - q * inv;
     qn[j] = 0u - inv;
-    mu64[j] = ~0ull / q;                               // floor((2^64 - 1)/q) = floor(2^64/q): q is odd, never divides 2^64
-    f62[j] = (uint32_t)((1ull << 62) / q);
+    qmu[j] = make_uint2(q, (uint32_t)((1ull << 53) / q));
     uint32_t psi = 0;
     for (uint32_t g = 2; g < 2000 && !psi; ++g) {
       uint32_t cand = powmod(g, (q - 1) / (2 * N), q);
@@ -228,24 +254,25 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     }
     uint32_t ninv = powmod(N % q, q - 2, q);
     scale_plain[j] = make_uint2(ninv, shoup(ninv, q));
-    uint32_t p26 = (uint32_t)((1ull << DIGIT_BITS) % q), cur = 1;
-    for (int d = 0; d < MAX_DIGITS_IN; ++d) {
-      uint4& slot = cdec[(size_t)(j / 4) * MAX_DIGITS_IN + d];
-      (&slot.x)[j % 4] = cur;
-      cur = mulmod(cur, p26, q);
+    uint32_t cur = 1;                                  // 2^(8 kb) mod q, byte cc at column 4 (j % 16) + cc of chunk j / 16
+    for (uint32_t kb = 0; kb < c->dec_KBimg; ++kb) {
+      for (uint32_t cc = 0; cc < 4; ++cc)
+        decB[(size_t)(j / 16) * dec_chunk + (size_t)(kb / 16) * DEC_NC * 16 + (size_t)(4 * (j % 16) + cc) * 16 + kb % 16] =
+            (uint8_t)(cur >> (8 * cc));
+      cur = mulmod(cur, 256u, q);
     }
   }
 #define UP(dst, vec)                                                                                   \
   if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
-  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_mu64, mu64) UP(d_f62, f62) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
-  UP(d_scale_plain, scale_plain) UP(d_cdec, cdec)
+  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
+  UP(d_scale_plain, scale_plain) UP(d_decB, decB)
 
   // ---- CRT targets -------------------------------------------------------------------------------------------------
   const bool ckks = (t == 0);
-  if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q)) != cudaSuccess ||
-      (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q)) != cudaSuccess ||
-      (e = build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ)) != cudaSuccess) {
+  if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
+      (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
+      (e = build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ, c->L_PQ + 2)) != cudaSuccess) {
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "CRT table build failed: " + m);
   }
 
@@ -265,7 +292,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     UP(d_muP, hmu)
     pp.muP_limbs = (uint32_t)mu.v.size();
     pp.g_limbs = c->L_PQ - c->L_P;
-    if ((pp.g_limbs + 1) + pp.muP_limbs > c->K2 + 1) { destroy(c); return fail(nullptr, FHE_ERR_UNSUPPORTED, "BGV: logP too small relative to logQ for the division scratch"); }
+    pp.scratch_limbs = (pp.g_limbs + 1) + pp.muP_limbs + 1;   // product q1 * mu of the divide-by-P (kernels_crt.cu)
     const uint32_t tt = (uint32_t)t;
     std::vector<uint32_t> p32(c->L_P + 2);
     uint32_t cur = 1 % tt, b32 = (uint32_t)((1ull << 32) % tt);

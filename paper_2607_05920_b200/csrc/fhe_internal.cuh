@@ -10,20 +10,25 @@
 
 namespace fhe {
 
-constexpr int DIGIT_BITS = 26;                 // decompose / CRT digit width: digit * 31-bit constant < 2^57,
-constexpr uint32_t DIGIT_MASK = (1u << DIGIT_BITS) - 1u;  // so up to 128 products fit a uint64 accumulator
-constexpr int MAX_DIGITS_IN = 128;             // decompose input: <= 8 chunks of 16 digits (13 limbs each)
-constexpr int MAX_LIMBS_IN = 104;
+constexpr int MAX_LIMBS_IN = 104;              // widest decompose input (limbs); 416 bytes of contraction
+constexpr int DEC_NC = 64;                     // decompose: columns per MMA / constant chunk = 16 primes x 4 constant bytes
+constexpr int DEC_GROUP_CHUNKS = 2;            // decompose: chunks accumulated in TMEM before an epilogue (128 columns)
+constexpr int CRT_ALPHA_COLS = 8;              // CRT: leading columns holding the byte sums of sum_i y_i floor(2^48 / q_i)
+constexpr int ALPHA_SHIFT = 48;
 
-// ---- CRT target: turns y_i = x_i * (M/q_i)^-1 mod q_i (i < K) into limbs of X = sum y_i (M/q_i) - alpha M ------------
+// ---- CRT target: turns y_i = x_i * (M/q_i)^-1 mod q_i (i < K) into limbs of V = sum y_i W_i + alpha * negM -------------
+// W_i = (M/q_i) mod T, negM = (-M) mod T, T = 2^(32 Lraw) (CKKS; masked later) or the odd modulus.  The sum is one
+// u8 x u8 -> s32 tensor-core contraction over the bytes of the y_i (umma.cuh): column 8 + e collects byte position e.
 struct CrtTarget {
   uint32_t K = 0;        // primes in the basis (prefix of the context's prime list)
-  uint32_t D = 0;        // 26-bit digits accumulated
-  uint32_t Dpad = 0;     // D rounded up to a multiple of 8 (table row stride)
-  uint32_t wbits = 26;   // digit width: 26 while K+1 <= 127 (uint64 accumulators cannot overflow), else 25 / 24
-  uint32_t Lraw = 0;     // 32-bit limbs of the raw accumulated value (ceil(wbits D / 32))
-  uint32_t* d_W = nullptr;   // [(K+1)][Dpad]: digits of W_i = (M/q_i) mod T, row K: (-M) mod T   (T: see ctx)
-  uint2* d_scale = nullptr;  // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
+  uint32_t KB = 0;       // contraction bytes: 4 K rounded up to a multiple of 32
+  uint32_t NC = 0;       // columns per constant chunk / MMA
+  uint32_t nchunks = 0;  // chunks; nchunks * NC <= 512 TMEM columns
+  uint32_t Lraw = 0;     // 32-bit limbs of V produced by the carry pass (4 Lraw value columns)
+  uint32_t Lx = 0;       // limbs of the per-coefficient column the post-processing works on (>= Lraw + 1)
+  uint8_t* d_B = nullptr;      // [nchunks][KB/16][NC][16]: shared-memory images of the constant chunks
+  uint32_t* d_negM = nullptr;  // [Lraw]
+  uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
 };
 
 enum PostMode : int {
@@ -42,7 +47,7 @@ struct PostParams {
   const uint32_t* d_P;         // [L_P+1]
   const uint32_t* d_PQ;        // [L_PQ+1]
   const uint32_t* d_muP;       // Barrett constant for division by P: floor(2^(32 (L_P + g)) / P), g = quotient limbs
-  uint32_t L_P, muP_limbs, g_limbs;
+  uint32_t L_P, muP_limbs, g_limbs, scratch_limbs;
   uint64_t mu1_Q, mu1_PQ;      // floor(2^(bits+62) / Q), floor(2^(bitsPQ+62) / PQ): one-word Barrett quotient estimates
   uint32_t t, Pinv_t;          // plaintext modulus and P^-1 mod t
   const uint32_t* d_pow32_t;   // [L_P+1]: 2^(32 i) mod t
@@ -60,12 +65,12 @@ struct Context {
   // device tables (all primes 0..Kmax-1)
   uint32_t* d_q = nullptr;        // [Kmax]
   uint32_t* d_qinv_neg = nullptr; // [Kmax] -q^-1 mod 2^32 (Montgomery)
-  uint64_t* d_mu64 = nullptr;     // [Kmax] floor(2^64 / q)  (reduction of 64-bit accumulators)
-  uint32_t* d_f62 = nullptr;      // [Kmax] floor(2^62 / q)  (alpha fixed point)
+  uint2* d_qmu = nullptr;         // [Kmax] (q, floor(2^53 / q)): one-word Barrett pair of the decompose epilogue
   uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion
   uint2* d_tw_inv = nullptr;      // [Kmax][N]: psi^-bitrev(k) and Shoup companion
   uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
-  uint4* d_cdec = nullptr;        // [ceil(Kmax/4)][MAX_DIGITS_IN]: 2^(26 d) mod q_j for 4 primes j = 4g..4g+3
+  uint8_t* d_decB = nullptr;      // [ceil(Kmax/16)][dec_KBimg/16][DEC_NC][16]: byte c of 2^(8 kb) mod q_j at column 4 j + c
+  uint32_t dec_KBimg = 0;         // contraction bytes covered by the decompose image (widest input, multiple of 32)
   CrtTarget tgt_pm, tgt_tensor, tgt_relin;
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
@@ -143,11 +148,11 @@ __device__ __forceinline__ uint32_t mont_redc(uint64_t t, uint32_t q, uint32_t q
   uint64_t u = t + (uint64_t)m * q;   // < 2^64: t < 2^63, m q < 2^63
   return csub((uint32_t)(u >> 32), q);
 }
-// reduce a 64-bit accumulator mod q with mu = floor(2^64 / q)
-__device__ __forceinline__ uint32_t barrett64(uint64_t x, uint32_t q, uint64_t mu) {
-  uint64_t h = __umul64hi(x, mu);
-  uint32_t r = (uint32_t)x - (uint32_t)h * q;   // x - h q in [0, 2q) fits 32 bits
-  return csub(r, q);
+// v < 2^49 -> v mod q with mu = floor(2^53 / q): the quotient estimate mulhi(v >> 21, mu) is floor(v/q) or one less
+// (v >> 21 < 2^28 and mu < 2^24 lose < 2^-4 + 2^-8 of a unit), so the 32-bit remainder lies in [0, 2q).
+__device__ __forceinline__ uint32_t barrett49(uint64_t v, uint32_t q, uint32_t mu) {
+  const uint32_t qh = __umulhi((uint32_t)(v >> 21), mu);
+  return csub((uint32_t)v - qh * q, q);
 }
 #endif
 

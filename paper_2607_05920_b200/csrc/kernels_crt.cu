@@ -7,7 +7,10 @@
 // frac(sum y_i/q_i) is within 1/4 of an integer and a 2^-22-accurate fixed-point sum decides alpha exactly
 // (DESIGN.md 5).  The sum is a dot product of (K+1) words with (K+1) constant multi-digit vectors, evaluated on
 // 26-bit digits so that products accumulate in uint64 without carries.
+#include <algorithm>
+
 #include "fhe_internal.cuh"
+#include "umma.cuh"
 
 namespace fhe {
 
@@ -103,77 +106,83 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// CRT kernel.  Block = 128 coefficients of one polynomial.
-//   phase 1  residues y[i][c] -> shared (coalesced), alpha per coefficient into row K
-//   phase 2  per thread: digits of V = sum_i y_i W_i accumulated 8 at a time, carries propagated, repacked to limbs
+// CRT kernel.  Block = 128 coefficients of one polynomial (thread = coefficient = TMEM lane).
+//   phase 1  the residues y[i][n] are staged as the byte matrix A[n][4 i + b] (umma.cuh) and contracted on the tensor
+//            cores with the constant image B: column 8 + e receives S_e = sum_{i,b} y_ib * byte_{e-b}(W_i), columns
+//            0..5 the byte sums of sum_i y_i floor(2^48 / q_i) (-> alpha)
+//   phase 2  per thread: V = sum_e S_e 2^(8 e) + alpha * negM, carries propagated four columns (one limb) at a time,
+//            limbs written to this thread's column in shared memory (which reuses the A image's space)
 //   phase 3  post-processing on the limb column (mask / divide-by-P + add [+ rescale] / BGV reductions), store
 // ------------------------------------------------------------------------------------------------------------------
 struct CrtArgs {
   const uint32_t* res; size_t res_poly_stride;
   uint32_t* out; size_t out_poly_stride;
   const uint32_t* add; size_t add_poly_stride;
-  const uint32_t* W; const uint32_t* f62;
-  uint32_t N, K, D, Dpad, Lraw, Lx, wbits;
+  const uint8_t* B; const uint32_t* negM;
+  uint32_t N, K, KB, NC, nchunks, Lraw, Lx, region_bytes;
 };
 
 __global__ void __launch_bounds__(TC)
 crt_kernel(CrtArgs a, PostParams pp) {
-  extern __shared__ uint32_t sm[];
-  uint32_t* ys = sm;                               // [(K+1)][TC]
-  uint32_t* xs = sm + (size_t)(a.K + 1) * TC;      // [Lx][TC]
-  const uint32_t tid = threadIdx.x;
+  using namespace umma;
+  extern __shared__ __align__(1024) uint8_t smem[];
+  __shared__ MmaPipe pipe;
+  __shared__ uint32_t tmem_slot;
+  uint8_t* sA = smem;                                          // [KB/16][128][16]; later the limb columns xs[Lx][TC]
+  uint8_t* sB0 = smem + a.region_bytes;
+  uint8_t* sB1 = sB0 + (size_t)a.KB * a.NC;
+  uint32_t* xs = reinterpret_cast<uint32_t*>(smem);
+  uint32_t* scratch = reinterpret_cast<uint32_t*>(sB0);        // BGV divide-by-P scratch column (B buffers are dead then)
+  const uint32_t tid = threadIdx.x, warp = tid >> 5;
   const uint32_t bpp = a.N / TC;
   const uint32_t poly = blockIdx.x / bpp;
   const uint32_t n = (blockIdx.x % bpp) * TC + tid;
-  const uint32_t* rin = a.res + (size_t)poly * a.res_poly_stride + n;
+  const uint32_t ncols_alloc = pow2_cols(a.nchunks * a.NC);
 
   // phase 1
-  uint64_t fsum = 0;
-  for (uint32_t i = 0; i < a.K; ++i) {
-    uint32_t y = rin[(size_t)i * a.N];
-    ys[i * TC + tid] = y;
-    fsum += ((uint64_t)y * __ldg(a.f62 + i)) >> 10;          // ~ (y/q_i) 2^52
-  }
-  const uint32_t alpha = (uint32_t)((fsum + (1ull << 51)) >> 52);
-  ys[a.K * TC + tid] = alpha;
-  // (each thread reads back only its own column: no barrier needed)
+  stage_rows(sA, a.res + (size_t)poly * a.res_poly_stride + (n - tid), a.N, a.K, a.KB, 0);
+  if (tid == 0) mma_pipe_init(&pipe);
+  fence_proxy_async();
+  __syncthreads();
+  if (warp == 0) tmem_alloc(&tmem_slot, ncols_alloc);           // after staging: a co-resident CTA may still hold TMEM
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tbase = tmem_slot;
+  PipeState st = {{0, 0}, {0, 0}, 0};
+  if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, a.NC, a.B, (size_t)a.KB * a.NC, a.nchunks, tbase);
+  mbar_wait(&pipe.done, 0);
+  __syncthreads();                                              // nobody overwrites the A image before all MMAs are done
+  tc_fence_after();
 
   // phase 2
   {
-    const uint32_t wb = a.wbits;
-    const uint64_t wmask = (1ull << wb) - 1ull;
-    uint64_t carry = 0, bitbuf = 0;
-    uint32_t nb = 0, lw = 0;
-    for (uint32_t dc = 0; dc < a.Dpad; dc += 8) {
-      uint64_t acc[8];
+    const uint32_t lane_addr = tbase + ((warp * 32u) << 16);
+    uint32_t t[32];
+    tmem_ld32(lane_addr, t);
+    uint64_t asum = 0;
 #pragma unroll
-      for (int e = 0; e < 8; ++e) acc[e] = 0;
-      const uint32_t* wrow = a.W + dc;
-      for (uint32_t i = 0; i <= a.K; ++i) {
-        const uint32_t y = ys[i * TC + tid];
-        const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(wrow + (size_t)i * a.Dpad));
-        const uint4 w1 = __ldg(reinterpret_cast<const uint4*>(wrow + (size_t)i * a.Dpad) + 1);
-        acc[0] += (uint64_t)y * w0.x; acc[1] += (uint64_t)y * w0.y; acc[2] += (uint64_t)y * w0.z; acc[3] += (uint64_t)y * w0.w;
-        acc[4] += (uint64_t)y * w1.x; acc[5] += (uint64_t)y * w1.y; acc[6] += (uint64_t)y * w1.z; acc[7] += (uint64_t)y * w1.w;
-      }
+    for (int e = 0; e < 6; ++e) asum += (uint64_t)t[e] << (8 * e);
+    const uint32_t alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
+    uint64_t carry = 0;
+    uint32_t l = 0;
+    // first load: columns 8..31 = limbs 0..5; later loads: eight limbs each
+    for (uint32_t col = 0; l < a.Lraw; col += 32) {
+      if (col) tmem_ld32(lane_addr + col, t);
 #pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        if (dc + e < a.D) {
-          uint64_t v = acc[e] + carry;
-          carry = v >> wb;
-          bitbuf |= (v & wmask) << nb;
-          nb += wb;
-          if (nb >= 32) {
-            if (lw < a.Lx) xs[lw * TC + tid] = (uint32_t)bitbuf;
-            ++lw;
-            bitbuf >>= 32;
-            nb -= 32;
-          }
-        }
+      for (int g = 0; g < 8; ++g) {
+        if ((col == 0 && g < CRT_ALPHA_COLS / 4) || l >= a.Lraw) continue;
+        uint64_t v = carry + (uint64_t)alpha * __ldg(a.negM + l);
+        v += (uint64_t)t[4 * g] + ((uint64_t)t[4 * g + 1] << 8) + ((uint64_t)t[4 * g + 2] << 16) + ((uint64_t)t[4 * g + 3] << 24);
+        xs[l * TC + tid] = (uint32_t)v;
+        carry = v >> 32;
+        ++l;
       }
     }
-    if (lw < a.Lx) { xs[lw * TC + tid] = (uint32_t)bitbuf; ++lw; }
-    for (; lw < a.Lx; ++lw) xs[lw * TC + tid] = 0;
+    for (; l < a.Lx; ++l) { xs[l * TC + tid] = (uint32_t)carry; carry = 0; }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tbase, ncols_alloc);            // release TMEM before the (long) post-processing
   }
 
   // phase 3
@@ -231,7 +240,7 @@ crt_kernel(CrtArgs a, PostParams pp) {
     col_barrett1(x, a.Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);   // x[0..LPQ) = xc
     // Barrett quotient estimate (HAC 14.42 generalised): q1 = xc >> 32(LP-1)  (g+1 limbs),
     // q3 = (q1 * mu) >> 32(g+1), mu = floor(2^(32 LPQ) / P)  (muP_limbs limbs); true quotient - q3 in {0,1,2}.
-    Col sc{ys + tid};                                // scratch column: (K+1) limbs, enough by construction
+    Col sc{scratch + tid};                           // scratch column: pp.scratch_limbs limbs (B buffers are dead by now)
     const uint32_t n1 = g + 1, nmu = pp.muP_limbs;
     {
       uint64_t acc_lo = 0; uint32_t acc_hi = 0;
@@ -329,13 +338,12 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   a.res = d_res; a.res_poly_stride = res_poly_stride;
   a.out = d_out; a.out_poly_stride = out_poly_stride;
   a.add = d_add; a.add_poly_stride = add_poly_stride;
-  a.W = tg.d_W; a.f62 = c->d_f62;
-  a.N = c->N; a.K = tg.K; a.D = tg.D; a.Dpad = tg.Dpad; a.Lraw = tg.Lraw; a.wbits = tg.wbits;
-  uint32_t Lx = tg.Lraw + 1;
-  if (Lx < pp.L + 2) Lx = pp.L + 2;
-  if (Lx < pp.L_PQ + 2 && (pp.mode == POST_BGV_RELIN || pp.mode == POST_CKKS_RELIN)) Lx = pp.L_PQ + 2;
-  a.Lx = Lx;
-  size_t smem = ((size_t)(tg.K + 1) + Lx) * TC * sizeof(uint32_t);
+  a.B = tg.d_B; a.negM = tg.d_negM;
+  a.N = c->N; a.K = tg.K; a.KB = tg.KB; a.NC = tg.NC; a.nchunks = tg.nchunks; a.Lraw = tg.Lraw; a.Lx = tg.Lx;
+  a.region_bytes = std::max(tg.KB * 128u, tg.Lx * 512u);
+  size_t tail = 2 * (size_t)tg.KB * tg.NC;
+  if (pp.mode == POST_BGV_RELIN && (size_t)pp.scratch_limbs * TC * 4 > tail) tail = (size_t)pp.scratch_limbs * TC * 4;
+  const size_t smem = a.region_bytes + tail;
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(crt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

@@ -1,4 +1,4 @@
-// kernels_ntt.cu -- S1 decompose (limb -> RNS), S2/S4 negacyclic NTT passes, S3 pointwise products.
+// kernels_ntt.cu -- S2/S4 negacyclic NTT passes, S3 pointwise products.
 //
 // NTT formulation (Eq. 8-9): merged-psi Cooley-Tukey forward / Gentleman-Sande inverse
 // (PAPER.md:352, 358); the psi^j "twist" of PAPER.md:346-350 is folded into the butterfly twiddles, so no separate
@@ -14,88 +14,6 @@
 #include "fhe_internal.cuh"
 
 namespace fhe {
-
-// ------------------------------------------------------------------------------------------------------------------
-// S1: decompose.  One thread per coefficient: limbs -> 26-bit digits in registers (13 limbs = 16 digits), then for
-// each group of 4 primes r_j = sum_d digit_d * (2^(26 d) mod q_j) accumulated in uint64.
-// ------------------------------------------------------------------------------------------------------------------
-template <int NCHUNK>
-__global__ void __launch_bounds__(128)
-decompose_kernel(uint32_t* __restrict__ res, size_t res_poly_stride, const uint32_t* __restrict__ limbs,
-                 size_t limb_poly_stride, uint32_t N, uint32_t Lin, uint32_t K, uint32_t mask_bits,
-                 const uint4* __restrict__ cdec, const uint32_t* __restrict__ qarr,
-                 const uint64_t* __restrict__ mu64) {
-  const uint32_t bpp = N / 128;                      // blocks per polynomial
-  const uint32_t poly = blockIdx.x / bpp;
-  const uint32_t n = (blockIdx.x % bpp) * 128 + threadIdx.x;
-  const uint32_t* in = limbs + (size_t)poly * limb_poly_stride + n;
-  uint32_t* out = res + (size_t)poly * res_poly_stride + n;
-
-  uint32_t dig[16 * NCHUNK];
-#pragma unroll
-  for (int c = 0; c < NCHUNK; ++c) {
-    uint32_t w[13];
-#pragma unroll
-    for (int i = 0; i < 13; ++i) {
-      uint32_t l = c * 13 + i;
-      uint32_t v = (l < Lin) ? __ldg(in + (size_t)l * N) : 0u;
-      if (mask_bits) {
-        uint32_t lo = l * 32;
-        if (lo >= mask_bits) v = 0;
-        else if (lo + 32 > mask_bits) v &= (1u << (mask_bits - lo)) - 1u;
-      }
-      w[i] = v;
-    }
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int bit = 26 * k, wi = bit >> 5, sh = bit & 31;
-      uint32_t v = w[wi] >> sh;
-      if (sh > 6) v |= w[wi + 1] << (32 - sh);
-      dig[c * 16 + k] = v & DIGIT_MASK;
-    }
-  }
-  const uint32_t ngroups = (K + 3) / 4;
-  for (uint32_t g = 0; g < ngroups; ++g) {
-    const uint4* cg = cdec + (size_t)g * MAX_DIGITS_IN;
-    uint64_t s0 = 0, s1 = 0, s2 = 0, s3 = 0;
-#pragma unroll
-    for (int d = 0; d < 16 * NCHUNK; ++d) {
-      uint4 c = __ldg(cg + d);
-      s0 += (uint64_t)dig[d] * c.x;
-      s1 += (uint64_t)dig[d] * c.y;
-      s2 += (uint64_t)dig[d] * c.z;
-      s3 += (uint64_t)dig[d] * c.w;
-    }
-    uint64_t s[4] = {s0, s1, s2, s3};
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      uint32_t j = g * 4 + e;
-      if (j < K) out[(size_t)j * N] = barrett64(s[e], __ldg(qarr + j), __ldg(mu64 + j));
-    }
-  }
-}
-
-cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_limbs,
-                             size_t limb_poly_stride, uint32_t npoly, uint32_t Lin, uint32_t K, uint32_t mask_bits,
-                             cudaStream_t s) {
-  if (npoly == 0) return cudaSuccess;
-  dim3 grid((c->N / 128) * npoly);
-  uint32_t eff_limbs = Lin;
-  if (mask_bits && (mask_bits + 31) / 32 < eff_limbs) eff_limbs = (mask_bits + 31) / 32;
-  int nchunk = (eff_limbs + 12) / 13;
-  LaunchTimer lt(c, KC_DECOMPOSE, s);
-#define DEC_CASE(NC)                                                                                              \
-  case NC:                                                                                                        \
-    decompose_kernel<NC><<<grid, 128, 0, s>>>(d_res, res_poly_stride, d_limbs, limb_poly_stride, c->N, Lin, K,  \
-                                                mask_bits, c->d_cdec, c->d_q, c->d_mu64);                         \
-    break;
-  switch (nchunk) {
-    DEC_CASE(1) DEC_CASE(2) DEC_CASE(3) DEC_CASE(4) DEC_CASE(5) DEC_CASE(6) DEC_CASE(7) DEC_CASE(8)
-    default: return cudaErrorInvalidValue;
-  }
-#undef DEC_CASE
-  return cudaGetLastError();
-}
 
 // ------------------------------------------------------------------------------------------------------------------
 // S2 / S4: local transform of n = 2^ln points with twiddle index base * m' + i', T transforms per block, radix-2
