@@ -150,7 +150,10 @@ crt_kernel(CrtArgs a, PostParams pp) {
   tc_fence_after();
   const uint32_t tbase = tmem_slot;
   PipeState st = {{0, 0}, {0, 0}, 0};
-  if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, a.NC, a.B, (size_t)a.KB * a.NC, a.nchunks, tbase);
+  if (warp == 0) {   // lane 0 issues; its warp mates park at the convergence barrier instead of polling beside it
+    if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, a.NC, a.B, (size_t)a.KB * a.NC, a.nchunks, tbase);
+    __syncwarp();
+  }
   mbar_wait(&pipe.done, 0);
   __syncthreads();                                              // nobody overwrites the A image before all MMAs are done
   tc_fence_after();
@@ -347,6 +350,8 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(crt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(crt_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     configured = smem;
   }

@@ -50,7 +50,10 @@ decompose_mma_kernel(DecArgs a) {
   PipeState st = {{0, 0}, {0, 0}, 0};
   for (uint32_t c0 = 0; c0 < a.nchunks; c0 += DEC_GROUP_CHUNKS) {
     const uint32_t nch = min((uint32_t)DEC_GROUP_CHUNKS, a.nchunks - c0);
-    if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, DEC_NC, a.B + (size_t)c0 * a.chunk_stride, a.chunk_stride, nch, tbase);
+    if (warp == 0) {   // lane 0 issues; its warp mates park at the convergence barrier instead of polling beside it
+      if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, DEC_NC, a.B + (size_t)c0 * a.chunk_stride, a.chunk_stride, nch, tbase);
+      __syncwarp();
+    }
     mbar_wait(&pipe.done, st.done_par);
     st.done_par ^= 1;
     __syncwarp();
@@ -93,10 +96,13 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride
   a.KB = (4 * eff + 31) / 32 * 32;
   a.nchunks = (K + 15) / 16;
   if (a.KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
-  const size_t smem = (size_t)a.KB * (TILE_M + 2 * DEC_NC);
+  const size_t smem = smem_for_tmem_residency((size_t)a.KB * (TILE_M + 2 * DEC_NC), DEC_GROUP_COLS);
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(decompose_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // several CTAs per SM are the latency hiding here: ask for the full shared-memory carveout, not the driver's guess
+    e = cudaFuncSetAttribute(decompose_mma_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     if (e != cudaSuccess) return e;
     configured = smem;
   }

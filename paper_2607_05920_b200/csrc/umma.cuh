@@ -88,6 +88,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+// Dynamic shared memory to request so that no more CTAs become resident on an SM than can hold `tmem_cols` TMEM
+// columns each (512 per SM): a CTA that blocks inside tcgen05.alloc holds up the SM's other tcgen05 traffic.
+inline size_t smem_for_tmem_residency(size_t smem_needed, uint32_t tmem_cols) {
+  const size_t per_sm = 227 * 1024;
+  const uint32_t max_ctas = 512 / tmem_cols;                 // 1, 2, 4, 8, 16
+  const size_t floor_bytes = per_sm / (max_ctas + 1) + 1024; // one more CTA would not fit (1 KB: per-CTA reserved + static)
+  return smem_needed > floor_bytes ? smem_needed : floor_bytes;
+}
+
 // ---- descriptors --------------------------------------------------------------------------------------------------------
 // Shared-memory matrix descriptor, K-major, no swizzle ("interleave"): element (row r, byte kb) of the operand sits at
 //   start + (r / 8) * sbo + (kb / 16) * lbo + (r % 8) * 16 + kb % 16.
@@ -171,28 +180,36 @@ __device__ __forceinline__ void mma_phase(MmaPipe* p, PipeState& st, const uint8
 }
 
 // Stage 128 rows of a word-major array into the A image: word w of row r comes from src[w * wstride + r].
-// Words >= nwords read as zero; if mask_bits != 0 the row's value is first reduced mod 2^mask_bits.
-// Thread t owns row t: four coalesced 128-byte loads per 16-byte chunk, one conflict-free 16-byte store.
+// Words >= nwords read as zero; if mask_bits != 0 the row's value is first reduced mod 2^mask_bits (callers pass
+// nwords <= ceil(mask_bits / 32)).  Thread t owns row t: 32 independent coalesced loads are in flight per thread
+// before the first dependent instruction (the loads are the only long-latency step of the kernels built on this),
+// then eight conflict-free 16-byte stores.
 __device__ __forceinline__ void stage_rows(uint8_t* sA, const uint32_t* __restrict__ src, size_t wstride, uint32_t nwords,
                                            uint32_t KB, uint32_t mask_bits) {
   const uint32_t t = threadIdx.x;
   const uint32_t nch = KB / 16;
   const uint32_t* p = src + t;
-#pragma unroll 4
-  for (uint32_t kc = 0; kc < nch; ++kc) {
-    uint32_t w[4];
+  for (uint32_t kc0 = 0; kc0 < nch; kc0 += 8) {
+    uint32_t w[32];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const uint32_t wi = kc * 4 + i;
-      uint32_t v = wi < nwords ? __ldg(p + (size_t)wi * wstride) : 0u;
-      if (mask_bits) {
-        const uint32_t lo = wi * 32;
-        if (lo >= mask_bits) v = 0;
-        else if (lo + 32 > mask_bits) v &= (1u << (mask_bits - lo)) - 1u;
-      }
-      w[i] = v;
+    for (int i = 0; i < 32; ++i) {
+      const uint32_t wi = kc0 * 4 + i;
+      w[i] = __ldg(p + (size_t)min(wi, nwords - 1) * wstride);     // clamped: always a valid address, no branch
     }
-    *reinterpret_cast<uint4*>(sA + (size_t)kc * ROWBLK + t * 16) = make_uint4(w[0], w[1], w[2], w[3]);
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+      if (kc0 * 4 + i >= nwords) w[i] = 0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c)
+      if (kc0 + c < nch)
+        *reinterpret_cast<uint4*>(sA + (size_t)(kc0 + c) * ROWBLK + t * 16) = make_uint4(w[4 * c], w[4 * c + 1], w[4 * c + 2], w[4 * c + 3]);
+  }
+  if (mask_bits & 31) {   // partial top word: each thread patches its own row (same thread wrote it)
+    const uint32_t wi = mask_bits >> 5;
+    if (wi < nwords) {
+      uint32_t* q = reinterpret_cast<uint32_t*>(sA + (size_t)(wi / 4) * ROWBLK + t * 16) + (wi % 4);
+      *q &= (1u << (mask_bits & 31)) - 1u;
+    }
   }
 }
 
