@@ -72,7 +72,7 @@ typedef struct {
  *   t  > 0 : BGV, t odd and < 2^31; Q = least odd integer > 2^logQ with Q = 1 (mod t), P likewise from logP
  *            (so logP == logQ gives P == Q)                                 (DESIGN.md 3-A10, A11)
  *   N a power of two, 2^8 <= N <= 2^16; 32 <= logQ; logQ, logP <= 2560.
- * Precomputes on the host and uploads: the NTT primes (31-bit, = 1 mod 2^17), psi/psi^-1 power
+ * Precomputes on the host and uploads: the NTT primes (30-bit, = 1 mod 2^17), psi/psi^-1 power
  * tables with Shoup companions, 2^(26 d) mod q_j and the CRT constants
  * (this build uses the direct form of Eq. 1).  Synchronises. */
 fhe_status fhe_ctx_create(fhe_ctx** out, uint32_t N, uint32_t logQ, uint32_t logP, uint64_t t);

@@ -37,12 +37,9 @@ fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const
     CK(launch_decompose(c, ws + comp * rp, 4 * rp, d_ct1 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
     CK(launch_decompose(c, ws + (2 + comp) * rp, 4 * rp, d_ct2 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
   }
-  CK(launch_ntt(c, ws, B * 4, K, false, nullptr, s), "ntt fwd");
-  CK(launch_pw_tensor(c, ws, B, K, s), "pointwise tensor");
-  // inverse on slots 0..2 of every item: items are 4 slots apart -> run per item group via npoly = B*4 would waste 25%;
-  // slots 0..2 of item b are contiguous [3][K][N], so launch per item
-  for (uint32_t b = 0; b < B; ++b)
-    CK(launch_ntt(c, ws + (size_t)b * 4 * rp, 3, K, true, c->tgt_tensor.d_scale, s), "ntt inv");
+  CK(launch_ntt_fwd(c, ws, B, 4, 4, K, s), "ntt fwd");
+  // pointwise tensor product in the registers of the first inverse pass: slots 0..2 <- INTT(d0^, d1^, d2^)
+  CK(launch_ntt_inv(c, ws, nullptr, B, 4, 3, K, PW_TENSOR, c->tgt_tensor.d_scale, s), "ntt inv");
   for (uint32_t b = 0; b < B; ++b)
     CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3 + (size_t)b * 3 * L * N, (size_t)L * N,
                   ws + (size_t)b * 4 * rp, rp, nullptr, 0, 3, s), "crt");
@@ -56,10 +53,8 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   const size_t rp = (size_t)K * N;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ws, 2 * rp, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, B, L, K, mask, s), "decompose d2");
-  for (uint32_t b = 0; b < B; ++b)
-    CK(launch_ntt(c, ws + (size_t)b * 2 * rp, 1, K, false, nullptr, s), "ntt fwd d2");
-  CK(launch_pw_relin(c, ws, c->d_evk_hat, B, K, s), "pointwise relin");
-  CK(launch_ntt(c, ws, B * 2, K, true, c->tgt_relin.d_scale, s), "ntt inv relin");
+  CK(launch_ntt_fwd(c, ws, B, 2, 1, K, s), "ntt fwd d2");
+  CK(launch_ntt_inv(c, ws, c->d_evk_hat, B, 2, 2, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt inv relin");
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
   for (uint32_t b = 0; b < B; ++b)
@@ -104,7 +99,7 @@ fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t w
   c->have_evk = false;
   const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
   CK(launch_decompose(c, c->d_evk_hat, (size_t)c->K2 * c->N, d_evk, (size_t)c->L_PQ * c->N, 2, c->L_PQ, c->K2, mask, s), "decompose evk");
-  CK(launch_ntt(c, c->d_evk_hat, 2, c->K2, false, nullptr, s), "ntt evk");
+  CK(launch_ntt_fwd(c, c->d_evk_hat, 1, 2, 2, c->K2, s), "ntt evk");
   c->have_evk = true;
   return FHE_OK;
 }
@@ -125,9 +120,8 @@ fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ra, rp, d_a, (size_t)L * N, batch, L, K, mask, s), "decompose a");
   CK(launch_decompose(c, rb, rp, d_b, (size_t)L * N, batch, L, K, mask, s), "decompose b");
-  CK(launch_ntt(c, ra, 2 * batch, K, false, nullptr, s), "ntt fwd");
-  CK(launch_pw_polymul(c, ra, rb, batch, K, s), "pointwise");
-  CK(launch_ntt(c, ra, batch, K, true, c->tgt_pm.d_scale, s), "ntt inv");
+  CK(launch_ntt_fwd(c, ra, 2 * batch, 1, 1, K, s), "ntt fwd");
+  CK(launch_ntt_inv(c, ra, rb, batch, 1, 1, K, PW_POLYMUL, c->tgt_pm.d_scale, s), "ntt inv");
   CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, (size_t)L * N, ra, rp, nullptr, 0, batch, s), "crt");
   return FHE_OK;
 }
@@ -222,7 +216,8 @@ fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
   if (!d_res || K == 0 || K > c->Kmax) return err(c, FHE_ERR_ARG, "bad argument");
-  CK(launch_ntt(c, d_res, npoly, K, inverse != 0, c->d_scale_plain, (cudaStream_t)stream), "ntt");
+  if (inverse) CK(launch_ntt_inv(c, d_res, nullptr, npoly, 1, 1, K, PW_NONE, c->d_scale_plain, (cudaStream_t)stream), "ntt inv");
+  else CK(launch_ntt_fwd(c, d_res, npoly, 1, 1, K, (cudaStream_t)stream), "ntt fwd");
   return FHE_OK;
 }
 

@@ -77,7 +77,7 @@ static BigU make_modulus(uint32_t log, uint64_t t) {
 static uint32_t primes_for(std::vector<uint32_t>& primes, const BigU& bound) {
   BigU M((uint64_t)1);
   uint32_t K = 0;
-  uint32_t cand = primes.empty() ? 0x80000001u - (1u << 17) : primes.back() - (1u << 17);
+  uint32_t cand = primes.empty() ? 0x40000001u - (1u << 17) : primes.back() - (1u << 17);   // q < 2^30: lazy butterflies keep values in [0, 4q)
   while (BigU::cmp(M, bound) <= 0) {
     if (K == primes.size()) {
       while (!is_prime32(cand)) cand -= (1u << 17);
@@ -207,7 +207,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   c->h_P.assign(c->L_P + 2, 0); P.to_limbs(c->h_P.data(), c->L_P + 2);
   c->h_PQ.assign(c->L_PQ + 2, 0); PQ.to_limbs(c->h_PQ.data(), c->L_PQ + 2);
 
-  // ---- primes: 31-bit, = 1 (mod 2^17), descending from 2^31; bounds DESIGN.md 3-A5 ------------
+  // ---- primes: 30-bit, = 1 (mod 2^17), descending from 2^30; bounds DESIGN.md 3-A5 ------------
   {
     BigU NQ2 = BigU::mul(Q, Q); NQ2.mul_small(N);
     BigU b_pm = NQ2; b_pm.mul_small(4);

@@ -104,21 +104,24 @@ struct LaunchTimer {
   ~LaunchTimer() { if (b) cudaEventRecord(b, s); }
 };
 
-// ---- launchers (kernels.cu) --------------------------------------------------------------------------------------
+// ---- launchers (kernels_*.cu) --------------------------------------------------------------------------------------
 // decompose: limbs [npoly][Lin][N] -> residues [npoly][K][N] (poly p of the input goes to out + out_poly_stride * p)
 cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_limbs,
                              size_t limb_poly_stride, uint32_t npoly, uint32_t Lin, uint32_t K, uint32_t mask_bits,
                              cudaStream_t s);
-// forward / inverse NTT in place on [npoly][K][N]; scale: per-prime final constant of the inverse ([K] uint2)
-cudaError_t launch_ntt(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, bool inverse, const uint2* d_scale,
-                       cudaStream_t s);
-// pointwise products (Montgomery: result carries a factor 2^-32 that the inverse scale removes)
-cudaError_t launch_pw_polymul(Context* c, uint32_t* d_a, const uint32_t* d_b, uint32_t batch, uint32_t K,
-                              cudaStream_t s);                      // a <- a*b, [batch][K][N]
-cudaError_t launch_pw_tensor(Context* c, uint32_t* d_r, uint32_t batch, uint32_t K, cudaStream_t s);
-// r: [batch][4][K][N] = (a0,a1,b0,b1)^ -> slots 0..2 = (d0,d1,d2)^
-cudaError_t launch_pw_relin(Context* c, uint32_t* d_r, const uint32_t* d_evk_hat, uint32_t batch, uint32_t K,
-                            cudaStream_t s);                        // r: [batch][2][K][N], slot0 = d2^ in
+// Transforms live in an item-major residue buffer [nitems][S][K][N] (S slots per item); slots 0..U-1 of every item
+// are transformed in place.  Forward output is in bit-reversed order and canonical ([0, q)).
+cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s);
+// Inverse, with the pointwise products (S3) formed in registers by the first pass (Montgomery: each product carries a
+// factor 2^-32 that d_scale removes):
+//   PW_NONE    plain inverse of slots 0..U-1
+//   PW_POLYMUL S = U = 1: data <- INTT(data * aux), aux = [nitems][K][N]
+//   PW_TENSOR  S = 4, U = 3: slots (a0, a1, b0, b1)^ -> slots 0..2 = INTT(a0 b0, a0 b1 + a1 b0, a1 b1)
+//   PW_RELIN   S = U = 2: slot 0 = d2^ -> slots 0, 1 = INTT(d2^ * aux[0], d2^ * aux[1]), aux = evk-hat [2][K][N]
+// d_scale: per-prime final constant ([K] uint2, value and Shoup companion).
+enum PwMode : int { PW_NONE = 0, PW_POLYMUL = 1, PW_TENSOR = 2, PW_RELIN = 3 };
+cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
+                           uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s);
 // CRT + post: residues [npoly][K][N] (poly p at d_res + p*res_poly_stride) -> limbs out [npoly][L][N]
 // d_add: for the relin modes, the polynomial added at the end (same indexing as out), else nullptr
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_poly_stride,

@@ -1,207 +1,398 @@
-// kernels_ntt.cu -- S2/S4 negacyclic NTT passes, S3 pointwise products.
+// kernels_ntt.cu -- S2/S4 negacyclic NTT (Eq. 8-9) with S3, the pointwise products (PAPER.md:354-356,
+// Eq. 7), folded into the first inverse pass.
 //
-// NTT formulation (Eq. 8-9): merged-psi Cooley-Tukey forward / Gentleman-Sande inverse
-// (PAPER.md:352, 358); the psi^j "twist" of PAPER.md:346-350 is folded into the butterfly twiddles, so no separate
-// twist pass exists.  tw_fwd[k] = psi^bitrev_logN(k), tw_inv[k] = psi^-bitrev_logN(k).  Forward stage with m
-// groups (m = 1, 2, .., N/2) pairs j and j + t, t = N/(2m), twiddle index m + (j >> log2(2t)).  Output of the
-// forward transform is in bit-reversed order; the pointwise products do not care, the inverse undoes it.
+// Formulation: merged-psi Cooley-Tukey forward / Gentleman-Sande inverse; the psi^j "twist" of
+// PAPER.md:346-350 lives in the butterfly twiddles, so there is no separate twist pass.  tw_fwd[k] = psi^bitrev(k),
+// tw_inv[k] = psi^-bitrev(k).  A forward stage with m groups pairs j and j + N/(2m) with twiddle index m + group;
+// the forward output is in bit-reversed order, the pointwise products do not care and the inverse undoes it.
 //
-// Two-pass split for N = N1 * N2 (the paper's "column NTT, twiddle, row NTT"): with the merged
-// twiddles the first log2 N1 stages act on columns (stride N2) with the N1-point table prefix, the last log2 N2
-// stages act on contiguous rows r with table indices (N1 + r) m' + i'.  Both are one "local transform with base":
-// twiddle index = base * m' + i' (base = 1 for columns / whole transforms, N1 + r for row r), so there is no separate
-// twiddle-multiplication pass and no transpose.
+// Split (the paper's two-pass / four-step idea): N = N1 * 256.  The first log2 N1 stages act on
+// "columns" (stride 256) with the N1-point prefix of the table, the last 8 stages on contiguous 256-point "rows" r with
+// table indices (N1 + r) m' + i'.  Both are one "local transform with base": twiddle index = base * m' + i' (base = 1
+// for columns, N1 + r for row r), so the paper's separate twiddle-multiplication pass and transpose do not exist.
+//
+// Each pass is register-tiled: a thread owns 16 points, runs four radix-2 stages on them in registers, trades points
+// with the other threads of its sub-transform through shared memory once, and runs the remaining (up to four) stages
+// in registers again.  Butterflies are Harvey's lazy ones with Shoup twiddles: values stay in [0, 4q) (forward) resp.
+// [0, 2q) (inverse), which is why the primes are below 2^30 (PAPER.md:312 allows 30- or 31-bit).  Only the last pass
+// of a transform brings values back to [0, q).
 #include "fhe_internal.cuh"
 
 namespace fhe {
 
-// ------------------------------------------------------------------------------------------------------------------
-// S2 / S4: local transform of n = 2^ln points with twiddle index base * m' + i', T transforms per block, radix-2
-// stages in shared memory (first correct version; the register-tiled version replaces it where it matters).
-// Layout of the tile in shared memory = flat load order f:
-//   column tile (COL): f = e * T + tt  <->  global  e * N2 + col0 + tt
-//   row tile    (ROW): f = tt * n + e  <->  global (row0 + tt) * n + e         (also the whole-transform case, T = 1)
-// ------------------------------------------------------------------------------------------------------------------
-template <bool INV, bool COL>
-__global__ void __launch_bounds__(256)
-ntt_tile_kernel(uint32_t* __restrict__ data, const uint2* __restrict__ tw_all, const uint32_t* __restrict__ qarr,
-                const uint2* __restrict__ scale, uint32_t N, uint32_t K, uint32_t ln, uint32_t lT, uint32_t N1,
-                uint32_t tiles_per_tr, bool apply_scale) {
-  extern __shared__ uint32_t sm[];
-  const uint32_t n = 1u << ln, T = 1u << lT;
-  const uint32_t tile = blockIdx.x % tiles_per_tr;
-  const uint32_t pp = blockIdx.x / tiles_per_tr;          // poly * K + prime
-  const uint32_t j = pp % K;
-  const uint32_t q = __ldg(qarr + j);
-  const uint2* tw = tw_all + (size_t)j * N;
-  uint32_t* g = data + (size_t)pp * N;
-  const uint32_t total = n * T;
-  const uint32_t N2 = COL ? (N / n) : n;
-
-  for (uint32_t f = threadIdx.x; f < total; f += blockDim.x) {
-    size_t off = COL ? ((size_t)(f >> lT) * N2 + tile * T + (f & (T - 1))) : ((size_t)tile * total + f);
-    sm[f] = g[off];
-  }
-  __syncthreads();
-
-  const uint32_t half = total >> 1;   // butterflies per stage in the tile
-  for (uint32_t st = 0; st < ln; ++st) {
-    const uint32_t sp = INV ? (ln - 1 - st) : st;     // stage parameter: m' = 2^sp
-    const uint32_t ltl = ln - 1 - sp;                 // log2 of the local butterfly stride
-    const uint32_t tl = 1u << ltl;
-    for (uint32_t x = threadIdx.x; x < half; x += blockDim.x) {
-      uint32_t tt, b;
-      if (COL) { tt = x & (T - 1); b = x >> lT; }
-      else     { b = x & ((n >> 1) - 1); tt = x >> (ln - 1); }
-      const uint32_t ip = b >> ltl, jj = b & (tl - 1);
-      const uint32_t e0 = (ip << (ltl + 1)) + jj, e1 = e0 + tl;
-      const uint32_t base = COL ? 1u : (N1 + tile * T + tt);   // N1 == 0 and tile == 0 for whole transforms -> +1 below
-      const uint32_t widx = (COL || N1) ? ((base << sp) + ip) : ((1u << sp) + ip);
-      const uint2 w = __ldg(tw + widx);
-      const uint32_t i0 = COL ? (e0 * T + tt) : (tt * n + e0);
-      const uint32_t i1 = COL ? (e1 * T + tt) : (tt * n + e1);
-      const uint32_t U = sm[i0], V = sm[i1];
-      if (!INV) {
-        const uint32_t Vw = mul_shoup(V, w.x, w.y, q);
-        sm[i0] = csub(U + Vw, q);
-        const uint32_t d = U - Vw;
-        sm[i1] = min(d, d + q);
-      } else {
-        sm[i0] = csub(U + V, q);
-        const uint32_t d = U - V;
-        sm[i1] = mul_shoup(min(d, d + q), w.x, w.y, q);
-      }
-    }
-    __syncthreads();
-  }
-  uint2 sc = make_uint2(0, 0);
-  if (apply_scale) sc = __ldg(scale + j);
-  for (uint32_t f = threadIdx.x; f < total; f += blockDim.x) {
-    size_t off = COL ? ((size_t)(f >> lT) * N2 + tile * T + (f & (T - 1))) : ((size_t)tile * total + f);
-    uint32_t v = sm[f];
-    if (apply_scale) v = mul_shoup(v, sc.x, sc.y, q);
-    g[off] = v;
-  }
+// ---- butterflies ----------------------------------------------------------------------------------------------------
+// forward: X, Y in [0, 4q) -> X + wY, X - wY in [0, 4q)
+__device__ __forceinline__ void bf_fwd(uint32_t& X, uint32_t& Y, const uint2 w, const uint32_t q, const uint32_t q2) {
+  const uint32_t x = min(X, X - q2);
+  const uint32_t t = mul_shoup_lazy(Y, w.x, w.y, q);
+  X = x + t;
+  Y = x - t + q2;
+}
+// inverse: X, Y in [0, 2q) -> X + Y, w (X - Y) in [0, 2q)
+__device__ __forceinline__ void bf_inv(uint32_t& X, uint32_t& Y, const uint2 w, const uint32_t q, const uint32_t q2) {
+  const uint32_t s = X + Y;
+  const uint32_t d = X - Y + q2;
+  X = min(s, s - q2);
+  Y = mul_shoup_lazy(d, w.x, w.y, q);
 }
 
-cudaError_t launch_ntt(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, bool inverse, const uint2* d_scale,
-                       cudaStream_t s) {
-  if (npoly == 0) return cudaSuccess;
-  const uint32_t N = c->N, logN = c->logN;
-  const uint32_t ntr = npoly * K;
-  if (logN <= 13) {   // one kernel: the whole transform in shared memory
-    size_t smem = (size_t)N * 4;
-    LaunchTimer lt(c, inverse ? KC_NTT_INV : KC_NTT_FWD, s);
-    if (!inverse)
-      ntt_tile_kernel<false, false><<<ntr, 256, smem, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, logN, 0, 0, 1, false);
-    else
-      ntt_tile_kernel<true, false><<<ntr, 256, smem, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, logN, 0, 0, 1, true);
-    return cudaGetLastError();
-  }
-  const uint32_t ln2 = 8, ln1 = logN - ln2, N1 = 1u << ln1, N2 = 1u << ln2;
-  const uint32_t lTc = 5, lTr = 4;                       // 32 columns / 16 rows per block
-  const uint32_t col_tiles = N2 >> lTc, row_tiles = N1 >> lTr;
-  const size_t smem_col = (size_t)N1 * (1u << lTc) * 4, smem_row = (size_t)N2 * (1u << lTr) * 4;
-  if (!inverse) {
-    { LaunchTimer lt(c, KC_NTT_FWD, s);
-    ntt_tile_kernel<false, true><<<ntr * col_tiles, 256, smem_col, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln1, lTc, N1, col_tiles, false); }
-    { LaunchTimer lt(c, KC_NTT_FWD, s);
-    ntt_tile_kernel<false, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_fwd, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false); }
+template <int NG>
+__device__ __forceinline__ void load_tw(const uint2* __restrict__ p, uint2 (&w)[8]) {
+  if constexpr (NG == 1) {
+    w[0] = __ldg(p);
   } else {
-    { LaunchTimer lt(c, KC_NTT_INV, s);
-    ntt_tile_kernel<true, false><<<ntr * row_tiles, 256, smem_row, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, ln2, lTr, N1, row_tiles, false); }
-    LaunchTimer lt(c, KC_NTT_INV, s);
-    ntt_tile_kernel<true, true><<<ntr * col_tiles, 256, smem_col, s>>>(d_res, c->d_tw_inv, c->d_q, d_scale, N, K, ln1, lTc, N1, col_tiles, true);
+#pragma unroll
+    for (int g = 0; g < NG; g += 2) {
+      const uint4 v = __ldg(reinterpret_cast<const uint4*>(p + g));
+      w[g] = make_uint2(v.x, v.y);
+      w[g + 1] = make_uint2(v.z, v.w);
+    }
   }
-  return cudaGetLastError();
 }
 
-// ------------------------------------------------------------------------------------------------------------------
-// S3: pointwise products in the NTT domain (Eq. 7), Montgomery form: each product carries 2^-32,
-// removed by the inverse transform's final constant.
-// ------------------------------------------------------------------------------------------------------------------
+// Stage with S = log2(groups inside the thread's points): H = E >> (S + 1) is the register stride, the thread's
+// 1 << S twiddles are consecutive table entries starting at `tw`.
+template <int E, int S, bool INV>
+__device__ __forceinline__ void reg_stage(uint32_t (&x)[16], const uint2* __restrict__ tw, uint32_t q, uint32_t q2) {
+  constexpr int NG = 1 << S, H = E >> (S + 1);
+  uint2 w[8];
+  load_tw<NG>(tw, w);
+#pragma unroll
+  for (int g = 0; g < NG; ++g)
+#pragma unroll
+    for (int k = 0; k < H; ++k) {
+      const int i0 = g * 2 * H + k;
+      if (!INV) bf_fwd(x[i0], x[i0 + H], w[g], q, q2);
+      else bf_inv(x[i0], x[i0 + H], w[g], q, q2);
+    }
+}
+
+// Phase A of a local transform of 2^LN points, LN > 4: the thread's 16 points differ in the top four index bits; the
+// first NS = min(4, LN - 4) stages of the local transform (phase B runs the last four).  The twiddles do not depend on
+// the thread: index (base << s) + g.
+template <bool INV, int NS>
+__device__ __forceinline__ void phase_a(uint32_t (&x)[16], const uint2* __restrict__ tw, uint32_t base, uint32_t q, uint32_t q2) {
+  if (!INV) {
+    reg_stage<16, 0, false>(x, tw + base, q, q2);
+    if constexpr (NS > 1) reg_stage<16, 1, false>(x, tw + 2 * base, q, q2);
+    if constexpr (NS > 2) reg_stage<16, 2, false>(x, tw + 4 * base, q, q2);
+    if constexpr (NS > 3) reg_stage<16, 3, false>(x, tw + 8 * base, q, q2);
+  } else {
+    if constexpr (NS > 3) reg_stage<16, 3, true>(x, tw + 8 * base, q, q2);
+    if constexpr (NS > 2) reg_stage<16, 2, true>(x, tw + 4 * base, q, q2);
+    if constexpr (NS > 1) reg_stage<16, 1, true>(x, tw + 2 * base, q, q2);
+    reg_stage<16, 0, true>(x, tw + base, q, q2);
+  }
+}
+// Phase B: the thread's E = min(16, 2^LN) points are contiguous, starting at local index tb * E; local stages
+// LN - log2(E) .. LN - 1.  Stage with S in-thread group bits uses twiddles ((base << s) + (tb << S)) + g, s = LN - log2 E + S.
+template <int LN, bool INV>
+__device__ __forceinline__ void phase_b(uint32_t (&x)[16], const uint2* __restrict__ tw, uint32_t base, uint32_t tb, uint32_t q, uint32_t q2) {
+  constexpr int LE = LN < 4 ? LN : 4, E = 1 << LE, S0 = LN - LE;
+#define STG(S) reg_stage<E, S, INV>(x, tw + (base << (S0 + S)) + (tb << S), q, q2)
+  if (!INV) {
+    if constexpr (LE > 0) STG(0);
+    if constexpr (LE > 1) STG(1);
+    if constexpr (LE > 2) STG(2);
+    if constexpr (LE > 3) STG(3);
+  } else {
+    if constexpr (LE > 3) STG(3);
+    if constexpr (LE > 2) STG(2);
+    if constexpr (LE > 1) STG(1);
+    if constexpr (LE > 0) STG(0);
+  }
+#undef STG
+}
+
+__device__ __forceinline__ uint32_t canon4(uint32_t v, uint32_t q, uint32_t q2) { v = min(v, v - q2); return min(v, v - q); }
+
+// Montgomery product: a b 2^-32 mod q in [0, q) (the inverse transform's final constant carries the 2^32)
 __device__ __forceinline__ uint32_t mm(uint32_t a, uint32_t b, uint32_t q, uint32_t qn) {
   return mont_redc((uint64_t)a * b, q, qn);
 }
 
+struct NttArgs {
+  uint32_t* data;            // transforms: item-major [nitems][S][K][N]; slots 0..U-1 of every item are transformed
+  const uint32_t* aux;       // PW_POLYMUL: b [nitems][K][N]; PW_RELIN: evk-hat [2][K][N]
+  const uint2* tw;           // [Kmax][N] twiddles of the direction
+  const uint32_t* q;         // [Kmax]
+  const uint32_t* qn;        // [Kmax] -q^-1 mod 2^32
+  const uint2* scale;        // [K] final constant of the inverse (with Shoup companion)
+  uint32_t N, K, N1, S, U, units;
+};
+
+// ------------------------------------------------------------------------------------------------------------------
+// Column pass: 2^LN-point transforms over elements e * 256 + c (c = column), in place.  A block owns T adjacent
+// columns of one (polynomial, prime); thread (t, cc) works on column cc; the block always has 256 threads and
+// 4096 points.  Shared-memory tile [e][cc]: every access of a warp is to 32 (or 16) consecutive words.
+// ------------------------------------------------------------------------------------------------------------------
+template <int LN, bool INV>
 __global__ void __launch_bounds__(256)
-pw_polymul_kernel(uint32_t* __restrict__ a, const uint32_t* __restrict__ b, uint32_t N4, uint32_t K,
-                  const uint32_t* __restrict__ qarr, const uint32_t* __restrict__ qnarr, uint32_t gx) {
-  const uint32_t pp = blockIdx.x / gx, j = pp % K, cx = blockIdx.x % gx;
-  const uint32_t q = __ldg(qarr + j), qn = __ldg(qnarr + j);
-  uint4* pa = reinterpret_cast<uint4*>(a) + (size_t)pp * N4;
-  const uint4* pb = reinterpret_cast<const uint4*>(b) + (size_t)pp * N4;
-  for (uint32_t i = cx * blockDim.x + threadIdx.x; i < N4; i += gx * blockDim.x) {
-    uint4 x = pa[i], y = pb[i];
-    x.x = mm(x.x, y.x, q, qn); x.y = mm(x.y, y.y, q, qn); x.z = mm(x.z, y.z, q, qn); x.w = mm(x.w, y.w, q, qn);
-    pa[i] = x;
+ntt_col_kernel(NttArgs a) {
+  constexpr int LE = LN < 4 ? LN : 4, E = 1 << LE;   // points per thread
+  constexpr int TPC = (1 << LN) / E;                 // threads per column
+  constexpr int T = 256 / TPC;                       // columns per block
+  __shared__ uint32_t sm[LN > 4 ? 4096 : 1];
+  const uint32_t tid = threadIdx.x, cc = tid % T, t = tid / T;
+  const uint32_t tiles = 256 / T;
+  const uint32_t tr = blockIdx.x / tiles, c0 = (blockIdx.x % tiles) * T;
+  const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
+  const uint2* tw = a.tw + (size_t)j * a.N;
+  uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + c0 + cc;
+  uint32_t x[16];
+
+  if constexpr (LN > 4) {
+    if (!INV) {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = g[(size_t)(i * TPC + t) * 256];
+      phase_a<false, LN - 4>(x, tw, 1, q, q2);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) sm[(i * TPC + t) * T + cc] = x[i];
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = sm[(t * 16 + i) * T + cc];
+      phase_b<LN, false>(x, tw, 1, t, q, q2);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[(size_t)(t * 16 + i) * 256] = x[i];
+    } else {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = g[(size_t)(t * 16 + i) * 256];
+      phase_b<LN, true>(x, tw, 1, t, q, q2);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) sm[(t * 16 + i) * T + cc] = x[i];
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = sm[(i * TPC + t) * T + cc];
+      phase_a<true, LN - 4>(x, tw, 1, q, q2);
+      const uint2 sc = __ldg(a.scale + j);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[(size_t)(i * TPC + t) * 256] = mul_shoup(x[i], sc.x, sc.y, q);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < E; ++i) x[i] = g[(size_t)i * 256];
+    phase_b<LN, INV>(x, tw, 1, 0, q, q2);
+    if (!INV) {
+#pragma unroll
+      for (int i = 0; i < E; ++i) g[(size_t)i * 256] = x[i];
+    } else {
+      const uint2 sc = __ldg(a.scale + j);
+#pragma unroll
+      for (int i = 0; i < E; ++i) g[(size_t)i * 256] = mul_shoup(x[i], sc.x, sc.y, q);
+    }
   }
 }
 
-// r: [batch][4][K][N] = (a0, a1, b0, b1) -> slots 0..2 = (a0 b0, a0 b1 + a1 b0, a1 b1)
-__global__ void __launch_bounds__(256)
-pw_tensor_kernel(uint32_t* __restrict__ r, uint32_t N4, uint32_t K, const uint32_t* __restrict__ qarr,
-                 const uint32_t* __restrict__ qnarr, uint32_t gx) {
-  const uint32_t pp = blockIdx.x / gx, cx = blockIdx.x % gx, j = pp % K, bi = pp / K;
-  const uint32_t q = __ldg(qarr + j), qn = __ldg(qnarr + j);
-  const size_t ps = (size_t)K * N4;   // poly stride in uint4
-  uint4* base = reinterpret_cast<uint4*>(r) + (size_t)bi * 4 * ps + (size_t)j * N4;
-  for (uint32_t i = cx * blockDim.x + threadIdx.x; i < N4; i += gx * blockDim.x) {
-    const uint4 a0 = base[i], a1 = base[ps + i], b0 = base[2 * ps + i], b1 = base[3 * ps + i];
-    uint4 d0, d1, d2;
-#define TP(c)                                                                     \
-  d0.c = mm(a0.c, b0.c, q, qn);                                                   \
-  d1.c = mont_redc((uint64_t)a0.c * b1.c + (uint64_t)a1.c * b0.c, q, qn);         \
-  d2.c = mm(a1.c, b1.c, q, qn);
-    TP(x) TP(y) TP(z) TP(w)
-#undef TP
-    base[i] = d0; base[ps + i] = d1; base[2 * ps + i] = d2;
+// ------------------------------------------------------------------------------------------------------------------
+// Row pass: 256-point transforms over contiguous rows, in place.  A block owns 16 rows, a half-warp one row.  The
+// exchange between the two register phases stays inside the half-warp (padded tile: 20 words per 16 points, 336 per
+// row, conflict-free for the scalar phase-A and the 128-bit phase-B accesses).
+// Forward: rows are the last pass, results leave canonical.  Inverse: rows are the first pass; PW selects what is
+// transformed (PwMode) -- the pointwise products are formed in registers from the forward-domain operands.
+// FINAL: there is no column pass (N = 256), so the inverse applies the scale here.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int ROW_SM = 336;
+
+__device__ __forceinline__ void row_fwd_core(uint32_t (&x)[16], uint32_t* srow, uint32_t t, const uint2* tw, uint32_t base,
+                                             uint32_t q, uint32_t q2) {
+  phase_a<false, 4>(x, tw, base, q, q2);
+#pragma unroll
+  for (int i = 0; i < 16; ++i) srow[i * 20 + t] = x[i];
+  __syncwarp();
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint4 v = *reinterpret_cast<const uint4*>(srow + t * 20 + 4 * k);
+    x[4 * k] = v.x; x[4 * k + 1] = v.y; x[4 * k + 2] = v.z; x[4 * k + 3] = v.w;
+  }
+  __syncwarp();
+  phase_b<8, false>(x, tw, base, t, q, q2);
+}
+// in: x = the thread's 16 contiguous points (values in [0, 2q)); out: x[i] = point i * 16 + t
+__device__ __forceinline__ void row_inv_core(uint32_t (&x)[16], uint32_t* srow, uint32_t t, const uint2* tw, uint32_t base,
+                                             uint32_t q, uint32_t q2) {
+  phase_b<8, true>(x, tw, base, t, q, q2);
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    *reinterpret_cast<uint4*>(srow + t * 20 + 4 * k) = make_uint4(x[4 * k], x[4 * k + 1], x[4 * k + 2], x[4 * k + 3]);
+  __syncwarp();
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = srow[i * 20 + t];
+  __syncwarp();
+  phase_a<true, 4>(x, tw, base, q, q2);
+}
+
+__device__ __forceinline__ void load16(uint32_t (&x)[16], const uint32_t* __restrict__ p) {
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const uint4 v = *reinterpret_cast<const uint4*>(p + 4 * k);
+    x[4 * k] = v.x; x[4 * k + 1] = v.y; x[4 * k + 2] = v.z; x[4 * k + 3] = v.w;
   }
 }
 
-// r: [batch][2][K][N], slot 0 = d2^ -> slot 0 = d2^ * evk_b^, slot 1 = d2^ * evk_a^
 __global__ void __launch_bounds__(256)
-pw_relin_kernel(uint32_t* __restrict__ r, const uint32_t* __restrict__ evk, uint32_t N4, uint32_t K,
-                const uint32_t* __restrict__ qarr, const uint32_t* __restrict__ qnarr, uint32_t gx) {
-  const uint32_t pp = blockIdx.x / gx, cx = blockIdx.x % gx, j = pp % K, bi = pp / K;
-  const uint32_t q = __ldg(qarr + j), qn = __ldg(qnarr + j);
-  const size_t ps = (size_t)K * N4;
-  uint4* base = reinterpret_cast<uint4*>(r) + (size_t)bi * 2 * ps + (size_t)j * N4;
-  const uint4* eb = reinterpret_cast<const uint4*>(evk) + (size_t)j * N4;
-  const uint4* ea = eb + ps;
-  for (uint32_t i = cx * blockDim.x + threadIdx.x; i < N4; i += gx * blockDim.x) {
-    const uint4 d = base[i], b = eb[i], a = ea[i];
-    uint4 xb, xa;
-    xb.x = mm(d.x, b.x, q, qn); xb.y = mm(d.y, b.y, q, qn); xb.z = mm(d.z, b.z, q, qn); xb.w = mm(d.w, b.w, q, qn);
-    xa.x = mm(d.x, a.x, q, qn); xa.y = mm(d.y, a.y, q, qn); xa.z = mm(d.z, a.z, q, qn); xa.w = mm(d.w, a.w, q, qn);
-    base[i] = xb; base[ps + i] = xa;
+ntt_row_fwd_kernel(NttArgs a) {
+  __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
+  const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
+  const uint32_t unit = blockIdx.x * 16 + rl;           // row of a transform: ((item * U + slot) * K + j) * N1 + r
+  if (unit >= a.units) return;                          // whole half-warps leave together; no block-wide barrier below
+  const uint32_t r = unit % a.N1, tr = unit / a.N1;
+  const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
+  const uint2* tw = a.tw + (size_t)j * a.N;
+  uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + (size_t)r * 256;
+  uint32_t x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = g[i * 16 + t];
+  row_fwd_core(x, sm + rl * ROW_SM, t, tw, a.N1 + r, q, q2);
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    *reinterpret_cast<uint4*>(g + t * 16 + 4 * k) = make_uint4(canon4(x[4 * k], q, q2), canon4(x[4 * k + 1], q, q2),
+                                                                canon4(x[4 * k + 2], q, q2), canon4(x[4 * k + 3], q, q2));
+}
+
+template <int PW, bool FINAL>
+__global__ void __launch_bounds__(256)
+ntt_row_inv_kernel(NttArgs a) {
+  __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
+  const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
+  const uint32_t unit = blockIdx.x * 16 + rl;           // PW_NONE: as forward; else ((item * K) + j) * N1 + r
+  if (unit >= a.units) return;
+  const uint32_t r = unit % a.N1, tr = unit / a.N1;
+  uint32_t* srow = sm + rl * ROW_SM;
+  const size_t roff = (size_t)r * 256;
+  const size_t KN = (size_t)a.K * a.N;
+
+  auto finish = [&](uint32_t (&x)[16], uint32_t* g, uint32_t j, uint32_t q, uint32_t q2, const uint2* tw) {
+    row_inv_core(x, srow, t, tw, a.N1 + r, q, q2);
+    if (FINAL) {
+      const uint2 sc = __ldg(a.scale + j);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[i * 16 + t] = mul_shoup(x[i], sc.x, sc.y, q);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[i * 16 + t] = x[i];
+    }
+  };
+
+  if constexpr (PW == PW_NONE) {
+    const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+    const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
+    const uint2* tw = a.tw + (size_t)j * a.N;
+    uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + roff;
+    uint32_t x[16];
+    load16(x, g + t * 16);
+    finish(x, g, j, q, q2, tw);
+  } else {
+    const uint32_t item = tr / a.K, j = tr % a.K;
+    const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
+    const uint2* tw = a.tw + (size_t)j * a.N;
+    const size_t poff = (size_t)j * a.N + roff;          // offset of this row inside a [K][N] polynomial
+    if constexpr (PW == PW_POLYMUL) {
+      uint32_t* g = a.data + (size_t)item * KN + poff;
+      uint32_t x[16], y[16];
+      load16(x, g + t * 16);
+      load16(y, a.aux + (size_t)item * KN + poff + t * 16);
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mm(x[i], y[i], q, qn);
+      finish(x, g, j, q, q2, tw);
+    } else if constexpr (PW == PW_TENSOR) {
+      uint32_t* g = a.data + (size_t)item * 4 * KN + poff;       // slots a0, a1, b0, b1 at g + slot * KN
+      uint32_t a0[16], a1[16], b0[16], b1[16], x[16];
+      load16(a0, g + t * 16);
+      load16(a1, g + KN + t * 16);
+      load16(b0, g + 2 * KN + t * 16);
+      load16(b1, g + 3 * KN + t * 16);
+      __syncwarp();   // every lane of the row holds its operands before slot 0 is overwritten
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
+      finish(x, g, j, q, q2, tw);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
+      finish(x, g + KN, j, q, q2, tw);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
+      finish(x, g + 2 * KN, j, q, q2, tw);
+    } else {   // PW_RELIN
+      uint32_t* g = a.data + (size_t)item * 2 * KN + poff;       // slot 0 = d2-hat
+      uint32_t d[16], e[16], x[16];
+      load16(d, g + t * 16);
+      load16(e, a.aux + poff + t * 16);
+      __syncwarp();
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e[i], q, qn);
+      finish(x, g, j, q, q2, tw);
+      load16(e, a.aux + KN + poff + t * 16);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e[i], q, qn);
+      finish(x, g + KN, j, q, q2, tw);
+    }
   }
 }
 
-static inline uint32_t pw_grid_x(uint32_t N4) { return (N4 + 255) / 256 > 16 ? 16 : (N4 + 255) / 256; }
+// ---- launchers ------------------------------------------------------------------------------------------------------
+template <bool INV>
+static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaStream_t s) {
+  const uint32_t ln1 = c->logN - 8;
+  LaunchTimer lt(c, INV ? KC_NTT_INV : KC_NTT_FWD, s);
+#define COL_CASE(LN)                                                                           \
+  case LN: {                                                                                   \
+    constexpr int TPC = (1 << LN) / ((LN) < 4 ? (1 << (LN)) : 16);                             \
+    ntt_col_kernel<LN, INV><<<ntr * TPC, 256, 0, s>>>(a);                                      \
+    break;                                                                                     \
+  }
+  switch (ln1) {   // blocks per transform = 256 / T = TPC
+    COL_CASE(1) COL_CASE(2) COL_CASE(3) COL_CASE(4) COL_CASE(5) COL_CASE(6) COL_CASE(7) COL_CASE(8)
+    default: return cudaErrorInvalidValue;
+  }
+#undef COL_CASE
+  return cudaGetLastError();
+}
 
-cudaError_t launch_pw_polymul(Context* c, uint32_t* d_a, const uint32_t* d_b, uint32_t batch, uint32_t K,
-                              cudaStream_t s) {
-  if (!batch) return cudaSuccess;
-  const uint32_t N4 = c->N / 4;
-  LaunchTimer lt(c, KC_POINTWISE, s);
-  pw_polymul_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_a, d_b, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
+cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s) {
+  if (!nitems || !U) return cudaSuccess;
+  NttArgs a;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U;
+  const uint32_t ntr = nitems * U * K;
+  a.units = ntr * a.N1;
+  if (c->logN > 8) {
+    cudaError_t e = launch_col<false>(c, a, ntr, s);
+    if (e != cudaSuccess) return e;
+  }
+  LaunchTimer lt(c, KC_NTT_FWD, s);
+  ntt_row_fwd_kernel<<<(a.units + 15) / 16, 256, 0, s>>>(a);
   return cudaGetLastError();
 }
-cudaError_t launch_pw_tensor(Context* c, uint32_t* d_r, uint32_t batch, uint32_t K, cudaStream_t s) {
-  if (!batch) return cudaSuccess;
-  const uint32_t N4 = c->N / 4;
-  LaunchTimer lt(c, KC_POINTWISE, s);
-  pw_tensor_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_r, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
-  return cudaGetLastError();
-}
-cudaError_t launch_pw_relin(Context* c, uint32_t* d_r, const uint32_t* d_evk_hat, uint32_t batch, uint32_t K,
-                            cudaStream_t s) {
-  if (!batch) return cudaSuccess;
-  const uint32_t N4 = c->N / 4;
-  LaunchTimer lt(c, KC_POINTWISE, s);
-  pw_relin_kernel<<<pw_grid_x(N4) * batch * K, 256, 0, s>>>(d_r, d_evk_hat, N4, K, c->d_q, c->d_qinv_neg, pw_grid_x(N4));
-  return cudaGetLastError();
+
+cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
+                           uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s) {
+  if (!nitems || !U) return cudaSuccess;
+  NttArgs a;
+  a.data = d_res; a.aux = d_aux; a.tw = c->d_tw_inv; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U;
+  const bool fin = c->logN == 8;
+  const uint32_t row_units = (pw_mode == PW_NONE ? nitems * U : nitems) * K * a.N1;
+  a.units = row_units;
+  const uint32_t blocks = (row_units + 15) / 16;
+  {
+    LaunchTimer lt(c, KC_NTT_INV, s);
+#define ROW_CASE(PW)                                                                  \
+  case PW:                                                                            \
+    if (fin) ntt_row_inv_kernel<PW, true><<<blocks, 256, 0, s>>>(a);                  \
+    else ntt_row_inv_kernel<PW, false><<<blocks, 256, 0, s>>>(a);                     \
+    break;
+    switch (pw_mode) {
+      ROW_CASE(PW_NONE) ROW_CASE(PW_POLYMUL) ROW_CASE(PW_TENSOR) ROW_CASE(PW_RELIN)
+      default: return cudaErrorInvalidValue;
+    }
+#undef ROW_CASE
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  if (!fin) return launch_col<true>(c, a, nitems * U * K, s);
+  return cudaSuccess;
 }
 
 }  // namespace fhe
