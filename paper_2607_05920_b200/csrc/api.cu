@@ -32,17 +32,13 @@ fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const
   const size_t rp = (size_t)K * N;           // residue poly stride
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   // slots (a0, a1, b0, b1) per batch item: ct1 polys go to slots 0,1 ; ct2 polys to slots 2,3
-  for (uint32_t comp = 0; comp < 2; ++comp) {
-    // all batch items of component `comp`: input poly stride 2*L*N, output stride 4*rp
-    CK(launch_decompose(c, ws + comp * rp, 4 * rp, d_ct1 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
-    CK(launch_decompose(c, ws + (2 + comp) * rp, 4 * rp, d_ct2 + (size_t)comp * L * N, (size_t)2 * L * N, B, L, K, mask, s), "decompose");
-  }
+  CK(launch_decompose(c, ws, 4 * rp, rp, d_ct1, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct1");
+  CK(launch_decompose(c, ws + 2 * rp, 4 * rp, rp, d_ct2, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct2");
   CK(launch_ntt_fwd(c, ws, B, 4, 4, K, s), "ntt fwd");
   // pointwise tensor product in the registers of the first inverse pass: slots 0..2 <- INTT(d0^, d1^, d2^)
   CK(launch_ntt_inv(c, ws, nullptr, B, 4, 3, K, PW_TENSOR, c->tgt_tensor.d_scale, s), "ntt inv");
-  for (uint32_t b = 0; b < B; ++b)
-    CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3 + (size_t)b * 3 * L * N, (size_t)L * N,
-                  ws + (size_t)b * 4 * rp, rp, nullptr, 0, 3, s), "crt");
+  CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3, (size_t)3 * L * N, (size_t)L * N, ws, 4 * rp, rp, nullptr, 0, 0,
+                B, 3, s), "crt");
   return FHE_OK;
 }
 
@@ -52,14 +48,13 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   const uint32_t N = c->N, L = c->L, K = c->K2;
   const size_t rp = (size_t)K * N;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
-  CK(launch_decompose(c, ws, 2 * rp, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, B, L, K, mask, s), "decompose d2");
+  CK(launch_decompose(c, ws, 2 * rp, 0, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, 0, B, 1, L, K, mask, s), "decompose d2");
   CK(launch_ntt_fwd(c, ws, B, 2, 1, K, s), "ntt fwd d2");
   CK(launch_ntt_inv(c, ws, c->d_evk_hat, B, 2, 2, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt inv relin");
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
-  for (uint32_t b = 0; b < B; ++b)
-    CK(launch_crt(c, c->tgt_relin, pp, d_out2 + (size_t)b * 2 * L * N, (size_t)L * N, ws + (size_t)b * 2 * rp, rp,
-                  d_in3 + (size_t)b * 3 * L * N, (size_t)L * N, 2, s), "crt relin");
+  CK(launch_crt(c, c->tgt_relin, pp, d_out2, (size_t)2 * L * N, (size_t)L * N, ws, 2 * rp, rp, d_in3, (size_t)3 * L * N,
+                (size_t)L * N, B, 2, s), "crt relin");
   return FHE_OK;
 }
 
@@ -98,7 +93,7 @@ fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t w
   }
   c->have_evk = false;
   const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
-  CK(launch_decompose(c, c->d_evk_hat, (size_t)c->K2 * c->N, d_evk, (size_t)c->L_PQ * c->N, 2, c->L_PQ, c->K2, mask, s), "decompose evk");
+  CK(launch_decompose(c, c->d_evk_hat, 0, (size_t)c->K2 * c->N, d_evk, 0, (size_t)c->L_PQ * c->N, 1, 2, c->L_PQ, c->K2, mask, s), "decompose evk");
   CK(launch_ntt_fwd(c, c->d_evk_hat, 1, 2, 2, c->K2, s), "ntt evk");
   c->have_evk = true;
   return FHE_OK;
@@ -118,11 +113,11 @@ fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const
   uint32_t* ra = (uint32_t*)d_ws;
   uint32_t* rb = ra + (size_t)batch * rp;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
-  CK(launch_decompose(c, ra, rp, d_a, (size_t)L * N, batch, L, K, mask, s), "decompose a");
-  CK(launch_decompose(c, rb, rp, d_b, (size_t)L * N, batch, L, K, mask, s), "decompose b");
+  CK(launch_decompose(c, ra, 0, rp, d_a, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose a");
+  CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose b");
   CK(launch_ntt_fwd(c, ra, 2 * batch, 1, 1, K, s), "ntt fwd");
   CK(launch_ntt_inv(c, ra, rb, batch, 1, 1, K, PW_POLYMUL, c->tgt_pm.d_scale, s), "ntt inv");
-  CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, (size_t)L * N, ra, rp, nullptr, 0, batch, s), "crt");
+  CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, 0, (size_t)L * N, ra, 0, rp, nullptr, 0, 0, 1, batch, s), "crt");
   return FHE_OK;
 }
 
@@ -208,7 +203,7 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
   if (!d_res || !d_limbs || K == 0 || K > c->Kmax || Lin == 0 || Lin > MAX_LIMBS_IN) return err(c, FHE_ERR_ARG, "bad argument");
-  CK(launch_decompose(c, d_res, (size_t)K * c->N, d_limbs, (size_t)Lin * c->N, npoly, Lin, K, mask_bits, (cudaStream_t)stream), "decompose");
+  CK(launch_decompose(c, d_res, 0, (size_t)K * c->N, d_limbs, 0, (size_t)Lin * c->N, 1, npoly, Lin, K, mask_bits, (cudaStream_t)stream), "decompose");
   return FHE_OK;
 }
 

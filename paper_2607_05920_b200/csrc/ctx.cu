@@ -97,16 +97,6 @@ static std::vector<uint8_t> bytes_of(const BigU& x, size_t n) {
   return o;
 }
 
-// Largest chunk width whose CRT kernel footprint (A image / limb columns + two constant buffers) still lets two CTAs
-// share an SM; 32 as the floor.
-static uint32_t pick_crt_nc(uint32_t KB, uint32_t ncols, uint32_t region_bytes) {
-  for (uint32_t nc : {128u, 64u}) {
-    if (nc / 2 >= ncols) continue;                       // do not pad a narrow target to a wide chunk
-    if ((size_t)region_bytes + 2 * (size_t)KB * nc + 1024 <= 112 * 1024) return nc;
-  }
-  return 32;
-}
-
 // CRT constants for the basis q_0..q_{K-1} and the target T (pow2: T = 2^(32 Lraw) with Lraw = ceil(width_bits/32);
 // else T = Tmod odd).  See fhe_internal.cuh (CrtTarget) and kernels_crt.cu for how the image is consumed.
 static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2, uint32_t width_bits,
@@ -120,17 +110,15 @@ static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2
   const uint32_t nbytes = 4 * tg.Lraw;
   const uint32_t ncols = CRT_ALPHA_COLS + nbytes;
   tg.Lx = std::max(tg.Lraw + 1, post_limbs);
-  const uint32_t region = std::max(tg.KB * 128u, tg.Lx * 512u);
-  tg.NC = pick_crt_nc(tg.KB, ncols, region);
-  tg.nchunks = (ncols + tg.NC - 1) / tg.NC;
-  if (tg.nchunks * tg.NC > 512) return cudaErrorInvalidValue;
+  constexpr uint32_t NC = 64;                                           // pipe::NC
+  tg.nchunks = (ncols + NC - 1) / NC;
   const BigU T = pow2 ? BigU::pow2(32 * tg.Lraw) : Tmod;
   BigU M((uint64_t)1);
   for (uint32_t i = 0; i < K; ++i) M.mul_small(c->h_q[i]);
-  const size_t chunk_bytes = (size_t)tg.KB * tg.NC;
+  const size_t chunk_bytes = (size_t)tg.KB * NC;
   std::vector<uint8_t> img(chunk_bytes * tg.nchunks, 0);
   auto put = [&](uint32_t kb, uint32_t col, uint8_t v) {
-    img[(size_t)(col / tg.NC) * chunk_bytes + (size_t)(kb / 16) * tg.NC * 16 + (size_t)(col % tg.NC) * 16 + kb % 16] = v;
+    img[(size_t)(col / NC) * chunk_bytes + (size_t)(kb / 16) * NC * 16 + (size_t)(col % NC) * 16 + kb % 16] = v;
   };
   std::vector<uint2> scale(K);
   for (uint32_t i = 0; i < K; ++i) {
@@ -314,6 +302,11 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   c->post_pm = pp;     c->post_pm.mode = ckks ? POST_CKKS_MASK : POST_BGV_MODQ;
   c->post_tensor = c->post_pm;
   c->post_relin = pp;  c->post_relin.mode = ckks ? POST_CKKS_RELIN : POST_BGV_RELIN;
+  if (!crt_target_fits(c->tgt_pm, c->post_pm) || !crt_target_fits(c->tgt_tensor, c->post_tensor) ||
+      !crt_target_fits(c->tgt_relin, c->post_relin)) {
+    destroy(c);
+    return fail(nullptr, FHE_ERR_UNSUPPORTED, "parameters too large for the conversion pipeline (TMEM columns / shared memory)");
+  }
   e = cudaDeviceSynchronize();
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, m); }
   *out = c;

@@ -11,8 +11,7 @@
 namespace fhe {
 
 constexpr int MAX_LIMBS_IN = 104;              // widest decompose input (limbs); 416 bytes of contraction
-constexpr int DEC_NC = 64;                     // decompose: columns per MMA / constant chunk = 16 primes x 4 constant bytes
-constexpr int DEC_GROUP_CHUNKS = 2;            // decompose: chunks accumulated in TMEM before an epilogue (128 columns)
+constexpr int DEC_NC = 64;                     // decompose: columns per constant chunk = 16 primes x 4 constant bytes (= pipe::NC)
 constexpr int CRT_ALPHA_COLS = 8;              // CRT: leading columns holding the byte sums of sum_i y_i floor(2^48 / q_i)
 constexpr int ALPHA_SHIFT = 48;
 
@@ -22,11 +21,10 @@ constexpr int ALPHA_SHIFT = 48;
 struct CrtTarget {
   uint32_t K = 0;        // primes in the basis (prefix of the context's prime list)
   uint32_t KB = 0;       // contraction bytes: 4 K rounded up to a multiple of 32
-  uint32_t NC = 0;       // columns per constant chunk / MMA
-  uint32_t nchunks = 0;  // chunks; nchunks * NC <= 512 TMEM columns
+  uint32_t nchunks = 0;  // 64-column chunks of the constant image (pipe::NC)
   uint32_t Lraw = 0;     // 32-bit limbs of V produced by the carry pass (4 Lraw value columns)
   uint32_t Lx = 0;       // limbs of the per-coefficient column the post-processing works on (>= Lraw + 1)
-  uint8_t* d_B = nullptr;      // [nchunks][KB/16][NC][16]: shared-memory images of the constant chunks
+  uint8_t* d_B = nullptr;      // [nchunks][KB/16][64][16]: shared-memory images of the constant chunks
   uint32_t* d_negM = nullptr;  // [Lraw]
   uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
 };
@@ -105,10 +103,11 @@ struct LaunchTimer {
 };
 
 // ---- launchers (kernels_*.cu) --------------------------------------------------------------------------------------
-// decompose: limbs [npoly][Lin][N] -> residues [npoly][K][N] (poly p of the input goes to out + out_poly_stride * p)
-cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_limbs,
-                             size_t limb_poly_stride, uint32_t npoly, uint32_t Lin, uint32_t K, uint32_t mask_bits,
-                             cudaStream_t s);
+// Polynomials of a launch are indexed (o, i), o < nouter, i < ninner, and live at base + o * outer + i * inner (words).
+// decompose: limbs [Lin][N] -> residues [K][N] per polynomial; mask_bits > 0 reduces the input mod 2^mask_bits first
+cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
+                             size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin,
+                             uint32_t K, uint32_t mask_bits, cudaStream_t s);
 // Transforms live in an item-major residue buffer [nitems][S][K][N] (S slots per item); slots 0..U-1 of every item
 // are transformed in place.  Forward output is in bit-reversed order and canonical ([0, q)).
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s);
@@ -122,11 +121,12 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
 enum PwMode : int { PW_NONE = 0, PW_POLYMUL = 1, PW_TENSOR = 2, PW_RELIN = 3 };
 cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
                            uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s);
-// CRT + post: residues [npoly][K][N] (poly p at d_res + p*res_poly_stride) -> limbs out [npoly][L][N]
-// d_add: for the relin modes, the polynomial added at the end (same indexing as out), else nullptr
-cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_poly_stride,
-                       const uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_add, size_t add_poly_stride,
-                       uint32_t npoly, cudaStream_t s);
+// CRT + post: residues [K][N] -> limbs [L][N] per polynomial (o, i); d_add: for the relin modes, the polynomial added
+// at the end, else nullptr
+cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
+                       const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
+                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s);
+bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the pipeline have the TMEM / shared memory for it
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -10,7 +10,7 @@
 #include <algorithm>
 
 #include "fhe_internal.cuh"
-#include "umma.cuh"
+#include "pipe.cuh"
 
 namespace fhe {
 
@@ -106,144 +106,130 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// CRT kernel.  Block = 128 coefficients of one polynomial (thread = coefficient = TMEM lane).
-//   phase 1  the residues y[i][n] are staged as the byte matrix A[n][4 i + b] (umma.cuh) and contracted on the tensor
-//            cores with the constant image B: column 8 + e receives S_e = sum_{i,b} y_ib * byte_{e-b}(W_i), columns
-//            0..5 the byte sums of sum_i y_i floor(2^48 / q_i) (-> alpha)
-//   phase 2  per thread: V = sum_e S_e 2^(8 e) + alpha * negM, carries propagated four columns (one limb) at a time,
-//            limbs written to this thread's column in shared memory (which reuses the A image's space)
-//   phase 3  post-processing on the limb column (mask / divide-by-P + add [+ rescale] / BGV reductions), store
+// CRT epilogue of the conversion pipeline (pipe.cuh).  The loaders stage the residues y[i][n] as the A operand (word i =
+// column i), the tensor cores contract them with the constant image B: column 8 + e receives
+// S_e = sum_{i,b} y_ib * byte_{e-b}(W_i), columns 0..5 the byte sums of sum_i y_i floor(2^48 / q_i) (-> alpha).  Here:
+//   carry pass   V = sum_e S_e 2^(8 e) + alpha * negM, four columns (one limb) at a time as the accumulator chunks
+//                arrive, limbs written to this thread's column xs[.][etid] in shared memory
+//   post         on the limb column: mask / divide-by-P + add [+ rescale] / BGV reductions, then the coalesced store.
+//                The polynomial added by the relin modes is prefetched into a second column with cp.async while the
+//                tile's MMAs run.
 // ------------------------------------------------------------------------------------------------------------------
-struct CrtArgs {
-  const uint32_t* res; size_t res_poly_stride;
-  uint32_t* out; size_t out_poly_stride;
-  const uint32_t* add; size_t add_poly_stride;
-  const uint8_t* B; const uint32_t* negM;
-  uint32_t N, K, KB, NC, nchunks, Lraw, Lx, region_bytes;
+struct CrtEpi {
+  struct Params {
+    uint32_t* out; size_t out_outer, out_inner;
+    const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
+    const uint32_t* negM;
+    uint32_t Lraw, Lx, adds_off, scratch_off;           // word offsets of the add column / BGV scratch column in the scratch
+    PostParams pp;
+  };
+  const Params& p;
+  const uint32_t N, etid;
+  uint32_t* xs;        // [Lx][TC]
+  uint32_t* adds;      // [L][TC]
+  uint32_t* scratch;   // [scratch_limbs][TC]
+  uint32_t* out = nullptr;
+  uint32_t alpha = 0, l = 0;
+  uint64_t carry = 0;
+
+  __device__ CrtEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_)
+      : p(p_), N(a.N), etid(etid_), xs(reinterpret_cast<uint32_t*>(sm)), adds(xs + p_.adds_off), scratch(xs + p_.scratch_off) {}
+
+  __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
+    out = p.out + (size_t)o * p.out_outer + (size_t)i * p.out_inner + n0 + etid;
+    l = 0; carry = 0;
+    if (p.add) {
+      const uint32_t* src = p.add + (size_t)o * p.add_outer + (size_t)i * p.add_inner + n0 + etid;
+      const uint32_t dst = umma::smem_u32(adds + etid);
+      for (uint32_t k = 0; k < p.pp.L; ++k)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + k * TC * 4), "l"(src + (size_t)k * N) : "memory");
+      asm volatile("cp.async.commit_group;" ::: "memory");
+    }
+  }
+  __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
+    int g0 = 0;
+    if (col0 == 0) {
+      uint64_t asum = 0;
+#pragma unroll
+      for (int e = 0; e < 6; ++e) asum += (uint64_t)t[e] << (8 * e);
+      alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
+      g0 = CRT_ALPHA_COLS / 4;
+    }
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      if (g < g0 || l >= p.Lraw) continue;
+      uint64_t v = carry + (uint64_t)alpha * __ldg(p.negM + l);
+      v += (uint64_t)t[4 * g] + ((uint64_t)t[4 * g + 1] << 8) + ((uint64_t)t[4 * g + 2] << 16) + ((uint64_t)t[4 * g + 3] << 24);
+      xs[l * TC + etid] = (uint32_t)v;
+      carry = v >> 32;
+      ++l;
+    }
+  }
+  __device__ void end_tile() {
+    for (; l < p.Lx; ++l) { xs[l * TC + etid] = (uint32_t)carry; carry = 0; }
+    if (p.add) asm volatile("cp.async.wait_group 0;" ::: "memory");
+    post();
+  }
+  __device__ void post();
 };
 
-__global__ void __launch_bounds__(TC)
-crt_kernel(CrtArgs a, PostParams pp) {
-  using namespace umma;
-  extern __shared__ __align__(1024) uint8_t smem[];
-  __shared__ MmaPipe pipe;
-  __shared__ uint32_t tmem_slot;
-  uint8_t* sA = smem;                                          // [KB/16][128][16]; later the limb columns xs[Lx][TC]
-  uint8_t* sB0 = smem + a.region_bytes;
-  uint8_t* sB1 = sB0 + (size_t)a.KB * a.NC;
-  uint32_t* xs = reinterpret_cast<uint32_t*>(smem);
-  uint32_t* scratch = reinterpret_cast<uint32_t*>(sB0);        // BGV divide-by-P scratch column (B buffers are dead then)
-  const uint32_t tid = threadIdx.x, warp = tid >> 5;
-  const uint32_t bpp = a.N / TC;
-  const uint32_t poly = blockIdx.x / bpp;
-  const uint32_t n = (blockIdx.x % bpp) * TC + tid;
-  const uint32_t ncols_alloc = pow2_cols(a.nchunks * a.NC);
-
-  // phase 1
-  stage_rows(sA, a.res + (size_t)poly * a.res_poly_stride + (n - tid), a.N, a.K, a.KB, 0);
-  if (tid == 0) mma_pipe_init(&pipe);
-  fence_proxy_async();
-  __syncthreads();
-  if (warp == 0) tmem_alloc(&tmem_slot, ncols_alloc);           // after staging: a co-resident CTA may still hold TMEM
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tbase = tmem_slot;
-  PipeState st = {{0, 0}, {0, 0}, 0};
-  if (warp == 0) {   // lane 0 issues; its warp mates park at the convergence barrier instead of polling beside it
-    if (tid == 0) mma_phase(&pipe, st, sA, sB0, sB1, a.KB, a.NC, a.B, (size_t)a.KB * a.NC, a.nchunks, tbase);
-    __syncwarp();
-  }
-  mbar_wait(&pipe.done, 0);
-  __syncthreads();                                              // nobody overwrites the A image before all MMAs are done
-  tc_fence_after();
-
-  // phase 2
-  {
-    const uint32_t lane_addr = tbase + ((warp * 32u) << 16);
-    uint32_t t[32];
-    tmem_ld32(lane_addr, t);
-    uint64_t asum = 0;
-#pragma unroll
-    for (int e = 0; e < 6; ++e) asum += (uint64_t)t[e] << (8 * e);
-    const uint32_t alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
-    uint64_t carry = 0;
-    uint32_t l = 0;
-    // first load: columns 8..31 = limbs 0..5; later loads: eight limbs each
-    for (uint32_t col = 0; l < a.Lraw; col += 32) {
-      if (col) tmem_ld32(lane_addr + col, t);
-#pragma unroll
-      for (int g = 0; g < 8; ++g) {
-        if ((col == 0 && g < CRT_ALPHA_COLS / 4) || l >= a.Lraw) continue;
-        uint64_t v = carry + (uint64_t)alpha * __ldg(a.negM + l);
-        v += (uint64_t)t[4 * g] + ((uint64_t)t[4 * g + 1] << 8) + ((uint64_t)t[4 * g + 2] << 16) + ((uint64_t)t[4 * g + 3] << 24);
-        xs[l * TC + tid] = (uint32_t)v;
-        carry = v >> 32;
-        ++l;
-      }
-    }
-    for (; l < a.Lx; ++l) { xs[l * TC + tid] = (uint32_t)carry; carry = 0; }
-    tc_fence_before();
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tbase, ncols_alloc);            // release TMEM before the (long) post-processing
-  }
-
-  // phase 3
-  Col x{xs + tid};
-  uint32_t* out = a.out + (size_t)poly * a.out_poly_stride + n;
+__device__ void CrtEpi::post() {
+  const PostParams& pp = p.pp;
+  const uint32_t Lx = p.Lx;
+  Col x{xs + etid};
+  Col ad{adds + etid};
   const uint32_t L = pp.L;
   if (pp.mode == POST_CKKS_MASK) {
     const uint32_t tm = top_mask(pp.logQ);
-    for (uint32_t l = 0; l < L; ++l) {
-      uint32_t v = x.get(l);
-      if (l == L - 1) v &= tm;
-      out[(size_t)l * a.N] = v;
+    for (uint32_t k = 0; k < L; ++k) {
+      uint32_t v = x.get(k);
+      if (k == L - 1) v &= tm;
+      out[(size_t)k * N] = v;
     }
     return;
   }
-  const uint32_t* addp = a.add + (size_t)poly * a.add_poly_stride + n;
   if (pp.mode == POST_CKKS_RELIN) {
     // k = ((X mod 2^logPQ + 2^(logP-1)) >> logP) mod 2^logQ ; bits above logP+logQ never reach k
-    col_add_pow2(x, pp.logP - 1, a.Lx);
-    uint32_t carry = 0;
+    col_add_pow2(x, pp.logP - 1, Lx);
+    uint32_t cy = 0;
     const uint32_t tm = top_mask(pp.logQ);
-    for (uint32_t l = 0; l < L; ++l) {               // in place: reads limbs >= l, writes limb l
-      uint32_t k = col_bits(x, pp.logP, l, a.Lx);
-      uint64_t s = (uint64_t)k + __ldg(addp + (size_t)l * a.N) + carry;
-      carry = (uint32_t)(s >> 32);
+    for (uint32_t k = 0; k < L; ++k) {               // in place: reads limbs >= k, writes limb k
+      uint32_t kk = col_bits(x, pp.logP, k, Lx);
+      uint64_t s = (uint64_t)kk + ad.get(k) + cy;
+      cy = (uint32_t)(s >> 32);
       uint32_t v = (uint32_t)s;
-      if (l == L - 1) v &= tm;
-      x.set(l, v);
+      if (k == L - 1) v &= tm;
+      x.set(k, v);
     }
     if (pp.rescale_bits == 0) {
-      for (uint32_t l = 0; l < L; ++l) out[(size_t)l * a.N] = x.get(l);
+      for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     } else {
-      const uint32_t p = pp.rescale_bits;
+      const uint32_t pb = pp.rescale_bits;
       x.set(L, 0);                                   // room for the rounding carry (Lx >= L + 1)
-      col_add_pow2(x, p - 1, L + 1);
-      const uint32_t nb = pp.logQ - p;               // result bits
+      col_add_pow2(x, pb - 1, L + 1);
+      const uint32_t nb = pp.logQ - pb;              // result bits
       const uint32_t Lr = (nb + 31) / 32;
       const uint32_t tm2 = top_mask(nb);
-      for (uint32_t l = 0; l < L; ++l) {
+      for (uint32_t k = 0; k < L; ++k) {
         uint32_t v = 0;
-        if (l < Lr) { v = col_bits(x, p, l, L + 1); if (l == Lr - 1) v &= tm2; }
-        out[(size_t)l * a.N] = v;
+        if (k < Lr) { v = col_bits(x, pb, k, L + 1); if (k == Lr - 1) v &= tm2; }
+        out[(size_t)k * N] = v;
       }
     }
     return;
   }
   if (pp.mode == POST_BGV_MODQ) {
-    col_barrett1(x, a.Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
-    for (uint32_t l = 0; l < L; ++l) out[(size_t)l * a.N] = x.get(l);
+    col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
+    for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     return;
   }
   // POST_BGV_RELIN: V -> xc = V mod PQ -> (q3, rem) = divmod(xc, P) -> centred r, kk -> (hi - kk + d) mod Q
   {
     const uint32_t LP = pp.L_P, LPQ = pp.L_PQ, g = pp.g_limbs;   // g = LPQ - LP
-    col_barrett1(x, a.Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);   // x[0..LPQ) = xc
+    col_barrett1(x, Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);     // x[0..LPQ) = xc
     // Barrett quotient estimate (HAC 14.42 generalised): q1 = xc >> 32(LP-1)  (g+1 limbs),
     // q3 = (q1 * mu) >> 32(g+1), mu = floor(2^(32 LPQ) / P)  (muP_limbs limbs); true quotient - q3 in {0,1,2}.
-    Col sc{scratch + tid};                           // scratch column: pp.scratch_limbs limbs (B buffers are dead by now)
+    Col sc{scratch + etid};
     const uint32_t n1 = g + 1, nmu = pp.muP_limbs;
     {
       uint64_t acc_lo = 0; uint32_t acc_hi = 0;
@@ -289,10 +275,10 @@ crt_kernel(CrtArgs a, PostParams pp) {
     {
       // compare 2*rem with P from the top limb down (2*rem has LP+1 limbs)
       int cmp = 0;
-      for (uint32_t l = LP + 1; l-- > 0 && cmp == 0;) {
-        uint32_t hi = l < LP ? x.get(l) : 0u, lo = l >= 1 ? x.get(l - 1) : 0u;
+      for (uint32_t k = LP + 1; k-- > 0 && cmp == 0;) {
+        uint32_t hi = k < LP ? x.get(k) : 0u, lo = k >= 1 ? x.get(k - 1) : 0u;
         uint32_t two = (hi << 1) | (lo >> 31);
-        uint32_t pv = l < LP ? __ldg(pp.d_P + l) : 0u;
+        uint32_t pv = k < LP ? __ldg(pp.d_P + k) : 0u;
         if (two != pv) cmp = two > pv ? 1 : -1;
       }
       neg = cmp > 0;
@@ -300,64 +286,72 @@ crt_kernel(CrtArgs a, PostParams pp) {
     if (neg) ++qinc;                                 // hi = q + 1, r = rem - P
     // r mod t
     uint64_t rt = 0;
-    for (uint32_t l = 0; l < LP; ++l) rt = (rt + (uint64_t)x.get(l) * __ldg(pp.d_pow32_t + l)) % pp.t;
+    for (uint32_t k = 0; k < LP; ++k) rt = (rt + (uint64_t)x.get(k) * __ldg(pp.d_pow32_t + k)) % pp.t;
     if (neg) { uint64_t Pt = __ldg(pp.d_pow32_t + LP); rt = (rt + pp.t - Pt) % pp.t; }   // d_pow32_t[LP] holds P mod t
     uint64_t kk = ((pp.t - rt) % pp.t) * pp.Pinv_t % pp.t;     // (-r P^-1) mod t in [0, t)
     const bool kneg = kk > pp.t / 2;                            // centred: kk - t
     const uint32_t kmag = kneg ? (uint32_t)(pp.t - kk) : (uint32_t)kk;
     // res = q3 + qinc - kk_centred, as an (L+1)-limb value in x[0..L], then mod Q, then + d mod Q
     {
-      // x[l] <- q3[l] for l <= L (q3 has nq = g+1 limbs; zero beyond)
       int64_t adj = (int64_t)qinc + (kneg ? (int64_t)kmag : -(int64_t)kmag);
-      // add signed small adj with carry/borrow propagation
-      int64_t c = adj;
-      for (uint32_t l = 0; l <= L; ++l) {
-        int64_t v = (int64_t)(l < nq ? q3.get(l) : 0u) + c;
-        x.set(l, (uint32_t)v);
-        c = v >> 32;
+      int64_t cc = adj;
+      for (uint32_t k = 0; k <= L; ++k) {
+        int64_t v = (int64_t)(k < nq ? q3.get(k) : 0u) + cc;
+        x.set(k, (uint32_t)v);
+        cc = v >> 32;
       }
-      // c == -1 here means the value is negative (only possible when q3 + qinc < kk): add Q
-      if (c < 0) { col_add(x, pp.d_Q, L + 1); }
+      // cc == -1 here means the value is negative (only possible when q3 + qinc < kk): add Q
+      if (cc < 0) { col_add(x, pp.d_Q, L + 1); }
       else if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
       // + d
-      uint32_t carry = 0;
-      for (uint32_t l = 0; l < L; ++l) {
-        uint64_t s = (uint64_t)x.get(l) + __ldg(addp + (size_t)l * a.N) + carry;
-        x.set(l, (uint32_t)s);
-        carry = (uint32_t)(s >> 32);
+      uint32_t cy = 0;
+      for (uint32_t k = 0; k < L; ++k) {
+        uint64_t s = (uint64_t)x.get(k) + ad.get(k) + cy;
+        x.set(k, (uint32_t)s);
+        cy = (uint32_t)(s >> 32);
       }
-      x.set(L, carry);
+      x.set(L, cy);
       if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
-      for (uint32_t l = 0; l < L; ++l) out[(size_t)l * a.N] = x.get(l);
+      for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     }
   }
 }
 
-cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_poly_stride,
-                       const uint32_t* d_res, size_t res_poly_stride, const uint32_t* d_add, size_t add_poly_stride,
-                       uint32_t npoly, cudaStream_t s) {
-  if (!npoly) return cudaSuccess;
-  CrtArgs a;
-  a.res = d_res; a.res_poly_stride = res_poly_stride;
-  a.out = d_out; a.out_poly_stride = out_poly_stride;
-  a.add = d_add; a.add_poly_stride = add_poly_stride;
-  a.B = tg.d_B; a.negM = tg.d_negM;
-  a.N = c->N; a.K = tg.K; a.KB = tg.KB; a.NC = tg.NC; a.nchunks = tg.nchunks; a.Lraw = tg.Lraw; a.Lx = tg.Lx;
-  a.region_bytes = std::max(tg.KB * 128u, tg.Lx * 512u);
-  size_t tail = 2 * (size_t)tg.KB * tg.NC;
-  if (pp.mode == POST_BGV_RELIN && (size_t)pp.scratch_limbs * TC * 4 > tail) tail = (size_t)pp.scratch_limbs * TC * 4;
-  const size_t smem = a.region_bytes + tail;
-  static size_t configured = 0;
-  if (smem > configured) {
-    cudaError_t e = cudaFuncSetAttribute(crt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(crt_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    if (e != cudaSuccess) return e;
-    configured = smem;
-  }
+// scratch layout of CrtEpi (words): xs [Lx][TC] | adds [L][TC] (relin modes) | BGV divide-by-P scratch [scratch_limbs][TC]
+static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, uint32_t& adds_off, uint32_t& scratch_off, size_t& bytes) {
+  const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
+  adds_off = tg.Lx * TC;
+  scratch_off = adds_off + (relin ? pp.L * TC : 0);
+  bytes = ((size_t)scratch_off + (pp.mode == POST_BGV_RELIN ? pp.scratch_limbs * TC : 0)) * 4;
+}
+
+bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
+  uint32_t ao, so; size_t bytes;
+  crt_scratch_layout(tg, pp, ao, so, bytes);
+  return pipe::make_plan(tg.KB, tg.nchunks, bytes).ok;
+}
+
+cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
+                       const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
+                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s) {
+  if (nouter * ninner == 0) return cudaSuccess;
+  CrtEpi::Params ep;
+  size_t epi_bytes;
+  crt_scratch_layout(tg, pp, ep.adds_off, ep.scratch_off, epi_bytes);
+  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes);
+  if (!plan.ok) return cudaErrorInvalidConfiguration;
+  const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
+  if (relin && !d_add) return cudaErrorInvalidValue;
+  pipe::PipeArgs a;
+  a.src = d_res; a.src_outer = res_outer; a.src_inner = res_inner;
+  a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = tg.K; a.mask_bits = 0;
+  a.B = tg.d_B; a.chunk_stride = (size_t)tg.KB * pipe::NC;
+  pipe::fill_args(a, plan);
+  ep.out = d_out; ep.out_outer = out_outer; ep.out_inner = out_inner;
+  ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;
+  ep.negM = tg.d_negM; ep.Lraw = tg.Lraw; ep.Lx = tg.Lx; ep.pp = pp;
   LaunchTimer lt(c, KC_CRT, s);
-  crt_kernel<<<(c->N / TC) * npoly, TC, smem, s>>>(a, pp);
-  return cudaGetLastError();
+  return pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
 }
 
 // ------------------------------------------------------------------------------------------------------------------
