@@ -42,7 +42,7 @@ __device__ __forceinline__ uint32_t col_bits(Col x, uint32_t sh, uint32_t l, uin
   uint32_t hi = (w + 1) < nl ? x.get(w + 1) : 0u;
   return (lo >> b) | (hi << (32 - b));
 }
-__device__ __forceinline__ uint32_t top_mask(uint32_t bits) { return (bits & 31) ? ((1u << (bits & 31)) - 1u) : 0xFFFFFFFFu; }
+__host__ __device__ __forceinline__ uint32_t top_mask(uint32_t bits) { return (bits & 31) ? ((1u << (bits & 31)) - 1u) : 0xFFFFFFFFu; }
 
 // x >= m ?  (x: nl limbs in the column, m: nl limbs in global memory)
 __device__ __forceinline__ bool col_ge(Col x, const uint32_t* __restrict__ m, uint32_t nl) {
@@ -110,34 +110,51 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 // column i), the tensor cores contract them with the constant image B: column 8 + e receives
 // S_e = sum_{i,b} y_ib * byte_{e-b}(W_i), columns 0..5 the byte sums of sum_i y_i floor(2^48 / q_i) (-> alpha).  Here:
 //   carry pass   V = sum_e S_e 2^(8 e) + alpha * negM, four columns (one limb) at a time as the accumulator chunks
-//                arrive, limbs written to this thread's column xs[.][etid] in shared memory
-//   post         on the limb column: mask / divide-by-P + add [+ rescale] / BGV reductions, then the coalesced store.
+//                arrive; everything but the two-instruction carry chain is independent across the limbs of a group
+//   post         CKKS: streamed, in registers -- mask (tensor / polymul), or shift by logP with rounding + add (d0, d1)
+//                [+ shift by the rescale bits with rounding] through one-limb delay lines, coalesced stores as the limbs
+//                come out.  BGV: the limbs go to this thread's column xs[.][etid] in shared memory and the multi-limb
+//                Barrett reductions run on the column (post()).
 //                The polynomial added by the relin modes is prefetched into a second column with cp.async while the
 //                tile's MMAs run.
 // ------------------------------------------------------------------------------------------------------------------
 struct CrtEpi {
+  static constexpr uint32_t GROUPS = 1, LOAD_WARPS = 8;
   struct Params {
     uint32_t* out; size_t out_outer, out_inner;
     const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
-    const uint32_t* negM;
-    uint32_t Lraw, Lx, adds_off, scratch_off;           // word offsets of the add column / BGV scratch column in the scratch
+    const uint32_t* negM;                               // [Lraw]
+    uint32_t Lraw, Lx, nl;                              // nl = limbs the chunks cover (16 per chunk minus the alpha columns)
+    uint32_t xs_off, adds_off, scratch_off;             // word offsets inside the scratch: negM table at 0, then the columns
+    // CKKS relin streaming constants: shift by logP = 32 ws + bs, rounding bit rbit in limb rb; rescale likewise (.2)
+    uint32_t ws, bs, rb, rbit, ws2, bs2, rb2, rbit2, Lr, tm2, tmq, lend;
     PostParams pp;
   };
   const Params& p;
   const uint32_t N, etid;
-  uint32_t* xs;        // [Lx][TC]
-  uint32_t* adds;      // [L][TC]
-  uint32_t* scratch;   // [scratch_limbs][TC]
+  const uint32_t* negm;  // [nl + 2] in shared memory, zero beyond Lraw
+  uint32_t* xs;          // [Lx][TC]   (BGV)
+  uint32_t* adds;        // [L][TC]    (relin modes)
+  uint32_t* scratch;     // [scratch_limbs][TC]  (BGV relin)
   uint32_t* out = nullptr;
-  uint32_t alpha = 0, l = 0;
+  uint32_t* optr = nullptr;
+  const uint32_t* aptr = nullptr;
+  uint32_t alpha = 0, yprev = 0, cy = 0, zprev = 0, cz = 0;
   uint64_t carry = 0;
 
-  __device__ CrtEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_)
-      : p(p_), N(a.N), etid(etid_), xs(reinterpret_cast<uint32_t*>(sm)), adds(xs + p_.adds_off), scratch(xs + p_.scratch_off) {}
+  __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t)
+      : p(p_), N(a.N), etid(etid_), negm(reinterpret_cast<const uint32_t*>(sm)),
+        xs(reinterpret_cast<uint32_t*>(sm) + p_.xs_off), adds(reinterpret_cast<uint32_t*>(sm) + p_.adds_off),
+        scratch(reinterpret_cast<uint32_t*>(sm) + p_.scratch_off) {
+    uint32_t* w = reinterpret_cast<uint32_t*>(sm);
+    for (uint32_t k = etid; k < p.nl + 2; k += TC) w[k] = k < p.Lraw ? __ldg(p.negM + k) : 0u;
+    pipe::epi_sync(TC);
+  }
 
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.out + (size_t)o * p.out_outer + (size_t)i * p.out_inner + n0 + etid;
-    l = 0; carry = 0;
+    optr = out; aptr = adds + etid;
+    carry = 0; yprev = 0; cy = 0; zprev = 0; cz = 0;
     if (p.add) {
       const uint32_t* src = p.add + (size_t)o * p.add_outer + (size_t)i * p.add_inner + n0 + etid;
       const uint32_t dst = umma::smem_u32(adds + etid);
@@ -146,6 +163,41 @@ struct CrtEpi {
       asm volatile("cp.async.commit_group;" ::: "memory");
     }
   }
+
+  // One limb of the CKKS relin stream: y = limb lg of V + 2^(logP-1).  Emits limb lg - 1 - ws of
+  // z = (d + (V + 2^(logP-1)) >> logP) mod 2^logQ, and from that, with rescaling, limb lg - 2 - ws - ws2 of the result.
+  // IN: the caller guarantees that no boundary (first / top limb, rounding limb, mask) falls on this limb.
+  template <bool IN>
+  __device__ __forceinline__ void relin_step(uint32_t lg, uint32_t y) {
+    if (IN || lg > p.ws) {
+      const uint32_t kidx = lg - 1 - p.ws;
+      const bool rescale = p.pp.rescale_bits != 0;
+      uint32_t z = 0;
+      if (IN || kidx < p.pp.L) {
+        const uint32_t kk = __funnelshift_r(yprev, y, p.bs);
+        const uint64_t s = (uint64_t)kk + *aptr + cy;
+        aptr += TC;
+        cy = (uint32_t)(s >> 32);
+        z = (uint32_t)s;
+        if (!IN && kidx == p.pp.L - 1) z &= p.tmq;
+        if (!rescale) { *optr = z; optr += N; }
+      }
+      if (rescale && (IN || kidx <= p.pp.L + p.ws2)) {            // limbs >= L of z are virtual: the rounding carry, then zero
+        const uint64_t s2 = (uint64_t)z + cz + ((!IN && kidx == p.rb2) ? p.rbit2 : 0u);
+        const uint32_t zz = (uint32_t)s2;
+        cz = (uint32_t)(s2 >> 32);
+        if (IN || kidx > p.ws2) {
+          const uint32_t m = kidx - 1 - p.ws2;
+          uint32_t v = __funnelshift_r(zprev, zz, p.bs2);
+          if (!IN) { if (m == p.Lr - 1) v &= p.tm2; if (m >= p.Lr) v = 0; }
+          if (IN || m < p.pp.L) { *optr = v; optr += N; }
+        }
+        zprev = zz;
+      }
+    }
+    yprev = y;
+  }
+
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     int g0 = 0;
     if (col0 == 0) {
@@ -155,19 +207,90 @@ struct CrtEpi {
       alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
       g0 = CRT_ALPHA_COLS / 4;
     }
+    const uint32_t l0 = col0 / 4 - CRT_ALPHA_COLS / 4;             // limb of group element 0 (wraps for col0 = 0; elements 0, 1 unused)
+    uint64_t P[8];                                                 // the limb's column sum + alpha * negM: independent of the carry
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
-      if (g < g0 || l >= p.Lraw) continue;
-      uint64_t v = carry + (uint64_t)alpha * __ldg(p.negM + l);
-      v += (uint64_t)t[4 * g] + ((uint64_t)t[4 * g + 1] << 8) + ((uint64_t)t[4 * g + 2] << 16) + ((uint64_t)t[4 * g + 3] << 24);
-      xs[l * TC + etid] = (uint32_t)v;
-      carry = v >> 32;
-      ++l;
+      if (g < g0) { P[g] = 0; continue; }
+      const uint64_t s01 = (uint64_t)t[4 * g + 1] * 256u + t[4 * g];
+      const uint64_t s23 = (uint64_t)t[4 * g + 3] * 256u + t[4 * g + 2];
+      P[g] = (uint64_t)alpha * negm[l0 + g] + s01 + (s23 << 16);
+    }
+    const int mode = p.pp.mode;
+    const uint32_t L = p.pp.L;
+    if (mode == POST_CKKS_MASK) {
+      if (g0 == 0 && l0 + 8 < L) {
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const uint64_t v = carry + P[g];
+          carry = v >> 32;
+          *optr = (uint32_t)v; optr += N;
+        }
+      } else {
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          if (g < g0) continue;
+          const uint64_t v = carry + P[g];
+          carry = v >> 32;
+          const uint32_t lg = l0 + g;
+          if (lg < L) { *optr = lg == L - 1 ? ((uint32_t)v & p.tmq) : (uint32_t)v; optr += N; }
+        }
+      }
+    } else if (mode == POST_CKKS_RELIN) {
+      const uint32_t k0 = l0 - 1 - p.ws;                           // first z limb this group emits (when l0 > ws)
+      const bool rescale = p.pp.rescale_bits != 0;
+      if (l0 + 8 > p.rb) asm volatile("cp.async.wait_group 0;" ::: "memory");   // the add column is read from here on
+      if (l0 + 8 <= p.rb) {                                        // far below the shift: only the carry matters
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          if (g < g0) continue;
+          const uint64_t v = carry + P[g];
+          carry = v >> 32;
+          yprev = (uint32_t)v;
+        }
+      } else if (g0 == 0 && l0 > p.ws && k0 + 8 < L &&
+                 (!rescale || (k0 > p.rb2 && k0 > p.ws2 && k0 + 8 - 1 - p.ws2 < p.Lr - 1))) {
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const uint64_t v = carry + P[g];
+          carry = v >> 32;
+          relin_step<true>(l0 + g, (uint32_t)v);
+        }
+      } else {
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          if (g < g0) continue;
+          const uint32_t lg = l0 + g;
+          const uint64_t v = carry + P[g] + (lg == p.rb ? p.rbit : 0u);
+          carry = v >> 32;
+          relin_step<false>(lg, (uint32_t)v);
+        }
+      }
+    } else {                                                       // BGV: the column in shared memory
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        if (g < g0) continue;
+        const uint64_t v = carry + P[g];
+        carry = v >> 32;
+        const uint32_t lg = l0 + g;
+        if (lg < p.Lx) xs[lg * TC + etid] = (uint32_t)v;
+      }
     }
   }
+
   __device__ void end_tile() {
-    for (; l < p.Lx; ++l) { xs[l * TC + etid] = (uint32_t)carry; carry = 0; }
+    const int mode = p.pp.mode;
+    if (mode == POST_CKKS_MASK) return;                            // the chunks cover all L limbs
     if (p.add) asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (mode == POST_CKKS_RELIN) {
+      for (uint32_t lg = p.nl; lg <= p.lend; ++lg) {               // limbs past the last chunk: the carry, then zeros
+        const uint64_t v = carry + (lg == p.rb ? p.rbit : 0u);
+        carry = v >> 32;
+        relin_step<false>(lg, (uint32_t)v);
+      }
+      return;
+    }
+    for (uint32_t lg = p.nl; lg < p.Lx; ++lg) { xs[lg * TC + etid] = (uint32_t)carry; carry = 0; }
     post();
   }
   __device__ void post();
@@ -179,45 +302,6 @@ __device__ void CrtEpi::post() {
   Col x{xs + etid};
   Col ad{adds + etid};
   const uint32_t L = pp.L;
-  if (pp.mode == POST_CKKS_MASK) {
-    const uint32_t tm = top_mask(pp.logQ);
-    for (uint32_t k = 0; k < L; ++k) {
-      uint32_t v = x.get(k);
-      if (k == L - 1) v &= tm;
-      out[(size_t)k * N] = v;
-    }
-    return;
-  }
-  if (pp.mode == POST_CKKS_RELIN) {
-    // k = ((X mod 2^logPQ + 2^(logP-1)) >> logP) mod 2^logQ ; bits above logP+logQ never reach k
-    col_add_pow2(x, pp.logP - 1, Lx);
-    uint32_t cy = 0;
-    const uint32_t tm = top_mask(pp.logQ);
-    for (uint32_t k = 0; k < L; ++k) {               // in place: reads limbs >= k, writes limb k
-      uint32_t kk = col_bits(x, pp.logP, k, Lx);
-      uint64_t s = (uint64_t)kk + ad.get(k) + cy;
-      cy = (uint32_t)(s >> 32);
-      uint32_t v = (uint32_t)s;
-      if (k == L - 1) v &= tm;
-      x.set(k, v);
-    }
-    if (pp.rescale_bits == 0) {
-      for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
-    } else {
-      const uint32_t pb = pp.rescale_bits;
-      x.set(L, 0);                                   // room for the rounding carry (Lx >= L + 1)
-      col_add_pow2(x, pb - 1, L + 1);
-      const uint32_t nb = pp.logQ - pb;              // result bits
-      const uint32_t Lr = (nb + 31) / 32;
-      const uint32_t tm2 = top_mask(nb);
-      for (uint32_t k = 0; k < L; ++k) {
-        uint32_t v = 0;
-        if (k < Lr) { v = col_bits(x, pb, k, L + 1); if (k == Lr - 1) v &= tm2; }
-        out[(size_t)k * N] = v;
-      }
-    }
-    return;
-  }
   if (pp.mode == POST_BGV_MODQ) {
     col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
     for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
@@ -317,17 +401,21 @@ __device__ void CrtEpi::post() {
   }
 }
 
-// scratch layout of CrtEpi (words): xs [Lx][TC] | adds [L][TC] (relin modes) | BGV divide-by-P scratch [scratch_limbs][TC]
-static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, uint32_t& adds_off, uint32_t& scratch_off, size_t& bytes) {
+// scratch layout of CrtEpi (words): negM table [nl + 2] | xs [Lx][TC] (BGV) | adds [L][TC] (relin modes) |
+// BGV divide-by-P scratch [scratch_limbs][TC]
+static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi::Params& ep, size_t& bytes) {
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
-  adds_off = tg.Lx * TC;
-  scratch_off = adds_off + (relin ? pp.L * TC : 0);
-  bytes = ((size_t)scratch_off + (pp.mode == POST_BGV_RELIN ? pp.scratch_limbs * TC : 0)) * 4;
+  const bool bgv = pp.mode == POST_BGV_MODQ || pp.mode == POST_BGV_RELIN;
+  ep.nl = tg.nchunks * (pipe::NC / 4) - CRT_ALPHA_COLS / 4;
+  ep.xs_off = (ep.nl + 2 + 31) / 32 * 32;
+  ep.adds_off = ep.xs_off + (bgv ? tg.Lx * TC : 0);
+  ep.scratch_off = ep.adds_off + (relin ? pp.L * TC : 0);
+  bytes = ((size_t)ep.scratch_off + (pp.mode == POST_BGV_RELIN ? pp.scratch_limbs * TC : 0)) * 4;
 }
 
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
-  uint32_t ao, so; size_t bytes;
-  crt_scratch_layout(tg, pp, ao, so, bytes);
+  CrtEpi::Params ep; size_t bytes;
+  crt_scratch_layout(tg, pp, ep, bytes);
   return pipe::make_plan(tg.KB, tg.nchunks, bytes).ok;
 }
 
@@ -337,7 +425,7 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   if (nouter * ninner == 0) return cudaSuccess;
   CrtEpi::Params ep;
   size_t epi_bytes;
-  crt_scratch_layout(tg, pp, ep.adds_off, ep.scratch_off, epi_bytes);
+  crt_scratch_layout(tg, pp, ep, epi_bytes);
   const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
@@ -350,6 +438,15 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   ep.out = d_out; ep.out_outer = out_outer; ep.out_inner = out_inner;
   ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;
   ep.negM = tg.d_negM; ep.Lraw = tg.Lraw; ep.Lx = tg.Lx; ep.pp = pp;
+  ep.tmq = top_mask(pp.logQ);
+  ep.ws = pp.logP >> 5; ep.bs = pp.logP & 31;
+  ep.rb = pp.logP ? (pp.logP - 1) >> 5 : 0; ep.rbit = pp.logP ? 1u << ((pp.logP - 1) & 31) : 0;
+  const uint32_t pb = pp.rescale_bits;
+  ep.ws2 = pb >> 5; ep.bs2 = pb & 31;
+  ep.rb2 = pb ? (pb - 1) >> 5 : 0; ep.rbit2 = pb ? 1u << ((pb - 1) & 31) : 0;
+  const uint32_t nb = pp.logQ - pb;
+  ep.Lr = (nb + 31) / 32; ep.tm2 = top_mask(nb);
+  ep.lend = ep.ws + pp.L + (pb ? ep.ws2 + 1 : 0);                 // last limb index the relin stream must see
   LaunchTimer lt(c, KC_CRT, s);
   return pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
 }

@@ -11,8 +11,10 @@
 
 namespace fhe {
 
-// Epilogue of the pipeline: a 64-column accumulator chunk holds the byte sums of 16 primes.
+// Epilogue of the pipeline: a 64-column accumulator chunk holds the byte sums of 16 primes; each of the two epilogue
+// warp groups takes 8 of them.  (q_j, floor(2^53 / q_j)) sit in shared memory, padded to whole chunks.
 struct DecEpi {
+  static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 4;   // 13 warps: at most 4 on an SM sub-partition, 128 registers each
   struct Params {
     uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
     const uint2* qmu;                             // (q_j, floor(2^53 / q_j))
@@ -20,22 +22,29 @@ struct DecEpi {
   };
   const Params& p;
   const uint32_t N, etid;
+  const uint2* tab;
   uint32_t* out = nullptr;
-  __device__ DecEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t*, uint32_t etid_) : p(p_), N(a.N), etid(etid_) {}
+  __device__ DecEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_, uint32_t grp)
+      : p(p_), N(a.N), etid(etid_), tab(reinterpret_cast<const uint2*>(sm)) {
+    uint2* w = reinterpret_cast<uint2*>(sm);
+    for (uint32_t j = grp * 128 + etid; j < a.nchunks * 16; j += 128 * GROUPS) w[j] = j < p.K ? __ldg(p.qmu + j) : make_uint2(1u, 0u);
+    pipe::epi_sync(128 * GROUPS);
+  }
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.res + (size_t)o * p.res_outer + (size_t)i * p.res_inner + n0 + etid;
   }
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     const uint32_t j0 = col0 / 4;
+    uint32_t* o = out + (size_t)j0 * N;
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
-      const uint32_t j = j0 + e;
-      if (j < p.K) {
-        const uint2 qm = __ldg(p.qmu + j);
-        const uint64_t lo = (uint64_t)t[4 * e + 1] * 256u + t[4 * e];
-        const uint64_t hi = (uint64_t)t[4 * e + 3] * 256u + t[4 * e + 2];
-        out[(size_t)j * N] = barrett49(lo + (hi << 16), qm.x, qm.y);
-      }
+      const uint2 qm = tab[j0 + e];
+      uint64_t v = (uint64_t)t[4 * e + 1] * 256u + t[4 * e];             // three wide multiply-adds: v < 2^49
+      v = (uint64_t)t[4 * e + 2] * 65536u + v;
+      v = (uint64_t)t[4 * e + 3] * 16777216u + v;
+      const uint32_t r = barrett49(v, qm.x, qm.y);
+      if (j0 + e < p.K) *o = r;
+      o += N;
     }
   }
   __device__ __forceinline__ void end_tile() {}
@@ -49,7 +58,7 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
   if (mask_bits && (mask_bits + 31) / 32 < eff) eff = (mask_bits + 31) / 32;
   const uint32_t KB = (4 * eff + 31) / 32 * 32;
   if (KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
-  const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, 0);
+  const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2));
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   pipe::PipeArgs a;
   a.src = d_limbs; a.src_outer = limb_outer; a.src_inner = limb_inner;

@@ -5,7 +5,7 @@
 // word-major array src[w][n] (umma.cuh).  One CTA per SM walks the 128-coefficient tiles of every polynomial of the
 // launch; inside it three roles run concurrently, tied together by mbarriers only:
 //
-//   loader warps (8)   global -> registers -> TMEM: thread (quarter, lane) owns tile row 32 quarter + lane, which is
+//   loader warps       global -> registers -> TMEM: thread (quarter, lane) owns tile row 32 quarter + lane, which is
 //                      TMEM lane 32 quarter + lane.  Word w of its coefficient is column w of the A operand: the i8
 //                      MMA reads an A operand held in TMEM as four K-bytes per 32-bit cell, little-endian -- exactly
 //                      the word-major data, so no transposition through shared memory exists.  Up to 64 coalesced
@@ -13,7 +13,7 @@
 //   MMA thread (1)     per tile and per 64-column chunk of the constant matrix (resident in shared memory, loaded once
 //                      per CTA with cp.async.bulk; streamed through a ring when it does not fit): KB/32
 //                      tcgen05.mma kind::i8 into one buffer of a ring of accumulator chunks in TMEM.
-//   epilogue warps (4) tcgen05.ld of a finished accumulator chunk, then the conversion's own arithmetic (an Epi
+//   epilogue warps     (4 or 8) tcgen05.ld of a finished accumulator chunk, then the conversion's own arithmetic (an Epi
 //                      functor: Barrett reduction and store for S1; carry pass, mod-Q / divide-by-P post-processing and
 //                      store for S5).
 //
@@ -27,10 +27,6 @@ namespace pipe {
 using namespace umma;
 
 constexpr uint32_t NC = 64;                                   // accumulator columns per chunk
-constexpr uint32_t EPI_WARPS = 4, LOAD_WARPS = 8;
-constexpr uint32_t MMA_WARP = EPI_WARPS + LOAD_WARPS;         // warp index of the MMA-issuing warp
-constexpr uint32_t NTHREADS = (MMA_WARP + 1) * 32;            // 416
-constexpr uint32_t EPI_THREADS = EPI_WARPS * 32;              // 128 = tile rows
 constexpr uint32_t MAX_SLOTS = 16, MAX_D = 4, MAX_A = 2;
 constexpr uint32_t CTRL_BYTES = 1024;
 constexpr size_t SMEM_LIMIT = 227 * 1024;
@@ -143,13 +139,24 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[32], uint32_t taddr_a,
 
 // ---- the kernel -------------------------------------------------------------------------------------------------------------
 // Epi: struct with
+//   static constexpr uint32_t LOAD_WARPS;                             4 or 8 loader warps (one or two per TMEM lane quarter)
+//   static constexpr uint32_t GROUPS;                                 1: every epilogue warp takes the 64 columns of a chunk
+//                                                                     2: warp group g takes columns [32 g, 32 g + 32) of it
 //   struct Params;                                                    by-value kernel argument
-//   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid);
+//   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid, uint32_t grp);
 //   __device__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0);  polynomial (o, i), first coefficient of the tile
 //   __device__ void consume(uint32_t col0, const uint32_t* t);        32 accumulator columns [col0, col0 + 32) of row etid
 //   __device__ void end_tile();
+// Warp roles: [0, 4 GROUPS) epilogue, then LOAD_WARPS loaders, then the MMA issuer.
+constexpr uint32_t nthreads(uint32_t groups, uint32_t load_warps) { return (4 * groups + load_warps + 1) * 32; }
+
+// barrier among the epilogue threads only (id 1; id 0 is __syncthreads)
+__device__ __forceinline__ void epi_sync(uint32_t nthr) { asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory"); }
+
 template <class Epi>
-__global__ void __launch_bounds__(NTHREADS, 1) pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename Epi::Params ep) {
+__global__ void __launch_bounds__(nthreads(Epi::GROUPS, Epi::LOAD_WARPS), 1)
+pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename Epi::Params ep) {
+  constexpr uint32_t EPIW = 4 * Epi::GROUPS, LOAD_WARPS = Epi::LOAD_WARPS, HALVES = LOAD_WARPS / 4, MMAW = EPIW + LOAD_WARPS;
   extern __shared__ __align__(1024) uint8_t smem[];
   Ctrl* ctl = reinterpret_cast<Ctrl*>(smem);
   uint8_t* sB = smem + a.b_off;
@@ -160,43 +167,48 @@ __global__ void __launch_bounds__(NTHREADS, 1) pipe_kernel(const __grid_constant
   const uint32_t a_cols = a.KB / 4;
   const uint32_t chunk_bytes = a.KB * NC;
   const bool resident = a.nslots >= a.nchunks;
+  const uint32_t dmask = a.nD - 1, dshift = a.nD == 4 ? 2 : 1;     // nD in {2, 4}
+  const uint32_t amask = a.nA - 1, ashift = a.nA - 1;              // nA in {1, 2}
 
   if (tid == 0) {
     for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], LOAD_WARPS * 32); mbar_init(&ctl->a_free[i], 1); }
-    for (uint32_t i = 0; i < MAX_D; ++i) { mbar_init(&ctl->d_full[i], 1); mbar_init(&ctl->d_free[i], EPI_THREADS); }
+    for (uint32_t i = 0; i < MAX_D; ++i) { mbar_init(&ctl->d_full[i], 1); mbar_init(&ctl->d_free[i], EPIW * 32); }
     for (uint32_t i = 0; i < MAX_SLOTS; ++i) { mbar_init(&ctl->b_full[i], 1); mbar_init(&ctl->b_free[i], 1); }
     fence_barrier_init();
   }
-  if (warp == MMA_WARP) tmem_alloc(&ctl->tmem_base, a.tmem_cols);
+  if (warp == MMAW) tmem_alloc(&ctl->tmem_base, a.tmem_cols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_a = ctl->tmem_base;                          // A buffers: columns [0, nA * a_cols)
   const uint32_t tmem_d = tmem_a + a.nA * a_cols;                  // accumulator ring: nD chunks of NC columns
 
-  if (warp == MMA_WARP) {
+  if (warp == MMAW) {
     // ===== MMA issuer (one thread) =====
     if (lane == 0 && mine) {
       const uint32_t total = mine * a.nchunks;
-      auto load_chunk = [&](uint32_t g) {                          // g: running chunk index over all my tiles
-        const uint32_t slot = g % a.nslots;
-        mbar_expect_tx(&ctl->b_full[slot], chunk_bytes);
-        bulk_g2s(sB + (size_t)slot * chunk_bytes, a.B + (size_t)(g % a.nchunks) * a.chunk_stride, chunk_bytes, &ctl->b_full[slot]);
+      uint32_t ld_slot = 0, ld_chunk = 0, ld_count = 0;            // next chunk to fetch: ring slot, chunk of the image
+      auto load_next = [&]() {
+        mbar_expect_tx(&ctl->b_full[ld_slot], chunk_bytes);
+        bulk_g2s(sB + (size_t)ld_slot * chunk_bytes, a.B + (size_t)ld_chunk * a.chunk_stride, chunk_bytes, &ctl->b_full[ld_slot]);
+        if (++ld_slot == a.nslots) ld_slot = 0;
+        if (++ld_chunk == a.nchunks) ld_chunk = 0;
+        ++ld_count;
       };
       const uint32_t pre = total < a.nslots ? total : a.nslots;
-      for (uint32_t g = 0; g < pre; ++g) load_chunk(g);
+      while (ld_count < pre) load_next();
       const uint32_t idesc = idesc_u8(NC);
       const uint32_t lboB = NC * 16;
-      uint32_t g = 0;
+      uint32_t g = 0, slot = 0, slot_par = 0;                      // running chunk index, its ring slot and the slot's use parity
+      uint32_t pslot = 0, pslot_par = 0;                           // the same for the previous chunk
       for (uint32_t k = 0; k < mine; ++k) {
-        const uint32_t abuf = k % a.nA;
-        mbar_wait(&ctl->a_full[abuf], (k / a.nA) & 1);
+        const uint32_t abuf = k & amask;
+        mbar_wait(&ctl->a_full[abuf], (k >> ashift) & 1);
         tc_fence_after();
         for (uint32_t c = 0; c < a.nchunks; ++c, ++g) {
-          const uint32_t slot = g % a.nslots;
-          if (!resident || k == 0) mbar_wait(&ctl->b_full[slot], (g / a.nslots) & 1);
-          const uint32_t dbuf = g % a.nD;
-          mbar_wait(&ctl->d_free[dbuf], ((g / a.nD) & 1) ^ 1);
+          if (!resident || k == 0) mbar_wait(&ctl->b_full[slot], slot_par);
+          const uint32_t dbuf = g & dmask;
+          mbar_wait(&ctl->d_free[dbuf], ((g >> dshift) & 1) ^ 1);
           tc_fence_after();
           const uint32_t baddr = smem_u32(sB + (size_t)slot * chunk_bytes);
           for (uint32_t ks = 0; ks < a.KB / KSTEP; ++ks) {
@@ -206,75 +218,92 @@ __global__ void __launch_bounds__(NTHREADS, 1) pipe_kernel(const __grid_constant
           mma_commit(&ctl->d_full[dbuf]);
           if (!resident) {
             mma_commit(&ctl->b_free[slot]);
-            if (g >= 1 && g - 1 + a.nslots < total) {              // the slot of the previous chunk is the next to refill
-              mbar_wait(&ctl->b_free[(g - 1) % a.nslots], ((g - 1) / a.nslots) & 1);
-              load_chunk(g - 1 + a.nslots);
+            if (g >= 1 && ld_count < total) {                      // the slot of the previous chunk is the next to refill
+              mbar_wait(&ctl->b_free[pslot], pslot_par);
+              load_next();
             }
           }
+          pslot = slot; pslot_par = slot_par;
+          if (++slot == a.nslots) { slot = 0; slot_par ^= 1; }
         }
         mma_commit(&ctl->a_free[abuf]);
       }
     }
     __syncwarp();
-  } else if (warp >= EPI_WARPS) {
+  } else if (warp >= EPIW) {
     // ===== loaders =====
-    const uint32_t lw = warp - EPI_WARPS, quarter = lw & 3, half = lw >> 2;
+    const uint32_t lw = warp - EPIW, quarter = lw & 3, half = lw >> 2;
     const uint32_t row = quarter * 32 + lane;
     const uint32_t nbatch = (a_cols + 31) / 32;
+    uint32_t tile = blockIdx.x;
+    uint32_t poly = tile / tpp, tin = tile % tpp;                  // advanced incrementally below
+    const uint32_t dpoly = gridDim.x / tpp, dtin = gridDim.x % tpp;
+    uint32_t po = poly / a.inner, pi = poly % a.inner;
     for (uint32_t k = 0; k < mine; ++k) {
-      const uint32_t tile = blockIdx.x + k * gridDim.x;
-      const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
-      const uint32_t* p = a.src + (size_t)(poly / a.inner) * a.src_outer + (size_t)(poly % a.inner) * a.src_inner + n0 + row;
-      const uint32_t abuf = k % a.nA;
+      const uint32_t* p = a.src + (size_t)po * a.src_outer + (size_t)pi * a.src_inner + tin * TILE_M + row;
+      const uint32_t abuf = k & amask;
       const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
       bool waited = false;
-      for (uint32_t b = half; b < nbatch; b += 4) {                // this warp's batches: half, half + 2, ... two at a time
+      for (uint32_t b = half; b < nbatch; b += 2 * HALVES) {       // this warp's batches, two at a time
         uint32_t w0[32], w1[32];
-        const bool two = b + 2 < nbatch;
+        const bool two = b + HALVES < nbatch;
         load_batch(w0, p, a.N, b, a.nwords);
-        if (two) load_batch(w1, p, a.N, b + 2, a.nwords);
+        if (two) load_batch(w1, p, a.N, b + HALVES, a.nwords);
         if (!waited) {                                             // loads are in flight while the buffer is still being read
-          mbar_wait(&ctl->a_free[abuf], ((k / a.nA) & 1) ^ 1);
+          mbar_wait(&ctl->a_free[abuf], ((k >> ashift) & 1) ^ 1);
           tc_fence_after();
           waited = true;
         }
         store_batch(w0, taddr, b, a.nwords, a_cols, a.mask_bits);
-        if (two) store_batch(w1, taddr, b + 2, a.nwords, a_cols, a.mask_bits);
+        if (two) store_batch(w1, taddr, b + HALVES, a.nwords, a_cols, a.mask_bits);
       }
-      if (!waited) mbar_wait(&ctl->a_free[abuf], ((k / a.nA) & 1) ^ 1);   // a warp without batches still keeps in step
+      if (!waited) mbar_wait(&ctl->a_free[abuf], ((k >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
       tmem_st_wait();
       tc_fence_before();
       mbar_arrive(&ctl->a_full[abuf]);
+      tin += dtin; poly += dpoly;
+      if (tin >= tpp) { tin -= tpp; ++poly; }
+      po = poly / a.inner; pi = poly % a.inner;
     }
   } else {
     // ===== epilogue =====
-    const uint32_t etid = tid;                                     // 0..127 = tile row = TMEM lane
-    const uint32_t lane_off = (warp * 32u) << 16;
-    Epi epi(ep, a, smem + a.epi_off, etid);
+    const uint32_t grp = warp >> 2;
+    const uint32_t etid = (warp & 3) * 32 + lane;                  // 0..127 = tile row = TMEM lane
+    const uint32_t lane_off = ((warp & 3) * 32u) << 16;
+    Epi epi(ep, a, smem + a.epi_off, etid, grp);
     uint32_t g = 0;
     for (uint32_t k = 0; k < mine; ++k) {
       const uint32_t tile = blockIdx.x + k * gridDim.x;
       const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
       epi.begin_tile(poly / a.inner, poly % a.inner, n0);
       for (uint32_t c = 0; c < a.nchunks; ++c, ++g) {
-        const uint32_t dbuf = g % a.nD;
-        mbar_wait(&ctl->d_full[dbuf], (g / a.nD) & 1);
+        const uint32_t dbuf = g & dmask;
+        mbar_wait(&ctl->d_full[dbuf], (g >> dshift) & 1);
         tc_fence_after();
-        uint32_t t[64];
-        tmem_ld32_nowait(tmem_d + dbuf * NC + lane_off, t);
-        tmem_ld32_nowait(tmem_d + dbuf * NC + 32 + lane_off, t + 32);
-        tmem_ld_wait();
-        tc_fence_before();
-        mbar_arrive(&ctl->d_free[dbuf]);                           // the accumulator chunk is in registers: hand it back
-        epi.consume(c * NC, t);
-        epi.consume(c * NC + 32, t + 32);
+        if constexpr (Epi::GROUPS == 1) {
+          uint32_t t[64];
+          tmem_ld32_nowait(tmem_d + dbuf * NC + lane_off, t);
+          tmem_ld32_nowait(tmem_d + dbuf * NC + 32 + lane_off, t + 32);
+          tmem_ld_wait();
+          tc_fence_before();
+          mbar_arrive(&ctl->d_free[dbuf]);                         // the accumulator chunk is in registers: hand it back
+          epi.consume(c * NC, t);
+          epi.consume(c * NC + 32, t + 32);
+        } else {
+          uint32_t t[32];
+          tmem_ld32_nowait(tmem_d + dbuf * NC + grp * 32 + lane_off, t);
+          tmem_ld_wait();
+          tc_fence_before();
+          mbar_arrive(&ctl->d_free[dbuf]);
+          epi.consume(c * NC + grp * 32, t);
+        }
       }
       epi.end_tile();
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == MMA_WARP) tmem_dealloc(tmem_a, a.tmem_cols);
+  if (warp == MMAW) tmem_dealloc(tmem_a, a.tmem_cols);
 }
 
 template <class Epi>
@@ -287,7 +316,7 @@ inline cudaError_t launch_pipe(const PipeArgs& a, const typename Epi::Params& ep
   }
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);
   const uint32_t grid = ntiles < (uint32_t)n_sm ? ntiles : (uint32_t)n_sm;
-  pipe_kernel<Epi><<<grid, NTHREADS, smem, s>>>(a, ep);
+  pipe_kernel<Epi><<<grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s>>>(a, ep);
   return cudaGetLastError();
 }
 #endif  // __CUDACC__
