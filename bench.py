@@ -54,21 +54,22 @@ def work_model(N, logQ, logP, L, L_PQ, K1, K2, B):
     dq = math.ceil(logQ / 26)                 # 26-bit digits of an input coefficient
     d_t = math.ceil(logQ / 26)                # CRT output digits, tensor
     d_r = math.ceil((logQ + logP) / (26 if K2 + 1 <= 127 else 25))
-    bfly = N // 2 * logN                      # butterflies per transform, 3 multiplies each (Shoup)
+    bf_col = N // 2 * (logN - 8)              # butterflies per transform in the column pass, 3 multiplies each (Shoup)
+    bf_row = N // 2 * 8                       # ... and in the 256-point rows (inside the fused row kernel)
     mul = {
         "decompose": B * N * (4 * K1 + K2) * (dq + 6),
-        "ntt_fwd": B * (4 * K1 + K2) * bfly * 3,
-        "ntt_inv": B * (3 * K1 + 2 * K2) * (bfly * 3 + N * 3),
-        "pointwise": B * N * (K1 * 4 * 3 + K2 * 2 * 3),
+        "ntt_fwd": B * (4 * K1 + K2) * bf_col * 3,
+        "pointwise": B * ((4 * K1 + K2) + (3 * K1 + 2 * K2)) * bf_row * 3 + B * N * (K1 * 4 * 3 + K2 * 2 * 3),
+        "ntt_inv": B * (3 * K1 + 2 * K2) * (bf_col * 3 + N * 3),
         "crt": B * N * (3 * ((K1 + 1) * d_t + K1) + 2 * ((K2 + 1) * d_r + K2)),
         "rescale": 0,
     }
     w = 4
-    byt = {   # bytes each class must move if every intermediate makes exactly one HBM round trip
+    byt = {   # bytes each class must move if every intermediate makes exactly one HBM round trip (DESIGN.md 7)
         "decompose": B * N * w * (4 * L + L + 4 * K1 + K2),
-        "ntt_fwd": B * N * w * 2 * 2 * (4 * K1 + K2),
-        "ntt_inv": B * N * w * 2 * 2 * (3 * K1 + 2 * K2),
-        "pointwise": B * N * w * (7 * K1 + 3 * K2) + N * w * 2 * K2,
+        "ntt_fwd": B * N * w * 2 * (4 * K1 + K2),                      # forward column pass, in place
+        "pointwise": B * N * w * (4 * K1 + 3 * K1 + K2 + 2 * K2 + 2 * K2),   # fused rows: operands in, products out, evk-hat per item
+        "ntt_inv": B * N * w * 2 * (3 * K1 + 2 * K2),                  # inverse column pass, in place
         "crt": B * N * w * (3 * K1 + 3 * L + 2 * K2 + 2 * L + 2 * L),
         "rescale": 0,
     }

@@ -34,9 +34,8 @@ fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const
   // slots (a0, a1, b0, b1) per batch item: ct1 polys go to slots 0,1 ; ct2 polys to slots 2,3
   CK(launch_decompose(c, ws, 4 * rp, rp, d_ct1, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct1");
   CK(launch_decompose(c, ws + 2 * rp, 4 * rp, rp, d_ct2, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct2");
-  CK(launch_ntt_fwd(c, ws, B, 4, 4, K, s), "ntt fwd");
-  // pointwise tensor product in the registers of the first inverse pass: slots 0..2 <- INTT(d0^, d1^, d2^)
-  CK(launch_ntt_inv(c, ws, nullptr, B, 4, 3, K, PW_TENSOR, c->tgt_tensor.d_scale, s), "ntt inv");
+  // forward columns, fused rows (tensor product in registers), inverse columns: slots 0..2 <- INTT(d0^, d1^, d2^)
+  CK(launch_ntt_product(c, ws, nullptr, B, K, PW_TENSOR, c->tgt_tensor.d_scale, s), "ntt tensor");
   CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3, (size_t)3 * L * N, (size_t)L * N, ws, 4 * rp, rp, nullptr, 0, 0,
                 B, 3, s), "crt");
   return FHE_OK;
@@ -49,8 +48,7 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   const size_t rp = (size_t)K * N;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ws, 2 * rp, 0, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, 0, B, 1, L, K, mask, s), "decompose d2");
-  CK(launch_ntt_fwd(c, ws, B, 2, 1, K, s), "ntt fwd d2");
-  CK(launch_ntt_inv(c, ws, c->d_evk_hat, B, 2, 2, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt inv relin");
+  CK(launch_ntt_product(c, ws, c->d_evk_hat, B, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt relin");
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
   CK(launch_crt(c, c->tgt_relin, pp, d_out2, (size_t)2 * L * N, (size_t)L * N, ws, 2 * rp, rp, d_in3, (size_t)3 * L * N,
@@ -115,8 +113,7 @@ fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ra, 0, rp, d_a, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose a");
   CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose b");
-  CK(launch_ntt_fwd(c, ra, 2 * batch, 1, 1, K, s), "ntt fwd");
-  CK(launch_ntt_inv(c, ra, rb, batch, 1, 1, K, PW_POLYMUL, c->tgt_pm.d_scale, s), "ntt inv");
+  CK(launch_ntt_product(c, ra, rb, batch, K, PW_POLYMUL, c->tgt_pm.d_scale, s), "ntt polymul");
   CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, 0, (size_t)L * N, ra, 0, rp, nullptr, 0, 0, 1, batch, s), "crt");
   return FHE_OK;
 }

@@ -121,6 +121,12 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
 enum PwMode : int { PW_NONE = 0, PW_POLYMUL = 1, PW_TENSOR = 2, PW_RELIN = 3 };
 cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
                            uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s);
+// The product path: forward column pass over the operand slots, ONE fused row pass (last forward pass, pointwise
+// products, first inverse pass, all in registers on the same 256-point row), inverse column pass over the result slots.
+// Same slot conventions as launch_ntt_inv's PW modes, but the operands arrive untransformed (decompose output); for
+// PW_POLYMUL d_aux (the b operand, [nitems][K][N]) is transformed in place too.
+cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
+                               const uint2* d_scale, cudaStream_t s);
 // CRT + post: residues [K][N] -> limbs [L][N] per polynomial (o, i); d_add: for the relin modes, the polynomial added
 // at the end, else nullptr
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,

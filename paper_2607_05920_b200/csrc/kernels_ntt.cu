@@ -114,11 +114,12 @@ __device__ __forceinline__ uint32_t mm(uint32_t a, uint32_t b, uint32_t q, uint3
 struct NttArgs {
   uint32_t* data;            // transforms: item-major [nitems][S][K][N]; slots 0..U-1 of every item are transformed
   const uint32_t* aux;       // PW_POLYMUL: b [nitems][K][N]; PW_RELIN: evk-hat [2][K][N]
-  const uint2* tw;           // [Kmax][N] twiddles of the direction
+  const uint2* tw;           // [Kmax][N] twiddles of the direction (fused row pass: inverse)
+  const uint2* tw2;          // fused row pass only: forward twiddles
   const uint32_t* q;         // [Kmax]
   const uint32_t* qn;        // [Kmax] -q^-1 mod 2^32
   const uint2* scale;        // [K] final constant of the inverse (with Shoup companion)
-  uint32_t N, K, N1, S, U, units;
+  uint32_t N, K, N1, S, U, units, nitems;
 };
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -331,6 +332,104 @@ ntt_row_inv_kernel(NttArgs a) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Fused row pass: the last forward pass, the pointwise products (S3) and the first inverse pass all act on the same
+// contiguous 256-point row of one prime, and the forward row pass leaves every thread with 16 contiguous points --
+// exactly what the inverse row pass starts from.  So the operands' rows are transformed forward in registers, the
+// products formed in registers, and the product rows transformed back, with no HBM round trip in between.
+// Operands after the forward rows: the first factor canonical ([0, q)), the second lazy ([0, 4q)): a b < 4 q^2 < 2^62,
+// a0 b1 + a1 b0 < 8 q^2 < 2^63 (q < 2^30), so mont_redc's precondition holds and its result is in [0, 2q) -- what the
+// inverse butterflies accept.
+// ------------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ldrow(uint32_t (&x)[16], const uint32_t* g, uint32_t t) {
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = g[i * 16 + t];
+}
+
+template <int PW, bool FINAL>
+__global__ void __launch_bounds__(256, 2)
+ntt_row_fused_kernel(NttArgs a) {
+  __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
+  const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
+  // unit = (j * N1 + r) * nitems + item: the half-warps of a block that share (j, r) share every twiddle of both
+  // directions (2 KB per row and direction, twice the row itself), so the tables cross L2 -> SM once per (j, r)
+  const uint32_t unit = blockIdx.x * 16 + rl;
+  if (unit >= a.units) return;
+  const uint32_t item = unit % a.nitems, jr = unit / a.nitems;
+  const uint32_t r = jr % a.N1, j = jr / a.N1;
+  uint32_t* srow = sm + rl * ROW_SM;
+  const size_t KN = (size_t)a.K * a.N;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
+  const uint2* twf = a.tw2 + (size_t)j * a.N;
+  const uint2* twi = a.tw + (size_t)j * a.N;
+  const uint32_t base = a.N1 + r;
+  const size_t poff = (size_t)j * a.N + (size_t)r * 256;
+
+  auto fwd = [&](uint32_t (&x)[16]) { row_fwd_core(x, srow, t, twf, base, q, q2); };
+  auto fwd_canon = [&](uint32_t (&x)[16]) {
+    row_fwd_core(x, srow, t, twf, base, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = canon4(x[i], q, q2);
+  };
+  auto finish = [&](uint32_t (&x)[16], uint32_t* g) {
+    row_inv_core(x, srow, t, twi, base, q, q2);
+    if (FINAL) {
+      const uint2 sc = __ldg(a.scale + j);
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[i * 16 + t] = mul_shoup(x[i], sc.x, sc.y, q);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 16; ++i) g[i * 16 + t] = x[i];
+    }
+  };
+
+  if constexpr (PW == PW_POLYMUL) {
+    uint32_t* g = a.data + (size_t)item * KN + poff;
+    uint32_t x[16], y[16];
+    ldrow(x, g, t);
+    ldrow(y, a.aux + (size_t)item * KN + poff, t);
+    fwd_canon(x);
+    fwd(y);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(x[i], y[i], q, qn);
+    finish(x, g);
+  } else if constexpr (PW == PW_TENSOR) {
+    uint32_t* g = a.data + (size_t)item * 4 * KN + poff;       // slots a0, a1, b0, b1 at g + slot * KN
+    uint32_t a0[16], a1[16], b0[16], b1[16], x[16];
+    ldrow(a0, g, t);
+    ldrow(a1, g + KN, t);
+    ldrow(b0, g + 2 * KN, t);
+    ldrow(b1, g + 3 * KN, t);
+    fwd_canon(a0);     // the exchange inside orders every lane's operand loads before the first store below
+    fwd_canon(a1);
+    fwd(b0);
+    fwd(b1);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
+    finish(x, g);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
+    finish(x, g + KN);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
+    finish(x, g + 2 * KN);
+  } else {   // PW_RELIN: slot 0 = d2 residues after the forward column pass; aux = evk-hat (fully transformed, canonical)
+    static_assert(PW == PW_RELIN, "fused row pass: unknown mode");
+    uint32_t* g = a.data + (size_t)item * 2 * KN + poff;
+    uint32_t d[16], e0[16], e1[16], x[16];
+    ldrow(d, g, t);
+    load16(e0, a.aux + poff + t * 16);
+    load16(e1, a.aux + KN + poff + t * 16);
+    fwd_canon(d);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e0[i], q, qn);
+    finish(x, g);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e1[i], q, qn);
+    finish(x, g + KN);
+  }
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------------------
 template <bool INV>
 static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaStream_t s) {
@@ -353,8 +452,8 @@ static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaSt
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s) {
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
-  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems;
   const uint32_t ntr = nitems * U * K;
   a.units = ntr * a.N1;
   if (c->logN > 8) {
@@ -370,8 +469,8 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, u
                            uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s) {
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
-  a.data = d_res; a.aux = d_aux; a.tw = c->d_tw_inv; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U;
+  a.data = d_res; a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems;
   const bool fin = c->logN == 8;
   const uint32_t row_units = (pw_mode == PW_NONE ? nitems * U : nitems) * K * a.N1;
   a.units = row_units;
@@ -392,6 +491,49 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, u
     if (e != cudaSuccess) return e;
   }
   if (!fin) return launch_col<true>(c, a, nitems * U * K, s);
+  return cudaSuccess;
+}
+
+// S2 + S3 + S4 of a product in three launches (four for PW_POLYMUL): forward column pass over the operand slots, the
+// fused row pass, inverse column pass over the result slots.
+cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
+                               const uint2* d_scale, cudaStream_t s) {
+  if (!nitems) return cudaSuccess;
+  uint32_t S, Uin, Uout;
+  switch (pw_mode) {
+    case PW_POLYMUL: S = 1; Uin = 1; Uout = 1; break;
+    case PW_TENSOR: S = 4; Uin = 4; Uout = 3; break;
+    case PW_RELIN: S = 2; Uin = 1; Uout = 2; break;
+    default: return cudaErrorInvalidValue;
+  }
+  NttArgs a;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems;
+  const bool fin = c->logN == 8;
+  cudaError_t e;
+  if (!fin) {
+    if ((e = launch_col<false>(c, a, nitems * Uin * K, s)) != cudaSuccess) return e;
+    if (pw_mode == PW_POLYMUL) {
+      a.data = d_aux;
+      if ((e = launch_col<false>(c, a, nitems * K, s)) != cudaSuccess) return e;
+      a.data = d_res;
+    }
+  }
+  a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = d_scale; a.U = Uout;
+  a.units = nitems * K * a.N1;
+  const uint32_t blocks = (a.units + 15) / 16;
+  {
+    LaunchTimer lt(c, KC_POINTWISE, s);
+#define FUSED_CASE(PW)                                                                 \
+  case PW:                                                                             \
+    if (fin) ntt_row_fused_kernel<PW, true><<<blocks, 256, 0, s>>>(a);                 \
+    else ntt_row_fused_kernel<PW, false><<<blocks, 256, 0, s>>>(a);                    \
+    break;
+    switch (pw_mode) { FUSED_CASE(PW_POLYMUL) FUSED_CASE(PW_TENSOR) FUSED_CASE(PW_RELIN) }
+#undef FUSED_CASE
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  if (!fin) return launch_col<true>(c, a, nitems * Uout * K, s);
   return cudaSuccess;
 }
 
