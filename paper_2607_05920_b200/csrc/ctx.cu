@@ -115,10 +115,10 @@ static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2
   const BigU T = pow2 ? BigU::pow2(32 * tg.Lraw) : Tmod;
   BigU M((uint64_t)1);
   for (uint32_t i = 0; i < K; ++i) M.mul_small(c->h_q[i]);
-  const size_t chunk_bytes = (size_t)tg.KB * NC;
-  std::vector<uint8_t> img(chunk_bytes * tg.nchunks, 0);
+  const size_t img_cols = (size_t)tg.nchunks * NC;                      // image [KB / 16][img_cols][16 bytes] (pipe.cuh)
+  std::vector<uint8_t> img((size_t)tg.KB * img_cols, 0);
   auto put = [&](uint32_t kb, uint32_t col, uint8_t v) {
-    img[(size_t)(col / NC) * chunk_bytes + (size_t)(kb / 16) * NC * 16 + (size_t)(col % NC) * 16 + kb % 16] = v;
+    img[((size_t)(kb / 16) * img_cols + col) * 16 + kb % 16] = v;
   };
   std::vector<uint2> scale(K);
   for (uint32_t i = 0; i < K; ++i) {
@@ -214,8 +214,8 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   std::vector<uint2> scale_plain(Kmax);
   // decompose constants: widest input is the evk (L_PQ limbs) or what fhe_debug_decompose may pass (MAX_LIMBS_IN)
   c->dec_KBimg = (4 * MAX_LIMBS_IN + 31) / 32 * 32;
-  const size_t dec_chunk = (size_t)c->dec_KBimg * DEC_NC;
-  std::vector<uint8_t> decB(dec_chunk * ((Kmax + 15) / 16), 0);
+  c->dec_cols = (Kmax + 15) / 16 * DEC_NC;               // image [dec_KBimg / 16][dec_cols][16 bytes] (pipe.cuh)
+  std::vector<uint8_t> decB((size_t)c->dec_KBimg * c->dec_cols, 0);
   c->h_psi.resize(Kmax);
   std::vector<uint2> twf((size_t)Kmax * N), twi((size_t)Kmax * N);
   std::vector<uint32_t> pw(N), ipw(N);
@@ -242,11 +242,10 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     }
     uint32_t ninv = powmod(N % q, q - 2, q);
     scale_plain[j] = make_uint2(ninv, shoup(ninv, q));
-    uint32_t cur = 1;                                  // 2^(8 kb) mod q, byte cc at column 4 (j % 16) + cc of chunk j / 16
+    uint32_t cur = 1;                                  // 2^(8 kb) mod q, byte cc at column 4 j + cc
     for (uint32_t kb = 0; kb < c->dec_KBimg; ++kb) {
       for (uint32_t cc = 0; cc < 4; ++cc)
-        decB[(size_t)(j / 16) * dec_chunk + (size_t)(kb / 16) * DEC_NC * 16 + (size_t)(4 * (j % 16) + cc) * 16 + kb % 16] =
-            (uint8_t)(cur >> (8 * cc));
+        decB[((size_t)(kb / 16) * c->dec_cols + 4 * j + cc) * 16 + kb % 16] = (uint8_t)(cur >> (8 * cc));
       cur = mulmod(cur, 256u, q);
     }
   }

@@ -24,7 +24,7 @@ struct CrtTarget {
   uint32_t nchunks = 0;  // 64-column chunks of the constant image (pipe::NC)
   uint32_t Lraw = 0;     // 32-bit limbs of V produced by the carry pass (4 Lraw value columns)
   uint32_t Lx = 0;       // limbs of the per-coefficient column the post-processing works on (>= Lraw + 1)
-  uint8_t* d_B = nullptr;      // [nchunks][KB/16][64][16]: shared-memory images of the constant chunks
+  uint8_t* d_B = nullptr;      // [KB/16][64 nchunks][16]: the constant matrix as K-major 16-byte core-matrix rows (pipe.cuh)
   uint32_t* d_negM = nullptr;  // [Lraw]
   uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
 };
@@ -67,7 +67,8 @@ struct Context {
   uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion
   uint2* d_tw_inv = nullptr;      // [Kmax][N]: psi^-bitrev(k) and Shoup companion
   uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
-  uint8_t* d_decB = nullptr;      // [ceil(Kmax/16)][dec_KBimg/16][DEC_NC][16]: byte c of 2^(8 kb) mod q_j at column 4 j + c
+  uint8_t* d_decB = nullptr;      // [dec_KBimg/16][dec_cols][16]: byte c of 2^(8 kb) mod q_j at column 4 j + c
+  uint32_t dec_cols = 0;          // columns of the decompose image: 64 ceil(Kmax / 16)
   uint32_t dec_KBimg = 0;         // contraction bytes covered by the decompose image (widest input, multiple of 32)
   CrtTarget tgt_pm, tgt_tensor, tgt_relin;
   PostParams post_pm, post_tensor, post_relin;

@@ -119,6 +119,7 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 //                tile's MMAs run.
 // ------------------------------------------------------------------------------------------------------------------
 struct CrtEpi {
+  static constexpr int LOAD_WORDS = 64, MAX_REGS = 128;    // 13 warps are allocated as 16: 16 x 32 x 128 = 64 K
   static constexpr uint32_t GROUPS = 1, LOAD_WARPS = 8;
   struct Params {
     uint32_t* out; size_t out_outer, out_inner;
@@ -416,7 +417,7 @@ static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
   CrtEpi::Params ep; size_t bytes;
   crt_scratch_layout(tg, pp, ep, bytes);
-  return pipe::make_plan(tg.KB, tg.nchunks, bytes).ok;
+  return pipe::make_plan(tg.KB, tg.nchunks, bytes, true).ok;
 }
 
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
@@ -426,14 +427,14 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   CrtEpi::Params ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);
-  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes);
+  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   if (relin && !d_add) return cudaErrorInvalidValue;
   pipe::PipeArgs a;
   a.src = d_res; a.src_outer = res_outer; a.src_inner = res_inner;
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = tg.K; a.mask_bits = 0;
-  a.B = tg.d_B; a.chunk_stride = (size_t)tg.KB * pipe::NC;
+  a.B = tg.d_B; a.b_cols = tg.nchunks * pipe::NC;
   pipe::fill_args(a, plan);
   ep.out = d_out; ep.out_outer = out_outer; ep.out_inner = out_inner;
   ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;

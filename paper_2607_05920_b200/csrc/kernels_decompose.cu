@@ -11,10 +11,15 @@
 
 namespace fhe {
 
-// Epilogue of the pipeline: a 64-column accumulator chunk holds the byte sums of 16 primes; each of the two epilogue
-// warp groups takes 8 of them.  (q_j, floor(2^53 / q_j)) sit in shared memory, padded to whole chunks.
+// Epilogue of the pipeline: a 64-column accumulator chunk holds the byte sums of 16 primes; each of the GROUPS epilogue
+// warp groups takes 16 / GROUPS of them.  (q_j, floor(2^53 / q_j)) sit in shared memory, padded to whole chunks.
+// Per residue: the low word of v = T0 + 2^8 T1 + 2^16 T2 + 2^24 T3 (< 2^49) exactly, an estimate vh <= v >> 21 that
+// is at most 20 short (the shifted-out bits of T1, T2 and T0 >> 21 < 16), and one Barrett step: qh = mulhi(vh, mu) is
+// floor(v / q) or one less (20 * 2^21 / q < 0.16 for q > 2^28), so the 32-bit remainder lies in [0, 2q).
 struct DecEpi {
-  static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 4;   // 13 warps: at most 4 on an SM sub-partition, 128 registers each
+  static constexpr int LOAD_WORDS = 40, MAX_REGS = 80;   // 21 warps are allocated as 24: 24 x 32 x 80 <= 64 K
+  static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 4;
+  static constexpr int PPG = 16 / GROUPS;                // primes per group and chunk
   struct Params {
     uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
     const uint2* qmu;                             // (q_j, floor(2^53 / q_j))
@@ -33,18 +38,24 @@ struct DecEpi {
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.res + (size_t)o * p.res_outer + (size_t)i * p.res_inner + n0 + etid;
   }
+  __device__ __forceinline__ uint32_t reduce(const uint32_t* t, const uint2 qm) const {
+    const uint32_t lo = t[0] + (t[1] << 8) + (t[2] << 16) + (t[3] << 24);
+    const uint32_t vh = (t[3] << 3) + (t[2] >> 5) + (t[1] >> 13);
+    const uint32_t qh = __umulhi(vh, qm.y);
+    return csub(lo - qh * qm.x, qm.x);
+  }
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     const uint32_t j0 = col0 / 4;
     uint32_t* o = out + (size_t)j0 * N;
+    if (j0 + PPG <= p.K) {
 #pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const uint2 qm = tab[j0 + e];
-      uint64_t v = (uint64_t)t[4 * e + 1] * 256u + t[4 * e];             // three wide multiply-adds: v < 2^49
-      v = (uint64_t)t[4 * e + 2] * 65536u + v;
-      v = (uint64_t)t[4 * e + 3] * 16777216u + v;
-      const uint32_t r = barrett49(v, qm.x, qm.y);
-      if (j0 + e < p.K) *o = r;
-      o += N;
+      for (int e = 0; e < PPG; ++e) { *o = reduce(t + 4 * e, tab[j0 + e]); o += N; }
+    } else {
+#pragma unroll
+      for (int e = 0; e < PPG; ++e) {
+        if (j0 + e < p.K) *o = reduce(t + 4 * e, tab[j0 + e]);
+        o += N;
+      }
     }
   }
   __device__ __forceinline__ void end_tile() {}
@@ -58,12 +69,12 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
   if (mask_bits && (mask_bits + 31) / 32 < eff) eff = (mask_bits + 31) / 32;
   const uint32_t KB = (4 * eff + 31) / 32 * 32;
   if (KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
-  const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2));
+  const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2), false);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   pipe::PipeArgs a;
   a.src = d_limbs; a.src_outer = limb_outer; a.src_inner = limb_inner;
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = eff; a.mask_bits = mask_bits;
-  a.B = c->d_decB; a.chunk_stride = (size_t)c->dec_KBimg * DEC_NC;
+  a.B = c->d_decB; a.b_cols = c->dec_cols;
   pipe::fill_args(a, plan);
   DecEpi::Params ep;
   ep.res = d_res; ep.res_outer = res_outer; ep.res_inner = res_inner; ep.qmu = c->d_qmu; ep.K = K;

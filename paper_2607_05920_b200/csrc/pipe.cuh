@@ -8,17 +8,25 @@
 //   loader warps       global -> registers -> TMEM: thread (quarter, lane) owns tile row 32 quarter + lane, which is
 //                      TMEM lane 32 quarter + lane.  Word w of its coefficient is column w of the A operand: the i8
 //                      MMA reads an A operand held in TMEM as four K-bytes per 32-bit cell, little-endian -- exactly
-//                      the word-major data, so no transposition through shared memory exists.  Up to 64 coalesced
-//                      loads are in flight per thread; the A operand is double-buffered.
-//   MMA thread (1)     per tile and per 64-column chunk of the constant matrix (resident in shared memory, loaded once
-//                      per CTA with cp.async.bulk; streamed through a ring when it does not fit): KB/32
-//                      tcgen05.mma kind::i8 into one buffer of a ring of accumulator chunks in TMEM.
-//   epilogue warps     (4 or 8) tcgen05.ld of a finished accumulator chunk, then the conversion's own arithmetic (an Epi
-//                      functor: Barrett reduction and store for S1; carry pass, mod-Q / divide-by-P post-processing and
-//                      store for S5).
+//                      the word-major data, so no transposition through shared memory exists.  The A operand is
+//                      double-buffered when tensor memory has the room.
+//   MMA thread (1)     per tile: KB/32 tcgen05.mma kind::i8 per SPAN of up to 256 accumulator columns.  A
+//                      tcgen05.mma costs ~100 cycles whatever its N, plus ~350 when it starts a new accumulator
+//                      (measured on B200), so the instruction is made as wide as the ISA allows (N = 256) and the K
+//                      loop as long as the operand: narrow 64-column MMAs left the tensor pipe as the bottleneck.
+//   epilogue warps     tcgen05.ld of 64 finished accumulator columns (a "chunk"), then the conversion's own arithmetic
+//                      (an Epi functor: Barrett reduction and store for S1; carry pass, mod-Q / divide-by-P
+//                      post-processing and store for S5).  A chunk's columns are handed back to the MMA thread as soon
+//                      as they are in registers, so the next tile's MMAs overlap this tile's arithmetic.
 //
-// TMEM budget: nA * KB/4 columns of A + nD * 64 columns of accumulators <= 512.
+// Tensor memory holds the A buffers and ONE set of accumulator columns for all chunks of a pass:
+//   nA * KB/4 + 64 * chunks_per_pass <= 512 columns.
+// When the constant matrix has more columns than that (or than shared memory holds), the launch runs several passes over
+// its tiles, pass p with columns [p * cpp * 64, ...) of B resident in shared memory (loaded once per pass per CTA).
 #pragma once
+#include <cstdio>
+#include <cstdlib>
+
 #include "umma.cuh"
 
 namespace fhe {
@@ -26,15 +34,17 @@ namespace pipe {
 
 using namespace umma;
 
-constexpr uint32_t NC = 64;                                   // accumulator columns per chunk
-constexpr uint32_t MAX_SLOTS = 16, MAX_D = 4, MAX_A = 2;
+constexpr uint32_t NC = 64;                                   // accumulator columns per chunk (the epilogue's unit)
+constexpr uint32_t SPAN = 4;                                  // chunks per MMA span: N = 256
+constexpr uint32_t MAX_CHUNKS = 8, MAX_SPANS = 2, MAX_A = 2;  // per pass (512 TMEM columns)
 constexpr uint32_t CTRL_BYTES = 1024;
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 
 struct Ctrl {
-  uint64_t a_full[MAX_A], a_free[MAX_A];      // A operand buffer written (256 loader arrivals) / consumed (MMA commit)
-  uint64_t d_full[MAX_D], d_free[MAX_D];      // accumulator chunk finished (MMA commit) / drained (128 epilogue arrivals)
-  uint64_t b_full[MAX_SLOTS], b_free[MAX_SLOTS];
+  uint64_t a_full[MAX_A], a_free[MAX_A];      // A buffer written (loader arrivals) / consumed (MMA commit)
+  uint64_t d_full[MAX_SPANS];                 // the span's accumulators finished (MMA commit)
+  uint64_t d_free[MAX_CHUNKS];                // the chunk's accumulators are in registers (epilogue arrivals)
+  uint64_t b_full, mma_done;                  // B of the pass landed (bulk copies) / every MMA of the pass finished
   uint32_t tmem_base;
 };
 static_assert(sizeof(Ctrl) <= CTRL_BYTES, "control block");
@@ -44,42 +54,54 @@ struct PipeArgs {
   // coefficient n at [w * N + n].  Words >= nwords read as zero; mask_bits != 0 reduces the row mod 2^mask_bits.
   const uint32_t* src; size_t src_outer, src_inner;
   uint32_t inner, npoly, N, nwords, mask_bits;
-  // contraction
-  const uint8_t* B; size_t chunk_stride;      // chunk c of the constant image at B + c * chunk_stride; KB * NC bytes used
-  uint32_t KB, nchunks, nslots, nA, nD, tmem_cols;
-  uint32_t epi_off, b_off;                    // byte offsets of the epilogue scratch and the B slots in dynamic smem
+  // contraction: the constant image is [kb / 16][b_cols][16 bytes] (K-major core matrices, no swizzle), KB bytes of
+  // contraction and nchunks * 64 columns of it are used
+  const uint8_t* B; uint32_t b_cols;
+  uint32_t KB, nchunks;
+  uint32_t npass, cpp;                        // passes over the tiles, chunks per pass (the last pass may have fewer)
+  uint32_t nA, tmem_cols;
+#ifdef PIPE_DBG
+  uint32_t dbg; unsigned long long* prof;
+#endif
+  uint32_t epi_off, b_off;                    // byte offsets of the epilogue scratch and of B in dynamic smem
 };
 
 // ---- host-side plan -----------------------------------------------------------------------------------------------------
 struct Plan {
-  uint32_t KB = 0, nchunks = 0, nslots = 0, nA = 0, nD = 0, tmem_cols = 0, epi_off = 0, b_off = 0;
+  uint32_t KB = 0, nchunks = 0, npass = 0, cpp = 0, nA = 0, tmem_cols = 0, epi_off = 0, b_off = 0;
   size_t smem = 0;
   bool ok = false;
 };
-inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes) {
+// single_pass: the epilogue carries state across the chunks of a tile (S5), so all columns must fit at once
+inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool single_pass) {
   Plan p;
   p.KB = KB; p.nchunks = nchunks;
   const uint32_t a_cols = KB / 4;
-  p.nD = (2 * a_cols + 4 * NC <= 512) ? 4 : 2;
-  p.nA = (2 * a_cols + p.nD * NC <= 512) ? 2 : 1;
-  const uint32_t cols = p.nA * a_cols + p.nD * NC;
-  if (cols > 512 || nchunks == 0) return p;
-  p.tmem_cols = 32;
-  while (p.tmem_cols < cols) p.tmem_cols <<= 1;
+  if (nchunks == 0 || a_cols + NC > 512) return p;
   p.epi_off = CTRL_BYTES;
   p.b_off = (uint32_t)((CTRL_BYTES + epi_bytes + 127) & ~(size_t)127);
-  const size_t chunk_bytes = (size_t)KB * NC;
-  if (p.b_off + 2 * chunk_bytes > SMEM_LIMIT) return p;
-  size_t fit = (SMEM_LIMIT - p.b_off) / chunk_bytes;
-  if (fit > MAX_SLOTS) fit = MAX_SLOTS;
-  p.nslots = nchunks <= fit ? nchunks : (uint32_t)fit;
-  if (p.nslots < nchunks && p.nslots < 2) return p;
-  p.smem = p.b_off + (size_t)p.nslots * chunk_bytes;
+  if (p.b_off + (size_t)KB * NC > SMEM_LIMIT) return p;
+  const uint32_t smem_chunks = (uint32_t)((SMEM_LIMIT - p.b_off) / ((size_t)KB * NC));
+  for (uint32_t nA = 2; nA >= 1 && !p.npass; --nA) {
+    if (nA * a_cols + NC > 512) continue;
+    uint32_t cap = (512 - nA * a_cols) / NC;                // chunks tensor memory holds beside the A buffers
+    if (cap > MAX_CHUNKS) cap = MAX_CHUNKS;
+    if (cap > smem_chunks) cap = smem_chunks;
+    if (cap == 0) continue;
+    const uint32_t npass = (nchunks + cap - 1) / cap;
+    if (single_pass && npass > 1) continue;                 // try nA = 1, which leaves more columns
+    p.nA = nA; p.npass = npass; p.cpp = (nchunks + npass - 1) / npass;
+  }
+  if (!p.npass) return p;
+  const uint32_t cols = p.nA * a_cols + p.cpp * NC;
+  p.tmem_cols = 32;
+  while (p.tmem_cols < cols) p.tmem_cols <<= 1;
+  p.smem = p.b_off + (size_t)p.cpp * KB * NC;
   p.ok = true;
   return p;
 }
 inline void fill_args(PipeArgs& a, const Plan& p) {
-  a.KB = p.KB; a.nchunks = p.nchunks; a.nslots = p.nslots; a.nA = p.nA; a.nD = p.nD; a.tmem_cols = p.tmem_cols;
+  a.KB = p.KB; a.nchunks = p.nchunks; a.npass = p.npass; a.cpp = p.cpp; a.nA = p.nA; a.tmem_cols = p.tmem_cols;
   a.epi_off = p.epi_off; a.b_off = p.b_off;
 }
 
@@ -116,36 +138,40 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// One batch of 32 words (A columns [32 b, 32 b + 32)) of this thread's row: issue the loads.
-__device__ __forceinline__ void load_batch(uint32_t (&w)[32], const uint32_t* __restrict__ p, size_t N, uint32_t b,
+// One batch of LR words (A columns [w0, w0 + LR)) of this thread's row: issue the loads ...
+template <int LR>
+__device__ __forceinline__ void load_batch(uint32_t (&w)[LR], const uint32_t* __restrict__ p, size_t N, uint32_t w0,
                                            uint32_t nwords) {
 #pragma unroll
-  for (int i = 0; i < 32; ++i) {
-    const uint32_t wi = b * 32 + i;
+  for (int i = 0; i < LR; ++i) {
+    const uint32_t wi = w0 + i;
     w[i] = wi < nwords ? __ldg(p + (size_t)wi * N) : 0u;        // warp-uniform predicate
   }
 }
-// ... then zero the padding, mask the top word and write the batch to TMEM columns [32 b, min(32 b + 32, a_cols)).
-__device__ __forceinline__ void store_batch(uint32_t (&w)[32], uint32_t taddr_a, uint32_t b, uint32_t nwords, uint32_t a_cols,
+// ... then mask the top word and write the batch to TMEM columns [w0, min(w0 + LR, a_cols)).
+template <int LR>
+__device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a, uint32_t w0, uint32_t a_cols,
                                             uint32_t mask_bits) {
 #pragma unroll
-  for (int i = 0; i < 32; ++i)
-    if ((mask_bits & 31) && b * 32 + i == (mask_bits >> 5)) w[i] &= (1u << (mask_bits & 31)) - 1u;
-  (void)nwords;
+  for (int i = 0; i < LR; ++i)
+    if ((mask_bits & 31) && w0 + i == (mask_bits >> 5)) w[i] &= (1u << (mask_bits & 31)) - 1u;
 #pragma unroll
-  for (int c = 0; c < 4; ++c)
-    if (b * 32 + c * 8 < a_cols) tmem_st8(taddr_a + b * 32 + c * 8, &w[c * 8]);
+  for (int c = 0; c < LR / 8; ++c)
+    if (w0 + c * 8 < a_cols) tmem_st8(taddr_a + w0 + c * 8, &w[c * 8]);
 }
 
 // ---- the kernel -------------------------------------------------------------------------------------------------------------
 // Epi: struct with
 //   static constexpr uint32_t LOAD_WARPS;                             4 or 8 loader warps (one or two per TMEM lane quarter)
-//   static constexpr uint32_t GROUPS;                                 1: every epilogue warp takes the 64 columns of a chunk
-//                                                                     2: warp group g takes columns [32 g, 32 g + 32) of it
+//   static constexpr int LOAD_WORDS, MAX_REGS;                        words of its row a loader thread has in flight
+//                                                                     (multiple of 8); register cap of the kernel
+//   static constexpr uint32_t GROUPS;                                 1, 2 or 4 epilogue warp groups: group g takes columns
+//                                                                     [g 64/GROUPS, (g + 1) 64/GROUPS) of every chunk
 //   struct Params;                                                    by-value kernel argument
 //   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid, uint32_t grp);
 //   __device__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0);  polynomial (o, i), first coefficient of the tile
-//   __device__ void consume(uint32_t col0, const uint32_t* t);        32 accumulator columns [col0, col0 + 32) of row etid
+//   __device__ void consume(uint32_t col0, const uint32_t* t);        64/GROUPS accumulator columns from col0 on, of row etid
+//                                                                     (GROUPS = 1: called twice per chunk, 32 columns each)
 //   __device__ void end_tile();
 // Warp roles: [0, 4 GROUPS) epilogue, then LOAD_WARPS loaders, then the MMA issuer.
 constexpr uint32_t nthreads(uint32_t groups, uint32_t load_warps) { return (4 * groups + load_warps + 1) * 32; }
@@ -153,10 +179,40 @@ constexpr uint32_t nthreads(uint32_t groups, uint32_t load_warps) { return (4 * 
 // barrier among the epilogue threads only (id 1; id 0 is __syncthreads)
 __device__ __forceinline__ void epi_sync(uint32_t nthr) { asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory"); }
 
+#ifdef PIPE_DBG
+#define PROF_T(v) const long long v = clock64()
+#define PROF_DECL(v) long long v = 0
+#define PROF_SET(v) v = clock64()
+#define PROF_ADD(i, a_, b_) do { if (blockIdx.x == 0) pacc[i] += (b_) - (a_); } while (0)
+#else
+#define PROF_T(v)
+#define PROF_DECL(v)
+#define PROF_SET(v)
+#define PROF_ADD(i, a_, b_)
+#endif
+
+template <int NCOL>
+__device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t* r) {
+  static_assert(NCOL == 16 || NCOL == 32, "epilogue slice");
+  if constexpr (NCOL == 32) {
+    tmem_ld32_nowait(taddr, r);
+  } else {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                   "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(taddr)
+                 : "memory");
+  }
+}
+
 template <class Epi>
-__global__ void __launch_bounds__(nthreads(Epi::GROUPS, Epi::LOAD_WARPS), 1)
+__global__ void __maxnreg__(Epi::MAX_REGS)   // 64 K registers / (warps rounded up to a multiple of 4) / 32
 pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename Epi::Params ep) {
-  constexpr uint32_t EPIW = 4 * Epi::GROUPS, LOAD_WARPS = Epi::LOAD_WARPS, HALVES = LOAD_WARPS / 4, MMAW = EPIW + LOAD_WARPS;
+  constexpr uint32_t GROUPS = Epi::GROUPS, EPIW = 4 * GROUPS, LOAD_WARPS = Epi::LOAD_WARPS, HALVES = LOAD_WARPS / 4,
+                     MMAW = EPIW + LOAD_WARPS, GC = NC / GROUPS;
+  constexpr int LR = Epi::LOAD_WORDS;
+  static_assert((GROUPS == 1 || GROUPS == 2 || GROUPS == 4) && (LOAD_WARPS == 4 || LOAD_WARPS == 8), "pipeline shape");
+  static_assert(((EPIW + LOAD_WARPS + 1 + 3) / 4 * 4) * 32 * Epi::MAX_REGS <= 65536, "one CTA must fit the register file");
   extern __shared__ __align__(1024) uint8_t smem[];
   Ctrl* ctl = reinterpret_cast<Ctrl*>(smem);
   uint8_t* sB = smem + a.b_off;
@@ -165,15 +221,13 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   const uint32_t ntiles = a.npoly * tpp;
   const uint32_t mine = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
   const uint32_t a_cols = a.KB / 4;
-  const uint32_t chunk_bytes = a.KB * NC;
-  const bool resident = a.nslots >= a.nchunks;
-  const uint32_t dmask = a.nD - 1, dshift = a.nD == 4 ? 2 : 1;     // nD in {2, 4}
   const uint32_t amask = a.nA - 1, ashift = a.nA - 1;              // nA in {1, 2}
 
   if (tid == 0) {
     for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], LOAD_WARPS * 32); mbar_init(&ctl->a_free[i], 1); }
-    for (uint32_t i = 0; i < MAX_D; ++i) { mbar_init(&ctl->d_full[i], 1); mbar_init(&ctl->d_free[i], EPIW * 32); }
-    for (uint32_t i = 0; i < MAX_SLOTS; ++i) { mbar_init(&ctl->b_full[i], 1); mbar_init(&ctl->b_free[i], 1); }
+    for (uint32_t i = 0; i < MAX_SPANS; ++i) mbar_init(&ctl->d_full[i], 1);
+    for (uint32_t i = 0; i < MAX_CHUNKS; ++i) mbar_init(&ctl->d_free[i], EPIW * 32);
+    mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
     fence_barrier_init();
   }
   if (warp == MMAW) tmem_alloc(&ctl->tmem_base, a.tmem_cols);
@@ -181,125 +235,187 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_a = ctl->tmem_base;                          // A buffers: columns [0, nA * a_cols)
-  const uint32_t tmem_d = tmem_a + a.nA * a_cols;                  // accumulator ring: nD chunks of NC columns
+  const uint32_t tmem_d = tmem_a + a.nA * a_cols;                  // chunk c of the pass: columns [c * NC, c * NC + NC)
 
   if (warp == MMAW) {
     // ===== MMA issuer (one thread) =====
     if (lane == 0 && mine) {
-      const uint32_t total = mine * a.nchunks;
-      uint32_t ld_slot = 0, ld_chunk = 0, ld_count = 0;            // next chunk to fetch: ring slot, chunk of the image
-      auto load_next = [&]() {
-        mbar_expect_tx(&ctl->b_full[ld_slot], chunk_bytes);
-        bulk_g2s(sB + (size_t)ld_slot * chunk_bytes, a.B + (size_t)ld_chunk * a.chunk_stride, chunk_bytes, &ctl->b_full[ld_slot]);
-        if (++ld_slot == a.nslots) ld_slot = 0;
-        if (++ld_chunk == a.nchunks) ld_chunk = 0;
-        ++ld_count;
-      };
-      const uint32_t pre = total < a.nslots ? total : a.nslots;
-      while (ld_count < pre) load_next();
-      const uint32_t idesc = idesc_u8(NC);
-      const uint32_t lboB = NC * 16;
-      uint32_t g = 0, slot = 0, slot_par = 0;                      // running chunk index, its ring slot and the slot's use parity
-      uint32_t pslot = 0, pslot_par = 0;                           // the same for the previous chunk
-      for (uint32_t k = 0; k < mine; ++k) {
-        const uint32_t abuf = k & amask;
-        mbar_wait(&ctl->a_full[abuf], (k >> ashift) & 1);
-        tc_fence_after();
-        for (uint32_t c = 0; c < a.nchunks; ++c, ++g) {
-          if (!resident || k == 0) mbar_wait(&ctl->b_full[slot], slot_par);
-          const uint32_t dbuf = g & dmask;
-          mbar_wait(&ctl->d_free[dbuf], ((g >> dshift) & 1) ^ 1);
-          tc_fence_after();
-          const uint32_t baddr = smem_u32(sB + (size_t)slot * chunk_bytes);
-          for (uint32_t ks = 0; ks < a.KB / KSTEP; ++ks) {
-            const uint64_t db = smem_desc(baddr + ks * 2 * lboB, lboB, 128);
-            mma_i8_ts(tmem_d + dbuf * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
-          }
-          mma_commit(&ctl->d_full[dbuf]);
-          if (!resident) {
-            mma_commit(&ctl->b_free[slot]);
-            if (g >= 1 && ld_count < total) {                      // the slot of the previous chunk is the next to refill
-              mbar_wait(&ctl->b_free[pslot], pslot_par);
-              load_next();
-            }
-          }
-          pslot = slot; pslot_par = slot_par;
-          if (++slot == a.nslots) { slot = 0; slot_par ^= 1; }
+#ifdef PIPE_DBG
+      long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+      PROF_T(m_start);
+      const uint32_t nkb = a.KB / 16;                              // 16-byte K blocks of the operands
+      uint32_t wi = 0;                                             // work item = (pass, tile) in issue order
+      for (uint32_t ps = 0; ps < a.npass; ++ps) {
+        const uint32_t c0 = ps * a.cpp;
+        const uint32_t nc = a.nchunks - c0 < a.cpp ? a.nchunks - c0 : a.cpp;     // chunks of this pass
+        const uint32_t nspan = (nc + SPAN - 1) / SPAN;
+        // B of the pass: span s as a dense image [nkb][w_s columns][16] at sB + span_off[s]
+        uint32_t span_off[MAX_SPANS], span_w[MAX_SPANS];
+        if (ps > 0) {                                              // the previous pass's MMAs still read sB
+          mma_commit(&ctl->mma_done);
+          mbar_wait(&ctl->mma_done, (ps - 1) & 1);
         }
-        mma_commit(&ctl->a_free[abuf]);
+        {
+          uint32_t off = 0;
+          mbar_expect_tx(&ctl->b_full, nc * NC * a.KB);
+          for (uint32_t sp = 0; sp < nspan; ++sp) {
+            const uint32_t w = ((nc - sp * SPAN < SPAN ? nc - sp * SPAN : SPAN)) * NC;
+            span_off[sp] = off; span_w[sp] = w;
+            const uint8_t* src = a.B + (size_t)(c0 + sp * SPAN) * NC * 16;
+            for (uint32_t kb = 0; kb < nkb; ++kb)
+              bulk_g2s(sB + off + (size_t)kb * w * 16, src + (size_t)kb * a.b_cols * 16, w * 16, &ctl->b_full);
+            off += nkb * w * 16;
+          }
+          mbar_wait(&ctl->b_full, ps & 1);
+        }
+        for (uint32_t k = 0; k < mine; ++k, ++wi) {
+          const uint32_t abuf = wi & amask;
+          PROF_T(m0);
+          mbar_wait(&ctl->a_full[abuf], (wi >> ashift) & 1);
+          tc_fence_after();
+          PROF_T(m1); PROF_ADD(1, m0, m1);
+          for (uint32_t sp = 0; sp < nspan; ++sp) {
+            PROF_T(m2);
+            const uint32_t cs = sp * SPAN, ce = cs + SPAN < nc ? cs + SPAN : nc;
+            for (uint32_t c = cs; c < ce; ++c) mbar_wait(&ctl->d_free[c], (wi & 1) ^ 1);
+            tc_fence_after();
+            PROF_T(m3); PROF_ADD(3, m2, m3);
+            const uint32_t idesc = idesc_u8(span_w[sp]);
+            const uint32_t lbo = span_w[sp] * 16;
+            const uint32_t baddr = smem_u32(sB + span_off[sp]);
+            for (uint32_t ks = 0; ks < a.KB / KSTEP; ++ks) {
+              const uint64_t db = smem_desc(baddr + ks * 2 * lbo, lbo, 128);
+#ifdef PIPE_DBG
+              if (!(a.dbg & 4))
+#endif
+              mma_i8_ts(tmem_d + cs * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
+            }
+            mma_commit(&ctl->d_full[sp]);
+            PROF_T(m4); PROF_ADD(4, m3, m4);
+          }
+          mma_commit(&ctl->a_free[abuf]);
+        }
       }
+#ifdef PIPE_DBG
+      { PROF_T(m_end); PROF_ADD(0, m_start, m_end); if (blockIdx.x == 0) for (int i = 0; i < 8; ++i) a.prof[i] = pacc[i]; }
+#endif
     }
     __syncwarp();
   } else if (warp >= EPIW) {
     // ===== loaders =====
     const uint32_t lw = warp - EPIW, quarter = lw & 3, half = lw >> 2;
     const uint32_t row = quarter * 32 + lane;
-    const uint32_t nbatch = (a_cols + 31) / 32;
-    uint32_t tile = blockIdx.x;
-    uint32_t poly = tile / tpp, tin = tile % tpp;                  // advanced incrementally below
-    const uint32_t dpoly = gridDim.x / tpp, dtin = gridDim.x % tpp;
-    uint32_t po = poly / a.inner, pi = poly % a.inner;
-    for (uint32_t k = 0; k < mine; ++k) {
-      const uint32_t* p = a.src + (size_t)po * a.src_outer + (size_t)pi * a.src_inner + tin * TILE_M + row;
-      const uint32_t abuf = k & amask;
-      const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
-      bool waited = false;
-      for (uint32_t b = half; b < nbatch; b += 2 * HALVES) {       // this warp's batches, two at a time
-        uint32_t w0[32], w1[32];
-        const bool two = b + HALVES < nbatch;
-        load_batch(w0, p, a.N, b, a.nwords);
-        if (two) load_batch(w1, p, a.N, b + HALVES, a.nwords);
-        if (!waited) {                                             // loads are in flight while the buffer is still being read
-          mbar_wait(&ctl->a_free[abuf], ((k >> ashift) & 1) ^ 1);
-          tc_fence_after();
-          waited = true;
+#ifdef PIPE_DBG
+    long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    PROF_T(l_start);
+    uint32_t wi = 0;
+    for (uint32_t ps = 0; ps < a.npass; ++ps) {
+      for (uint32_t k = 0; k < mine; ++k, ++wi) {
+        const uint32_t tile = blockIdx.x + k * gridDim.x;
+        const uint32_t poly = tile / tpp, tin = tile % tpp;
+        const uint32_t po = poly / a.inner, pi = poly % a.inner;
+        const uint32_t* p = a.src + (size_t)po * a.src_outer + (size_t)pi * a.src_inner + tin * TILE_M + row;
+        const uint32_t abuf = wi & amask;
+        const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
+        bool waited = false;
+        for (uint32_t w0 = half * LR; w0 < a_cols; w0 += HALVES * LR) {   // this warp's batches of LR words
+          uint32_t w[LR];
+          PROF_T(l0);
+#ifdef PIPE_DBG
+          if (a.dbg & 2) {
+#pragma unroll
+            for (int i = 0; i < LR; ++i) w[i] = i;
+          } else
+#endif
+          load_batch<LR>(w, p, a.N, w0, a.nwords);
+          PROF_T(l1); PROF_ADD(1, l0, l1);
+          if (!waited) {                                           // loads are in flight while the buffer is still being read
+            mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
+            tc_fence_after();
+            waited = true;
+          }
+          PROF_T(l2); PROF_ADD(2, l1, l2);
+          store_batch<LR>(w, taddr, w0, a_cols, a.mask_bits);
+          PROF_T(l3); PROF_ADD(3, l2, l3);
         }
-        store_batch(w0, taddr, b, a.nwords, a_cols, a.mask_bits);
-        if (two) store_batch(w1, taddr, b + HALVES, a.nwords, a_cols, a.mask_bits);
+        if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
+        PROF_T(l4);
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(&ctl->a_full[abuf]);
+        PROF_T(l5); PROF_ADD(4, l4, l5);
       }
-      if (!waited) mbar_wait(&ctl->a_free[abuf], ((k >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
-      tmem_st_wait();
-      tc_fence_before();
-      mbar_arrive(&ctl->a_full[abuf]);
-      tin += dtin; poly += dpoly;
-      if (tin >= tpp) { tin -= tpp; ++poly; }
-      po = poly / a.inner; pi = poly % a.inner;
     }
+#ifdef PIPE_DBG
+    { PROF_T(l_end); PROF_ADD(0, l_start, l_end); if (blockIdx.x == 0 && lw == 0 && lane == 0) for (int i = 0; i < 8; ++i) a.prof[8 + i] = pacc[i]; }
+#endif
   } else {
     // ===== epilogue =====
     const uint32_t grp = warp >> 2;
     const uint32_t etid = (warp & 3) * 32 + lane;                  // 0..127 = tile row = TMEM lane
     const uint32_t lane_off = ((warp & 3) * 32u) << 16;
     Epi epi(ep, a, smem + a.epi_off, etid, grp);
-    uint32_t g = 0;
-    for (uint32_t k = 0; k < mine; ++k) {
-      const uint32_t tile = blockIdx.x + k * gridDim.x;
-      const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
-      epi.begin_tile(poly / a.inner, poly % a.inner, n0);
-      for (uint32_t c = 0; c < a.nchunks; ++c, ++g) {
-        const uint32_t dbuf = g & dmask;
-        mbar_wait(&ctl->d_full[dbuf], (g >> dshift) & 1);
-        tc_fence_after();
-        if constexpr (Epi::GROUPS == 1) {
-          uint32_t t[64];
-          tmem_ld32_nowait(tmem_d + dbuf * NC + lane_off, t);
-          tmem_ld32_nowait(tmem_d + dbuf * NC + 32 + lane_off, t + 32);
-          tmem_ld_wait();
-          tc_fence_before();
-          mbar_arrive(&ctl->d_free[dbuf]);                         // the accumulator chunk is in registers: hand it back
-          epi.consume(c * NC, t);
-          epi.consume(c * NC + 32, t + 32);
-        } else {
-          uint32_t t[32];
-          tmem_ld32_nowait(tmem_d + dbuf * NC + grp * 32 + lane_off, t);
-          tmem_ld_wait();
-          tc_fence_before();
-          mbar_arrive(&ctl->d_free[dbuf]);
-          epi.consume(c * NC + grp * 32, t);
+#ifdef PIPE_DBG
+    long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+#endif
+    PROF_T(e_start);
+    uint32_t wi = 0;
+    for (uint32_t ps = 0; ps < a.npass; ++ps) {
+      const uint32_t c0 = ps * a.cpp;
+      const uint32_t nc = a.nchunks - c0 < a.cpp ? a.nchunks - c0 : a.cpp;
+      for (uint32_t k = 0; k < mine; ++k, ++wi) {
+        const uint32_t tile = blockIdx.x + k * gridDim.x;
+        const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
+        PROF_T(e0);
+        epi.begin_tile(poly / a.inner, poly % a.inner, n0);
+        PROF_T(e1); PROF_ADD(4, e0, e1);
+        for (uint32_t c = 0; c < nc; ++c) {
+          PROF_T(e2);
+          if (c % SPAN == 0) {
+            mbar_wait(&ctl->d_full[c / SPAN], wi & 1);
+            tc_fence_after();
+          }
+          PROF_T(e3); PROF_ADD(1, e2, e3);
+          if constexpr (GROUPS == 1) {
+            uint32_t t[64];
+            tmem_ld32_nowait(tmem_d + c * NC + lane_off, t);
+            tmem_ld32_nowait(tmem_d + c * NC + 32 + lane_off, t + 32);
+            tmem_ld_wait();
+            tc_fence_before();
+            mbar_arrive(&ctl->d_free[c]);                          // the accumulator chunk is in registers: hand it back
+            PROF_T(e4); PROF_ADD(2, e3, e4);
+#ifdef PIPE_DBG
+            if (!(a.dbg & 1) || t[0] == 0x12345678u)
+#endif
+            {
+              epi.consume((c0 + c) * NC, t);
+              epi.consume((c0 + c) * NC + 32, t + 32);
+            }
+            PROF_T(e5); PROF_ADD(3, e4, e5);
+          } else {
+            uint32_t t[GC];
+            tmem_ld_cols<GC>(tmem_d + c * NC + grp * GC + lane_off, t);
+            tmem_ld_wait();
+            tc_fence_before();
+            mbar_arrive(&ctl->d_free[c]);
+            PROF_T(e4); PROF_ADD(2, e3, e4);
+#ifdef PIPE_DBG
+            if (!(a.dbg & 1) || t[0] == 0x12345678u)
+#endif
+            epi.consume((c0 + c) * NC + grp * GC, t);
+            PROF_T(e5); PROF_ADD(3, e4, e5);
+          }
         }
+        PROF_T(e6);
+        epi.end_tile();
+        PROF_T(e7); PROF_ADD(4, e6, e7);
       }
-      epi.end_tile();
     }
+#ifdef PIPE_DBG
+    { PROF_T(e_end); PROF_ADD(0, e_start, e_end); if (blockIdx.x == 0 && warp == 0 && lane == 0) for (int i = 0; i < 8; ++i) a.prof[16 + i] = pacc[i]; }
+#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -307,16 +423,34 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
 }
 
 template <class Epi>
-inline cudaError_t launch_pipe(const PipeArgs& a, const typename Epi::Params& ep, size_t smem, int n_sm, cudaStream_t s) {
+inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params& ep, size_t smem, int n_sm, cudaStream_t s) {
   static size_t configured = 0;
   if (smem > configured) {
     cudaError_t e = cudaFuncSetAttribute(pipe_kernel<Epi>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = smem;
   }
+  PipeArgs a = a_in;
+#ifdef PIPE_DBG
+  static unsigned long long* d_prof = nullptr;
+  if (!d_prof) cudaMalloc(&d_prof, 24 * 8);
+  cudaMemsetAsync(d_prof, 0, 24 * 8, s);
+  a.dbg = getenv("PIPE_DBG") ? atoi(getenv("PIPE_DBG")) : 0;
+  a.prof = d_prof;
+#endif
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);
   const uint32_t grid = ntiles < (uint32_t)n_sm ? ntiles : (uint32_t)n_sm;
   pipe_kernel<Epi><<<grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s>>>(a, ep);
+#ifdef PIPE_DBG
+  if (getenv("PIPE_PROF")) {
+    unsigned long long h[24];
+    cudaStreamSynchronize(s);
+    cudaMemcpy(h, d_prof, sizeof(h), cudaMemcpyDeviceToHost);
+    const uint32_t per = (ntiles + grid - 1) / grid;
+    fprintf(stderr, "[pipe groups %u npoly %u nwords %u nchunks %u npass %u cpp %u nA %u tiles/cta %u]\n  mma: total %llu a_full %llu d_free %llu issue %llu\n  load: total %llu issue %llu a_free %llu store %llu stwait %llu\n  epi: total %llu d_full %llu ld %llu consume %llu tile %llu\n",
+            Epi::GROUPS, a.npoly, a.nwords, a.nchunks, a.npass, a.cpp, a.nA, per, h[0], h[1], h[3], h[4], h[8], h[9], h[10], h[11], h[12], h[16], h[17], h[18], h[19], h[20]);
+  }
+#endif
   return cudaGetLastError();
 }
 #endif  // __CUDACC__
