@@ -121,6 +121,7 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 struct CrtEpi {
   static constexpr int LOAD_WORDS = 64, MAX_REGS = 128;    // 13 warps are allocated as 16: 16 x 32 x 128 = 64 K
   static constexpr uint32_t GROUPS = 1, LOAD_WARPS = 8;
+  static constexpr bool LOAD_ALT = false;
   struct Params {
     uint32_t* out; size_t out_outer, out_inner;
     const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr

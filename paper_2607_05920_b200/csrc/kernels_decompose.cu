@@ -17,8 +17,9 @@ namespace fhe {
 // is at most 20 short (the shifted-out bits of T1, T2 and T0 >> 21 < 16), and one Barrett step: qh = mulhi(vh, mu) is
 // floor(v / q) or one less (20 * 2^21 / q < 0.16 for q > 2^28), so the 32-bit remainder lies in [0, 2q).
 struct DecEpi {
-  static constexpr int LOAD_WORDS = 40, MAX_REGS = 80;   // 21 warps are allocated as 24: 24 x 32 x 80 <= 64 K
-  static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 4;
+  static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
+  static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
+  static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: the loaders' round trip bounds S1
   static constexpr int PPG = 16 / GROUPS;                // primes per group and chunk
   struct Params {
     uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
@@ -70,7 +71,7 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
   const uint32_t KB = (4 * eff + 31) / 32 * 32;
   if (KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
   const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2), false);
-  if (!plan.ok) return cudaErrorInvalidConfiguration;
+  if (!plan.ok || plan.nA != 2) return cudaErrorInvalidConfiguration;
   pipe::PipeArgs a;
   a.src = d_limbs; a.src_outer = limb_outer; a.src_inner = limb_inner;
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = eff; a.mask_bits = mask_bits;

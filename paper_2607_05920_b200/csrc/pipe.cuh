@@ -24,9 +24,6 @@
 // When the constant matrix has more columns than that (or than shared memory holds), the launch runs several passes over
 // its tiles, pass p with columns [p * cpp * 64, ...) of B resident in shared memory (loaded once per pass per CTA).
 #pragma once
-#include <cstdio>
-#include <cstdlib>
-
 #include "umma.cuh"
 
 namespace fhe {
@@ -60,9 +57,6 @@ struct PipeArgs {
   uint32_t KB, nchunks;
   uint32_t npass, cpp;                        // passes over the tiles, chunks per pass (the last pass may have fewer)
   uint32_t nA, tmem_cols;
-#ifdef PIPE_DBG
-  uint32_t dbg; unsigned long long* prof;
-#endif
   uint32_t epi_off, b_off;                    // byte offsets of the epilogue scratch and of B in dynamic smem
 };
 
@@ -163,6 +157,9 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 // ---- the kernel -------------------------------------------------------------------------------------------------------------
 // Epi: struct with
 //   static constexpr uint32_t LOAD_WARPS;                             4 or 8 loader warps (one or two per TMEM lane quarter)
+//   static constexpr bool LOAD_ALT;                                   8 loader warps only.  false: the two warps of a lane quarter
+//                                                                     split the words of every tile; true: they take alternate
+//                                                                     tiles whole (two tiles' loads in flight; needs nA = 2)
 //   static constexpr int LOAD_WORDS, MAX_REGS;                        words of its row a loader thread has in flight
 //                                                                     (multiple of 8); register cap of the kernel
 //   static constexpr uint32_t GROUPS;                                 1, 2 or 4 epilogue warp groups: group g takes columns
@@ -179,17 +176,6 @@ constexpr uint32_t nthreads(uint32_t groups, uint32_t load_warps) { return (4 * 
 // barrier among the epilogue threads only (id 1; id 0 is __syncthreads)
 __device__ __forceinline__ void epi_sync(uint32_t nthr) { asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory"); }
 
-#ifdef PIPE_DBG
-#define PROF_T(v) const long long v = clock64()
-#define PROF_DECL(v) long long v = 0
-#define PROF_SET(v) v = clock64()
-#define PROF_ADD(i, a_, b_) do { if (blockIdx.x == 0) pacc[i] += (b_) - (a_); } while (0)
-#else
-#define PROF_T(v)
-#define PROF_DECL(v)
-#define PROF_SET(v)
-#define PROF_ADD(i, a_, b_)
-#endif
 
 template <int NCOL>
 __device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t* r) {
@@ -211,6 +197,8 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   constexpr uint32_t GROUPS = Epi::GROUPS, EPIW = 4 * GROUPS, LOAD_WARPS = Epi::LOAD_WARPS, HALVES = LOAD_WARPS / 4,
                      MMAW = EPIW + LOAD_WARPS, GC = NC / GROUPS;
   constexpr int LR = Epi::LOAD_WORDS;
+  constexpr bool ALT = Epi::LOAD_ALT;
+  static_assert(!ALT || LOAD_WARPS == 8, "alternating loaders come in pairs");
   static_assert((GROUPS == 1 || GROUPS == 2 || GROUPS == 4) && (LOAD_WARPS == 4 || LOAD_WARPS == 8), "pipeline shape");
   static_assert(((EPIW + LOAD_WARPS + 1 + 3) / 4 * 4) * 32 * Epi::MAX_REGS <= 65536, "one CTA must fit the register file");
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -224,7 +212,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   const uint32_t amask = a.nA - 1, ashift = a.nA - 1;              // nA in {1, 2}
 
   if (tid == 0) {
-    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], LOAD_WARPS * 32); mbar_init(&ctl->a_free[i], 1); }
+    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], (ALT ? 4 : LOAD_WARPS) * 32); mbar_init(&ctl->a_free[i], 1); }
     for (uint32_t i = 0; i < MAX_SPANS; ++i) mbar_init(&ctl->d_full[i], 1);
     for (uint32_t i = 0; i < MAX_CHUNKS; ++i) mbar_init(&ctl->d_free[i], EPIW * 32);
     mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
@@ -240,10 +228,6 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   if (warp == MMAW) {
     // ===== MMA issuer (one thread) =====
     if (lane == 0 && mine) {
-#ifdef PIPE_DBG
-      long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-      PROF_T(m_start);
       const uint32_t nkb = a.KB / 16;                              // 16-byte K blocks of the operands
       uint32_t wi = 0;                                             // work item = (pass, tile) in issue order
       for (uint32_t ps = 0; ps < a.npass; ++ps) {
@@ -271,48 +255,34 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         }
         for (uint32_t k = 0; k < mine; ++k, ++wi) {
           const uint32_t abuf = wi & amask;
-          PROF_T(m0);
           mbar_wait(&ctl->a_full[abuf], (wi >> ashift) & 1);
           tc_fence_after();
-          PROF_T(m1); PROF_ADD(1, m0, m1);
           for (uint32_t sp = 0; sp < nspan; ++sp) {
-            PROF_T(m2);
             const uint32_t cs = sp * SPAN, ce = cs + SPAN < nc ? cs + SPAN : nc;
             for (uint32_t c = cs; c < ce; ++c) mbar_wait(&ctl->d_free[c], (wi & 1) ^ 1);
             tc_fence_after();
-            PROF_T(m3); PROF_ADD(3, m2, m3);
             const uint32_t idesc = idesc_u8(span_w[sp]);
             const uint32_t lbo = span_w[sp] * 16;
             const uint32_t baddr = smem_u32(sB + span_off[sp]);
             for (uint32_t ks = 0; ks < a.KB / KSTEP; ++ks) {
               const uint64_t db = smem_desc(baddr + ks * 2 * lbo, lbo, 128);
-#ifdef PIPE_DBG
-              if (!(a.dbg & 4))
-#endif
               mma_i8_ts(tmem_d + cs * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
             }
             mma_commit(&ctl->d_full[sp]);
-            PROF_T(m4); PROF_ADD(4, m3, m4);
           }
           mma_commit(&ctl->a_free[abuf]);
         }
       }
-#ifdef PIPE_DBG
-      { PROF_T(m_end); PROF_ADD(0, m_start, m_end); if (blockIdx.x == 0) for (int i = 0; i < 8; ++i) a.prof[i] = pacc[i]; }
-#endif
     }
     __syncwarp();
   } else if (warp >= EPIW) {
     // ===== loaders =====
     const uint32_t lw = warp - EPIW, quarter = lw & 3, half = lw >> 2;
     const uint32_t row = quarter * 32 + lane;
-#ifdef PIPE_DBG
-    long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    PROF_T(l_start);
     uint32_t wi = 0;
     for (uint32_t ps = 0; ps < a.npass; ++ps) {
       for (uint32_t k = 0; k < mine; ++k, ++wi) {
+        if (ALT && (wi & 1) != half) continue;
         const uint32_t tile = blockIdx.x + k * gridDim.x;
         const uint32_t poly = tile / tpp, tin = tile % tpp;
         const uint32_t po = poly / a.inner, pi = poly % a.inner;
@@ -320,47 +290,28 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         const uint32_t abuf = wi & amask;
         const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
         bool waited = false;
-        for (uint32_t w0 = half * LR; w0 < a_cols; w0 += HALVES * LR) {   // this warp's batches of LR words
+        for (uint32_t w0 = ALT ? 0 : half * LR; w0 < a_cols; w0 += (ALT ? 1 : HALVES) * LR) {   // this warp's batches of LR words
           uint32_t w[LR];
-          PROF_T(l0);
-#ifdef PIPE_DBG
-          if (a.dbg & 2) {
-#pragma unroll
-            for (int i = 0; i < LR; ++i) w[i] = i;
-          } else
-#endif
           load_batch<LR>(w, p, a.N, w0, a.nwords);
-          PROF_T(l1); PROF_ADD(1, l0, l1);
           if (!waited) {                                           // loads are in flight while the buffer is still being read
             mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
             tc_fence_after();
             waited = true;
           }
-          PROF_T(l2); PROF_ADD(2, l1, l2);
           store_batch<LR>(w, taddr, w0, a_cols, a.mask_bits);
-          PROF_T(l3); PROF_ADD(3, l2, l3);
         }
         if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
-        PROF_T(l4);
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&ctl->a_full[abuf]);
-        PROF_T(l5); PROF_ADD(4, l4, l5);
       }
     }
-#ifdef PIPE_DBG
-    { PROF_T(l_end); PROF_ADD(0, l_start, l_end); if (blockIdx.x == 0 && lw == 0 && lane == 0) for (int i = 0; i < 8; ++i) a.prof[8 + i] = pacc[i]; }
-#endif
   } else {
     // ===== epilogue =====
     const uint32_t grp = warp >> 2;
     const uint32_t etid = (warp & 3) * 32 + lane;                  // 0..127 = tile row = TMEM lane
     const uint32_t lane_off = ((warp & 3) * 32u) << 16;
     Epi epi(ep, a, smem + a.epi_off, etid, grp);
-#ifdef PIPE_DBG
-    long long pacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-#endif
-    PROF_T(e_start);
     uint32_t wi = 0;
     for (uint32_t ps = 0; ps < a.npass; ++ps) {
       const uint32_t c0 = ps * a.cpp;
@@ -368,16 +319,12 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
       for (uint32_t k = 0; k < mine; ++k, ++wi) {
         const uint32_t tile = blockIdx.x + k * gridDim.x;
         const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
-        PROF_T(e0);
         epi.begin_tile(poly / a.inner, poly % a.inner, n0);
-        PROF_T(e1); PROF_ADD(4, e0, e1);
         for (uint32_t c = 0; c < nc; ++c) {
-          PROF_T(e2);
           if (c % SPAN == 0) {
             mbar_wait(&ctl->d_full[c / SPAN], wi & 1);
             tc_fence_after();
           }
-          PROF_T(e3); PROF_ADD(1, e2, e3);
           if constexpr (GROUPS == 1) {
             uint32_t t[64];
             tmem_ld32_nowait(tmem_d + c * NC + lane_off, t);
@@ -385,37 +332,22 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
             tmem_ld_wait();
             tc_fence_before();
             mbar_arrive(&ctl->d_free[c]);                          // the accumulator chunk is in registers: hand it back
-            PROF_T(e4); PROF_ADD(2, e3, e4);
-#ifdef PIPE_DBG
-            if (!(a.dbg & 1) || t[0] == 0x12345678u)
-#endif
             {
               epi.consume((c0 + c) * NC, t);
               epi.consume((c0 + c) * NC + 32, t + 32);
             }
-            PROF_T(e5); PROF_ADD(3, e4, e5);
           } else {
             uint32_t t[GC];
             tmem_ld_cols<GC>(tmem_d + c * NC + grp * GC + lane_off, t);
             tmem_ld_wait();
             tc_fence_before();
             mbar_arrive(&ctl->d_free[c]);
-            PROF_T(e4); PROF_ADD(2, e3, e4);
-#ifdef PIPE_DBG
-            if (!(a.dbg & 1) || t[0] == 0x12345678u)
-#endif
             epi.consume((c0 + c) * NC + grp * GC, t);
-            PROF_T(e5); PROF_ADD(3, e4, e5);
           }
         }
-        PROF_T(e6);
         epi.end_tile();
-        PROF_T(e7); PROF_ADD(4, e6, e7);
       }
     }
-#ifdef PIPE_DBG
-    { PROF_T(e_end); PROF_ADD(0, e_start, e_end); if (blockIdx.x == 0 && warp == 0 && lane == 0) for (int i = 0; i < 8; ++i) a.prof[16 + i] = pacc[i]; }
-#endif
   }
   tc_fence_before();
   __syncthreads();
@@ -431,26 +363,9 @@ inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params&
     configured = smem;
   }
   PipeArgs a = a_in;
-#ifdef PIPE_DBG
-  static unsigned long long* d_prof = nullptr;
-  if (!d_prof) cudaMalloc(&d_prof, 24 * 8);
-  cudaMemsetAsync(d_prof, 0, 24 * 8, s);
-  a.dbg = getenv("PIPE_DBG") ? atoi(getenv("PIPE_DBG")) : 0;
-  a.prof = d_prof;
-#endif
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);
   const uint32_t grid = ntiles < (uint32_t)n_sm ? ntiles : (uint32_t)n_sm;
   pipe_kernel<Epi><<<grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s>>>(a, ep);
-#ifdef PIPE_DBG
-  if (getenv("PIPE_PROF")) {
-    unsigned long long h[24];
-    cudaStreamSynchronize(s);
-    cudaMemcpy(h, d_prof, sizeof(h), cudaMemcpyDeviceToHost);
-    const uint32_t per = (ntiles + grid - 1) / grid;
-    fprintf(stderr, "[pipe groups %u npoly %u nwords %u nchunks %u npass %u cpp %u nA %u tiles/cta %u]\n  mma: total %llu a_full %llu d_free %llu issue %llu\n  load: total %llu issue %llu a_free %llu store %llu stwait %llu\n  epi: total %llu d_full %llu ld %llu consume %llu tile %llu\n",
-            Epi::GROUPS, a.npoly, a.nwords, a.nchunks, a.npass, a.cpp, a.nA, per, h[0], h[1], h[3], h[4], h[8], h[9], h[10], h[11], h[12], h[16], h[17], h[18], h[19], h[20]);
-  }
-#endif
   return cudaGetLastError();
 }
 #endif  // __CUDACC__
