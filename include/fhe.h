@@ -121,9 +121,12 @@ fhe_status fhe_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, ui
 fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct1, const uint32_t* d_ct2,
                                   uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
 
-/* Same computation as fhe_mult_relin_rescale with HOST buffers (pageable or pinned): copies the inputs to the
- * device, runs, copies the result back and synchronises `stream`.  d_ws must additionally hold the device copies:
- * fhe_workspace_bytes(op) + 3 ciphertext batches.  Used for the end-to-end ("e2e") measurement. */
+/* Same computation as fhe_mult_relin_rescale with HOST buffers (pageable or pinned; pinned for full PCIe speed):
+ * copies the inputs to the device, runs, copies the result back and returns when h_out2 is complete (`stream` and the
+ * context's two copy streams are synchronised).  Batch items are independent, so the call is pipelined item by item:
+ * the host->device copy of item i + 1, the kernels of item i (on `stream`) and the device->host copy of item i - 1
+ * overlap.  d_ws must additionally hold the device copies: fhe_workspace_bytes(op) + 3 ciphertext batches.  Used for
+ * the end-to-end ("e2e") measurement. */
 fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uint32_t* h_ct1, const uint32_t* h_ct2,
                                        uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
 

@@ -185,12 +185,33 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
   cudaStream_t s = (cudaStream_t)stream;
   char* base = (char*)d_ws + inner;
   uint32_t* d1 = (uint32_t*)base; uint32_t* d2 = (uint32_t*)(base + ctb); uint32_t* d_o = (uint32_t*)(base + 2 * ctb);
-  const size_t bytes = (size_t)batch * 2 * c->L * c->N * 4;
-  CK(cudaMemcpyAsync(d1, h_ct1, bytes, cudaMemcpyHostToDevice, s), "H2D ct1");
-  CK(cudaMemcpyAsync(d2, h_ct2, bytes, cudaMemcpyHostToDevice, s), "H2D ct2");
-  fhe_status st = fhe_mult_relin_rescale(ctx, d_o, d1, d2, p_bits, batch, d_ws, inner, stream);
-  if (st != FHE_OK) return st;
-  CK(cudaMemcpyAsync(h_out2, d_o, bytes, cudaMemcpyDeviceToHost, s), "D2H out");
+  // Batch items are independent, so the call is pipelined in pieces of `per` items over three streams: piece i + 1 is
+  // on its way to the device (copy stream) while piece i runs on the caller's stream and piece i - 1 goes back to
+  // the host (second copy stream): the PCIe transfers of both directions overlap each other and the kernels.
+  const uint32_t per = (batch + Context::HOST_PIECES - 1) / Context::HOST_PIECES;
+  const uint32_t pieces = (batch + per - 1) / per;
+  const size_t item_words = (size_t)2 * c->L * c->N;
+  CK(cudaEventRecord(c->ev_start, s), "event");
+  CK(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0), "wait");          // the staging buffers are free once `s` gets here
+  CK(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0), "wait");
+  for (uint32_t i = 0; i < pieces; ++i) {
+    const uint32_t b0 = i * per, nb = batch - b0 < per ? batch - b0 : per;
+    const size_t off = (size_t)b0 * item_words, bytes = (size_t)nb * item_words * 4;
+    CK(cudaMemcpyAsync(d1 + off, h_ct1 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct1");
+    CK(cudaMemcpyAsync(d2 + off, h_ct2 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct2");
+    CK(cudaEventRecord(c->ev_in[i], c->s_h2d), "event");
+  }
+  for (uint32_t i = 0; i < pieces; ++i) {
+    const uint32_t b0 = i * per, nb = batch - b0 < per ? batch - b0 : per;
+    const size_t off = (size_t)b0 * item_words, bytes = (size_t)nb * item_words * 4;
+    CK(cudaStreamWaitEvent(s, c->ev_in[i], 0), "wait");
+    fhe_status st = fhe_mult_relin_rescale(ctx, d_o + off, d1 + off, d2 + off, p_bits, nb, d_ws, inner, stream);
+    if (st != FHE_OK) return st;
+    CK(cudaEventRecord(c->ev_done[i], s), "event");
+    CK(cudaStreamWaitEvent(c->s_d2h, c->ev_done[i], 0), "wait");
+    CK(cudaMemcpyAsync(h_out2 + off, d_o + off, bytes, cudaMemcpyDeviceToHost, c->s_d2h), "D2H out");
+  }
+  CK(cudaStreamSynchronize(c->s_d2h), "sync");
   CK(cudaStreamSynchronize(s), "sync");
   return FHE_OK;
 }

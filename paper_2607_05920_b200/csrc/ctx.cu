@@ -167,6 +167,13 @@ static void destroy(Context* c) {
   for (void* p : c->allocs) cudaFree(p);
   if (c->d_evk_hat) cudaFree(c->d_evk_hat);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
+  if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
+  if (c->ev_start) cudaEventDestroy(c->ev_start);
+  for (int i = 0; i < Context::HOST_PIECES; ++i) {
+    if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
+    if (c->ev_done[i]) cudaEventDestroy(c->ev_done[i]);
+  }
   delete c;
 }
 
@@ -184,6 +191,13 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming);
+  for (int i = 0; i < Context::HOST_PIECES && e == cudaSuccess; ++i) {
+    e = cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[i], cudaEventDisableTiming);
+  }
   if (e != cudaSuccess) { std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "no CUDA device: " + m); }
 
   const BigU Q = make_modulus(logQ, t), P = make_modulus(logP, t);

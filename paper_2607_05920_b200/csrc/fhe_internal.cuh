@@ -76,6 +76,10 @@ struct Context {
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
   bool have_evk = false;
+  // copy streams and events of the host-buffer entry point (created with the context; the hot path creates nothing)
+  static constexpr int HOST_PIECES = 32;
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  cudaEvent_t ev_start = nullptr, ev_in[HOST_PIECES] = {}, ev_done[HOST_PIECES] = {};
   // bookkeeping
   mutable std::string err;
   uint64_t launches = 0;
