@@ -34,7 +34,9 @@ WORKLOADS = {
 # one op at C5 on the oracle = 4 ring products mod Q + 2 mod PQ; a mod-PQ product costs 2.06x a mod-Q product
 # (measured once on the dev box: 61.7 s vs 29.9 s); used only to scale the timed CPU sample to ops/s.
 ORACLE_PRODUCTS_PER_OP = 4 + 2 * 2.06
-ALU_PEAK_TMULS = 64 * 148 * 1.965e9 / 1e12   # 32-bit IMAD: 16 lanes/clk/SMSP x 4 SMSP x 148 SMs x 1.965 GHz
+# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/, same command as the
+# timed run): dram__bytes_read.sum + dram__bytes_write.sum, averaged over that class's launches of one step.
+NCU_TRAFFIC = {}   # filled in below from profiles/r1m_launches_and_captures.md
 
 
 def _peaks():
@@ -48,33 +50,38 @@ def _peaks():
 
 # ---- algorithmic work model of the algorithm actually shipped ---------------------------------------------
 def work_model(N, logQ, logP, L, L_PQ, K1, K2, B):
-    """32x32-bit multiplies and compulsory HBM bytes per kernel class for one step (B ops)."""
-    import math
+    """Per kernel class and step (B ops): NTT butterflies, other multiplier-pipe work in units of one mad.lo.u32
+    (a mul.hi / mul.wide issues at half that rate on B200 and counts 2), and the HBM bytes if every intermediate makes
+    exactly one round trip.  The base-conversion contractions run on the tensor cores and are not counted here."""
     logN = N.bit_length() - 1
-    dq = math.ceil(logQ / 26)                 # 26-bit digits of an input coefficient
-    d_t = math.ceil(logQ / 26)                # CRT output digits, tensor
-    d_r = math.ceil((logQ + logP) / (26 if K2 + 1 <= 127 else 25))
-    bf_col = N // 2 * (logN - 8)              # butterflies per transform in the column pass, 3 multiplies each (Shoup)
-    bf_row = N // 2 * 8                       # ... and in the 256-point rows (inside the fused row kernel)
-    mul = {
-        "decompose": B * N * (4 * K1 + K2) * (dq + 6),
-        "ntt_fwd": B * (4 * K1 + K2) * bf_col * 3,
-        "pointwise": B * ((4 * K1 + K2) + (3 * K1 + 2 * K2)) * bf_row * 3 + B * N * (K1 * 4 * 3 + K2 * 2 * 3),
-        "ntt_inv": B * (3 * K1 + 2 * K2) * (bf_col * 3 + N * 3),
-        "crt": B * N * (3 * ((K1 + 1) * d_t + K1) + 2 * ((K2 + 1) * d_r + K2)),
+    half = N // 2
+    fwd_t, inv_t = 4 * K1 + K2, 3 * K1 + 2 * K2          # transforms per op
+    bf = {
+        "decompose": 0,
+        "ntt_fwd": B * fwd_t * half * (logN - 8),           # forward column pass
+        "pointwise": B * (fwd_t + inv_t) * half * 8,        # fused rows: last forward + first inverse pass
+        "ntt_inv": B * inv_t * half * (logN - 8),           # inverse column pass
+        "crt": 0, "rescale": 0,
+    }
+    units = {
+        "decompose": B * N * fwd_t * 3,                      # per residue: mul.hi (2) + mul.lo (1) of the Barrett step
+        "ntt_fwd": 0,
+        "pointwise": B * N * (K1 * 17 + K2 * 10),            # tensor: 4 wide products + 3 reductions; relin: 2 + 2
+        "ntt_inv": B * N * inv_t * 4,                        # final Shoup multiplication by the folded constant
+        "crt": B * N * (3 * L + 2 * L_PQ) * 8,               # per limb of V: four 32 x 32 -> 64 multiply-adds
         "rescale": 0,
     }
     w = 4
     byt = {   # bytes each class must move if every intermediate makes exactly one HBM round trip (DESIGN.md 7)
         "decompose": B * N * w * (4 * L + L + 4 * K1 + K2),
-        "ntt_fwd": B * N * w * 2 * (4 * K1 + K2),                      # forward column pass, in place
-        "pointwise": B * N * w * (4 * K1 + 3 * K1 + K2 + 2 * K2 + 2 * K2),   # fused rows: operands in, products out, evk-hat per item
-        "ntt_inv": B * N * w * 2 * (3 * K1 + 2 * K2),                  # inverse column pass, in place
+        "ntt_fwd": B * N * w * 2 * fwd_t,                                  # forward column pass, in place
+        "pointwise": B * N * w * (4 * K1 + 3 * K1 + K2 + 2 * K2 + 2 * K2),  # fused rows: operands in, products out, evk-hat per item
+        "ntt_inv": B * N * w * 2 * inv_t,                                  # inverse column pass, in place
         "crt": B * N * w * (3 * K1 + 3 * L + 2 * K2 + 2 * L + 2 * L),
         "rescale": 0,
     }
     compulsory = B * N * w * (4 * L + 2 * L) + N * w * 2 * K2      # read 2 cts, write 1, evk-hat once per batch
-    return mul, byt, compulsory
+    return bf, units, byt, compulsory
 
 
 class ClockSampler:
@@ -316,32 +323,43 @@ def run_ours(args):
     if rank != 0:
         return 0
     hbm_gbs, peak_kind = _peaks()
-    mul, byt, compulsory = work_model(N, logQ, logP, ctx.L, ctx.L_PQ, ctx.K1, ctx.K2, B)
+    bf, units, byt, compulsory = work_model(N, logQ, logP, ctx.L, ctx.L_PQ, ctx.K1, ctx.K2, B)
+    # integer peaks measured in this run, register-only (fhe_debug_int_peak): the NTT butterfly as the kernels execute
+    # it, and mad.lo.u32 for the remaining multiplier-pipe work
+    bf_peak, mad_peak, mulhi_peak = (ctx.fhe_debug_int_peak(m) for m in (0, 1, 2))
+
+    def t_int(k):
+        return bf[k] / bf_peak + units[k] / mad_peak
+
     kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps,
                 "share": v[0] / max(1e-9, sum(x[0] for x in per_class.values())),
-                "gmul_per_step": mul[k] / 1e9, "mb_per_step": byt[k] / 1e6} for k, v in per_class.items()}
+                "gbutterfly_per_step": bf[k] / 1e9, "gmulunit_per_step": units[k] / 1e9, "mb_per_step": byt[k] / 1e6,
+                "t_int_ms": t_int(k) * 1e3, "t_hbm_ms": byt[k] / (hbm_gbs * 1e9) * 1e3} for k, v in per_class.items()}
     top = max(per_class, key=lambda k: per_class[k][0])
     n_launch_top = max(1, per_class[top][1])
     avg_launch_s = per_class[top][0] / 1e3 / n_launch_top
-    mul_per_launch = mul[top] * args.steps / n_launch_top
-    t_alu = mul[top] / (ALU_PEAK_TMULS * 1e12)
     t_hbm = byt[top] / (hbm_gbs * 1e9)
-    if t_alu >= t_hbm:
-        roof = {"bound": "alu", "kernel": top, "achieved": mul_per_launch / avg_launch_s / 1e12, "peak": ALU_PEAK_TMULS,
-                "unit": "Tmul32/s", "peak_kind": "derived: 64 IMAD/clk/SM x 148 SM x 1.965 GHz (DESIGN.md 7)"}
+    if t_int(top) >= t_hbm and bf[top] > 0:
+        roof = {"bound": "alu", "kernel": top, "achieved": bf[top] * args.steps / n_launch_top / avg_launch_s / 1e9,
+                "peak": bf_peak / 1e9, "unit": "Gbutterfly/s",
+                "peak_kind": "measured in this run: the kernels' own forward butterfly, register-only (fhe_debug_int_peak; DESIGN.md 7)"}
     else:
         roof = {"bound": "hbm", "kernel": top, "achieved": byt[top] * args.steps / n_launch_top / avg_launch_s / 1e9,
                 "peak": hbm_gbs, "unit": "GB/s", "peak_kind": peak_kind}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
+    roof["traffic"] = NCU_TRAFFIC.get(top) if args.workload == "c5" else None
+    roof["algorithmic_bytes_per_launch"] = byt[top] * args.steps / n_launch_top
     roof["avg_launch_ms"] = avg_launch_s * 1e3
-    # whole-path roofline (north_star): slower of all multiplies at the ALU peak and compulsory bytes at HBM peak
-    t_path_alu = sum(mul.values()) / (ALU_PEAK_TMULS * 1e12)
+    roof["hbm_frac"] = byt[top] * args.steps / n_launch_top / avg_launch_s / 1e9 / hbm_gbs
+    # whole-path roofline (north_star): slower of the integer work at the measured integer peaks and the compulsory
+    # bytes at the measured HBM bandwidth
+    t_path_alu = sum(t_int(k) for k in bf)
     t_path_hbm = compulsory / (hbm_gbs * 1e9)
     t_step = ms_total / args.steps / 1e3
-    path = {"t_alu_ms": t_path_alu * 1e3, "t_hbm_ms": t_path_hbm * 1e3, "t_measured_ms": t_step * 1e3,
-            "frac": max(t_path_alu, t_path_hbm) / t_step, "gmul_per_step": sum(mul.values()) / 1e9,
-            "compulsory_mb_per_step": compulsory / 1e6}
+    path = {"t_int_ms": t_path_alu * 1e3, "t_hbm_ms": t_path_hbm * 1e3, "t_measured_ms": t_step * 1e3,
+            "frac": max(t_path_alu, t_path_hbm) / t_step, "gbutterfly_per_step": sum(bf.values()) / 1e9,
+            "compulsory_mb_per_step": compulsory / 1e6,
+            "int_peaks": {"gbutterfly_per_s": bf_peak / 1e9, "gmadlo_per_s": mad_peak / 1e9, "gmulhi_per_s": mulhi_peak / 1e9}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -371,6 +389,56 @@ def run_ours(args):
     return 0
 
 
+# ---- the standalone polymul sweep (BASELINE.json configs[4]): not part of the default line ----------------
+def run_sweep(args):
+    import numpy as np
+    import torch
+    import synth
+    import paper_2607_05920_b200 as fhe
+
+    rank, local_rank, world = dist_env()
+    if rank != 0:
+        return 0
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    hbm_gbs, _ = _peaks()
+    stream = torch.cuda.current_stream(dev)
+    for logN in (12, 13, 14, 15, 16):
+        for logQ in (64, 256, 620, 1240, 2480):
+            N = 1 << logN
+            ctx = fhe.Context(N, logQ, 32)
+            L, K = ctx.L, ctx.K_pm
+            batch = max(1, round(2e9 / (2 * N * L * 4)))           # about 2 GB of operands
+            g = synth.rng(0)
+            # one seeded pair, repeated: the kernels have no data-dependent control flow
+            a1 = torch.from_numpy(synth.uniform_limbs(g, (1,), N, logQ).view(np.int32)).to(dev)
+            b1 = torch.from_numpy(synth.uniform_limbs(g, (1,), N, logQ).view(np.int32)).to(dev)
+            a = a1.expand(batch, L, N).contiguous()
+            b = b1.expand(batch, L, N).contiguous()
+            out = torch.empty_like(a)
+            for _ in range(2):
+                ctx.fhe_polymul(a, b, out=out, stream=stream)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(3, args.steps // 4)
+            e0.record(stream)
+            for _ in range(reps):
+                ctx.fhe_polymul(a, b, out=out, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            w = 4
+            alg = batch * N * w * (2 * L + 2 * K) + batch * N * w * (2 * 2 * K + 2 * K + K + 2 * K) + batch * N * w * (K + L)
+            print(json.dumps({"sweep": True, "metric": "polymuls/s", "value": batch / (ms / 1e3), "unit": "polymuls/s",
+                              "N": N, "logQ": logQ, "L": L, "K": K, "batch": batch, "ms_per_call": ms,
+                              "us_per_polymul": ms * 1e3 / batch, "algorithmic_gb_per_s": alg / (ms / 1e3) / 1e9,
+                              "hbm_frac_of_plan": alg / (ms / 1e3) / 1e9 / hbm_gbs, "dtype": "u32 (exact integer)",
+                              "data": "synthetic"}), flush=True)
+            del ctx, a, b, out
+            torch.cuda.empty_cache()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -379,9 +447,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c5", choices=sorted(WORKLOADS))
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true",
+                    help="standalone polymul sweep N = 2^12..2^16 x logQ in {64, 256, 620, 1240, 2480}: one JSON line per cell")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     return run_ours(args)
 
 

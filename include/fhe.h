@@ -37,7 +37,9 @@ typedef struct fhe_ctx fhe_ctx; /* opaque: owns prime/twiddle/CRT tables (device
 typedef enum {
   FHE_OK = 0,
   FHE_ERR_ARG = 1,         /* NULL pointer, misaligned pointer, bad size, batch == 0 handled as OK no-op */
-  FHE_ERR_UNSUPPORTED = 2, /* parameter combination the library does not implement */
+  FHE_ERR_UNSUPPORTED = 2, /* parameter combination the library does not implement; also returned by fhe_he_mult /
+                              fhe_relinearize / fhe_mult_relin_rescale when that call's CRT target (constant matrix in
+                              shared memory, accumulators in tensor memory) does not fit the SM while fhe_polymul's does */
   FHE_ERR_STATE = 3,       /* e.g. fhe_relinearize before fhe_set_evk */
   FHE_ERR_CUDA = 4,        /* a CUDA runtime call failed; text in fhe_last_error */
   FHE_ERR_NOMEM = 5        /* host or device allocation failed, or workspace too small */
@@ -142,6 +144,11 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
  * order: res[bitrev(i)] = sum_j a_j psi^((2i+1) j).  inverse != 0: expects that order, returns natural order,
  * scaled by N^-1 only (no CRT constant folded in). */
 fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream);
+/* Calibration for the roofline report: register-only throughput, in operations per second over the
+ * whole device, of mode 0: the forward NTT butterfly exactly as the kernels execute it (Eq. 8: one
+ * Shoup modular multiplication, one add, one subtract, lazy corrections); 1: mad.lo.u32; 2: mul.hi.u32.  Allocates
+ * a scratch buffer, launches a few milliseconds of work on `stream` and synchronises: not a hot-path call. */
+fhe_status fhe_debug_int_peak(fhe_ctx* ctx, int mode, double* per_second, void* stream);
 /* Number of kernel launches the context has enqueued so far (for bench.py's gpu_launches). */
 uint64_t fhe_debug_launch_count(const fhe_ctx* ctx);
 /* Per-kernel device timing for the roofline report.  enable != 0: every later launch is bracketed by a CUDA event

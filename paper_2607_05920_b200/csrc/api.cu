@@ -126,6 +126,7 @@ fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, co
   if (!d_out3 || !d_ct1 || !d_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out3, 16) || misaligned(d_ct1, 16) || misaligned(d_ct2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
   if (ws_bytes < ws_tensor(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  if (!c->fit_tensor) return err(c, FHE_ERR_UNSUPPORTED, "tensor-product CRT target too large for the conversion pipeline");
   return do_he_mult(c, d_out3, d_ct1, d_ct2, batch, (uint32_t*)d_ws, (cudaStream_t)stream);
 }
 
@@ -138,6 +139,7 @@ fhe_status fhe_relinearize(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in3
   if (misaligned(d_out2, 16) || misaligned(d_in3, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
   if (!c->have_evk) return err(c, FHE_ERR_STATE, "no evk installed (call fhe_set_evk first)");
   if (ws_bytes < ws_relin(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  if (!c->fit_relin) return err(c, FHE_ERR_UNSUPPORTED, "relinearisation CRT target too large for the conversion pipeline");
   return do_relin(c, d_out2, d_in3, batch, (uint32_t*)d_ws, 0, (cudaStream_t)stream);
 }
 
@@ -165,6 +167,7 @@ fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t
   if (c->t != 0 && p_bits != 0) return err(c, FHE_ERR_UNSUPPORTED, "rescale is CKKS-only");
   if (p_bits >= c->logQ) return err(c, FHE_ERR_ARG, "p_bits out of range");
   if (ws_bytes < fhe_workspace_bytes(ctx, FHE_OP_MULT_RELIN_RESCALE, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  if (!c->fit_tensor || !c->fit_relin) return err(c, FHE_ERR_UNSUPPORTED, "CRT target too large for the conversion pipeline");
   cudaStream_t s = (cudaStream_t)stream;
   uint32_t* d3 = (uint32_t*)d_ws;
   uint32_t* ws = (uint32_t*)((char*)d_ws + ws_d3(c, batch));
@@ -213,6 +216,14 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
   }
   CK(cudaStreamSynchronize(c->s_d2h), "sync");
   CK(cudaStreamSynchronize(s), "sync");
+  return FHE_OK;
+}
+
+fhe_status fhe_debug_int_peak(fhe_ctx* ctx, int mode, double* per_second, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (!per_second || mode < 0 || mode > 2) return err(c, FHE_ERR_ARG, "bad argument");
+  CK(measure_int_peak(c, mode, per_second, (cudaStream_t)stream), "int peak");
   return FHE_OK;
 }
 

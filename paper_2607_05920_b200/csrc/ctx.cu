@@ -315,8 +315,12 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   c->post_pm = pp;     c->post_pm.mode = ckks ? POST_CKKS_MASK : POST_BGV_MODQ;
   c->post_tensor = c->post_pm;
   c->post_relin = pp;  c->post_relin.mode = ckks ? POST_CKKS_RELIN : POST_BGV_RELIN;
-  if (!crt_target_fits(c->tgt_pm, c->post_pm) || !crt_target_fits(c->tgt_tensor, c->post_tensor) ||
-      !crt_target_fits(c->tgt_relin, c->post_relin)) {
+  // A target whose constant matrix or accumulators exceed shared / tensor memory disables the calls that need it
+  // (FHE_ERR_UNSUPPORTED from those calls); the context is refused only when not even the plain product fits.
+  c->fit_pm = crt_target_fits(c->tgt_pm, c->post_pm);
+  c->fit_tensor = crt_target_fits(c->tgt_tensor, c->post_tensor);
+  c->fit_relin = crt_target_fits(c->tgt_relin, c->post_relin);
+  if (!c->fit_pm) {
     destroy(c);
     return fail(nullptr, FHE_ERR_UNSUPPORTED, "parameters too large for the conversion pipeline (TMEM columns / shared memory)");
   }

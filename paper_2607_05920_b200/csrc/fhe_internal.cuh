@@ -71,6 +71,7 @@ struct Context {
   uint32_t dec_cols = 0;          // columns of the decompose image: 64 ceil(Kmax / 16)
   uint32_t dec_KBimg = 0;         // contraction bytes covered by the decompose image (widest input, multiple of 32)
   CrtTarget tgt_pm, tgt_tensor, tgt_relin;
+  bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
   // evk-hat
@@ -137,6 +138,8 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
                        const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
                        size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s);
+// register-only throughput of the NTT butterfly (mode 0), mad.lo.u32 (1), mul.hi.u32 (2) on this device, per second
+cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s);
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the pipeline have the TMEM / shared memory for it
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);

@@ -430,6 +430,76 @@ ntt_row_fused_kernel(NttArgs a) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Calibration of the roofline the NTT kernels are held against ("calibrate the integer peak in the same
+// run with a register-only microbenchmark of the actual mix").  MODE 0: the forward butterfly itself (bf_fwd: one
+// IMAD.HI, two IMAD, three adds / min) on 16 registers per thread with register-resident twiddles, no memory traffic;
+// MODE 1: mad.lo.u32 alone; MODE 2: mul.hi.u32 alone.  Measured on B200: 32-bit multiply-add issues at 64 lanes per
+// clock per SM, multiply-high at 32, add / min at 128 on another pipe -- so a butterfly costs 4 + 2 + 2 = 8 cycles of
+// the multiplier pipe per warp and the pipe, not the issue slots or HBM, bounds the NTT arithmetic.
+// ------------------------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(256)
+int_peak_kernel(uint32_t* out, uint32_t q, uint2 w0, uint2 w1, uint32_t rounds) {
+  uint32_t x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = (threadIdx.x * 16 + i) * 2654435761u % q;
+  const uint32_t q2 = 2 * q;
+  for (uint32_t r = 0; r < rounds; ++r) {
+    if (MODE == 0) {
+#pragma unroll
+      for (int h = 8; h >= 1; h >>= 1)
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+          if (!(i & h)) bf_fwd(x[i], x[i + h], (i & 1) ? w1 : w0, q, q2);
+    } else {
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+          if (MODE == 1) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(x[i]) : "r"(w0.x), "r"(w1.x));
+          else asm volatile("mul.hi.u32 %0, %0, %1;" : "+r"(x[i]) : "r"(w0.y));
+        }
+    }
+  }
+  uint32_t acc = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) acc ^= x[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
+// ops per second of MODE on the whole device: 8 blocks of 256 threads per SM, `rounds` chosen for a few milliseconds
+cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s) {
+  const uint32_t q = c->h_q[0], rounds = 4096;
+  const uint32_t w = c->h_psi[0];
+  const uint2 w0 = make_uint2(w, (uint32_t)(((uint64_t)w << 32) / q)), w1 = make_uint2(q - w, (uint32_t)(((uint64_t)(q - w) << 32) / q));
+  const uint32_t blocks = 8 * (uint32_t)c->n_sm;
+  uint32_t* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, (size_t)blocks * 256 * 4);
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  float best = 1e30f;
+  for (int rep = 0; rep < 4; ++rep) {                              // first repetition is the warm-up
+    cudaEventRecord(e0, s);
+    if (mode == 0) int_peak_kernel<0><<<blocks, 256, 0, s>>>(d, q, w0, w1, rounds);
+    else if (mode == 1) int_peak_kernel<1><<<blocks, 256, 0, s>>>(d, q, w0, w1, rounds);
+    else int_peak_kernel<2><<<blocks, 256, 0, s>>>(d, q, w0, w1, rounds);
+    cudaEventRecord(e1, s);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0;
+    cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms < best) best = ms;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d);
+  if (e != cudaSuccess) return e;
+  const double per_thread = mode == 0 ? 32.0 : 64.0;               // butterflies resp. instructions per thread and round
+  *per_s = per_thread * rounds * 256.0 * blocks / (best * 1e-3);
+  return cudaSuccess;
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------------------
 template <bool INV>
 static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaStream_t s) {

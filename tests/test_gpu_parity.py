@@ -348,3 +348,71 @@ def test_c4_bgv_full_size():
             want = _relin_coeff_bgv(prm, out3[b], list(evk), k)
             assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
     assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, 0), t2)
+
+
+# ---- shapes that make the conversion pipeline take its other paths -------------------------------------------------------
+def test_decompose_extreme_byte_sums_and_two_passes():
+    """Every input byte 0xFF (the largest accumulator columns the Barrett step sees), a one-hot input, and a prime count
+    whose accumulator columns exceed tensor memory, so the launch runs two passes over its tiles (pipe.cuh)."""
+    fhe = _lib()
+    N, logQ = 512, 2480
+    ctx = fhe.Context(N, logQ, 32)
+    Lin = ctx.L
+    K = ctx.K_pm
+    assert (K + 15) // 16 > 6            # more 64-column chunks than fit beside the A buffers in 512 TMEM columns
+    q, _ = ctx.primes(K)
+    limbs = np.zeros((3, Lin, N), dtype=np.uint32)
+    limbs[0] = 0xFFFFFFFF
+    limbs[1, Lin - 1, :] = 0x80000000
+    limbs[2] = synth.uniform_limbs(synth.rng(5), (), N, 32 * Lin)
+    res = tensor_to_np(ctx.fhe_debug_decompose(limbs_np_to_tensor(limbs), K, 0))
+    for p in range(3):
+        vals = from_limbs(limbs[p])
+        for j in (0, 15, 16, 95, 96, K - 1):
+            want = np.array([v % q[j] for v in vals], dtype=np.uint32)
+            assert np.array_equal(res[p, j], want), (p, j)
+
+
+def test_polymul_widest_sweep_cell_sampled():
+    """A cell of the polymul sweep at logQ = 2480 (78 limbs, K > 160): two-pass decompose, single-buffered A operand
+    in the CRT.  Sampled coefficients from the definition (Eq. 5-6)."""
+    fhe = _lib()
+    N, logQ, batch = 1 << 12, 2480, 3
+    ctx = fhe.Context(N, logQ, 32)
+    assert ctx.L == 78 and ctx.K_pm > 160
+    g = synth.rng(2480)
+    a = synth.uniform_limbs(g, (batch,), N, logQ)
+    b = synth.uniform_limbs(g, (batch,), N, logQ)
+    out = tensor_to_np(ctx.fhe_polymul(limbs_np_to_tensor(a), limbs_np_to_tensor(b)))
+    Q = 1 << logQ
+    rnd = np.random.default_rng(3)
+    for i in range(batch):
+        ai, bi = from_limbs(a[i]), from_limbs(b[i])
+        for k in [0, 1, 127, 128, N - 1] + [int(v) for v in rnd.integers(0, N, size=4)]:
+            assert coeff_from_limbs(out[i], k) == ring.pm_coeff(ai, bi, k, Q)
+
+
+@pytest.mark.parametrize("batch", [1, 5, 37])
+def test_host_entry_point_equals_device_path(batch):
+    """fhe_mult_relin_rescale_host pipelines the batch in pieces over three streams (37 items: ragged pieces of two);
+    its result must be the device path's, bit for bit."""
+    fhe = _lib()
+    N, logQ, logP, p = 256, 128, 128, 40
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(77)
+    ct1 = limbs_np_to_tensor(synth.uniform_limbs(g, (batch, 2), N, logQ))
+    ct2 = limbs_np_to_tensor(synth.uniform_limbs(g, (batch, 2), N, logQ))
+    ctx.fhe_set_evk(limbs_np_to_tensor(synth.uniform_limbs(g, (2,), N, logQ + logP)))
+    want = ctx.fhe_mult_relin_rescale(ct1, ct2, p)
+    torch.cuda.synchronize()
+    h1, h2 = ct1.cpu().pin_memory(), ct2.cpu().pin_memory()
+    got = ctx.fhe_mult_relin_rescale_host(h1, h2, p)
+    assert torch.equal(got, want.cpu())
+
+
+def test_empty_batch_is_a_no_op():
+    fhe = _lib()
+    ctx = fhe.Context(256, 64, 32)
+    a = torch.empty((0, ctx.L, 256), dtype=torch.int32, device="cuda")
+    out = ctx.fhe_polymul(a, a)
+    assert out.shape[0] == 0
