@@ -85,9 +85,11 @@ def work_model(N, logQ, logP, L, L_PQ, K1, K2, B):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line).  nvidia-smi needs a
+    few hundred milliseconds to start, so the sampler is started before the warm-up, waited on until its first line
+    is there, and only the samples whose timestamps fall inside [mark_start(), mark_end()] are kept."""
 
-    FIELDS = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    FIELDS = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
               "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
               "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -95,18 +97,31 @@ class ClockSampler:
         self.idx = gpu_index
         self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         self.proc = None
+        self.t0 = self.t1 = None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits", "-lms", "100"],
+                ["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=self.tmp, stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
+            return
+        deadline = time.time() + 3.0
+        while time.time() < deadline and os.path.getsize(self.tmp.name) == 0:
+            time.sleep(0.02)
+
+    def mark_start(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
 
     def stop(self):
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.proc is not None:
+            time.sleep(0.05)
             self.proc.terminate()
             try:
                 self.proc.wait(timeout=5)
@@ -117,15 +132,27 @@ class ClockSampler:
             with open(self.tmp.name) as f:
                 rows = [r.strip().split(", ") for r in f if r.strip()]
             os.unlink(self.tmp.name)
-            sm = sorted(float(r[1]) for r in rows if len(r) >= 9)
+            rows = [r for r in rows if len(r) >= 10]
+            keep = []
+            for r in rows:
+                try:
+                    ts = datetime.datetime.strptime(r[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                except Exception:
+                    continue
+                if self.t0 is not None and self.t1 is not None and self.t0 - 0.02 <= ts <= self.t1 + 0.02:
+                    keep.append(r)
+            out["samples_total"] = len(rows)
+            if not keep:            # region shorter than the sampling period: fall back to the samples around it
+                keep = rows[-3:]
+            sm = sorted(float(r[2]) for r in keep)
             if sm:
                 out["sm_mhz"] = sm[len(sm) // 2]
-                out["sm_max_mhz"] = float(rows[0][2])
+                out["sm_max_mhz"] = float(keep[0][3])
                 out["samples"] = len(sm)
                 names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
                 seen = set()
-                for r in rows:
-                    for name, val in zip(names, r[5:9]):
+                for r in keep:
+                    for name, val in zip(names, r[6:10]):
                         if val.strip().lower().startswith("active"):
                             seen.add(name)
                 out["reasons"] = sorted(seen)
@@ -268,13 +295,13 @@ def run_ours(args):
     def step():
         ctx.fhe_mult_relin_rescale(ct1, ct2, p_bits, out=out, stream=stream)
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler.mark_start()
     # ---- timed region: K steps, device time on the launching stream, max over ranks ----
     l0 = ctx.launch_count()
     barrier(world)
@@ -288,7 +315,6 @@ def run_ours(args):
     barrier(world)
     ms_total = max_over_ranks(e0.elapsed_time(e1), world, dev)
     launches = ctx.launch_count() - l0
-    clocks = sampler.stop() if rank == 0 else None
     _, total_units = shard_units(B, world)
     value = total_units * args.steps / (ms_total / 1e3)
 
@@ -318,6 +344,8 @@ def run_ours(args):
         ctx.fhe_mult_relin_rescale_host(h1, h2, p_bits, h_out=hout, stream=stream)   # synchronises the stream itself
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3, world, dev)
     e2e_value = total_units * e2e_steps / (e2e_ms / 1e3)
+    sampler.mark_end()       # the timed, the instrumented and the end-to-end steps: all of them the same load
+    clocks = sampler.stop() if rank == 0 else None
     ct_bytes = B * 2 * ctx.L * N * 4
 
     if rank != 0:

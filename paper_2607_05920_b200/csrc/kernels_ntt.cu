@@ -128,7 +128,7 @@ struct NttArgs {
 // 4096 points.  Shared-memory tile [e][cc]: every access of a warp is to 32 (or 16) consecutive words.
 // ------------------------------------------------------------------------------------------------------------------
 template <int LN, bool INV>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 6)
 ntt_col_kernel(NttArgs a) {
   constexpr int LE = LN < 4 ? LN : 4, E = 1 << LE;   // points per thread
   constexpr int TPC = (1 << LN) / E;                 // threads per column
