@@ -470,7 +470,7 @@ int_peak_kernel(uint32_t* out, uint32_t q, uint2 w0, uint2 w1, uint32_t rounds) 
 
 // ops per second of MODE on the whole device: 8 blocks of 256 threads per SM, `rounds` chosen for a few milliseconds
 cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s) {
-  const uint32_t q = c->h_q[0], rounds = 4096;
+  const uint32_t q = c->h_q[0], rounds = 1024;
   const uint32_t w = c->h_psi[0];
   const uint2 w0 = make_uint2(w, (uint32_t)(((uint64_t)w << 32) / q)), w1 = make_uint2(q - w, (uint32_t)(((uint64_t)(q - w) << 32) / q));
   const uint32_t blocks = 8 * (uint32_t)c->n_sm;
