@@ -55,6 +55,10 @@ def test_single_process_plumbing_is_identity():
     import bench
     assert bench.max_over_ranks(3.5, 1) == 3.5
     assert bench.shard_units(4, 1) == (4, 4)
-    mul, byt, comp = bench.work_model(1 << 16, 1240, 1240, 39, 78, 81, 121, 4)
+    bf, units, byt, comp = bench.work_model(1 << 16, 1240, 1240, 39, 78, 81, 121, 4)
     assert comp == 4 * 65536 * 4 * 6 * 39 + 65536 * 4 * 2 * 121
-    assert all(v >= 0 for v in mul.values()) and mul["crt"] > mul["pointwise"]
+    # every transform has N/2 log2 N butterflies: 8 of the 16 stages in the column passes, 8 in the fused rows
+    transforms = 4 * ((4 * 81 + 121) + (3 * 81 + 2 * 121))
+    assert sum(bf.values()) == transforms * 32768 * 16
+    assert bf["pointwise"] == bf["ntt_fwd"] + bf["ntt_inv"]
+    assert all(v >= 0 for v in units.values()) and all(v >= 0 for v in byt.values())
