@@ -144,6 +144,11 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
  * order: res[bitrev(i)] = sum_j a_j psi^((2i+1) j).  inverse != 0: expects that order, returns natural order,
  * scaled by N^-1 only (no CRT constant folded in). */
 fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream);
+/* The CKKS relinearisation CRT decides the one carry out of the low logP bits of x from 96-bit truncated constants and
+ * recomputes a coefficient exactly when the `bits` fractional bits below the rounding position are all ones (default
+ * and maximum 58: the truncation error is below 2^-58, so nothing else can be wrong).  A smaller value
+ * only sends more coefficients down the exact path -- results are identical -- which is how the tests reach it. */
+fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits);
 /* Calibration for the roofline report: register-only throughput, in operations per second over the
  * whole device, of mode 0: the forward NTT butterfly exactly as the kernels execute it (Eq. 8: one
  * Shoup modular multiplication, one add, one subtract, lazy corrections); 1: mad.lo.u32; 2: mul.hi.u32.  Allocates

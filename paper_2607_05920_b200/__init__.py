@@ -23,7 +23,7 @@ EXPORTS = [
     "fhe_ctx_create", "fhe_ctx_destroy", "fhe_ctx_info", "fhe_last_error", "fhe_get_modulus", "fhe_workspace_bytes",
     "fhe_set_evk", "fhe_polymul", "fhe_he_mult", "fhe_relinearize", "fhe_rescale", "fhe_mult_relin_rescale",
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
-    "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak",
+    "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
 ]
 
 
@@ -86,6 +86,8 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_debug_ntt.restype = c_int
     lib.fhe_debug_launch_count.argtypes = [vp]
     lib.fhe_debug_launch_count.restype = c_uint64
+    lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
+    lib.fhe_debug_crt_ambiguity.restype = c_int
     lib.fhe_debug_int_peak.argtypes = [vp, c_int, POINTER(ctypes.c_double), vp]
     lib.fhe_debug_int_peak.restype = c_int
     lib.fhe_debug_timing.argtypes = [vp, c_int]
@@ -186,6 +188,9 @@ class Context:
         return int(self._lib.fhe_debug_launch_count(self._h))
 
     KERNEL_CLASSES = ("decompose", "ntt_fwd", "ntt_inv", "pointwise", "crt", "rescale")
+
+    def fhe_debug_crt_ambiguity(self, bits: int):
+        self._check(self._lib.fhe_debug_crt_ambiguity(self._h, bits))
 
     def fhe_debug_int_peak(self, mode: int, stream=None) -> float:
         """Register-only throughput per second of 0: the NTT butterfly, 1: mad.lo.u32, 2: mul.hi.u32 (whole device)."""

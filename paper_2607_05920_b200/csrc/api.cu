@@ -51,6 +51,7 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   CK(launch_ntt_product(c, ws, c->d_evk_hat, B, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt relin");
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
+  pp.amb_bits = c->amb_bits;
   CK(launch_crt(c, c->tgt_relin, pp, d_out2, (size_t)2 * L * N, (size_t)L * N, ws, 2 * rp, rp, d_in3, (size_t)3 * L * N,
                 (size_t)L * N, B, 2, s), "crt relin");
   return FHE_OK;
@@ -216,6 +217,14 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
   }
   CK(cudaStreamSynchronize(c->s_d2h), "sync");
   CK(cudaStreamSynchronize(s), "sync");
+  return FHE_OK;
+}
+
+fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (bits < 1 || bits > TOP_AMB) return err(c, FHE_ERR_ARG, "bits out of range");
+  c->amb_bits = bits;
   return FHE_OK;
 }
 

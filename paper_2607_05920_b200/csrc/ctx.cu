@@ -150,6 +150,77 @@ static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2
   return upload(c, &tg.d_scale, scale);
 }
 
+// bits [lo, lo + n) of x
+static BigU bit_range(const BigU& x, uint32_t lo, uint32_t n) {
+  BigU r;
+  r.v.assign((n + 31) / 32, 0u);
+  for (uint32_t i = 0; i < n; ++i)
+    if (x.bit(lo + i)) r.v[i / 32] |= 1u << (i % 32);
+  r.trim();
+  return r;
+}
+
+// The CKKS relin target in its "top" form (fhe_internal.cuh): image columns 0..7 alpha, 8..31 the byte
+// positions of sum_i y_i Wt_i (Wt_i = top TOP_BITS bits of W_i mod 2^logP), 32.. those of sum_i y_i Wh_i mod 2^(32 L)
+// (Wh_i = W_i >> logP).  The negM table is [Nt (TOP_LIMBS) | Nh (L)].  The full constants go along for the exact path.
+static cudaError_t build_target_top(Context* c, CrtTarget& tg, uint32_t K, uint32_t logP, uint32_t logQ) {
+  constexpr uint32_t NC = 64;
+  const uint32_t L = (logQ + 31) / 32;
+  tg.K = K;
+  tg.KB = (4 * K + 31) / 32 * 32;
+  tg.top = true;
+  tg.Lraw = TOP_LIMBS + L;
+  tg.Lx = tg.Lraw + 1;
+  tg.Lfull = (logP + logQ + 31) / 32;
+  const uint32_t hbytes = 4 * L, tbytes = TOP_BITS / 8;
+  const uint32_t ncols = CRT_ALPHA_COLS + 4 * TOP_LIMBS + hbytes;
+  tg.nchunks = (ncols + NC - 1) / NC;
+  BigU M((uint64_t)1);
+  for (uint32_t i = 0; i < K; ++i) M.mul_small(c->h_q[i]);
+  const size_t img_cols = (size_t)tg.nchunks * NC;
+  std::vector<uint8_t> img((size_t)tg.KB * img_cols, 0);
+  auto put = [&](uint32_t kb, uint32_t col, uint8_t v) { img[((size_t)(kb / 16) * img_cols + col) * 16 + kb % 16] = v; };
+  std::vector<uint2> scale(K);
+  std::vector<uint32_t> wfull((size_t)K * tg.Lfull, 0u);
+  for (uint32_t i = 0; i < K; ++i) {
+    const uint32_t q = c->h_q[i];
+    BigU Mi = M;
+    if (Mi.divmod_small(q) != 0) return cudaErrorUnknown;
+    const uint32_t inv = powmod(Mi.mod_small(q), q - 2, q);            // (M/q_i)^-1 mod q_i
+    const BigU W = Mi.low_bits(logP + logQ);
+    W.to_limbs(wfull.data() + (size_t)i * tg.Lfull, tg.Lfull);
+    const std::vector<uint8_t> Wt = bytes_of(bit_range(W, logP - TOP_BITS, TOP_BITS), tbytes);
+    const std::vector<uint8_t> Wh = bytes_of(bit_range(W, logP, logQ), hbytes);
+    const uint64_t F = (1ull << ALPHA_SHIFT) / q;
+    for (uint32_t b = 0; b < 4; ++b) {                                  // byte b of y_i weighs 2^(8 b)
+      for (uint32_t cc = 0; cc < 3; ++cc) put(4 * i + b, b + cc, (uint8_t)(F >> (8 * cc)));
+      for (uint32_t e = 0; e < tbytes; ++e) put(4 * i + b, CRT_ALPHA_COLS + b + e, Wt[e]);
+      for (uint32_t e = b; e < hbytes; ++e) put(4 * i + b, CRT_ALPHA_COLS + 4 * TOP_LIMBS + e, Wh[e - b]);
+    }
+    const uint32_t ninv = powmod(c->N % q, q - 2, q);
+    const uint32_t r32 = (uint32_t)((1ull << 32) % q);
+    const uint32_t sc = mulmod(mulmod(ninv, inv, q), r32, q);
+    scale[i] = make_uint2(sc, shoup(sc, q));
+  }
+  std::vector<uint32_t> negM(tg.Lraw, 0u), negfull(tg.Lfull, 0u);
+  {
+    const BigU T = BigU::pow2(logP + logQ);
+    BigU Mt = M.low_bits(logP + logQ), neg;
+    if (!Mt.is_zero()) { neg = T; neg.sub(Mt); }
+    neg.to_limbs(negfull.data(), negfull.size());
+    bit_range(neg, logP - TOP_BITS, TOP_BITS).to_limbs(negM.data(), TOP_LIMBS);
+    bit_range(neg, logP, logQ).to_limbs(negM.data() + TOP_LIMBS, L);
+  }
+  cudaError_t e = upload(c, &tg.d_B, img);
+  if (e != cudaSuccess) return e;
+  if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
+  if ((e = upload(c, &tg.d_Wfull, wfull)) != cudaSuccess) return e;
+  if ((e = upload(c, &tg.d_negMfull, negfull)) != cudaSuccess) return e;
+  std::vector<uint32_t> flags(1 + 3 * (size_t)TOP_MAX_FLAGS, 0u);
+  if ((e = upload(c, &c->d_flags, flags)) != cudaSuccess) return e;
+  return upload(c, &tg.d_scale, scale);
+}
+
 static uint64_t mu1_of(const BigU& m) {   // floor(2^(bits(m)+62) / m), in (2^62, 2^63]
   BigU q, r;
   BigU::divmod(BigU::pow2(m.bits() + 62), m, q, r);
@@ -273,7 +344,8 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   const bool ckks = (t == 0);
   if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
       (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
-      (e = build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ, c->L_PQ + 2)) != cudaSuccess) {
+      (e = (ckks && logP >= TOP_BITS) ? build_target_top(c, c->tgt_relin, c->K2, logP, logQ)
+                                      : build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ, c->L_PQ + 2)) != cudaSuccess) {
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "CRT table build failed: " + m);
   }
 

@@ -27,7 +27,17 @@ struct CrtTarget {
   uint8_t* d_B = nullptr;      // [KB/16][64 nchunks][16]: the constant matrix as K-major 16-byte core-matrix rows (pipe.cuh)
   uint32_t* d_negM = nullptr;  // [Lraw]
   uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
+  // "Top" form of the CKKS relin target: the output needs floor((V mod 2^(logP+logQ) + 2^(logP-1)) >> logP)
+  // mod 2^logQ only, i.e. the high logQ bits of W_i exactly and ONE carry out of the low logP bits.  That carry is taken
+  // from the top TOP_BITS bits of the low parts (columns 8..31 of the image, then 4 L columns of the high parts); the
+  // truncation can change it only when the TOP_AMB fractional bits below it are all ones, in which case the coefficient
+  // is flagged and recomputed exactly from the full constants by crt_exact_kernel.
+  bool top = false;
+  uint32_t Lfull = 0;              // limbs of the full constants: ceil((logP + logQ) / 32)
+  uint32_t* d_Wfull = nullptr;     // [K][Lfull]: (M/q_i) mod 2^(logP+logQ)
+  uint32_t* d_negMfull = nullptr;  // [Lfull]
 };
+constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58, TOP_MAX_FLAGS = 65536;
 
 enum PostMode : int {
   POST_CKKS_MASK = 0,    // out = X mod 2^logQ
@@ -40,6 +50,7 @@ struct PostParams {
   int mode;
   uint32_t L, L_PQ, logQ, logP, bitsQ, bitsP, bitsPQ;
   uint32_t rescale_bits;       // POST_CKKS_RELIN only; 0 = none
+  uint32_t amb_bits;           // top-form relin target: fractional bits that must all be ones to flag a coefficient
   // BGV constants (device pointers, little-endian limbs)
   const uint32_t* d_Q;         // [L+1]
   const uint32_t* d_P;         // [L_P+1]
@@ -74,6 +85,8 @@ struct Context {
   bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
+  uint32_t* d_flags = nullptr;    // [1 + 3 TOP_MAX_FLAGS]: count, then (outer, inner, n) of the coefficients to recompute
+  uint32_t amb_bits = TOP_AMB;    // fhe_debug_crt_ambiguity lowers it so that tests reach the exact path
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
   bool have_evk = false;

@@ -126,7 +126,8 @@ struct CrtEpi {
     uint32_t* out; size_t out_outer, out_inner;
     const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
     const uint32_t* negM;                               // [Lraw]
-    uint32_t Lraw, Lx, nl;                              // nl = limbs the chunks cover (16 per chunk minus the alpha columns)
+    uint32_t Lraw, Lx, nl, ntab;                        // nl = limbs of V the chunks cover; ntab = entries of the negM table
+    uint32_t top, amb_bits; uint32_t* flags;             // top-form relin target (fhe_internal.cuh): flag list of the exact path
     uint32_t xs_off, adds_off, scratch_off;             // word offsets inside the scratch: negM table at 0, then the columns
     // CKKS relin streaming constants: shift by logP = 32 ws + bs, rounding bit rbit in limb rb; rescale likewise (.2)
     uint32_t ws, bs, rb, rbit, ws2, bs2, rb2, rbit2, Lr, tm2, tmq, lend;
@@ -143,13 +144,14 @@ struct CrtEpi {
   const uint32_t* aptr = nullptr;
   uint32_t alpha = 0, yprev = 0, cy = 0, zprev = 0, cz = 0;
   uint64_t carry = 0;
+  uint32_t cur_o = 0, cur_i = 0, cur_n = 0;
 
   __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t)
       : p(p_), N(a.N), etid(etid_), negm(reinterpret_cast<const uint32_t*>(sm)),
         xs(reinterpret_cast<uint32_t*>(sm) + p_.xs_off), adds(reinterpret_cast<uint32_t*>(sm) + p_.adds_off),
         scratch(reinterpret_cast<uint32_t*>(sm) + p_.scratch_off) {
     uint32_t* w = reinterpret_cast<uint32_t*>(sm);
-    for (uint32_t k = etid; k < p.nl + 2; k += TC) w[k] = k < p.Lraw ? __ldg(p.negM + k) : 0u;
+    for (uint32_t k = etid; k < p.ntab; k += TC) w[k] = k < p.Lraw ? __ldg(p.negM + k) : 0u;
     pipe::epi_sync(TC);
   }
 
@@ -157,6 +159,7 @@ struct CrtEpi {
     out = p.out + (size_t)o * p.out_outer + (size_t)i * p.out_inner + n0 + etid;
     optr = out; aptr = adds + etid;
     carry = 0; yprev = 0; cy = 0; zprev = 0; cz = 0;
+    cur_o = o; cur_i = i; cur_n = n0 + etid;
     if (p.add) {
       const uint32_t* src = p.add + (size_t)o * p.add_outer + (size_t)i * p.add_inner + n0 + etid;
       const uint32_t dst = umma::smem_u32(adds + etid);
@@ -200,6 +203,32 @@ struct CrtEpi {
     yprev = y;
   }
 
+  // Top-form relin target, first 32 columns of a tile: P[2..8) are the six limbs of S_t = sum_i y_i Wt_i + alpha Nt, the
+  // low part of V cut down to its top TOP_BITS bits.  The carry into the high part is round(S_t / 2^96); the cut-off
+  // bits can add less than 2^-58 to S_t / 2^96, so the rounding is certain unless the amb_bits fractional bits below the
+  // rounding position are all ones -- then the coefficient is put on the list crt_exact_kernel works off.
+  __device__ __forceinline__ void top_carry(const uint64_t* P) {
+    uint32_t sl[TOP_LIMBS];
+    uint64_t cr = 0;
+#pragma unroll
+    for (int g = 0; g < (int)TOP_LIMBS; ++g) {
+      const uint64_t v = cr + P[g + 2];
+      sl[g] = (uint32_t)v;
+      cr = v >> 32;
+    }
+    const uint64_t r2 = (uint64_t)sl[2] + 0x80000000u;             // + 2^95
+    const uint64_t r3 = (uint64_t)sl[3] + (r2 >> 32);
+    const uint64_t r4 = (uint64_t)sl[4] + (r3 >> 32);
+    carry = (r3 & 0xFFFFFFFFu) | (r4 << 32);                      // bits 96.. of S_t + 2^95 (S_t < 2^134)
+    const uint64_t frac = ((uint64_t)(uint32_t)r2 << 32) | sl[1];  // fractional bits 32..95
+    if ((frac >> (64 - p.amb_bits)) == (~0ull >> (64 - p.amb_bits))) {
+      const uint32_t idx = atomicAdd(p.flags, 1u);
+      if (idx < TOP_MAX_FLAGS) {
+        p.flags[1 + 3 * idx] = cur_o; p.flags[2 + 3 * idx] = cur_i; p.flags[3 + 3 * idx] = cur_n;
+      }
+    }
+  }
+
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     int g0 = 0;
     if (col0 == 0) {
@@ -209,7 +238,7 @@ struct CrtEpi {
       alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
       g0 = CRT_ALPHA_COLS / 4;
     }
-    const uint32_t l0 = col0 / 4 - CRT_ALPHA_COLS / 4;             // limb of group element 0 (wraps for col0 = 0; elements 0, 1 unused)
+    uint32_t l0 = col0 / 4 - CRT_ALPHA_COLS / 4;                   // limb of group element 0 (wraps for col0 = 0; elements 0, 1 unused)
     uint64_t P[8];                                                 // the limb's column sum + alpha * negM: independent of the carry
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
@@ -217,6 +246,10 @@ struct CrtEpi {
       const uint64_t s01 = (uint64_t)t[4 * g + 1] * 256u + t[4 * g];
       const uint64_t s23 = (uint64_t)t[4 * g + 3] * 256u + t[4 * g + 2];
       P[g] = (uint64_t)alpha * negm[l0 + g] + s01 + (s23 << 16);
+    }
+    if (p.top) {
+      if (col0 == 0) { top_carry(P); return; }
+      l0 -= TOP_LIMBS;                                             // from here on l0 counts limbs of the high part
     }
     const int mode = p.pp.mode;
     const uint32_t L = p.pp.L;
@@ -403,13 +436,99 @@ __device__ void CrtEpi::post() {
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// The exact path of the top-form relin target: one thread per flagged coefficient recomputes the whole output
+// coefficient from the full constants -- V = sum_i y_i W_i + alpha negM mod 2^(logP+logQ) limb by limb, divide by P with
+// rounding, add d, optional rescale (the formulas of DESIGN.md 3, A3/A4) -- and overwrites what the pipeline stored.
+// Expected work: 2^-58 of the coefficients; the launch costs a few microseconds when the list is empty.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr uint32_t EXACT_MAX_LIMBS = 168;
+struct ExactArgs {
+  const uint32_t* flags;
+  const uint32_t* res; size_t res_outer, res_inner;
+  const uint32_t* add; size_t add_outer, add_inner;
+  uint32_t* out; size_t out_outer, out_inner;
+  const uint32_t* W; const uint32_t* negM; const uint32_t* q;
+  uint32_t N, K, Lfull, L, logP, logQ, rescale_bits;
+};
+
+// x[0..n) += 2^bit
+__device__ inline void big_add_pow2(uint32_t* x, uint32_t n, uint32_t bit) {
+  uint32_t l = bit >> 5, add = 1u << (bit & 31);
+  while (l < n && add) { const uint32_t v = x[l]; x[l] = v + add; add = (v + add) < v ? 1u : 0u; ++l; }
+}
+// x[0..n) = (x >> sh) over n + extra limbs of input, then reduced mod 2^bits
+__device__ inline void big_shr_mask(uint32_t* x, uint32_t nin, uint32_t sh, uint32_t bits, uint32_t nout) {
+  const uint32_t w = sh >> 5, b = sh & 31;
+  for (uint32_t l = 0; l < nout; ++l) {
+    const uint32_t lo = l + w < nin ? x[l + w] : 0u, hi = l + w + 1 < nin ? x[l + w + 1] : 0u;
+    uint32_t v = b ? (lo >> b) | (hi << (32 - b)) : lo;
+    if (32 * l >= bits) v = 0; else if (bits - 32 * l < 32) v &= (1u << (bits - 32 * l)) - 1u;
+    x[l] = v;
+  }
+}
+
+__global__ void __launch_bounds__(64)
+crt_exact_kernel(ExactArgs a) {
+  const uint32_t cnt = min(a.flags[0], TOP_MAX_FLAGS);
+  uint32_t V[EXACT_MAX_LIMBS + 2];
+  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
+    const uint32_t o = a.flags[1 + 3 * e], i = a.flags[2 + 3 * e], n = a.flags[3 + 3 * e];
+    const uint32_t* y = a.res + (size_t)o * a.res_outer + (size_t)i * a.res_inner + n;
+    const uint32_t nl = a.Lfull + 2;
+    for (uint32_t l = 0; l < nl; ++l) V[l] = 0;
+    uint64_t asum = 0;
+    for (uint32_t j = 0; j < a.K; ++j) {
+      const uint32_t yj = y[(size_t)j * a.N];
+      asum += (uint64_t)yj * ((1ull << ALPHA_SHIFT) / a.q[j]);
+      uint64_t cr = 0;
+      const uint32_t* w = a.W + (size_t)j * a.Lfull;
+      for (uint32_t l = 0; l < a.Lfull; ++l) {
+        const uint64_t t = (uint64_t)yj * w[l] + V[l] + cr;
+        V[l] = (uint32_t)t; cr = t >> 32;
+      }
+      for (uint32_t l = a.Lfull; l < nl && cr; ++l) { const uint64_t t = (uint64_t)V[l] + cr; V[l] = (uint32_t)t; cr = t >> 32; }
+    }
+    const uint32_t alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
+    {
+      uint64_t cr = 0;
+      for (uint32_t l = 0; l < a.Lfull; ++l) {
+        const uint64_t t = (uint64_t)alpha * a.negM[l] + V[l] + cr;
+        V[l] = (uint32_t)t; cr = t >> 32;
+      }
+    }
+    // x = V mod 2^(logP+logQ); k = ((x + 2^(logP-1)) >> logP) mod 2^logQ
+    big_shr_mask(V, a.Lfull, 0, a.logP + a.logQ, a.Lfull);
+    V[a.Lfull] = V[a.Lfull + 1] = 0;
+    big_add_pow2(V, a.Lfull + 1, a.logP - 1);
+    big_shr_mask(V, a.Lfull + 1, a.logP, a.logQ, a.L);
+    // z = (d + k) mod 2^logQ
+    const uint32_t* d = a.add + (size_t)o * a.add_outer + (size_t)i * a.add_inner + n;
+    uint32_t cy = 0;
+    for (uint32_t l = 0; l < a.L; ++l) {
+      const uint64_t t = (uint64_t)V[l] + d[(size_t)l * a.N] + cy;
+      V[l] = (uint32_t)t; cy = (uint32_t)(t >> 32);
+    }
+    V[a.L] = 0;                                                    // the carry out of 2^(32 L) is dropped by the mask below
+    big_shr_mask(V, a.L, 0, a.logQ, a.L);
+    if (a.rescale_bits) {
+      V[a.L] = 0;
+      big_add_pow2(V, a.L + 1, a.rescale_bits - 1);
+      big_shr_mask(V, a.L + 1, a.rescale_bits, a.logQ - a.rescale_bits, a.L);
+    }
+    uint32_t* dst = a.out + (size_t)o * a.out_outer + (size_t)i * a.out_inner + n;
+    for (uint32_t l = 0; l < a.L; ++l) dst[(size_t)l * a.N] = V[l];
+  }
+}
+
 // scratch layout of CrtEpi (words): negM table [nl + 2] | xs [Lx][TC] (BGV) | adds [L][TC] (relin modes) |
 // BGV divide-by-P scratch [scratch_limbs][TC]
 static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi::Params& ep, size_t& bytes) {
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   const bool bgv = pp.mode == POST_BGV_MODQ || pp.mode == POST_BGV_RELIN;
-  ep.nl = tg.nchunks * (pipe::NC / 4) - CRT_ALPHA_COLS / 4;
-  ep.xs_off = (ep.nl + 2 + 31) / 32 * 32;
+  ep.ntab = tg.nchunks * (pipe::NC / 4);
+  ep.nl = ep.ntab - CRT_ALPHA_COLS / 4 - (tg.top ? TOP_LIMBS : 0);
+  ep.xs_off = (ep.ntab + 31) / 32 * 32;
   ep.adds_off = ep.xs_off + (bgv ? tg.Lx * TC : 0);
   ep.scratch_off = ep.adds_off + (relin ? pp.L * TC : 0);
   bytes = ((size_t)ep.scratch_off + (pp.mode == POST_BGV_RELIN ? pp.scratch_limbs * TC : 0)) * 4;
@@ -441,16 +560,35 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;
   ep.negM = tg.d_negM; ep.Lraw = tg.Lraw; ep.Lx = tg.Lx; ep.pp = pp;
   ep.tmq = top_mask(pp.logQ);
-  ep.ws = pp.logP >> 5; ep.bs = pp.logP & 31;
-  ep.rb = pp.logP ? (pp.logP - 1) >> 5 : 0; ep.rbit = pp.logP ? 1u << ((pp.logP - 1) & 31) : 0;
+  const uint32_t shiftP = tg.top ? 0 : pp.logP;                  // the top form hands the epilogue V >> logP directly
+  ep.ws = shiftP >> 5; ep.bs = shiftP & 31;
+  ep.rb = shiftP ? (shiftP - 1) >> 5 : 0; ep.rbit = shiftP ? 1u << ((shiftP - 1) & 31) : 0;
+  ep.top = tg.top ? 1 : 0; ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = c->d_flags;
   const uint32_t pb = pp.rescale_bits;
   ep.ws2 = pb >> 5; ep.bs2 = pb & 31;
   ep.rb2 = pb ? (pb - 1) >> 5 : 0; ep.rbit2 = pb ? 1u << ((pb - 1) & 31) : 0;
   const uint32_t nb = pp.logQ - pb;
   ep.Lr = (nb + 31) / 32; ep.tm2 = top_mask(nb);
   ep.lend = ep.ws + pp.L + (pb ? ep.ws2 + 1 : 0);                 // last limb index the relin stream must see
+  if (tg.top) {
+    cudaError_t e = cudaMemsetAsync(c->d_flags, 0, sizeof(uint32_t), s);
+    if (e != cudaSuccess) return e;
+  }
+  cudaError_t e;
+  {
+    LaunchTimer lt(c, KC_CRT, s);
+    e = pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
+  }
+  if (e != cudaSuccess || !tg.top) return e;
   LaunchTimer lt(c, KC_CRT, s);
-  return pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
+  ExactArgs x;
+  x.flags = c->d_flags; x.res = d_res; x.res_outer = res_outer; x.res_inner = res_inner;
+  x.add = d_add; x.add_outer = add_outer; x.add_inner = add_inner;
+  x.out = d_out; x.out_outer = out_outer; x.out_inner = out_inner;
+  x.W = tg.d_Wfull; x.negM = tg.d_negMfull; x.q = c->d_q;
+  x.N = c->N; x.K = tg.K; x.Lfull = tg.Lfull; x.L = pp.L; x.logP = pp.logP; x.logQ = pp.logQ; x.rescale_bits = pp.rescale_bits;
+  crt_exact_kernel<<<32, 64, 0, s>>>(x);
+  return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------------------------

@@ -416,3 +416,33 @@ def test_empty_batch_is_a_no_op():
     a = torch.empty((0, ctx.L, 256), dtype=torch.int32, device="cuda")
     out = ctx.fhe_polymul(a, a)
     assert out.shape[0] == 0
+
+
+@pytest.mark.parametrize("bits", [1, 4, 58])
+@pytest.mark.parametrize("logQ,logP", [(128, 128), (100, 96), (218, 250)])
+def test_relin_top_form_and_its_exact_path(bits, logQ, logP):
+    """The CKKS relin CRT takes the carry out of the low logP bits from 96-bit truncated constants and
+    recomputes flagged coefficients exactly.  With the flag threshold lowered to 1 or 4 fractional bits half resp. 1/16
+    of the coefficients go down the exact path; every setting must give the oracle's limbs, with and without rescale."""
+    fhe = _lib()
+    N, B, p = 256, 2, 40
+    prm = scheme.Params(N, logQ, logP, 0)
+    ctx = fhe.Context(N, logQ, logP)
+    ctx.fhe_debug_crt_ambiguity(bits)
+    g = synth.rng(900 + bits + logP)
+    d3_np = synth.uniform_limbs(g, (B, 3), N, logQ)
+    evk_np = synth.uniform_limbs(g, (2,), N, logQ + logP)
+    d3 = [[from_limbs(d3_np[i, k]) for k in range(3)] for i in range(B)]
+    evk = tuple(from_limbs(evk_np[k]) for k in range(2))
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk_np))
+    r2 = ctx.fhe_relinearize(limbs_np_to_tensor(d3_np))
+    want2 = [scheme.relinearize(prm, tuple(d3[i]), evk) for i in range(B)]
+    assert tensor_to_polys(r2) == [[list(q) for q in w] for w in want2]
+    # fused path (he_mult -> relin -> rescale) against the oracle's three calls
+    ct_np = synth.uniform_limbs(g, (2, B, 2), N, logQ)
+    fused = ctx.fhe_mult_relin_rescale(limbs_np_to_tensor(ct_np[0]), limbs_np_to_tensor(ct_np[1]), p)
+    for i in range(B):
+        c1 = tuple(from_limbs(ct_np[0, i, k]) for k in range(2))
+        c2 = tuple(from_limbs(ct_np[1, i, k]) for k in range(2))
+        want = scheme.rescale(prm, scheme.relinearize(prm, scheme.he_mult(prm, c1, c2), evk), p)
+        assert tensor_to_polys(fused[i]) == [list(q) for q in want]
