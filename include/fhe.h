@@ -132,6 +132,20 @@ fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t
 fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uint32_t* h_ct1, const uint32_t* h_ct2,
                                        uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream);
 
+/* ---- NEXT-1: coefficient-wise ciphertext operations and the level drop -------------------------------
+ * The paper lists them by name (add_pairwise_into, sub_pairwise_into, negate_pairwise_into, PAPER.md:654-662;
+ * moddownBy_pairwise_into).  Polynomials are limb-major [L][N], `npoly` of them back to back (a batch of B
+ * ciphertexts is 2 B polynomials); inputs canonical in [0, Q), outputs canonical.  In place (d_out == d_a) is allowed.
+ *   fhe_add / fhe_sub / fhe_negate   (a + b) mod Q, (a - b) mod Q, (-a) mod Q, CKKS (Q = 2^logQ) and BGV (odd Q).
+ *   fhe_moddown                      CKKS only: every coefficient mod 2^new_logq, 1 <= new_logq <= logQ, same L-limb stride
+ *                                    (the limbs above new_logq are written as zero).  A ciphertext at the lower level is
+ *                                    then used with a context created for logQ = new_logq (its evk is the original one
+ *                                    reduced mod 2^(logP + new_logq): fhe_set_evk masks on load when given L_PQ' limbs). */
+fhe_status fhe_add(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream);
+fhe_status fhe_sub(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream);
+fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32_t npoly, void* stream);
+fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream);
+
 /* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
 
 /* Host copies of the first `count` NTT primes and the primitive 2N-th roots psi_j the tables were built from. */

@@ -131,3 +131,30 @@ def rescale(prm: Params, ct, p: int):
     assert prm.is_ckks and 1 <= p < prm.logQ
     Q2 = 1 << (prm.logQ - p)
     return tuple([round_shift(int(c), p) % Q2 for c in comp] for comp in ct)
+
+
+# ---- NEXT-1: the coefficient-wise ciphertext operations and the level drop -----------------------------
+# The paper lists them by name only (add_pairwise_into, sub_pairwise_into, negate_pairwise_into, PAPER.md:654-662;
+# moddownBy_pairwise_into, "modulus switching operation to reduce ciphertext level").  In the ring
+# Z_Q[X]/(X^N+1) they are the component-wise definitions below on canonical representatives in [0, Q); with
+# Q = 2^logq dropping to a smaller power of two is reduction mod 2^logq' (A3 / A12 conventions).
+def ct_add(prm: Params, ct1, ct2):
+    Q = prm.Q
+    return tuple([(x + y) % Q for x, y in zip(a, b)] for a, b in zip(ct1, ct2))
+
+
+def ct_sub(prm: Params, ct1, ct2):
+    Q = prm.Q
+    return tuple([(x - y) % Q for x, y in zip(a, b)] for a, b in zip(ct1, ct2))
+
+
+def ct_negate(prm: Params, ct):
+    Q = prm.Q
+    return tuple([(-x) % Q for x in a] for a in ct)
+
+
+def moddown(prm: Params, ct, new_logq: int):
+    """CKKS only: the same ciphertext one or more levels down, every coefficient mod 2^new_logq."""
+    assert prm.is_ckks and 1 <= new_logq <= prm.logQ
+    m = 1 << new_logq
+    return tuple([x % m for x in a] for a in ct)

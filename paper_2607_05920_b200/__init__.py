@@ -24,6 +24,7 @@ EXPORTS = [
     "fhe_set_evk", "fhe_polymul", "fhe_he_mult", "fhe_relinearize", "fhe_rescale", "fhe_mult_relin_rescale",
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
+    "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown",
 ]
 
 
@@ -86,6 +87,10 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_debug_ntt.restype = c_int
     lib.fhe_debug_launch_count.argtypes = [vp]
     lib.fhe_debug_launch_count.restype = c_uint64
+    lib.fhe_add.argtypes = lib.fhe_sub.argtypes = [vp, vp, vp, vp, c_uint32, vp]
+    lib.fhe_negate.argtypes = [vp, vp, vp, c_uint32, vp]
+    lib.fhe_moddown.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
+    lib.fhe_add.restype = lib.fhe_sub.restype = lib.fhe_negate.restype = lib.fhe_moddown.restype = c_int
     lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
     lib.fhe_debug_crt_ambiguity.restype = c_int
     lib.fhe_debug_int_peak.argtypes = [vp, c_int, POINTER(ctypes.c_double), vp]
@@ -282,6 +287,33 @@ class Context:
         self._check(self._lib.fhe_mult_relin_rescale_host(self._h, h_out.data_ptr(), h_ct1.data_ptr(), h_ct2.data_ptr(),
                                                           p_bits, batch, ws.data_ptr(), nb, self._stream(stream)))
         return h_out
+
+    # ---- NEXT-1: coefficient-wise operations on [..., L, N] tensors (any leading shape) ----
+    def _elem(self, fn, a, b, out, extra=()):
+        npoly = a.numel() // (self.L * self.N)
+        n = npoly * self.L * self.N
+        out = self._torch_empty_like(a) if out is None else out
+        args = [self._h, _dev_ptr(out, n, "out"), _dev_ptr(a, n, "a")]
+        if b is not None:
+            args.append(_dev_ptr(b, n, "b"))
+        self._check(fn(*args, *extra, npoly, self._stream(None)))
+        return out
+
+    @staticmethod
+    def _torch_empty_like(a):
+        return _torch().empty_like(a)
+
+    def fhe_add(self, a, b, out=None):
+        return self._elem(self._lib.fhe_add, a, b, out)
+
+    def fhe_sub(self, a, b, out=None):
+        return self._elem(self._lib.fhe_sub, a, b, out)
+
+    def fhe_negate(self, a, out=None):
+        return self._elem(self._lib.fhe_negate, a, None, out)
+
+    def fhe_moddown(self, a, new_logq: int, out=None):
+        return self._elem(self._lib.fhe_moddown, a, None, out, extra=(new_logq,))
 
     # ---- debug entry points --------------------------------------------------------------------------------------
     def fhe_debug_decompose(self, limbs, K: int, mask_bits: int = 0, stream=None):

@@ -220,6 +220,35 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
   return FHE_OK;
 }
 
+// ---- NEXT-1: coefficient-wise operations (kernels_elem.cu) --------------------------------------------------------------
+static fhe_status elem_call(fhe_ctx* ctx, int op, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
+                            uint32_t bits, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (npoly == 0) return FHE_OK;
+  if (!d_out || !d_a || (op <= 1 && !d_b)) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out, 16) || misaligned(d_a, 16) || (op <= 1 && misaligned(d_b, 16))) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (c->N < 256) return err(c, FHE_ERR_UNSUPPORTED, "N < 256");
+  CK(launch_elem(c, op, d_out, d_a, d_b, npoly, bits, (cudaStream_t)stream), "elementwise");
+  return FHE_OK;
+}
+fhe_status fhe_add(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream) {
+  return elem_call(ctx, 0, d_out, d_a, d_b, npoly, ctx ? C(ctx)->logQ : 0, stream);
+}
+fhe_status fhe_sub(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream) {
+  return elem_call(ctx, 1, d_out, d_a, d_b, npoly, ctx ? C(ctx)->logQ : 0, stream);
+}
+fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32_t npoly, void* stream) {
+  return elem_call(ctx, 2, d_out, d_a, nullptr, npoly, ctx ? C(ctx)->logQ : 0, stream);
+}
+fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (c->t != 0) return err(c, FHE_ERR_UNSUPPORTED, "moddown is CKKS-only");
+  if (new_logq < 1 || new_logq > c->logQ) return err(c, FHE_ERR_ARG, "new_logq out of range");
+  return elem_call(ctx, 3, d_out, d_in, nullptr, npoly, new_logq, stream);
+}
+
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);

@@ -154,6 +154,10 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
 // register-only throughput of the NTT butterfly (mode 0), mad.lo.u32 (1), mul.hi.u32 (2) on this device, per second
 cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s);
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the pipeline have the TMEM / shared memory for it
+// coefficient-wise ring operations (kernels_elem.cu): op 0 add, 1 sub, 2 negate, 3 reduce mod 2^bits (CKKS); bits = the
+// modulus width the result is masked to (CKKS)
+cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
+                        uint32_t bits, cudaStream_t s);
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -1,0 +1,120 @@
+// kernels_elem.cu -- NEXT-1: the coefficient-wise ciphertext operations the paper lists by name
+// (add_pairwise_into, sub_pairwise_into, negate_pairwise_into) and the level drop
+// (moddownBy_pairwise_into) on limb-major polynomials [L][N] with canonical coefficients in [0, Q).
+// HBM-bound streaming kernels: one thread per coefficient, so every limb access of a warp is one 128-byte line; the
+// carry / borrow runs along the limbs inside the thread.
+//   CKKS (Q = 2^logQ):  the sum / difference wraps mod 2^(32 L) by itself; the top limb is masked.
+//   BGV  (odd Q):       a + b in [0, 2Q): subtract Q when >= Q; a - b: add Q on borrow; -a = Q - a for a != 0.
+//                       The comparison with Q needs all limbs, so the coefficient is kept in a local array.
+#include "fhe_internal.cuh"
+
+namespace fhe {
+
+constexpr uint32_t ELEM_MAX_LIMBS = 88;   // logQ <= 2560 (+ one limb for an odd Q just above 2^logQ)
+
+enum ElemOp : int { EL_ADD = 0, EL_SUB = 1, EL_NEG = 2, EL_MODDOWN = 3 };
+
+__device__ __forceinline__ uint32_t top_mask32(uint32_t bits) { return (bits & 31) ? ((1u << (bits & 31)) - 1u) : 0xFFFFFFFFu; }
+
+template <int OP>
+__global__ void __launch_bounds__(256)
+elem_ckks_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, const uint32_t* __restrict__ b, uint32_t N,
+                 uint32_t L, uint32_t bits) {
+  const uint32_t bpp = N / 256;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
+  const size_t base = (size_t)poly * L * N + n;
+  const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);     // limbs that hold bits; the rest of the L limbs are zero
+  uint32_t carry = OP == EL_NEG ? 1u : 0u;                          // -a = ~a + 1
+  for (uint32_t l = 0; l < L; ++l) {
+    uint32_t v = 0;
+    if (l < Lb) {
+      const uint32_t x = a[base + (size_t)l * N];
+      if (OP == EL_ADD) {
+        const uint64_t s = (uint64_t)x + b[base + (size_t)l * N] + carry;
+        v = (uint32_t)s; carry = (uint32_t)(s >> 32);
+      } else if (OP == EL_SUB) {
+        const uint32_t y = b[base + (size_t)l * N];
+        const uint32_t d = x - y, d2 = d - carry;
+        carry = (x < y) | (d < carry);
+        v = d2;
+      } else if (OP == EL_NEG) {
+        const uint64_t s = (uint64_t)(~x) + carry;
+        v = (uint32_t)s; carry = (uint32_t)(s >> 32);
+      } else {
+        v = x;
+      }
+      if (l == Lb - 1) v &= tm;
+    }
+    out[base + (size_t)l * N] = v;
+  }
+}
+
+template <int OP>
+__global__ void __launch_bounds__(256)
+elem_bgv_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, const uint32_t* __restrict__ b,
+                const uint32_t* __restrict__ Q, uint32_t N, uint32_t L) {
+  const uint32_t bpp = N / 256;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
+  const size_t base = (size_t)poly * L * N + n;
+  uint32_t r[ELEM_MAX_LIMBS];
+  if (OP == EL_ADD) {
+    uint32_t carry = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      const uint64_t s = (uint64_t)a[base + (size_t)l * N] + b[base + (size_t)l * N] + carry;
+      r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
+    }
+    bool ge = carry != 0;                                           // sum >= 2^(32 L) > Q
+    if (!ge) {
+      ge = true;
+      for (uint32_t l = L; l-- > 0;) { const uint32_t q = __ldg(Q + l); if (r[l] != q) { ge = r[l] > q; break; } }
+    }
+    uint32_t borrow = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = r[l];
+      if (ge) { const uint32_t q = __ldg(Q + l); const uint32_t d = v - q, d2 = d - borrow; borrow = (v < q) | (d < borrow); v = d2; }
+      out[base + (size_t)l * N] = v;
+    }
+  } else {                                                          // a - b (EL_NEG: 0 - a)
+    uint32_t borrow = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      const uint32_t x = OP == EL_NEG ? 0u : a[base + (size_t)l * N];
+      const uint32_t y = OP == EL_NEG ? a[base + (size_t)l * N] : b[base + (size_t)l * N];
+      const uint32_t d = x - y, d2 = d - borrow;
+      borrow = (x < y) | (d < borrow);
+      r[l] = d2;
+    }
+    uint32_t carry = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = r[l];
+      if (borrow) { const uint64_t s = (uint64_t)v + __ldg(Q + l) + carry; v = (uint32_t)s; carry = (uint32_t)(s >> 32); }
+      out[base + (size_t)l * N] = v;
+    }
+  }
+}
+
+cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
+                        uint32_t bits, cudaStream_t s) {
+  if (!npoly) return cudaSuccess;
+  if (c->L > ELEM_MAX_LIMBS) return cudaErrorInvalidValue;
+  const uint32_t grid = (c->N / 256) * npoly;
+  LaunchTimer lt(c, KC_RESCALE, s);
+  if (c->t == 0) {
+    switch (op) {
+      case EL_ADD: elem_ckks_kernel<EL_ADD><<<grid, 256, 0, s>>>(d_out, d_a, d_b, c->N, c->L, bits); break;
+      case EL_SUB: elem_ckks_kernel<EL_SUB><<<grid, 256, 0, s>>>(d_out, d_a, d_b, c->N, c->L, bits); break;
+      case EL_NEG: elem_ckks_kernel<EL_NEG><<<grid, 256, 0, s>>>(d_out, d_a, d_a, c->N, c->L, bits); break;
+      case EL_MODDOWN: elem_ckks_kernel<EL_MODDOWN><<<grid, 256, 0, s>>>(d_out, d_a, d_a, c->N, c->L, bits); break;
+      default: return cudaErrorInvalidValue;
+    }
+  } else {
+    switch (op) {
+      case EL_ADD: elem_bgv_kernel<EL_ADD><<<grid, 256, 0, s>>>(d_out, d_a, d_b, c->d_Qlimbs, c->N, c->L); break;
+      case EL_SUB: elem_bgv_kernel<EL_SUB><<<grid, 256, 0, s>>>(d_out, d_a, d_b, c->d_Qlimbs, c->N, c->L); break;
+      case EL_NEG: elem_bgv_kernel<EL_NEG><<<grid, 256, 0, s>>>(d_out, d_a, d_a, c->d_Qlimbs, c->N, c->L); break;
+      default: return cudaErrorInvalidValue;
+    }
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace fhe

@@ -446,3 +446,58 @@ def test_relin_top_form_and_its_exact_path(bits, logQ, logP):
         c2 = tuple(from_limbs(ct_np[1, i, k]) for k in range(2))
         want = scheme.rescale(prm, scheme.relinearize(prm, scheme.he_mult(prm, c1, c2), evk), p)
         assert tensor_to_polys(fused[i]) == [list(q) for q in want]
+
+
+# ---- NEXT-1: coefficient-wise operations, level drop, and a depth-2 circuit across two levels ----------------
+@pytest.mark.parametrize("N,logQ,t", [(256, 128, 0), (1024, 218, 0), (256, 100, 257), (1024, 437, 65537)])
+def test_next1_add_sub_negate_match_the_oracle(N, logQ, t):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logQ, t)
+    ctx = fhe.Context(N, logQ, logQ, t)
+    g = synth.rng(50 + N + logQ)
+    Q = prm.Q
+    rnd = np.random.default_rng(N + logQ)
+    def rand_ct():
+        ct = tuple([int.from_bytes(rnd.bytes((Q.bit_length() + 7) // 8 + 8), "little") % Q for _ in range(N)] for _ in range(2))
+        ct[0][0], ct[0][1], ct[1][0] = 0, Q - 1, Q - 1          # the ends of the range
+        return ct
+    c1, c2 = rand_ct(), rand_ct()
+    d1, d2 = polys_to_tensor([list(c1)], ctx.L), polys_to_tensor([list(c2)], ctx.L)
+    assert tensor_to_polys(ctx.fhe_add(d1, d2))[0] == [list(p) for p in scheme.ct_add(prm, c1, c2)]
+    assert tensor_to_polys(ctx.fhe_sub(d1, d2))[0] == [list(p) for p in scheme.ct_sub(prm, c1, c2)]
+    assert tensor_to_polys(ctx.fhe_negate(d1))[0] == [list(p) for p in scheme.ct_negate(prm, c1)]
+    assert torch.equal(ctx.fhe_sub(ctx.fhe_add(d1, d2), d2), d1)
+
+
+def test_next1_moddown_and_depth_two_circuit_over_two_levels():
+    """(z1 z2) z3 on CKKS: multiply + relinearise + rescale at logQ = 128, drop the factor z3 to the new level with
+    fhe_moddown, multiply again with a context for logQ = 88 whose evk is the original one reduced mod 2^(logP + 88).
+    Every ciphertext equals the oracle's limb for limb; the final decryption is within 2^-20 of the slot product."""
+    fhe = _lib()
+    N, logQ, logP, p = 1 << 10, 128, 128, 40
+    prm, s, evk, cts1, cts2, zs = _ckks_setup(N, logQ, logP, 2, seed=5)
+    hi = fhe.Context(N, logQ, logP)
+    hi.fhe_set_evk(polys_to_tensor(list(evk), hi.L_PQ))
+    # level 1: ct12 = rescale(relin(ct1 * ct2)) has modulus 2^88
+    ct12 = hi.fhe_mult_relin_rescale(polys_to_tensor([cts1[0]], hi.L), polys_to_tensor([cts2[0]], hi.L), p)
+    want12 = scheme.rescale(prm, scheme.relinearize(prm, scheme.he_mult(prm, cts1[0], cts2[0]), evk), p)
+    assert tensor_to_polys(ct12)[0] == [list(q) for q in want12]
+    logq1 = logQ - p
+    # the third factor comes down to the same level by moddown
+    ct3 = hi.fhe_moddown(polys_to_tensor([cts1[1]], hi.L), logq1)
+    want3 = scheme.moddown(prm, cts1[1], logq1)
+    assert tensor_to_polys(ct3)[0] == [list(q) for q in want3]
+    # level 2 context: logQ = 88 (3 limbs), evk mod 2^(logP + 88)
+    prm1 = scheme.Params(N, logq1, logP, 0)
+    lo = fhe.Context(N, logq1, logP)
+    evk1 = tuple([x % prm1.PQ for x in e] for e in evk)
+    lo.fhe_set_evk(polys_to_tensor(list(evk1), lo.L_PQ))
+    a = ct12[..., : lo.L, :].contiguous()
+    b = ct3[..., : lo.L, :].contiguous()
+    out = lo.fhe_mult_relin_rescale(a, b, p)
+    want = scheme.rescale(prm1, scheme.relinearize(prm1, scheme.he_mult(prm1, want12, want3), evk1), p)
+    got = tensor_to_polys(out)[0]
+    assert got == [list(q) for q in want]
+    mu = harness.decrypt(tuple(got), s, 1 << (logq1 - p))
+    z = harness.decode(mu, N, 2.0 ** 40)
+    assert np.max(np.abs(z - zs[0][0] * zs[0][1] * zs[1][0])) <= 2.0 ** -20

@@ -319,3 +319,41 @@ def test_r4_bgv_exact(N, logQ, t, hwt):
     assert all(e % t == 0 for e in err) and max(abs(e) for e in err) < t * N * 64
     zero = [0] * N
     assert scheme.relinearize(prm, (d[0], d[1], zero), evk) == (d[0], d[1])
+
+
+# ---- NEXT-1: coefficient-wise operations and the level drop (parity unpinned by the paper: names only) --------------------
+def test_next1_elementwise_ops_are_the_ring_operations_and_decrypt_homomorphically():
+    """ct_add / ct_sub / ct_negate: group laws on random data, and Dec(add) = Dec(ct1) + Dec(ct2) mod Q exactly (the
+    decryption map c0 + c1 s is linear); BGV: plaintexts add mod t.  moddown: Dec(moddown(ct)) = Dec(ct) mod 2^logq'."""
+    import numpy as np
+    import synth
+    from oracle import harness, scheme
+    N, logQ, logP = 64, 100, 100
+    prm = scheme.Params(N, logQ, logP, 0)
+    g = synth.rng(31)
+    s, _ = harness.keygen(prm, g, hwt=16)
+    z1, z2 = synth.unit_disk(g, N // 2), synth.unit_disk(g, N // 2)
+    ct1 = harness.encrypt(prm, g, s, harness.encode(z1, N, 2.0 ** 30))
+    ct2 = harness.encrypt(prm, g, s, harness.encode(z2, N, 2.0 ** 30))
+    Q = prm.Q
+    add, sub, neg = scheme.ct_add(prm, ct1, ct2), scheme.ct_sub(prm, ct1, ct2), scheme.ct_negate(prm, ct2)
+    assert scheme.ct_sub(prm, add, ct2) == tuple(list(a) for a in ct1)
+    assert scheme.ct_add(prm, ct1, neg) == sub
+    assert scheme.ct_add(prm, ct2, neg) == tuple([0] * N for _ in range(2))
+    d1, d2 = harness.decrypt(ct1, s, Q), harness.decrypt(ct2, s, Q)
+    assert [x % Q for x in harness.decrypt(add, s, Q)] == [(a + b) % Q for a, b in zip(d1, d2)]
+    assert np.max(np.abs(harness.decode(harness.decrypt(add, s, Q), N, 2.0 ** 30) - (z1 + z2))) < 1e-6
+    assert np.max(np.abs(harness.decode(harness.decrypt(sub, s, Q), N, 2.0 ** 30) - (z1 - z2))) < 1e-6
+    low = scheme.moddown(prm, ct1, 70)
+    assert all(0 <= x < (1 << 70) for a in low for x in a)
+    assert [x % (1 << 70) for x in harness.decrypt(low, s, 1 << 70)] == [x % (1 << 70) for x in d1]
+    assert np.max(np.abs(harness.decode(harness.decrypt(low, s, 1 << 70), N, 2.0 ** 30) - z1)) < 1e-6
+    # BGV: exact mod t
+    prb = scheme.Params(N, 60, 60, 257)
+    sb, _ = harness.keygen(prb, g, hwt=None)
+    m1 = [int(v) for v in g.integers(0, 257, size=N)]
+    m2 = [int(v) for v in g.integers(0, 257, size=N)]
+    c1, c2 = harness.encrypt(prb, g, sb, m1), harness.encrypt(prb, g, sb, m2)
+    assert harness.decrypt_bgv(scheme.ct_add(prb, c1, c2), sb, prb) == [(a + b) % 257 for a, b in zip(m1, m2)]
+    assert harness.decrypt_bgv(scheme.ct_sub(prb, c1, c2), sb, prb) == [(a - b) % 257 for a, b in zip(m1, m2)]
+    assert harness.decrypt_bgv(scheme.ct_negate(prb, c1), sb, prb) == [(-a) % 257 for a in m1]
