@@ -431,6 +431,47 @@ def run_sweep(args):
     dev = torch.device("cuda", local_rank)
     hbm_gbs, _ = _peaks()
     stream = torch.cuda.current_stream(dev)
+    # NEXT-1 streaming kernels at the C5 shape: a batch of 64 ciphertexts (2.6 GB of traffic per call), against HBM
+    ctx = fhe.Context(1 << 16, 1240, 1240)
+    g = synth.rng(0)
+    x1 = torch.from_numpy(synth.uniform_limbs(g, (1, 2), 1 << 16, 1240).view(np.int32)).to(dev).expand(64, 2, ctx.L, 1 << 16).contiguous()
+    x2 = x1.clone()
+    y = torch.empty_like(x1)
+    for name, fn, nbuf in (("fhe_add", lambda: ctx.fhe_add(x1, x2, out=y), 3), ("fhe_sub", lambda: ctx.fhe_sub(x1, x2, out=y), 3),
+                           ("fhe_negate", lambda: ctx.fhe_negate(x1, out=y), 2), ("fhe_moddown", lambda: ctx.fhe_moddown(x1, 1200, out=y), 2)):
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(5):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 5
+        byts = nbuf * x1.numel() * 4
+        print(json.dumps({"sweep": True, "metric": name + " ciphertexts/s", "value": 64 / (ms / 1e3), "unit": "ciphertexts/s",
+                          "N": 1 << 16, "logQ": 1240, "batch": 64, "ms_per_call": ms, "gb_per_s": byts / (ms / 1e3) / 1e9,
+                          "roofline": {"bound": "hbm", "achieved": byts / (ms / 1e3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                                       "frac": byts / (ms / 1e3) / 1e9 / hbm_gbs}, "data": "synthetic"}), flush=True)
+    # NEXT-2: rotation (automorphism + key switch with a rotation key) of a batch of 4 ciphertexts at the C5 shape
+    ctx.fhe_set_rotation_key(0, 5, torch.from_numpy(synth.uniform_limbs(g, (2,), 1 << 16, 2480).view(np.int32)).to(dev))
+    xr = x1[:4].contiguous()
+    yr = torch.empty_like(xr)
+    for _ in range(3):
+        ctx.fhe_rotate(xr, 0, out=yr, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(10):
+        ctx.fhe_rotate(xr, 0, out=yr, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 10
+    print(json.dumps({"sweep": True, "metric": "fhe_rotate ciphertexts/s", "value": 4 / (ms / 1e3), "unit": "ciphertexts/s",
+                      "N": 1 << 16, "logQ": 1240, "logP": 1240, "batch": 4, "ms_per_call": ms, "data": "synthetic"}), flush=True)
+    del ctx, x1, x2, y, xr, yr
+    torch.cuda.empty_cache()
     for logN in (12, 13, 14, 15, 16):
         for logQ in (64, 256, 620, 1240, 2480):
             N = 1 << logN

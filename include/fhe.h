@@ -51,7 +51,8 @@ typedef enum {            /* `op` argument of fhe_workspace_bytes */
   FHE_OP_RELINEARIZE = 2,
   FHE_OP_RESCALE = 3,     /* needs no workspace: returns 0 */
   FHE_OP_MULT_RELIN_RESCALE = 4,
-  FHE_OP_SET_EVK = 5
+  FHE_OP_SET_EVK = 5,
+  FHE_OP_ROTATE = 6
 } fhe_op;
 
 typedef struct {
@@ -145,6 +146,19 @@ fhe_status fhe_add(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uin
 fhe_status fhe_sub(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream);
 fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32_t npoly, void* stream);
 fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream);
+
+/* ---- NEXT-2: slot rotation and conjugation ------------------------------------
+ * A rotation is the Galois automorphism X -> X^k (k odd, k < 2N; k = 2N - 1 conjugates) applied to both components,
+ * followed by a key switch from sigma_k(s) back to s: out = (sigma(c0) + kb, ka), (kb, ka) = round(sigma(c1) * rk / P)
+ * with the same divide-by-P rule as fhe_relinearize (A2/A3/A10) and a key of the same form as the evk,
+ * rk = (b', a') mod PQ, b' = -a' s + e' + P sigma_k(s) (BGV: t e').
+ *   fhe_set_rotation_key   installs the key for Galois element k in `slot` (0..15): decompose + forward NTT, once per key;
+ *                          d_key [2][L_PQ][N] as for fhe_set_evk.
+ *   fhe_rotate             d_in2, d_out2 [B][2][L][N]; d_ws >= fhe_workspace_bytes(FHE_OP_ROTATE, batch).
+ *                          FHE_ERR_STATE when the slot holds no key. */
+fhe_status fhe_set_rotation_key(fhe_ctx* ctx, uint32_t slot, uint32_t k, const uint32_t* d_key, void* stream);
+fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uint32_t slot, uint32_t batch, void* d_ws,
+                      size_t ws_bytes, void* stream);
 
 /* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
 

@@ -107,3 +107,31 @@ def decode(m, N: int, scale: float) -> np.ndarray:
     mf = np.array([float(int(x)) for x in m], dtype=np.float64)
     v = np.fft.ifft(mf * np.exp(1j * np.pi * k / N)) * N
     return v[: N // 2] / scale
+
+
+def rotkeygen(prm: Params, g: np.random.Generator, s, k: int, sigma: float = 3.2):
+    """Rotation / conjugation key for the Galois element k (DESIGN 3, NEXT-2 reading): rk = (b', a') mod PQ,
+    b' = -a' s + e' + P sigma_k(s)  (BGV: t e')."""
+    from .scheme import automorphism
+    N, PQ = prm.N, prm.PQ
+    e = synth.gaussian_error(g, N, sigma)
+    a = synth.uniform_big(g, N, (PQ - 1).bit_length() - (0 if prm.is_ckks else 1))
+    sk = automorphism([v % PQ for v in s], k, PQ)
+    a_s = pm_secret(a, s, PQ)
+    mult = 1 if prm.is_ckks else prm.t
+    b = [(-x + mult * int(ee) + prm.P * y) % PQ for x, ee, y in zip(a_s, e, sk)]
+    return b, a
+
+
+def slot_image(N: int, k: int):
+    """Where the automorphism X -> X^k sends the slots of `encode` (roots zeta_j = exp(i pi (2j+1)/N), j < N/2):
+    (sigma_k m)(zeta_j) = m(zeta_j^k) = m(zeta_j') with 2j'+1 = k (2j+1) mod 2N.  Returns (src, conj): new slot j holds
+    z[src[j]], conjugated where conj[j] (j' >= N/2 is the conjugate of slot N-1-j')."""
+    src, conj = [], []
+    for j in range(N // 2):
+        jp = ((k * (2 * j + 1)) % (2 * N) - 1) // 2
+        if jp < N // 2:
+            src.append(jp); conj.append(False)
+        else:
+            src.append(N - 1 - jp); conj.append(True)
+    return src, conj

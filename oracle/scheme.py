@@ -158,3 +158,29 @@ def moddown(prm: Params, ct, new_logq: int):
     assert prm.is_ckks and 1 <= new_logq <= prm.logQ
     m = 1 << new_logq
     return tuple([x % m for x in a] for a in ct)
+
+
+# ---- NEXT-2: slot rotation / conjugation --------------------------------------------------------------------
+# The paper names the operations (conjugate_pairwise_into, leftrotate_broadcast_into with "precomputed Galois / rotation
+# keys") and gives no formula.  Reading: the Galois automorphism sigma_k: a(X) -> a(X^k) on both
+# components, then the key switch of A2 / A3 / A10 with the key rk = (b', a'), b' = -a' s + e' + P sigma_k(s): the triple
+# (sigma(c0), 0, sigma(c1)) decrypts under (1, s, sigma_k(s)) exactly like a tensor triple under (1, s, s^2), so the
+# relinearisation procedure applies unchanged.
+def automorphism(a, k: int, M: int) -> list:
+    """a(X^k) mod (X^N + 1, M), k odd: coefficient i moves to i k mod 2N, negated when that is >= N."""
+    N = len(a)
+    assert k % 2 == 1
+    out = [0] * N
+    for i, x in enumerate(a):
+        j = (i * k) % (2 * N)
+        if j < N:
+            out[j] = x % M
+        else:
+            out[j - N] = (-x) % M
+    return out
+
+
+def rotate(prm: Params, ct, k: int, rk):
+    Q = prm.Q
+    d = (automorphism(ct[0], k, Q), [0] * prm.N, automorphism(ct[1], k, Q))
+    return relinearize(prm, d, rk)

@@ -43,12 +43,13 @@ fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const
 
 // relin core: in3 [B][3][L][N] -> out2 [B][2][L][N]; ws: [B][2][K2][N]; rescale_bits fused into the CRT epilogue
 fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_t B, uint32_t* ws, uint32_t rescale_bits,
-                    cudaStream_t s) {
+                    cudaStream_t s, const uint32_t* d_key_hat = nullptr) {
+  if (!d_key_hat) d_key_hat = c->d_evk_hat;
   const uint32_t N = c->N, L = c->L, K = c->K2;
   const size_t rp = (size_t)K * N;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ws, 2 * rp, 0, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, 0, B, 1, L, K, mask, s), "decompose d2");
-  CK(launch_ntt_product(c, ws, c->d_evk_hat, B, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt relin");
+  CK(launch_ntt_product(c, ws, const_cast<uint32_t*>(d_key_hat), B, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt relin");
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
   pp.amb_bits = c->amb_bits;
@@ -74,8 +75,23 @@ size_t fhe_workspace_bytes(const fhe_ctx* ctx, int op, uint32_t batch) {
       return (a > b ? a : b) + ws_d3(c, batch);
     }
     case FHE_OP_SET_EVK: return ws_evk(c);
+    case FHE_OP_ROTATE: return ws_relin(c, batch) + ws_d3(c, batch);
     default: return 0;
   }
+}
+
+// decompose + forward NTT of a key (b', a') mod PQ into *slot ([2][K2][N], allocated on first use)
+static fhe_status install_key(Context* c, uint32_t** slot, const uint32_t* d_key, cudaStream_t s) {
+  const size_t bytes = (size_t)2 * c->K2 * c->N * 4;
+  if (!*slot) {
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return err(c, FHE_ERR_NOMEM, "key allocation failed"); }
+    *slot = (uint32_t*)p;
+  }
+  const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
+  CK(launch_decompose(c, *slot, 0, (size_t)c->K2 * c->N, d_key, 0, (size_t)c->L_PQ * c->N, 1, 2, c->L_PQ, c->K2, mask, s), "decompose key");
+  CK(launch_ntt_fwd(c, *slot, 1, 2, 2, c->K2, s), "ntt key");
+  return FHE_OK;
 }
 
 fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t ws_bytes, void* stream) {
@@ -83,19 +99,42 @@ fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t w
   Context* c = C(ctx);
   (void)d_ws; (void)ws_bytes;
   if (!d_evk || misaligned(d_evk, 16)) return err(c, FHE_ERR_ARG, "d_evk NULL or misaligned");
-  cudaStream_t s = (cudaStream_t)stream;
-  const size_t bytes = (size_t)2 * c->K2 * c->N * 4;
-  if (!c->d_evk_hat) {
-    void* p = nullptr;
-    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return err(c, FHE_ERR_NOMEM, "evk-hat allocation failed"); }
-    c->d_evk_hat = (uint32_t*)p;
-  }
   c->have_evk = false;
-  const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
-  CK(launch_decompose(c, c->d_evk_hat, 0, (size_t)c->K2 * c->N, d_evk, 0, (size_t)c->L_PQ * c->N, 1, 2, c->L_PQ, c->K2, mask, s), "decompose evk");
-  CK(launch_ntt_fwd(c, c->d_evk_hat, 1, 2, 2, c->K2, s), "ntt evk");
+  fhe_status st = install_key(c, &c->d_evk_hat, d_evk, (cudaStream_t)stream);
+  if (st != FHE_OK) return st;
   c->have_evk = true;
   return FHE_OK;
+}
+
+fhe_status fhe_set_rotation_key(fhe_ctx* ctx, uint32_t slot, uint32_t k, const uint32_t* d_key, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (slot >= (uint32_t)Context::MAX_ROT_KEYS) return err(c, FHE_ERR_ARG, "key slot out of range");
+  if (!(k & 1) || k >= 2 * c->N) return err(c, FHE_ERR_ARG, "Galois element must be odd and below 2N");
+  if (!d_key || misaligned(d_key, 16)) return err(c, FHE_ERR_ARG, "d_key NULL or misaligned");
+  c->rot_k[slot] = 0;
+  fhe_status st = install_key(c, &c->d_rot_hat[slot], d_key, (cudaStream_t)stream);
+  if (st != FHE_OK) return st;
+  c->rot_k[slot] = k;
+  return FHE_OK;
+}
+
+fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uint32_t slot, uint32_t batch, void* d_ws,
+                      size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_in2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_in2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (slot >= (uint32_t)Context::MAX_ROT_KEYS || !c->rot_k[slot]) return err(c, FHE_ERR_STATE, "no rotation key in this slot");
+  if (c->N < 256) return err(c, FHE_ERR_UNSUPPORTED, "N < 256");
+  if (!c->fit_relin) return err(c, FHE_ERR_UNSUPPORTED, "relinearisation CRT target too large for the conversion pipeline");
+  if (ws_bytes < ws_relin(c, batch) + ws_d3(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  cudaStream_t s = (cudaStream_t)stream;
+  uint32_t* d3 = (uint32_t*)d_ws;
+  uint32_t* ws = (uint32_t*)((char*)d_ws + ws_d3(c, batch));
+  CK(launch_automorphism(c, d3, d_in2, c->rot_k[slot], batch, s), "automorphism");
+  return do_relin(c, d_out2, d3, batch, ws, 0, s, c->d_rot_hat[slot]);
 }
 
 fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,

@@ -237,6 +237,7 @@ static void destroy(Context* c) {
   if (!c) return;
   for (void* p : c->allocs) cudaFree(p);
   if (c->d_evk_hat) cudaFree(c->d_evk_hat);
+  for (int i = 0; i < Context::MAX_ROT_KEYS; ++i) if (c->d_rot_hat[i]) cudaFree(c->d_rot_hat[i]);
   for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
   if (c->s_d2h) cudaStreamDestroy(c->s_d2h);

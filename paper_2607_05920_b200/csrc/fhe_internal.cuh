@@ -90,6 +90,10 @@ struct Context {
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
   bool have_evk = false;
+  // rotation / conjugation keys (NEXT-2): same form as the evk, one per slot, with the Galois element they belong to
+  static constexpr int MAX_ROT_KEYS = 16;
+  uint32_t* d_rot_hat[MAX_ROT_KEYS] = {};
+  uint32_t rot_k[MAX_ROT_KEYS] = {};
   // copy streams and events of the host-buffer entry point (created with the context; the hot path creates nothing)
   static constexpr int HOST_PIECES = 32;
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
@@ -158,6 +162,9 @@ bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the p
 // modulus width the result is masked to (CKKS)
 cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
                         uint32_t bits, cudaStream_t s);
+// Galois automorphism X -> X^k (k odd) of ciphertexts (kernels_elem.cu): in2 [B][2][L][N] -> out3 [B][3][L][N] =
+// (sigma(c0), 0, sigma(c1)), the triple the key switch of a rotation consumes
+cudaError_t launch_automorphism(Context* c, uint32_t* d_out3, const uint32_t* d_in2, uint32_t k, uint32_t batch, cudaStream_t s);
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -92,6 +92,67 @@ elem_bgv_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, cons
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// NEXT-2: Galois automorphism sigma_k: a(X) -> a(X^k) mod (X^N + 1), k odd (rotation of the CKKS slots; k = 2N - 1 is
+// the conjugation).  Coefficient i moves to position i k mod 2N, with a sign flip when that is
+// >= N.  Gather form: out[n] = a[i] for i' = n k^-1 mod 2N < N (i = i'), else -a[i' - N].  Ciphertext component 0 goes
+// to slot 0 of the triple, component 1 to slot 2, slot 1 is zeroed: the key switch adds (round(sigma(c1) rk / P)) to
+// (sigma(c0), 0).  Reads are a permutation (one 32-byte sector per word); the kernel is a small part of a rotation.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+automorphism_kernel(uint32_t* __restrict__ out3, const uint32_t* __restrict__ in2, const uint32_t* __restrict__ Q, uint32_t N,
+                    uint32_t L, uint32_t bits, uint32_t kinv, uint32_t ckks) {
+  const uint32_t bpp = N / 256;
+  const uint32_t item = blockIdx.x / (3 * bpp), rem = blockIdx.x % (3 * bpp), slot = rem / bpp;
+  const uint32_t n = (rem % bpp) * 256 + threadIdx.x;
+  uint32_t* dst = out3 + ((size_t)item * 3 + slot) * L * N + n;
+  if (slot == 1) {
+    for (uint32_t l = 0; l < L; ++l) dst[(size_t)l * N] = 0;
+    return;
+  }
+  const uint32_t ip = (uint32_t)(((uint64_t)n * kinv) & (2 * N - 1));
+  const bool neg = ip >= N;
+  const uint32_t* src = in2 + ((size_t)item * 2 + (slot ? 1 : 0)) * L * N + (neg ? ip - N : ip);
+  if (!neg) {
+    for (uint32_t l = 0; l < L; ++l) dst[(size_t)l * N] = src[(size_t)l * N];
+    return;
+  }
+  if (ckks) {                                                       // -a mod 2^bits: two's complement, top limb masked
+    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
+    uint32_t carry = 1;
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = 0;
+      if (l < Lb) {
+        const uint64_t s = (uint64_t)(~src[(size_t)l * N]) + carry;
+        v = (uint32_t)s; carry = (uint32_t)(s >> 32);
+        if (l == Lb - 1) v &= tm;
+      }
+      dst[(size_t)l * N] = v;
+    }
+  } else {                                                          // Q - a, and 0 stays 0
+    uint32_t any = 0;
+    for (uint32_t l = 0; l < L; ++l) any |= src[(size_t)l * N];
+    uint32_t borrow = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      const uint32_t q = any ? __ldg(Q + l) : 0u, y = src[(size_t)l * N];
+      const uint32_t d = q - y, d2 = d - borrow;
+      borrow = (q < y) | (d < borrow);
+      dst[(size_t)l * N] = d2;
+    }
+  }
+}
+
+cudaError_t launch_automorphism(Context* c, uint32_t* d_out3, const uint32_t* d_in2, uint32_t k, uint32_t batch, cudaStream_t s) {
+  if (!batch) return cudaSuccess;
+  const uint32_t twoN = 2 * c->N;
+  uint32_t kinv = 1;                                                // k^-1 mod 2N (k odd): Newton iteration mod 2^32, then reduce
+  for (int it = 0; it < 5; ++it) kinv *= 2u - k * kinv;
+  kinv &= twoN - 1;
+  LaunchTimer lt(c, KC_RESCALE, s);
+  automorphism_kernel<<<(c->N / 256) * 3 * batch, 256, 0, s>>>(d_out3, d_in2, c->d_Qlimbs, c->N, c->L, c->logQ, kinv, c->t == 0 ? 1u : 0u);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
                         uint32_t bits, cudaStream_t s) {
   if (!npoly) return cudaSuccess;

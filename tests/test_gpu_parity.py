@@ -501,3 +501,39 @@ def test_next1_moddown_and_depth_two_circuit_over_two_levels():
     mu = harness.decrypt(tuple(got), s, 1 << (logq1 - p))
     z = harness.decode(mu, N, 2.0 ** 40)
     assert np.max(np.abs(z - zs[0][0] * zs[0][1] * zs[1][0])) <= 2.0 ** -20
+
+
+# ---- NEXT-2: rotation / conjugation = automorphism + key switch with a rotation key ----------------------
+@pytest.mark.parametrize("N,logQ,logP,t,ks", [(1 << 10, 128, 128, 0, (5, 25, 2047)), (256, 100, 100, 257, (3, 511)),
+                                              (1 << 12, 218, 250, 0, (5,))])
+def test_next2_rotate_matches_the_oracle(N, logQ, logP, t, ks):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logP, t)
+    g = synth.rng(60 + N)
+    s, _ = harness.keygen(prm, g, hwt=64 if t == 0 else None)
+    ctx = fhe.Context(N, logQ, logP, t)
+    B = 2
+    if t == 0:
+        zs = [synth.unit_disk(g, N // 2) for _ in range(B)]
+        cts = [harness.encrypt(prm, g, s, harness.encode(z, N, 2.0 ** 40)) for z in zs]
+    else:
+        ms = [[int(v) for v in g.integers(0, t, size=N)] for _ in range(B)]
+        cts = [harness.encrypt(prm, g, s, m) for m in ms]
+    d = polys_to_tensor([list(c) for c in cts], ctx.L)
+    for slot, k in enumerate(ks):
+        rk = harness.rotkeygen(prm, g, s, k)
+        ctx.fhe_set_rotation_key(slot, k, polys_to_tensor(list(rk), ctx.L_PQ))
+        got = tensor_to_polys(ctx.fhe_rotate(d, slot))
+        for i in range(B):
+            want = scheme.rotate(prm, cts[i], k, rk)
+            assert got[i] == [list(p) for p in want], (k, i)
+        if t == 0:
+            src, conj = harness.slot_image(N, k)
+            z = harness.decode(harness.decrypt(tuple(got[0]), s, prm.Q), N, 2.0 ** 40)
+            want = np.array([np.conj(zs[0][j]) if c else zs[0][j] for j, c in zip(src, conj)])
+            assert np.max(np.abs(z - want)) <= 2.0 ** -20
+        else:
+            assert harness.decrypt_bgv(tuple(got[0]), s, prm) == scheme.automorphism(ms[0], k, t)
+    # an empty slot is an error, not a silent no-op
+    with pytest.raises(fhe.FheError):
+        ctx.fhe_rotate(d, len(ks))

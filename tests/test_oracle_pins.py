@@ -357,3 +357,49 @@ def test_next1_elementwise_ops_are_the_ring_operations_and_decrypt_homomorphical
     assert harness.decrypt_bgv(scheme.ct_add(prb, c1, c2), sb, prb) == [(a + b) % 257 for a, b in zip(m1, m2)]
     assert harness.decrypt_bgv(scheme.ct_sub(prb, c1, c2), sb, prb) == [(a - b) % 257 for a, b in zip(m1, m2)]
     assert harness.decrypt_bgv(scheme.ct_negate(prb, c1), sb, prb) == [(-a) % 257 for a in m1]
+
+
+# ---- NEXT-2: automorphism, rotation key switch (parity unpinned by the paper: names only) ---------------------------------
+def test_next2_automorphism_is_the_substitution_and_rotation_permutes_the_slots():
+    import numpy as np
+    import synth
+    from oracle import harness, ring, scheme
+    N, M = 16, 97
+    g = synth.rng(41)
+    a = [int(v) for v in g.integers(0, M, size=N)]
+    b = [int(v) for v in g.integers(0, M, size=N)]
+    # sigma_k(X) = X^k reduced mod X^N + 1; sigma_1 = id; sigma_k sigma_j = sigma_{kj}; ring homomorphism
+    X = [0, 1] + [0] * (N - 2)
+    for k in (3, 5, 2 * N - 1):
+        want = [0] * N
+        want[k % N] = 1 if k < N else M - 1
+        assert scheme.automorphism(X, k, M) == want
+        assert scheme.automorphism(ring.pm(a, b, M), k, M) == ring.pm(scheme.automorphism(a, k, M), scheme.automorphism(b, k, M), M)
+    assert scheme.automorphism(a, 1, M) == a
+    assert scheme.automorphism(scheme.automorphism(a, 3, M), 5, M) == scheme.automorphism(a, 15, M)
+    # direct evaluation: (sigma_k a)(x) = a(x^k) at a root of X^N + 1 mod 97 (x = 19^3 has order 32 = 2N)
+    x = next(v for v in range(2, M) if pow(v, N, M) == M - 1)
+    ev = lambda p, y: sum(c * pow(y, i, M) for i, c in enumerate(p)) % M
+    assert ev(scheme.automorphism(a, 5, M), x) == ev(a, pow(x, 5, M))
+    # end to end on CKKS: Dec(rotate(ct)) decodes to the permuted (and, for k = 2N - 1, conjugated) slots
+    N, logQ, logP = 64, 100, 100
+    prm = scheme.Params(N, logQ, logP, 0)
+    s, _ = harness.keygen(prm, g, hwt=16)
+    z = synth.unit_disk(g, N // 2)
+    ct = harness.encrypt(prm, g, s, harness.encode(z, N, 2.0 ** 30))
+    for k in (5, 25, 2 * N - 1):
+        rk = harness.rotkeygen(prm, g, s, k)
+        out = scheme.rotate(prm, ct, k, rk)
+        got = harness.decode(harness.decrypt(out, s, prm.Q), N, 2.0 ** 30)
+        src, conj = harness.slot_image(N, k)
+        want = np.array([np.conj(z[i]) if c else z[i] for i, c in zip(src, conj)])
+        assert np.max(np.abs(got - want)) < 1e-6
+    src, conj = harness.slot_image(N, 2 * N - 1)
+    assert src == list(range(N // 2)) and all(conj)
+    # BGV: the plaintext polynomial is mapped by the same automorphism, exactly mod t
+    prb = scheme.Params(N, 60, 60, 257)
+    sb, _ = harness.keygen(prb, g, hwt=None)
+    m = [int(v) for v in g.integers(0, 257, size=N)]
+    cb = harness.encrypt(prb, g, sb, m)
+    rkb = harness.rotkeygen(prb, g, sb, 5)
+    assert harness.decrypt_bgv(scheme.rotate(prb, cb, 5, rkb), sb, prb) == scheme.automorphism(m, 5, 257)
