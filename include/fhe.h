@@ -52,7 +52,8 @@ typedef enum {            /* `op` argument of fhe_workspace_bytes */
   FHE_OP_RESCALE = 3,     /* needs no workspace: returns 0 */
   FHE_OP_MULT_RELIN_RESCALE = 4,
   FHE_OP_SET_EVK = 5,
-  FHE_OP_ROTATE = 6
+  FHE_OP_ROTATE = 6,
+  FHE_OP_MULT_PLAIN = 7
 } fhe_op;
 
 typedef struct {
@@ -159,6 +160,15 @@ fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint
 fhe_status fhe_set_rotation_key(fhe_ctx* ctx, uint32_t slot, uint32_t k, const uint32_t* d_key, void* stream);
 fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uint32_t slot, uint32_t batch, void* d_ws,
                       size_t ws_bytes, void* stream);
+
+/* ---- NEXT-3: ciphertext x plaintext, pairwise and broadcast -----------------
+ * out[i] = (c0_i * m_j, c1_i * m_j) mod (X^N + 1, Q) with j = i / group: group = 1 multiplies ciphertext i by its own
+ * plaintext polynomial (multconstvec_pairwise), group = batch lifts ONE plaintext over the whole tensor
+ * (multconst_broadcast).  d_ct, d_out2 [B][2][L][N]; d_pt [ceil(B / group)][L][N], an ENCODED plaintext (the caller rescales
+ * afterwards as after any multiplication); d_ws >= fhe_workspace_bytes(FHE_OP_MULT_PLAIN, batch).  The shared operand is
+ * decomposed and column-transformed once per plaintext; the same kernels as fhe_polymul do the rest. */
+fhe_status fhe_mult_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                          uint32_t group, void* d_ws, size_t ws_bytes, void* stream);
 
 /* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
 

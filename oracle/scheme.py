@@ -184,3 +184,12 @@ def rotate(prm: Params, ct, k: int, rk):
     Q = prm.Q
     d = (automorphism(ct[0], k, Q), [0] * prm.N, automorphism(ct[1], k, Q))
     return relinearize(prm, d, rk)
+
+
+# ---- NEXT-3: ciphertext x plaintext ----------------------------------------------------------------------
+# multconstvec_pairwise_into / multconst_broadcast_into: "element-wise multiplication with
+# per-ciphertext constants" / "of a single constant across a ciphertext tensor".  On an encoded plaintext polynomial m
+# this is the ring product on both components (decryption is linear: (c0 + c1 s) m = c0 m + (c1 m) s).
+def mult_plain(prm: Params, ct, m):
+    Q = prm.Q
+    return pm(ct[0], m, Q), pm(ct[1], m, Q)

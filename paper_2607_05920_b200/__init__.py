@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfhe_b200.so")
 
 FHE_OK, FHE_ERR_ARG, FHE_ERR_UNSUPPORTED, FHE_ERR_STATE, FHE_ERR_CUDA, FHE_ERR_NOMEM = range(6)
-OP_POLYMUL, OP_HE_MULT, OP_RELINEARIZE, OP_RESCALE, OP_MULT_RELIN_RESCALE, OP_SET_EVK, OP_ROTATE = range(7)
+OP_POLYMUL, OP_HE_MULT, OP_RELINEARIZE, OP_RESCALE, OP_MULT_RELIN_RESCALE, OP_SET_EVK, OP_ROTATE, OP_MULT_PLAIN = range(8)
 _STATUS_NAMES = ["FHE_OK", "FHE_ERR_ARG", "FHE_ERR_UNSUPPORTED", "FHE_ERR_STATE", "FHE_ERR_CUDA", "FHE_ERR_NOMEM"]
 
 # every symbol include/fhe.h declares (tests/test_abi.py checks the header against this and the .so)
@@ -24,7 +24,7 @@ EXPORTS = [
     "fhe_set_evk", "fhe_polymul", "fhe_he_mult", "fhe_relinearize", "fhe_rescale", "fhe_mult_relin_rescale",
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
-    "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_set_rotation_key", "fhe_rotate",
+    "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
 ]
 
 
@@ -87,6 +87,8 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_debug_ntt.restype = c_int
     lib.fhe_debug_launch_count.argtypes = [vp]
     lib.fhe_debug_launch_count.restype = c_uint64
+    lib.fhe_mult_plain.argtypes = [vp, vp, vp, vp, c_uint32, c_uint32, vp, c_size_t, vp]
+    lib.fhe_mult_plain.restype = c_int
     lib.fhe_set_rotation_key.argtypes = [vp, c_uint32, c_uint32, vp, vp]
     lib.fhe_set_rotation_key.restype = c_int
     lib.fhe_rotate.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp, c_size_t, vp]
@@ -291,6 +293,19 @@ class Context:
         self._check(self._lib.fhe_mult_relin_rescale_host(self._h, h_out.data_ptr(), h_ct1.data_ptr(), h_ct2.data_ptr(),
                                                           p_bits, batch, ws.data_ptr(), nb, self._stream(stream)))
         return h_out
+
+    # ---- NEXT-3: ciphertext x plaintext, pairwise (group = 1) or broadcast (group = batch) ----
+    def fhe_mult_plain(self, ct, pt, group: int = 1, out=None, stream=None):
+        batch = ct.shape[0]
+        n = batch * 2 * self.L * self.N
+        npt = (batch + group - 1) // group
+        out = self._empty(batch, 2, self.L, self.N) if out is None else out
+        nb = self.workspace_bytes(OP_MULT_PLAIN, batch)
+        ws = self._workspace(nb)
+        self._check(self._lib.fhe_mult_plain(self._h, _dev_ptr(out, n, "out"), _dev_ptr(ct, n, "ct"),
+                                             _dev_ptr(pt, npt * self.L * self.N, "pt"), batch, group, ws.data_ptr(), nb,
+                                             self._stream(stream)))
+        return out
 
     # ---- NEXT-2: rotation / conjugation ----
     def fhe_set_rotation_key(self, slot: int, k: int, key, stream=None):

@@ -76,6 +76,7 @@ size_t fhe_workspace_bytes(const fhe_ctx* ctx, int op, uint32_t batch) {
     }
     case FHE_OP_SET_EVK: return ws_evk(c);
     case FHE_OP_ROTATE: return ws_relin(c, batch) + ws_d3(c, batch);
+    case FHE_OP_MULT_PLAIN: return ws_polymul(c, 2 * batch);
     default: return 0;
   }
 }
@@ -137,6 +138,21 @@ fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uin
   return do_relin(c, d_out2, d3, batch, ws, 0, s, c->d_rot_hat[slot]);
 }
 
+// out[i] = a[i] * b[i / group] mod (X^N + 1, Q) for i < npoly; ws: [npoly + ceil(npoly / group)][K_pm][N]
+static fhe_status do_polymul(Context* c, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly,
+                             uint32_t group, uint32_t* ws, cudaStream_t s) {
+  const uint32_t N = c->N, L = c->L, K = c->K_pm, nb = (npoly + group - 1) / group;
+  const size_t rp = (size_t)K * N;
+  uint32_t* ra = ws;
+  uint32_t* rb = ra + (size_t)npoly * rp;
+  const uint32_t mask = c->t == 0 ? c->logQ : 0;
+  CK(launch_decompose(c, ra, 0, rp, d_a, 0, (size_t)L * N, 1, npoly, L, K, mask, s), "decompose a");
+  CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, nb, L, K, mask, s), "decompose b");
+  CK(launch_ntt_product(c, ra, rb, npoly, K, PW_POLYMUL, c->tgt_pm.d_scale, s, group), "ntt polymul");
+  CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, 0, (size_t)L * N, ra, 0, rp, nullptr, 0, 0, 1, npoly, s), "crt");
+  return FHE_OK;
+}
+
 fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,
                        void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
@@ -145,17 +161,20 @@ fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const
   if (!d_out || !d_a || !d_b || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out, 16) || misaligned(d_a, 16) || misaligned(d_b, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
   if (ws_bytes < ws_polymul(c, batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
-  cudaStream_t s = (cudaStream_t)stream;
-  const uint32_t N = c->N, L = c->L, K = c->K_pm;
-  const size_t rp = (size_t)K * N;
-  uint32_t* ra = (uint32_t*)d_ws;
-  uint32_t* rb = ra + (size_t)batch * rp;
-  const uint32_t mask = c->t == 0 ? c->logQ : 0;
-  CK(launch_decompose(c, ra, 0, rp, d_a, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose a");
-  CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, batch, L, K, mask, s), "decompose b");
-  CK(launch_ntt_product(c, ra, rb, batch, K, PW_POLYMUL, c->tgt_pm.d_scale, s), "ntt polymul");
-  CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, 0, (size_t)L * N, ra, 0, rp, nullptr, 0, 0, 1, batch, s), "crt");
-  return FHE_OK;
+  return do_polymul(c, d_out, d_a, d_b, batch, 1, (uint32_t*)d_ws, (cudaStream_t)stream);
+}
+
+fhe_status fhe_mult_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                          uint32_t group, void* d_ws, size_t ws_bytes, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_ct || !d_pt || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_ct, 16) || misaligned(d_pt, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (group == 0) return err(c, FHE_ERR_ARG, "group must be at least 1");
+  if (ws_bytes < ws_polymul(c, 2 * batch)) return err(c, FHE_ERR_NOMEM, "workspace too small");
+  // both components of ciphertext i times plaintext i / group: 2 batch polynomials, operand shared by 2 group of them
+  return do_polymul(c, d_out2, d_ct, d_pt, 2 * batch, 2 * group, (uint32_t*)d_ws, (cudaStream_t)stream);
 }
 
 fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, const uint32_t* d_ct2, uint32_t batch,

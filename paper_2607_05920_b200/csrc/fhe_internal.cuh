@@ -148,8 +148,9 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, u
 // products, first inverse pass, all in registers on the same 256-point row), inverse column pass over the result slots.
 // Same slot conventions as launch_ntt_inv's PW modes, but the operands arrive untransformed (decompose output); for
 // PW_POLYMUL d_aux (the b operand, [nitems][K][N]) is transformed in place too.
+// aux_group (PW_POLYMUL): item i multiplies aux polynomial i / aux_group, of which there are ceil(nitems / aux_group).
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
-                               const uint2* d_scale, cudaStream_t s);
+                               const uint2* d_scale, cudaStream_t s, uint32_t aux_group = 1);
 // CRT + post: residues [K][N] -> limbs [L][N] per polynomial (o, i); d_add: for the relin modes, the polynomial added
 // at the end, else nullptr
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,

@@ -120,6 +120,7 @@ struct NttArgs {
   const uint32_t* qn;        // [Kmax] -q^-1 mod 2^32
   const uint2* scale;        // [K] final constant of the inverse (with Shoup companion)
   uint32_t N, K, N1, S, U, units, nitems;
+  uint32_t aux_group;        // PW_POLYMUL: item i multiplies aux polynomial i / aux_group (1: pairwise; > 1: shared operand)
 };
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -387,7 +388,7 @@ ntt_row_fused_kernel(NttArgs a) {
     uint32_t* g = a.data + (size_t)item * KN + poff;
     uint32_t x[16], y[16];
     ldrow(x, g, t);
-    ldrow(y, a.aux + (size_t)item * KN + poff, t);
+    ldrow(y, a.aux + (size_t)(item / a.aux_group) * KN + poff, t);
     fwd_canon(x);
     fwd(y);
 #pragma unroll
@@ -523,7 +524,7 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
   a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
   const uint32_t ntr = nitems * U * K;
   a.units = ntr * a.N1;
   if (c->logN > 8) {
@@ -540,7 +541,7 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, u
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
   a.data = d_res; a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
   const bool fin = c->logN == 8;
   const uint32_t row_units = (pw_mode == PW_NONE ? nitems * U : nitems) * K * a.N1;
   a.units = row_units;
@@ -567,7 +568,7 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, u
 // S2 + S3 + S4 of a product in three launches (four for PW_POLYMUL): forward column pass over the operand slots, the
 // fused row pass, inverse column pass over the result slots.
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
-                               const uint2* d_scale, cudaStream_t s) {
+                               const uint2* d_scale, cudaStream_t s, uint32_t aux_group) {
   if (!nitems) return cudaSuccess;
   uint32_t S, Uin, Uout;
   switch (pw_mode) {
@@ -578,14 +579,14 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   }
   NttArgs a;
   a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems; a.aux_group = aux_group ? aux_group : 1;
   const bool fin = c->logN == 8;
   cudaError_t e;
   if (!fin) {
     if ((e = launch_col<false>(c, a, nitems * Uin * K, s)) != cudaSuccess) return e;
     if (pw_mode == PW_POLYMUL) {
       a.data = d_aux;
-      if ((e = launch_col<false>(c, a, nitems * K, s)) != cudaSuccess) return e;
+      if ((e = launch_col<false>(c, a, ((nitems + a.aux_group - 1) / a.aux_group) * K, s)) != cudaSuccess) return e;
       a.data = d_res;
     }
   }

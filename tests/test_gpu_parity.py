@@ -537,3 +537,21 @@ def test_next2_rotate_matches_the_oracle(N, logQ, logP, t, ks):
     # an empty slot is an error, not a silent no-op
     with pytest.raises(fhe.FheError):
         ctx.fhe_rotate(d, len(ks))
+
+
+# ---- NEXT-3: ciphertext x plaintext, pairwise and broadcast ----------------------------------------------
+@pytest.mark.parametrize("N,logQ,t,B,group", [(1024, 128, 0, 3, 1), (1024, 128, 0, 5, 5), (256, 100, 257, 4, 2), (4096, 218, 0, 5, 2)])
+def test_next3_mult_plain_pairwise_and_broadcast(N, logQ, t, B, group):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, 32 if t == 0 else logQ, t)
+    ctx = fhe.Context(N, logQ, prm.logP, t)
+    g = synth.rng(70 + N + B)
+    Q = prm.Q
+    npt = (B + group - 1) // group
+    ct_np = synth.uniform_limbs(g, (B, 2), N, logQ)      # uniform below 2^logQ < Q: valid canonical inputs for both schemes
+    pt_np = synth.uniform_limbs(g, (npt,), N, logQ)
+    out = tensor_to_polys(ctx.fhe_mult_plain(limbs_np_to_tensor(ct_np), limbs_np_to_tensor(pt_np), group))
+    for i in range(B):
+        ct = tuple(from_limbs(ct_np[i, k]) for k in range(2))
+        want = scheme.mult_plain(prm, ct, from_limbs(pt_np[i // group]))
+        assert out[i] == [list(p) for p in want], i

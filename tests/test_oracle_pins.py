@@ -403,3 +403,33 @@ def test_next2_automorphism_is_the_substitution_and_rotation_permutes_the_slots(
     cb = harness.encrypt(prb, g, sb, m)
     rkb = harness.rotkeygen(prb, g, sb, 5)
     assert harness.decrypt_bgv(scheme.rotate(prb, cb, 5, rkb), sb, prb) == scheme.automorphism(m, 5, 257)
+
+
+# ---- NEXT-3: ciphertext x plaintext (parity unpinned by the paper: names only) ---------------------------------------------
+def test_next3_mult_plain_multiplies_the_slots_and_is_exact_mod_t():
+    import numpy as np
+    import synth
+    from oracle import harness, ring, scheme
+    g = synth.rng(43)
+    N, logQ, logP = 64, 120, 120
+    prm = scheme.Params(N, logQ, logP, 0)
+    s, _ = harness.keygen(prm, g, hwt=16)
+    z, w = synth.unit_disk(g, N // 2), synth.unit_disk(g, N // 2)
+    ct = harness.encrypt(prm, g, s, harness.encode(z, N, 2.0 ** 30))
+    m = [v % prm.Q for v in harness.encode(w, N, 2.0 ** 30)]
+    out = scheme.mult_plain(prm, ct, m)
+    # linearity of decryption: Dec(out) = Dec(ct) * m exactly in the ring
+    d = [v % prm.Q for v in harness.decrypt(ct, s, prm.Q)]
+    assert [v % prm.Q for v in harness.decrypt(out, s, prm.Q)] == ring.pm(d, m, prm.Q)
+    got = harness.decode(harness.decrypt(scheme.rescale(prm, out, 30), s, 1 << (logQ - 30)), N, 2.0 ** 30)
+    assert np.max(np.abs(got - z * w)) < 1e-6
+    # the constant polynomial 1 is the identity, 0 annihilates
+    one = [1] + [0] * (N - 1)
+    assert scheme.mult_plain(prm, ct, one) == (list(ct[0]), list(ct[1]))
+    assert scheme.mult_plain(prm, ct, [0] * N) == ([0] * N, [0] * N)
+    prb = scheme.Params(N, 60, 60, 257)
+    sb, _ = harness.keygen(prb, g, hwt=None)
+    m1 = [int(v) for v in g.integers(0, 257, size=N)]
+    m2 = [int(v) for v in g.integers(0, 257, size=N)]
+    cb = harness.encrypt(prb, g, sb, m1)
+    assert harness.decrypt_bgv(scheme.mult_plain(prb, cb, m2), sb, prb) == ring.pm(m1, m2, 257)
