@@ -336,7 +336,7 @@ fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
   if (!d_res || K == 0 || K > c->Kmax) return err(c, FHE_ERR_ARG, "bad argument");
-  if (inverse) CK(launch_ntt_inv(c, d_res, nullptr, npoly, 1, 1, K, PW_NONE, c->d_scale_plain, (cudaStream_t)stream), "ntt inv");
+  if (inverse) CK(launch_ntt_inv(c, d_res, npoly, 1, 1, K, c->d_scale_plain, (cudaStream_t)stream), "ntt inv");
   else CK(launch_ntt_fwd(c, d_res, npoly, 1, 1, K, (cudaStream_t)stream), "ntt fwd");
   return FHE_OK;
 }

@@ -134,20 +134,18 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
 // Transforms live in an item-major residue buffer [nitems][S][K][N] (S slots per item); slots 0..U-1 of every item
 // are transformed in place.  Forward output is in bit-reversed order and canonical ([0, q)).
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s);
-// Inverse, with the pointwise products (S3) formed in registers by the first pass (Montgomery: each product carries a
-// factor 2^-32 that d_scale removes):
-//   PW_NONE    plain inverse of slots 0..U-1
-//   PW_POLYMUL S = U = 1: data <- INTT(data * aux), aux = [nitems][K][N]
-//   PW_TENSOR  S = 4, U = 3: slots (a0, a1, b0, b1)^ -> slots 0..2 = INTT(a0 b0, a0 b1 + a1 b0, a1 b1)
-//   PW_RELIN   S = U = 2: slot 0 = d2^ -> slots 0, 1 = INTT(d2^ * aux[0], d2^ * aux[1]), aux = evk-hat [2][K][N]
+// Plain inverse of slots 0..U-1 (the debug entry point; the products go through launch_ntt_product).
 // d_scale: per-prime final constant ([K] uint2, value and Shoup companion).
 enum PwMode : int { PW_NONE = 0, PW_POLYMUL = 1, PW_TENSOR = 2, PW_RELIN = 3 };
-cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
-                           uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s);
+cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K,
+                           const uint2* d_scale, cudaStream_t s);
 // The product path: forward column pass over the operand slots, ONE fused row pass (last forward pass, pointwise
 // products, first inverse pass, all in registers on the same 256-point row), inverse column pass over the result slots.
-// Same slot conventions as launch_ntt_inv's PW modes, but the operands arrive untransformed (decompose output); for
-// PW_POLYMUL d_aux (the b operand, [nitems][K][N]) is transformed in place too.
+// The operands arrive untransformed (decompose output) in an item-major buffer [nitems][S][K][N]:
+//   PW_POLYMUL S = 1: data <- INTT(NTT(data) * NTT(aux)), aux = [ceil(nitems / aux_group)][K][N], transformed in place too
+//   PW_TENSOR  S = 4: slots (a0, a1, b0, b1) -> slots 0..2 = INTT(a0^ b0^, a0^ b1^ + a1^ b0^, a1^ b1^)
+//   PW_RELIN   S = 2: slot 0 = d2 -> slots 0, 1 = INTT(d2^ * aux[0], d2^ * aux[1]), aux = a key already in the NTT domain [2][K][N]
+// (Montgomery products: each carries a factor 2^-32 that d_scale removes.)
 // aux_group (PW_POLYMUL): item i multiplies aux polynomial i / aux_group, of which there are ceil(nitems / aux_group).
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
                                const uint2* d_scale, cudaStream_t s, uint32_t aux_group = 1);

@@ -1,5 +1,5 @@
 // kernels_ntt.cu -- S2/S4 negacyclic NTT (Eq. 8-9) with S3, the pointwise products (PAPER.md:354-356,
-// Eq. 7), folded into the first inverse pass.
+// Eq. 7), formed in registers between the last forward and the first inverse pass (ntt_row_fused_kernel).
 //
 // Formulation: merged-psi Cooley-Tukey forward / Gentleman-Sande inverse; the psi^j "twist" of
 // PAPER.md:346-350 lives in the butterfly twiddles, so there is no separate twist pass.  tw_fwd[k] = psi^bitrev(k),
@@ -253,83 +253,28 @@ ntt_row_fwd_kernel(NttArgs a) {
                                                                 canon4(x[4 * k + 2], q, q2), canon4(x[4 * k + 3], q, q2));
 }
 
-template <int PW, bool FINAL>
+template <bool FINAL>
 __global__ void __launch_bounds__(256)
 ntt_row_inv_kernel(NttArgs a) {
   __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
   const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
-  const uint32_t unit = blockIdx.x * 16 + rl;           // PW_NONE: as forward; else ((item * K) + j) * N1 + r
+  const uint32_t unit = blockIdx.x * 16 + rl;           // row of a transform, as in the forward row pass
   if (unit >= a.units) return;
   const uint32_t r = unit % a.N1, tr = unit / a.N1;
-  uint32_t* srow = sm + rl * ROW_SM;
-  const size_t roff = (size_t)r * 256;
-  const size_t KN = (size_t)a.K * a.N;
-
-  auto finish = [&](uint32_t (&x)[16], uint32_t* g, uint32_t j, uint32_t q, uint32_t q2, const uint2* tw) {
-    row_inv_core(x, srow, t, tw, a.N1 + r, q, q2);
-    if (FINAL) {
-      const uint2 sc = __ldg(a.scale + j);
+  const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
+  const uint2* tw = a.tw + (size_t)j * a.N;
+  uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + (size_t)r * 256;
+  uint32_t x[16];
+  load16(x, g + t * 16);
+  row_inv_core(x, sm + rl * ROW_SM, t, tw, a.N1 + r, q, q2);
+  if (FINAL) {
+    const uint2 sc = __ldg(a.scale + j);
 #pragma unroll
-      for (int i = 0; i < 16; ++i) g[i * 16 + t] = mul_shoup(x[i], sc.x, sc.y, q);
-    } else {
-#pragma unroll
-      for (int i = 0; i < 16; ++i) g[i * 16 + t] = x[i];
-    }
-  };
-
-  if constexpr (PW == PW_NONE) {
-    const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
-    const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
-    const uint2* tw = a.tw + (size_t)j * a.N;
-    uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + roff;
-    uint32_t x[16];
-    load16(x, g + t * 16);
-    finish(x, g, j, q, q2, tw);
+    for (int i = 0; i < 16; ++i) g[i * 16 + t] = mul_shoup(x[i], sc.x, sc.y, q);
   } else {
-    const uint32_t item = tr / a.K, j = tr % a.K;
-    const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
-    const uint2* tw = a.tw + (size_t)j * a.N;
-    const size_t poff = (size_t)j * a.N + roff;          // offset of this row inside a [K][N] polynomial
-    if constexpr (PW == PW_POLYMUL) {
-      uint32_t* g = a.data + (size_t)item * KN + poff;
-      uint32_t x[16], y[16];
-      load16(x, g + t * 16);
-      load16(y, a.aux + (size_t)item * KN + poff + t * 16);
-      __syncwarp();
 #pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mm(x[i], y[i], q, qn);
-      finish(x, g, j, q, q2, tw);
-    } else if constexpr (PW == PW_TENSOR) {
-      uint32_t* g = a.data + (size_t)item * 4 * KN + poff;       // slots a0, a1, b0, b1 at g + slot * KN
-      uint32_t a0[16], a1[16], b0[16], b1[16], x[16];
-      load16(a0, g + t * 16);
-      load16(a1, g + KN + t * 16);
-      load16(b0, g + 2 * KN + t * 16);
-      load16(b1, g + 3 * KN + t * 16);
-      __syncwarp();   // every lane of the row holds its operands before slot 0 is overwritten
-#pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
-      finish(x, g, j, q, q2, tw);
-#pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
-      finish(x, g + KN, j, q, q2, tw);
-#pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
-      finish(x, g + 2 * KN, j, q, q2, tw);
-    } else {   // PW_RELIN
-      uint32_t* g = a.data + (size_t)item * 2 * KN + poff;       // slot 0 = d2-hat
-      uint32_t d[16], e[16], x[16];
-      load16(d, g + t * 16);
-      load16(e, a.aux + poff + t * 16);
-      __syncwarp();
-#pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e[i], q, qn);
-      finish(x, g, j, q, q2, tw);
-      load16(e, a.aux + KN + poff + t * 16);
-#pragma unroll
-      for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e[i], q, qn);
-      finish(x, g + KN, j, q, q2, tw);
-    }
+    for (int i = 0; i < 16; ++i) g[i * 16 + t] = x[i];
   }
 }
 
@@ -536,28 +481,19 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
   return cudaGetLastError();
 }
 
-cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, const uint32_t* d_aux, uint32_t nitems, uint32_t S, uint32_t U,
-                           uint32_t K, int pw_mode, const uint2* d_scale, cudaStream_t s) {
+cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K,
+                           const uint2* d_scale, cudaStream_t s) {
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
-  a.data = d_res; a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_inv; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
   const bool fin = c->logN == 8;
-  const uint32_t row_units = (pw_mode == PW_NONE ? nitems * U : nitems) * K * a.N1;
-  a.units = row_units;
-  const uint32_t blocks = (row_units + 15) / 16;
+  a.units = nitems * U * K * a.N1;
+  const uint32_t blocks = (a.units + 15) / 16;
   {
     LaunchTimer lt(c, KC_NTT_INV, s);
-#define ROW_CASE(PW)                                                                  \
-  case PW:                                                                            \
-    if (fin) ntt_row_inv_kernel<PW, true><<<blocks, 256, 0, s>>>(a);                  \
-    else ntt_row_inv_kernel<PW, false><<<blocks, 256, 0, s>>>(a);                     \
-    break;
-    switch (pw_mode) {
-      ROW_CASE(PW_NONE) ROW_CASE(PW_POLYMUL) ROW_CASE(PW_TENSOR) ROW_CASE(PW_RELIN)
-      default: return cudaErrorInvalidValue;
-    }
-#undef ROW_CASE
+    if (fin) ntt_row_inv_kernel<true><<<blocks, 256, 0, s>>>(a);
+    else ntt_row_inv_kernel<false><<<blocks, 256, 0, s>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
