@@ -38,9 +38,9 @@ constexpr uint32_t CTRL_BYTES = 1024;
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 
 struct Ctrl {
-  uint64_t a_full[MAX_A], a_free[MAX_A];      // A buffer written (loader arrivals) / consumed (MMA commit)
+  uint64_t a_full[MAX_A], a_free[MAX_A];      // A buffer written (one arrival per loader warp) / consumed (MMA commit)
   uint64_t d_full[MAX_SPANS];                 // the span's accumulators finished (MMA commit)
-  uint64_t d_free[MAX_CHUNKS];                // the chunk's accumulators are in registers (epilogue arrivals)
+  uint64_t d_free[MAX_CHUNKS];                // the chunk's accumulators are in registers (one arrival per epilogue warp)
   uint64_t b_full, mma_done;                  // B of the pass landed (bulk copies) / every MMA of the pass finished
   uint32_t tmem_base;
 };
@@ -212,9 +212,11 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   const uint32_t amask = a.nA - 1, ashift = a.nA - 1;              // nA in {1, 2}
 
   if (tid == 0) {
-    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], (ALT ? 4 : LOAD_WARPS) * 32); mbar_init(&ctl->a_free[i], 1); }
+    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], ALT ? 4 : LOAD_WARPS); mbar_init(&ctl->a_free[i], 1); }
     for (uint32_t i = 0; i < MAX_SPANS; ++i) mbar_init(&ctl->d_full[i], 1);
-    for (uint32_t i = 0; i < MAX_CHUNKS; ++i) mbar_init(&ctl->d_free[i], EPIW * 32);
+    // one arrival per WARP (its lane 0, after the warp-collective tcgen05.wait): hundreds of per-thread arrivals on one
+    // mbarrier serialise in shared memory and were a quarter of the epilogue's time
+    for (uint32_t i = 0; i < MAX_CHUNKS; ++i) mbar_init(&ctl->d_free[i], EPIW);
     mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
     fence_barrier_init();
   }
@@ -303,7 +305,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
         tmem_st_wait();
         tc_fence_before();
-        mbar_arrive(&ctl->a_full[abuf]);
+        if (lane == 0) mbar_arrive(&ctl->a_full[abuf]);
       }
     }
   } else {
@@ -331,7 +333,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
             tmem_ld32_nowait(tmem_d + c * NC + 32 + lane_off, t + 32);
             tmem_ld_wait();
             tc_fence_before();
-            mbar_arrive(&ctl->d_free[c]);                          // the accumulator chunk is in registers: hand it back
+            if (lane == 0) mbar_arrive(&ctl->d_free[c]);           // the accumulator chunk is in registers: hand it back
             {
               epi.consume((c0 + c) * NC, t);
               epi.consume((c0 + c) * NC + 32, t + 32);
@@ -341,7 +343,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
             tmem_ld_cols<GC>(tmem_d + c * NC + grp * GC + lane_off, t);
             tmem_ld_wait();
             tc_fence_before();
-            mbar_arrive(&ctl->d_free[c]);
+            if (lane == 0) mbar_arrive(&ctl->d_free[c]);
             epi.consume((c0 + c) * NC + grp * GC, t);
           }
         }
