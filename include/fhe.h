@@ -147,6 +147,9 @@ fhe_status fhe_add(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uin
 fhe_status fhe_sub(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t npoly, void* stream);
 fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32_t npoly, void* stream);
 fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream);
+/* out = X^k * in mod (X^N + 1, Q), 0 <= k < 2N, per polynomial: a signed rotation of the coefficients.  k = N/2 multiplies
+ * the CKKS slots by the imaginary unit (imult_pairwise_into), k = 3N/2 by -i.  NOT in place. */
+fhe_status fhe_mul_monomial(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, void* stream);
 
 /* ---- NEXT-2: slot rotation and conjugation ------------------------------------
  * A rotation is the Galois automorphism X -> X^k (k odd, k < 2N; k = 2N - 1 conjugates) applied to both components,

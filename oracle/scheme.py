@@ -193,3 +193,16 @@ def rotate(prm: Params, ct, k: int, rk):
 def mult_plain(prm: Params, ct, m):
     Q = prm.Q
     return pm(ct[0], m, Q), pm(ct[1], m, Q)
+
+
+def mul_monomial(prm: Params, ct, k: int):
+    """X^k * ct, 0 <= k < 2N: the ring product with a monomial on every component (a signed rotation of the coefficients,
+    pin P3).  k = N/2 multiplies every CKKS slot by the imaginary unit (imult_pairwise_into):
+    zeta_j^(N/2) = exp(i pi (2j+1)/2) = +-i ... the sign alternates with j, see tests."""
+    N, Q = prm.N, prm.Q
+    mono = [0] * N
+    if k < N:
+        mono[k] = 1
+    else:
+        mono[k - N] = Q - 1
+    return tuple(pm(a, mono, Q) for a in ct)

@@ -24,7 +24,7 @@ EXPORTS = [
     "fhe_set_evk", "fhe_polymul", "fhe_he_mult", "fhe_relinearize", "fhe_rescale", "fhe_mult_relin_rescale",
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
-    "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
+    "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_mul_monomial", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
 ]
 
 
@@ -96,6 +96,8 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_add.argtypes = lib.fhe_sub.argtypes = [vp, vp, vp, vp, c_uint32, vp]
     lib.fhe_negate.argtypes = [vp, vp, vp, c_uint32, vp]
     lib.fhe_moddown.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
+    lib.fhe_mul_monomial.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
+    lib.fhe_mul_monomial.restype = c_int
     lib.fhe_add.restype = lib.fhe_sub.restype = lib.fhe_negate.restype = lib.fhe_moddown.restype = c_int
     lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
     lib.fhe_debug_crt_ambiguity.restype = c_int
@@ -345,6 +347,9 @@ class Context:
 
     def fhe_negate(self, a, out=None):
         return self._elem(self._lib.fhe_negate, a, None, out)
+
+    def fhe_mul_monomial(self, a, k: int, out=None):
+        return self._elem(self._lib.fhe_mul_monomial, a, None, out, extra=(k,))
 
     def fhe_moddown(self, a, new_logq: int, out=None):
         return self._elem(self._lib.fhe_moddown, a, None, out, extra=(new_logq,))

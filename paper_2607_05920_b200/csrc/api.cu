@@ -299,6 +299,17 @@ fhe_status fhe_sub(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uin
 fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32_t npoly, void* stream) {
   return elem_call(ctx, 2, d_out, d_a, nullptr, npoly, ctx ? C(ctx)->logQ : 0, stream);
 }
+fhe_status fhe_mul_monomial(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (npoly == 0) return FHE_OK;
+  if (!d_out || !d_in || d_out == d_in) return err(c, FHE_ERR_ARG, "NULL or aliasing pointer");
+  if (misaligned(d_out, 16) || misaligned(d_in, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (k >= 2 * c->N) return err(c, FHE_ERR_ARG, "k must be below 2N");
+  if (c->N < 256) return err(c, FHE_ERR_UNSUPPORTED, "N < 256");
+  CK(launch_monomial(c, d_out, d_in, k, npoly, (cudaStream_t)stream), "monomial");
+  return FHE_OK;
+}
 fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);

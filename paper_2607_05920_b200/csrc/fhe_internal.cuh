@@ -164,6 +164,8 @@ cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a
 // Galois automorphism X -> X^k (k odd) of ciphertexts (kernels_elem.cu): in2 [B][2][L][N] -> out3 [B][3][L][N] =
 // (sigma(c0), 0, sigma(c1)), the triple the key switch of a rotation consumes
 cudaError_t launch_automorphism(Context* c, uint32_t* d_out3, const uint32_t* d_in2, uint32_t k, uint32_t batch, cudaStream_t s);
+// out = X^k * in mod (X^N + 1, Q), 0 <= k < 2N, per polynomial (kernels_elem.cu); out must not alias in
+cudaError_t launch_monomial(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, cudaStream_t s);
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -142,6 +142,54 @@ automorphism_kernel(uint32_t* __restrict__ out3, const uint32_t* __restrict__ in
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Multiplication by the monomial X^k, 0 <= k < 2N: a signed rotation of the coefficients (X^N = -1).  k = N/2 is the
+// multiplication by the imaginary unit of the CKKS slots (imult_pairwise_into), k = 3N/2 its inverse.
+// out[n] = a[n - k] for n >= k (mod 2N bookkeeping below), negated when the index wraps an odd number of times.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+monomial_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, const uint32_t* __restrict__ Q, uint32_t N,
+                uint32_t L, uint32_t bits, uint32_t k, uint32_t ckks) {
+  const uint32_t bpp = N / 256;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
+  const uint32_t ip = (n + 2 * N - k) & (2 * N - 1);                // source index mod 2N: X^k X^ip = X^n
+  const bool neg = ip >= N;
+  const uint32_t* src = in + (size_t)poly * L * N + (neg ? ip - N : ip);
+  uint32_t* dst = out + (size_t)poly * L * N + n;
+  if (!neg) {
+    for (uint32_t l = 0; l < L; ++l) dst[(size_t)l * N] = src[(size_t)l * N];
+  } else if (ckks) {
+    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
+    uint32_t carry = 1;
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = 0;
+      if (l < Lb) {
+        const uint64_t s = (uint64_t)(~src[(size_t)l * N]) + carry;
+        v = (uint32_t)s; carry = (uint32_t)(s >> 32);
+        if (l == Lb - 1) v &= tm;
+      }
+      dst[(size_t)l * N] = v;
+    }
+  } else {
+    uint32_t any = 0;
+    for (uint32_t l = 0; l < L; ++l) any |= src[(size_t)l * N];
+    uint32_t borrow = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+      const uint32_t q = any ? __ldg(Q + l) : 0u, y = src[(size_t)l * N];
+      const uint32_t d = q - y, d2 = d - borrow;
+      borrow = (q < y) | (d < borrow);
+      dst[(size_t)l * N] = d2;
+    }
+  }
+}
+
+cudaError_t launch_monomial(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, cudaStream_t s) {
+  if (!npoly) return cudaSuccess;
+  LaunchTimer lt(c, KC_RESCALE, s);
+  monomial_kernel<<<(c->N / 256) * npoly, 256, 0, s>>>(d_out, d_in, c->d_Qlimbs, c->N, c->L, c->logQ, k, c->t == 0 ? 1u : 0u);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_automorphism(Context* c, uint32_t* d_out3, const uint32_t* d_in2, uint32_t k, uint32_t batch, cudaStream_t s) {
   if (!batch) return cudaSuccess;
   const uint32_t twoN = 2 * c->N;

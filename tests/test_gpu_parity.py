@@ -555,3 +555,17 @@ def test_next3_mult_plain_pairwise_and_broadcast(N, logQ, t, B, group):
         ct = tuple(from_limbs(ct_np[i, k]) for k in range(2))
         want = scheme.mult_plain(prm, ct, from_limbs(pt_np[i // group]))
         assert out[i] == [list(p) for p in want], i
+
+
+@pytest.mark.parametrize("N,logQ,t", [(256, 128, 0), (1024, 218, 0), (256, 100, 257)])
+def test_next1_mul_monomial_matches_the_oracle(N, logQ, t):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logQ, t)
+    ctx = fhe.Context(N, logQ, logQ, t)
+    Q = prm.Q
+    rnd = np.random.default_rng(N + logQ + 3)
+    ct = tuple([int.from_bytes(rnd.bytes((Q.bit_length() + 7) // 8 + 8), "little") % Q for _ in range(N)] for _ in range(2))
+    ct[0][0], ct[0][1], ct[1][N - 1] = 0, Q - 1, 1
+    d = polys_to_tensor([list(ct)], ctx.L)
+    for k in (0, 1, N // 2, N - 1, N, 3 * N // 2, 2 * N - 1):
+        assert tensor_to_polys(ctx.fhe_mul_monomial(d, k))[0] == [list(p) for p in scheme.mul_monomial(prm, ct, k)], k

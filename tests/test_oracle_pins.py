@@ -433,3 +433,29 @@ def test_next3_mult_plain_multiplies_the_slots_and_is_exact_mod_t():
     m2 = [int(v) for v in g.integers(0, 257, size=N)]
     cb = harness.encrypt(prb, g, sb, m1)
     assert harness.decrypt_bgv(scheme.mult_plain(prb, cb, m2), sb, prb) == ring.pm(m1, m2, 257)
+
+
+def test_next1_mul_monomial_is_the_signed_rotation_and_multiplies_slots_by_powers_of_the_roots():
+    import numpy as np
+    import synth
+    from oracle import harness, scheme
+    N, logQ = 64, 100
+    prm = scheme.Params(N, logQ, logQ, 0)
+    g = synth.rng(47)
+    a = [int(v) for v in g.integers(0, 1 << 62, size=N)]
+    Q = prm.Q
+    for k in (0, 1, N // 2, N - 1, N, N + 5, 2 * N - 1):
+        got = scheme.mul_monomial(prm, (a,), k)[0]
+        want = [0] * N
+        for i, x in enumerate(a):                     # X^k X^i = +-X^((i + k) mod N)
+            j = (i + k) % (2 * N)
+            want[j % N] = x % Q if j < N else (-x) % Q
+        assert got == want
+    # slots: (X^k m)(zeta_j) = zeta_j^k m(zeta_j); k = N/2 gives zeta_j^(N/2) = exp(i pi (2j+1)/2) = i (-1)^j
+    s, _ = harness.keygen(prm, g, hwt=16)
+    z = synth.unit_disk(g, N // 2)
+    ct = harness.encrypt(prm, g, s, harness.encode(z, N, 2.0 ** 30))
+    out = scheme.mul_monomial(prm, ct, N // 2)
+    got = harness.decode(harness.decrypt(out, s, Q), N, 2.0 ** 30)
+    want = np.array([1j * (-1) ** j * z[j] for j in range(N // 2)])
+    assert np.max(np.abs(got - want)) < 1e-6
