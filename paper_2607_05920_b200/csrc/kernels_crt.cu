@@ -119,9 +119,10 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 //                tile's MMAs run.
 // ------------------------------------------------------------------------------------------------------------------
 struct CrtEpi {
-  static constexpr int LOAD_WORDS = 64, MAX_REGS = 128;    // 13 warps are allocated as 16: 16 x 32 x 128 = 64 K
-  static constexpr uint32_t GROUPS = 1, LOAD_WARPS = 8;
+  static constexpr int LOAD_WORDS = 64, MAX_REGS = 96;     // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
+  static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;
   static constexpr bool LOAD_ALT = false;
+  static constexpr bool TILE_ALT = true;                   // two whole epilogues on alternate tiles: the epilogue bounds S5
   struct Params {
     uint32_t* out; size_t out_outer, out_inner;
     const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
@@ -146,13 +147,13 @@ struct CrtEpi {
   uint64_t carry = 0;
   uint32_t cur_o = 0, cur_i = 0, cur_n = 0;
 
-  __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t)
+  __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t, uint32_t bar)
       : p(p_), N(a.N), etid(etid_), negm(reinterpret_cast<const uint32_t*>(sm)),
         xs(reinterpret_cast<uint32_t*>(sm) + p_.xs_off), adds(reinterpret_cast<uint32_t*>(sm) + p_.adds_off),
         scratch(reinterpret_cast<uint32_t*>(sm) + p_.scratch_off) {
     uint32_t* w = reinterpret_cast<uint32_t*>(sm);
     for (uint32_t k = etid; k < p.ntab; k += TC) w[k] = k < p.Lraw ? __ldg(p.negM + k) : 0u;
-    pipe::epi_sync(TC);
+    pipe::epi_sync(bar, TC);
   }
 
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
@@ -537,7 +538,7 @@ static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
   CrtEpi::Params ep; size_t bytes;
   crt_scratch_layout(tg, pp, ep, bytes);
-  return pipe::make_plan(tg.KB, tg.nchunks, bytes, true).ok;
+  return pipe::make_plan(tg.KB, tg.nchunks, bytes, true, CrtEpi::TILE_ALT).ok;
 }
 
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
@@ -547,7 +548,7 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   CrtEpi::Params ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);
-  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true);
+  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true, CrtEpi::TILE_ALT);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   if (relin && !d_add) return cudaErrorInvalidValue;

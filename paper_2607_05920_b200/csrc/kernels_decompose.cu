@@ -19,6 +19,7 @@ namespace fhe {
 struct DecEpi {
   static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
   static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
+  static constexpr bool TILE_ALT = false;
   static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: the loaders' round trip bounds S1
   static constexpr int PPG = 16 / GROUPS;                // primes per group and chunk
   struct Params {
@@ -30,11 +31,11 @@ struct DecEpi {
   const uint32_t N, etid;
   const uint2* tab;
   uint32_t* out = nullptr;
-  __device__ DecEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_, uint32_t grp)
+  __device__ DecEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_, uint32_t grp, uint32_t bar)
       : p(p_), N(a.N), etid(etid_), tab(reinterpret_cast<const uint2*>(sm)) {
     uint2* w = reinterpret_cast<uint2*>(sm);
     for (uint32_t j = grp * 128 + etid; j < a.nchunks * 16; j += 128 * GROUPS) w[j] = j < p.K ? __ldg(p.qmu + j) : make_uint2(1u, 0u);
-    pipe::epi_sync(128 * GROUPS);
+    pipe::epi_sync(bar, 128 * GROUPS);
   }
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.res + (size_t)o * p.res_outer + (size_t)i * p.res_inner + n0 + etid;

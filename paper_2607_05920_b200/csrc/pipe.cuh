@@ -39,8 +39,8 @@ constexpr size_t SMEM_LIMIT = 227 * 1024;
 
 struct Ctrl {
   uint64_t a_full[MAX_A], a_free[MAX_A];      // A buffer written (one arrival per loader warp) / consumed (MMA commit)
-  uint64_t d_full[MAX_SPANS];                 // the span's accumulators finished (MMA commit)
-  uint64_t d_free[MAX_CHUNKS];                // the chunk's accumulators are in registers (one arrival per epilogue warp)
+  uint64_t d_full[2][MAX_SPANS];              // [accumulator set] the span's accumulators finished (MMA commit)
+  uint64_t d_free[2][MAX_CHUNKS];                // the chunk's accumulators are in registers (one arrival per epilogue warp)
   uint64_t b_full, mma_done;                  // B of the pass landed (bulk copies) / every MMA of the pass finished
   uint32_t tmem_base;
 };
@@ -56,26 +56,34 @@ struct PipeArgs {
   const uint8_t* B; uint32_t b_cols;
   uint32_t KB, nchunks;
   uint32_t npass, cpp;                        // passes over the tiles, chunks per pass (the last pass may have fewer)
-  uint32_t nA, tmem_cols;
+  uint32_t nA, nsets, tmem_cols;              // nsets: accumulator column sets (2: tiles alternate between them, TILE_ALT)
+  uint32_t epi_stride;                        // TILE_ALT: bytes between the scratch regions of the two epilogue groups
   uint32_t epi_off, b_off;                    // byte offsets of the epilogue scratch and of B in dynamic smem
 };
 
 // ---- host-side plan -----------------------------------------------------------------------------------------------------
 struct Plan {
-  uint32_t KB = 0, nchunks = 0, npass = 0, cpp = 0, nA = 0, tmem_cols = 0, epi_off = 0, b_off = 0;
+  uint32_t KB = 0, nchunks = 0, npass = 0, cpp = 0, nA = 0, nsets = 1, tmem_cols = 0, epi_off = 0, b_off = 0, epi_stride = 0;
   size_t smem = 0;
   bool ok = false;
 };
 // single_pass: the epilogue carries state across the chunks of a tile (S5), so all columns must fit at once
-inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool single_pass) {
+// tile_alt: two epilogue groups on alternate tiles, each with its own accumulator set and scratch region; taken when two
+// sets of all chunks fit beside ONE A buffer (single pass), else the plan falls back to one set served by group 0 alone.
+inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool single_pass, bool tile_alt = false) {
   Plan p;
   p.KB = KB; p.nchunks = nchunks;
   const uint32_t a_cols = KB / 4;
   if (nchunks == 0 || a_cols + NC > 512) return p;
   p.epi_off = CTRL_BYTES;
-  p.b_off = (uint32_t)((CTRL_BYTES + epi_bytes + 127) & ~(size_t)127);
+  p.epi_stride = (uint32_t)((epi_bytes + 127) & ~(size_t)127);
+  p.b_off = CTRL_BYTES + (tile_alt ? 2 : 1) * p.epi_stride;
   if (p.b_off + (size_t)KB * NC > SMEM_LIMIT) return p;
   const uint32_t smem_chunks = (uint32_t)((SMEM_LIMIT - p.b_off) / ((size_t)KB * NC));
+  if (tile_alt && a_cols + 2 * nchunks * NC <= 512 && nchunks <= MAX_CHUNKS &&
+      p.b_off + (size_t)nchunks * KB * NC <= SMEM_LIMIT) {
+    p.nA = 1; p.nsets = 2; p.npass = 1; p.cpp = nchunks;
+  }
   for (uint32_t nA = 2; nA >= 1 && !p.npass; --nA) {
     if (nA * a_cols + NC > 512) continue;
     uint32_t cap = (512 - nA * a_cols) / NC;                // chunks tensor memory holds beside the A buffers
@@ -87,7 +95,7 @@ inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool sing
     p.nA = nA; p.npass = npass; p.cpp = (nchunks + npass - 1) / npass;
   }
   if (!p.npass) return p;
-  const uint32_t cols = p.nA * a_cols + p.cpp * NC;
+  const uint32_t cols = p.nA * a_cols + p.nsets * p.cpp * NC;
   p.tmem_cols = 32;
   while (p.tmem_cols < cols) p.tmem_cols <<= 1;
   p.smem = p.b_off + (size_t)p.cpp * KB * NC;
@@ -95,7 +103,8 @@ inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool sing
   return p;
 }
 inline void fill_args(PipeArgs& a, const Plan& p) {
-  a.KB = p.KB; a.nchunks = p.nchunks; a.npass = p.npass; a.cpp = p.cpp; a.nA = p.nA; a.tmem_cols = p.tmem_cols;
+  a.KB = p.KB; a.nchunks = p.nchunks; a.npass = p.npass; a.cpp = p.cpp; a.nA = p.nA; a.nsets = p.nsets; a.tmem_cols = p.tmem_cols;
+  a.epi_stride = p.epi_stride;
   a.epi_off = p.epi_off; a.b_off = p.b_off;
 }
 
@@ -165,7 +174,10 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 //   static constexpr uint32_t GROUPS;                                 1, 2 or 4 epilogue warp groups: group g takes columns
 //                                                                     [g 64/GROUPS, (g + 1) 64/GROUPS) of every chunk
 //   struct Params;                                                    by-value kernel argument
-//   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid, uint32_t grp);
+//   static constexpr bool TILE_ALT;                                   GROUPS = 2 only: the groups are two whole epilogues on
+//                                                                     alternate tiles (own accumulator set, scratch, Epi object)
+//   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid, uint32_t grp, uint32_t bar);
+//                                                                     bar: named barrier of the threads sharing this scratch (epi_sync)
 //   __device__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0);  polynomial (o, i), first coefficient of the tile
 //   __device__ void consume(uint32_t col0, const uint32_t* t);        64/GROUPS accumulator columns from col0 on, of row etid
 //                                                                     (GROUPS = 1: called twice per chunk, 32 columns each)
@@ -173,8 +185,8 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 // Warp roles: [0, 4 GROUPS) epilogue, then LOAD_WARPS loaders, then the MMA issuer.
 constexpr uint32_t nthreads(uint32_t groups, uint32_t load_warps) { return (4 * groups + load_warps + 1) * 32; }
 
-// barrier among the epilogue threads only (id 1; id 0 is __syncthreads)
-__device__ __forceinline__ void epi_sync(uint32_t nthr) { asm volatile("bar.sync 1, %0;" ::"r"(nthr) : "memory"); }
+// barrier among the epilogue threads that share a scratch region (id >= 1; id 0 is __syncthreads)
+__device__ __forceinline__ void epi_sync(uint32_t bar, uint32_t nthr) { asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(nthr) : "memory"); }
 
 
 template <int NCOL>
@@ -213,10 +225,13 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
 
   if (tid == 0) {
     for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], ALT ? 4 : LOAD_WARPS); mbar_init(&ctl->a_free[i], 1); }
-    for (uint32_t i = 0; i < MAX_SPANS; ++i) mbar_init(&ctl->d_full[i], 1);
+    for (uint32_t i = 0; i < MAX_SPANS; ++i) { mbar_init(&ctl->d_full[0][i], 1); mbar_init(&ctl->d_full[1][i], 1); }
     // one arrival per WARP (its lane 0, after the warp-collective tcgen05.wait): hundreds of per-thread arrivals on one
     // mbarrier serialise in shared memory and were a quarter of the epilogue's time
-    for (uint32_t i = 0; i < MAX_CHUNKS; ++i) mbar_init(&ctl->d_free[i], EPIW);
+    for (uint32_t i = 0; i < MAX_CHUNKS; ++i) {
+      mbar_init(&ctl->d_free[0][i], Epi::TILE_ALT ? 4 : EPIW);
+      mbar_init(&ctl->d_free[1][i], Epi::TILE_ALT ? 4 : EPIW);
+    }
     mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
     fence_barrier_init();
   }
@@ -261,16 +276,17 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
           tc_fence_after();
           for (uint32_t sp = 0; sp < nspan; ++sp) {
             const uint32_t cs = sp * SPAN, ce = cs + SPAN < nc ? cs + SPAN : nc;
-            for (uint32_t c = cs; c < ce; ++c) mbar_wait(&ctl->d_free[c], (wi & 1) ^ 1);
+            const uint32_t dset = a.nsets == 2 ? (wi & 1) : 0, duse = a.nsets == 2 ? (wi >> 1) : wi;   // the set's use count
+            for (uint32_t c = cs; c < ce; ++c) mbar_wait(&ctl->d_free[dset][c], (duse & 1) ^ 1);
             tc_fence_after();
             const uint32_t idesc = idesc_u8(span_w[sp]);
             const uint32_t lbo = span_w[sp] * 16;
             const uint32_t baddr = smem_u32(sB + span_off[sp]);
             for (uint32_t ks = 0; ks < a.KB / KSTEP; ++ks) {
               const uint64_t db = smem_desc(baddr + ks * 2 * lbo, lbo, 128);
-              mma_i8_ts(tmem_d + cs * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
+              mma_i8_ts(tmem_d + (dset * a.cpp + cs) * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
             }
-            mma_commit(&ctl->d_full[sp]);
+            mma_commit(&ctl->d_full[dset][sp]);
           }
           mma_commit(&ctl->a_free[abuf]);
         }
@@ -292,15 +308,18 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         const uint32_t abuf = wi & amask;
         const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
         bool waited = false;
-        for (uint32_t w0 = ALT ? 0 : half * LR; w0 < a_cols; w0 += (ALT ? 1 : HALVES) * LR) {   // this warp's batches of LR words
+        // the warps of a lane quarter share the row: contiguous, equal ranges of its words (multiples of 8), LR at a time
+        const uint32_t wph = ALT ? a_cols : ((a_cols + HALVES - 1) / HALVES + 7) / 8 * 8;
+        const uint32_t w_lo = ALT ? 0 : half * wph, w_hi = w_lo + wph < a_cols ? w_lo + wph : a_cols;
+        for (uint32_t w0 = w_lo; w0 < w_hi; w0 += LR) {
           uint32_t w[LR];
-          load_batch<LR>(w, p, a.N, w0, a.nwords);
+          load_batch<LR>(w, p, a.N, w0, w_hi < a.nwords ? w_hi : a.nwords);
           if (!waited) {                                           // loads are in flight while the buffer is still being read
             mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
             tc_fence_after();
             waited = true;
           }
-          store_batch<LR>(w, taddr, w0, a_cols, a.mask_bits);
+          store_batch<LR>(w, taddr, w0, w_hi, a.mask_bits);
         }
         if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
         tmem_st_wait();
@@ -313,7 +332,37 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
     const uint32_t grp = warp >> 2;
     const uint32_t etid = (warp & 3) * 32 + lane;                  // 0..127 = tile row = TMEM lane
     const uint32_t lane_off = ((warp & 3) * 32u) << 16;
-    Epi epi(ep, a, smem + a.epi_off, etid, grp);
+    if constexpr (Epi::TILE_ALT) {
+      // two groups, each a whole epilogue of its own on the tiles wi = grp (mod 2): own accumulator set, own scratch
+      // region, own Epi object -- no state crosses between them.  With one set only (plan fallback) group 0 does it all.
+      const uint32_t nset = a.nsets;
+      if (grp < nset) {
+        Epi epi(ep, a, smem + a.epi_off + grp * a.epi_stride, etid, 0, 1 + grp);
+        const uint32_t tset = tmem_d + grp * a.cpp * NC;
+        const uint32_t nc = a.nchunks;                             // single pass
+        for (uint32_t wi = grp, use = 0; wi < mine; wi += nset, ++use) {
+          const uint32_t tile = blockIdx.x + wi * gridDim.x;
+          const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
+          epi.begin_tile(poly / a.inner, poly % a.inner, n0);
+          for (uint32_t c = 0; c < nc; ++c) {
+            if (c % SPAN == 0) {
+              mbar_wait(&ctl->d_full[grp][c / SPAN], use & 1);
+              tc_fence_after();
+            }
+            uint32_t t[64];
+            tmem_ld32_nowait(tset + c * NC + lane_off, t);
+            tmem_ld32_nowait(tset + c * NC + 32 + lane_off, t + 32);
+            tmem_ld_wait();
+            tc_fence_before();
+            if (lane == 0) mbar_arrive(&ctl->d_free[grp][c]);     // the accumulator chunk is in registers: hand it back
+            epi.consume(c * NC, t);
+            epi.consume(c * NC + 32, t + 32);
+          }
+          epi.end_tile();
+        }
+      }
+    } else {
+    Epi epi(ep, a, smem + a.epi_off, etid, grp, 1);
     uint32_t wi = 0;
     for (uint32_t ps = 0; ps < a.npass; ++ps) {
       const uint32_t c0 = ps * a.cpp;
@@ -324,7 +373,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         epi.begin_tile(poly / a.inner, poly % a.inner, n0);
         for (uint32_t c = 0; c < nc; ++c) {
           if (c % SPAN == 0) {
-            mbar_wait(&ctl->d_full[c / SPAN], wi & 1);
+            mbar_wait(&ctl->d_full[0][c / SPAN], wi & 1);
             tc_fence_after();
           }
           if constexpr (GROUPS == 1) {
@@ -333,22 +382,21 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
             tmem_ld32_nowait(tmem_d + c * NC + 32 + lane_off, t + 32);
             tmem_ld_wait();
             tc_fence_before();
-            if (lane == 0) mbar_arrive(&ctl->d_free[c]);           // the accumulator chunk is in registers: hand it back
-            {
-              epi.consume((c0 + c) * NC, t);
-              epi.consume((c0 + c) * NC + 32, t + 32);
-            }
+            if (lane == 0) mbar_arrive(&ctl->d_free[0][c]);        // the accumulator chunk is in registers: hand it back
+            epi.consume((c0 + c) * NC, t);
+            epi.consume((c0 + c) * NC + 32, t + 32);
           } else {
             uint32_t t[GC];
             tmem_ld_cols<GC>(tmem_d + c * NC + grp * GC + lane_off, t);
             tmem_ld_wait();
             tc_fence_before();
-            if (lane == 0) mbar_arrive(&ctl->d_free[c]);
+            if (lane == 0) mbar_arrive(&ctl->d_free[0][c]);
             epi.consume((c0 + c) * NC + grp * GC, t);
           }
         }
         epi.end_tile();
       }
+    }
     }
   }
   tc_fence_before();
