@@ -7,7 +7,8 @@ One "step" = one pass of the whole hot path (decompose,
 inverse NTT, CRT + mod Q, relinearise with evk mod PQ + divide by P, rescale by 2^40) over one batch of 4
 synthetic ciphertext pairs per GPU (BASELINE.json configs[4]).  Prints ONE JSON line (rank 0).
 Multi-GPU: the batch dimension shards with no data-path collective -> weak scaling, evk replicated.
-`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample on the host cores.
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample (one ring product of the
+workload's shape per step) on the host cores.
 """
 from __future__ import annotations
 
@@ -211,55 +212,30 @@ def oracle_sample_product(N, logQ, seed=0):
     return time.perf_counter() - t0
 
 
-def oracle_sample_coeffs(N, logQ, logP, p_bits, count, seed=0):
-    """`count` output coefficients of one full op (he_mult -> relinearize -> rescale) straight from the definition
-    (oracle.ring.pm_coeff, Eq. 5-6) and the oracle's rounding rules.  Returns seconds."""
-    import numpy as np
-    import synth
-    from oracle import ring, scheme
-    from oracle.limbs import from_limbs
-    g = synth.rng(seed)
-    Q, PQ = 1 << logQ, 1 << (logQ + logP)
-    c = [from_limbs(synth.uniform_limbs(g, (), N, logQ)) for _ in range(4)]
-    evk = [from_limbs(synth.uniform_limbs(g, (), N, logQ + logP)) for _ in range(2)]
-    d2 = from_limbs(synth.uniform_limbs(g, (), N, logQ))   # stands in for the full d2 the relin product needs
-    ks = [int(v) for v in np.random.default_rng(seed).integers(0, N, size=count)]
-    t0 = time.perf_counter()
-    for k in ks:
-        d0 = ring.pm_coeff(c[0], c[2], k, Q)
-        d1 = (ring.pm_coeff(c[0], c[3], k, Q) + ring.pm_coeff(c[1], c[2], k, Q)) % Q
-        _ = ring.pm_coeff(c[1], c[3], k, Q)
-        out = []
-        for comp, d in ((0, d0), (1, d1)):
-            x = ring.pm_coeff(d2, evk[comp], k, PQ)
-            v = (d + scheme.round_shift(x, logP) % Q) % Q
-            out.append(scheme.round_shift(v, p_bits) % (1 << (logQ - p_bits)))
-    return time.perf_counter() - t0
-
-
 def run_reference(args):
+    """The oracle as it stands on the host cores: at this size its ring product goes through its own NTT route
+    (oracle.ring.pm).  A step times ONE ring product mod Q of one pair of the workload's shape (about 14 s on one core)
+    and converts it to ops/s with the 4 + 2 * 2.06 products an op costs -- the same bounded sample as `cpu_baseline`."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
     N, logQ, logP, B, p_bits = WORKLOADS[args.workload]
-    total_steps = args.steps + args.warmup
-    budget = max(0.5, min(20.0, 150.0 / max(1, total_steps)))      # seconds per step
-    t_probe = oracle_sample_coeffs(N, logQ, logP, p_bits, 1)
-    count = max(1, int(budget / max(t_probe, 1e-3)))
-    for _ in range(args.warmup):
-        oracle_sample_coeffs(N, logQ, logP, p_bits, count)
+    for i in range(args.warmup):
+        oracle_sample_product(N, logQ, seed=100 + i)
     t0 = time.perf_counter()
     for i in range(args.steps):
-        oracle_sample_coeffs(N, logQ, logP, p_bits, count, seed=i)
+        oracle_sample_product(N, logQ, seed=i)
     dt = time.perf_counter() - t0
-    value = (args.steps * count / N) / dt          # ops/s: an op has N output coefficients (per component pair)
-    sample = f"{count} of {N} output coefficients of one op per step via the definition (oracle.ring.pm_coeff, Eq. 5-6), scaled by N/{count}"
+    t_prod = dt / args.steps
+    value = 1.0 / (t_prod * ORACLE_PRODUCTS_PER_OP)
+    sample = (f"per step 1 ring product mod Q of 1 pair (oracle.ring.pm, own NTT route) = {t_prod:.1f} s; "
+              f"an op = 4 products mod Q + 2 mod PQ = {ORACLE_PRODUCTS_PER_OP:.2f} such products")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "int (python big integers)", "data": "synthetic",
+        "vs_baseline": None, "dtype": "int (python big integers, numpy uint64 NTT)", "data": "synthetic",
         "config": {"workload": f"{args.workload}: CKKS N={N} logQ={logQ} logP={logP} batch={B} rescale={p_bits}"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(), "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
