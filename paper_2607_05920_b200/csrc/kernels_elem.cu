@@ -33,10 +33,8 @@ elem_ckks_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, con
         const uint64_t s = (uint64_t)x + b[base + (size_t)l * N] + carry;
         v = (uint32_t)s; carry = (uint32_t)(s >> 32);
       } else if (OP == EL_SUB) {
-        const uint32_t y = b[base + (size_t)l * N];
-        const uint32_t d = x - y, d2 = d - carry;
-        carry = (x < y) | (d < carry);
-        v = d2;
+        const uint64_t d = (uint64_t)x - b[base + (size_t)l * N] - carry;   // >= -2^32: the borrow is the sign
+        v = (uint32_t)d; carry = (uint32_t)(d >> 63);
       } else if (OP == EL_NEG) {
         const uint64_t s = (uint64_t)(~x) + carry;
         v = (uint32_t)s; carry = (uint32_t)(s >> 32);
