@@ -141,6 +141,12 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// streaming load: read once, no L1 line allocated for it
+__device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
 // One batch of LR words (A columns [w0, w0 + LR)) of this thread's row: issue the loads ...
 template <int LR>
 __device__ __forceinline__ void load_batch(uint32_t (&w)[LR], const uint32_t* __restrict__ p, size_t N, uint32_t w0,
@@ -148,7 +154,7 @@ __device__ __forceinline__ void load_batch(uint32_t (&w)[LR], const uint32_t* __
 #pragma unroll
   for (int i = 0; i < LR; ++i) {
     const uint32_t wi = w0 + i;
-    w[i] = wi < nwords ? __ldg(p + (size_t)wi * N) : 0u;        // warp-uniform predicate
+    w[i] = wi < nwords ? ld_stream(p + (size_t)wi * N) : 0u;    // warp-uniform predicate
   }
 }
 // ... then mask the top word and write the batch to TMEM columns [w0, min(w0 + LR, a_cols)).
