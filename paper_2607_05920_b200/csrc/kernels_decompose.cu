@@ -17,11 +17,11 @@ namespace fhe {
 // is at most 20 short (the shifted-out bits of T1, T2 and T0 >> 21 < 16), and one Barrett step: qh = mulhi(vh, mu) is
 // floor(v / q) or one less (20 * 2^21 / q < 0.16 for q > 2^28), so the 32-bit remainder lies in [0, 2q).
 struct DecEpi {
-  static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
-  static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
+  static constexpr int LOAD_WORDS = 40, MAX_REGS = 96;   // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
+  static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;   // measured: 1 group 0.229 ms, 2 groups 0.202 ms, 4 groups 0.215 ms per C5 step
   static constexpr bool TILE_ALT = false;
   static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: the loaders' round trip bounds S1
-  static constexpr int PPG = 16 / GROUPS;                // primes per group and chunk
+  static constexpr int PPG = GROUPS == 1 ? 8 : 16 / GROUPS;   // primes per consume call (GROUPS = 1: two calls per chunk)
   struct Params {
     uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
     const uint2* qmu;                             // (q_j, floor(2^53 / q_j))
