@@ -104,6 +104,47 @@ __device__ __forceinline__ void phase_b(uint32_t (&x)[16], const uint2* __restri
 #undef STG
 }
 
+// The same stages on NOPS sequences that share every twiddle (adjacent columns of one prime in the column pass): the
+// twiddles are loaded once per stage.
+template <int NOPS, int E, int S, bool INV>
+__device__ __forceinline__ void reg_stage_multi(uint32_t (&x)[NOPS][16], const uint2* __restrict__ tw, uint32_t q, uint32_t q2) {
+  constexpr int NG = 1 << S, H = E >> (S + 1);
+  uint2 w[8];
+  load_tw<NG>(tw, w);
+#pragma unroll
+  for (int o = 0; o < NOPS; ++o)
+#pragma unroll
+    for (int g = 0; g < NG; ++g)
+#pragma unroll
+      for (int k = 0; k < H; ++k) {
+        const int i0 = g * 2 * H + k;
+        if (!INV) bf_fwd(x[o][i0], x[o][i0 + H], w[g], q, q2);
+        else bf_inv(x[o][i0], x[o][i0 + H], w[g], q, q2);
+      }
+}
+template <int NOPS, bool INV, int NS>
+__device__ __forceinline__ void phase_a_multi(uint32_t (&x)[NOPS][16], const uint2* __restrict__ tw, uint32_t base, uint32_t q, uint32_t q2) {
+  if (!INV) {
+    reg_stage_multi<NOPS, 16, 0, false>(x, tw + base, q, q2);
+    if constexpr (NS > 1) reg_stage_multi<NOPS, 16, 1, false>(x, tw + 2 * base, q, q2);
+    if constexpr (NS > 2) reg_stage_multi<NOPS, 16, 2, false>(x, tw + 4 * base, q, q2);
+    if constexpr (NS > 3) reg_stage_multi<NOPS, 16, 3, false>(x, tw + 8 * base, q, q2);
+  } else {
+    if constexpr (NS > 3) reg_stage_multi<NOPS, 16, 3, true>(x, tw + 8 * base, q, q2);
+    if constexpr (NS > 2) reg_stage_multi<NOPS, 16, 2, true>(x, tw + 4 * base, q, q2);
+    if constexpr (NS > 1) reg_stage_multi<NOPS, 16, 1, true>(x, tw + 2 * base, q, q2);
+    reg_stage_multi<NOPS, 16, 0, true>(x, tw + base, q, q2);
+  }
+}
+template <int NOPS, int LN, bool INV>
+__device__ __forceinline__ void phase_b_multi(uint32_t (&x)[NOPS][16], const uint2* __restrict__ tw, uint32_t base, uint32_t tb, uint32_t q, uint32_t q2) {
+  constexpr int S0 = LN - 4;
+#define STGM(S) reg_stage_multi<NOPS, 16, S, INV>(x, tw + (base << (S0 + S)) + (tb << S), q, q2)
+  if (!INV) { STGM(0); STGM(1); STGM(2); STGM(3); }
+  else { STGM(3); STGM(2); STGM(1); STGM(0); }
+#undef STGM
+}
+
 __device__ __forceinline__ uint32_t canon4(uint32_t v, uint32_t q, uint32_t q2) { v = min(v, v - q2); return min(v, v - q); }
 
 // Montgomery product: a b 2^-32 mod q in [0, q) (the inverse transform's final constant carries the 2^32)
@@ -183,6 +224,57 @@ ntt_col_kernel(NttArgs a) {
 #pragma unroll
       for (int i = 0; i < E; ++i) g[(size_t)i * 256] = mul_shoup(x[i], sc.x, sc.y, q);
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Column pass, two adjacent columns per thread (LN > 4): the same transforms as ntt_col_kernel, but a thread moves its
+// points as 8-byte pairs, so that a warp access is two full 128-byte lines of two rows instead of two half lines, and the
+// two columns share the twiddles of every stage.  A block owns 2 T2 adjacent columns of one (polynomial, prime).
+// ------------------------------------------------------------------------------------------------------------------
+template <int LN, bool INV>
+__global__ void __launch_bounds__(256, 3)
+ntt_col2_kernel(NttArgs a) {
+  static_assert(LN > 4 && LN <= 8, "paired column pass: 32..256-point columns");
+  constexpr int TPC = (1 << LN) / 16;                // threads per column pair
+  constexpr int T2 = 256 / TPC;                      // column pairs per block
+  constexpr int W = 2 * T2;                          // columns per block = words per tile row
+  __shared__ __align__(8) uint32_t sm[8192];
+  const uint32_t tid = threadIdx.x, cp = tid % T2, t = tid / T2;
+  constexpr uint32_t tiles = 256 / W;
+  const uint32_t tr = blockIdx.x / tiles, c0 = (blockIdx.x % tiles) * W;
+  const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
+  const uint2* tw = a.tw + (size_t)j * a.N;
+  uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + c0 + 2 * cp;
+  uint32_t x[2][16];
+  auto ld2 = [&](const uint32_t* p, int i) { const uint2 v = *reinterpret_cast<const uint2*>(p); x[0][i] = v.x; x[1][i] = v.y; };
+  if (!INV) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) ld2(g + (size_t)(i * TPC + t) * 256, i);
+    phase_a_multi<2, false, LN - 4>(x, tw, 1, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) *reinterpret_cast<uint2*>(sm + (i * TPC + t) * W + 2 * cp) = make_uint2(x[0][i], x[1][i]);
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 16; ++i) ld2(sm + (t * 16 + i) * W + 2 * cp, i);
+    phase_b_multi<2, LN, false>(x, tw, 1, t, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) *reinterpret_cast<uint2*>(g + (size_t)(t * 16 + i) * 256) = make_uint2(x[0][i], x[1][i]);
+  } else {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) ld2(g + (size_t)(t * 16 + i) * 256, i);
+    phase_b_multi<2, LN, true>(x, tw, 1, t, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) *reinterpret_cast<uint2*>(sm + (t * 16 + i) * W + 2 * cp) = make_uint2(x[0][i], x[1][i]);
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 16; ++i) ld2(sm + (i * TPC + t) * W + 2 * cp, i);
+    phase_a_multi<2, true, LN - 4>(x, tw, 1, q, q2);
+    const uint2 sc = __ldg(a.scale + j);
+#pragma unroll
+    for (int i = 0; i < 16; ++i)
+      *reinterpret_cast<uint2*>(g + (size_t)(i * TPC + t) * 256) = make_uint2(mul_shoup(x[0][i], sc.x, sc.y, q), mul_shoup(x[1][i], sc.x, sc.y, q));
   }
 }
 
@@ -458,11 +550,18 @@ static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaSt
     ntt_col_kernel<LN, INV><<<ntr * TPC, 256, 0, s>>>(a);                                      \
     break;                                                                                     \
   }
-  switch (ln1) {   // blocks per transform = 256 / T = TPC
-    COL_CASE(1) COL_CASE(2) COL_CASE(3) COL_CASE(4) COL_CASE(5) COL_CASE(6) COL_CASE(7) COL_CASE(8)
+#define COL2_CASE(LN)                                                                          \
+  case LN: {                                                                                   \
+    constexpr int TPC = (1 << LN) / 16;                                                        \
+    ntt_col2_kernel<LN, INV><<<ntr * (256 / (2 * (256 / TPC))), 256, 0, s>>>(a);               \
+    break;                                                                                     \
+  }
+  switch (ln1) {   // blocks per transform = 256 / T = TPC (single columns) or TPC / 2 (column pairs)
+    COL_CASE(1) COL_CASE(2) COL_CASE(3) COL_CASE(4) COL2_CASE(5) COL2_CASE(6) COL2_CASE(7) COL2_CASE(8)
     default: return cudaErrorInvalidValue;
   }
 #undef COL_CASE
+#undef COL2_CASE
   return cudaGetLastError();
 }
 
