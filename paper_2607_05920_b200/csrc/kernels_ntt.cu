@@ -233,7 +233,7 @@ ntt_col_kernel(NttArgs a) {
 // two columns share the twiddles of every stage.  A block owns 2 T2 adjacent columns of one (polynomial, prime).
 // ------------------------------------------------------------------------------------------------------------------
 template <int LN, bool INV>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(256, 4)
 ntt_col2_kernel(NttArgs a) {
   static_assert(LN > 4 && LN <= 8, "paired column pass: 32..256-point columns");
   constexpr int TPC = (1 << LN) / 16;                // threads per column pair
