@@ -37,7 +37,7 @@ WORKLOADS = {
 ORACLE_PRODUCTS_PER_OP = 4 + 2 * 2.06
 # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/, same command as the
 # timed run): dram__bytes_read.sum + dram__bytes_write.sum, averaged over that class's launches of one step.
-NCU_TRAFFIC = {"pointwise": 604.3e6}   # profiles/r1x_launches_and_captures.md: (440.1 + 219.2 + 329.8 + 219.5) MB / 2 launches
+NCU_TRAFFIC = {"pointwise": 605.3e6}   # profiles/r1y_launches_and_captures.md: (440.2 + 218.6 + 329.8 + 221.9) MB / 2 launches
 
 
 def _peaks():
