@@ -439,19 +439,27 @@ ntt_row_fused_kernel(NttArgs a) {
     ldrow(a1, g + KN, t);
     ldrow(b0, g + 2 * KN, t);
     ldrow(b1, g + 3 * KN, t);
-    fwd_canon(a0);     // the exchange inside orders every lane's operand loads before the first store below
+    // The exchange inside the first transform orders every lane's operand loads before the first store below.
+    fwd_canon(a0);
     fwd_canon(a1);
     fwd(b0);
     fwd(b1);
+    // One copy of the inverse transform's code, looped over the three outputs (uniform branches form the products):
+    // fully unrolled the kernel is 55 KB of straight-line code and stalled on instruction fetch more than on anything else.
+#pragma unroll 1
+    for (int op = 0; op < 3; ++op) {
+      if (op == 0) {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
-    finish(x, g);
+        for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
+      } else if (op == 1) {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
-    finish(x, g + KN);
+        for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
+      } else {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
-    finish(x, g + 2 * KN);
+        for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
+      }
+      finish(x, g + (size_t)op * KN);
+    }
   } else {   // PW_RELIN: slot 0 = d2 residues after the forward column pass; aux = evk-hat (fully transformed, canonical)
     static_assert(PW == PW_RELIN, "fused row pass: unknown mode");
     uint32_t* g = a.data + (size_t)item * 2 * KN + poff;
