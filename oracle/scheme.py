@@ -195,6 +195,20 @@ def mult_plain(prm: Params, ct, m):
     return pm(ct[0], m, Q), pm(ct[1], m, Q)
 
 
+def add_plain(prm: Params, ct, m):
+    """ct + plaintext polynomial m (addconst_pairwise / _broadcast: names only): the plaintext is added
+    to component 0, since Dec = c0 + c1 s is linear and Dec of (m, 0) is m."""
+    Q = prm.Q
+    return [(x + y) % Q for x, y in zip(ct[0], m)], list(ct[1])
+
+
+def mult_scalar(prm: Params, ct, k: int):
+    """ct times the integer constant k (multconst with a scalar: names only): every coefficient of both
+    components times k mod Q; k may be negative."""
+    Q = prm.Q
+    return tuple([(x * k) % Q for x in a] for a in ct)
+
+
 def mul_monomial(prm: Params, ct, k: int):
     """X^k * ct, 0 <= k < 2N: the ring product with a monomial on every component (a signed rotation of the coefficients,
     pin P3).  k = N/2 multiplies every CKKS slot by the imaginary unit (imult_pairwise_into):

@@ -459,3 +459,46 @@ def test_next1_mul_monomial_is_the_signed_rotation_and_multiplies_slots_by_power
     got = harness.decode(harness.decrypt(out, s, Q), N, 2.0 ** 30)
     want = np.array([1j * (-1) ** j * z[j] for j in range(N // 2)])
     assert np.max(np.abs(got - want)) < 1e-6
+
+
+def test_next3_add_plain_and_mult_scalar_are_linear_under_decryption():
+    """add_plain: Dec(ct + m) = Dec(ct) + m exactly mod Q (CKKS: slots add; BGV: plaintexts add mod t).  mult_scalar:
+    k = 3 equals ct + ct + ct (the pinned ct_add), k = -1 the pinned ct_negate, k = 0 the zero ciphertext, Dec scales by k;
+    both agree with the ring product by the constant polynomial (pm, pinned by P1-P4)."""
+    import numpy as np
+    import synth
+    from oracle import harness, scheme
+    from oracle.ring import pm
+    N, logQ = 64, 100
+    prm = scheme.Params(N, logQ, logQ, 0)
+    g = synth.rng(37)
+    s, _ = harness.keygen(prm, g, hwt=16)
+    z1, z2 = synth.unit_disk(g, N // 2), synth.unit_disk(g, N // 2)
+    Q = prm.Q
+    ct = harness.encrypt(prm, g, s, harness.encode(z1, N, 2.0 ** 30))
+    m = [x % Q for x in harness.encode(z2, N, 2.0 ** 30)]
+    ap = scheme.add_plain(prm, ct, m)
+    d = harness.decrypt(ct, s, Q)
+    assert [x % Q for x in harness.decrypt(ap, s, Q)] == [(a + b) % Q for a, b in zip(d, m)]
+    assert np.max(np.abs(harness.decode(harness.decrypt(ap, s, Q), N, 2.0 ** 30) - (z1 + z2))) < 1e-6
+    assert list(ap[1]) == list(ct[1])
+    three = scheme.mult_scalar(prm, ct, 3)
+    assert three == scheme.ct_add(prm, scheme.ct_add(prm, ct, ct), ct)
+    assert scheme.mult_scalar(prm, ct, -1) == scheme.ct_negate(prm, ct)
+    assert scheme.mult_scalar(prm, ct, 0) == tuple([0] * N for _ in range(2))
+    for k in (7, -5, 2 ** 31 - 1, -(2 ** 31 - 1)):
+        got = scheme.mult_scalar(prm, ct, k)
+        const = [k % Q] + [0] * (N - 1)
+        assert got == tuple(pm(a, const, Q) for a in ct)
+        assert [x % Q for x in harness.decrypt(got, s, Q)] == [(x * k) % Q for x in d]
+    assert np.max(np.abs(harness.decode(harness.decrypt(scheme.mult_scalar(prm, ct, -5), s, Q), N, 2.0 ** 30) + 5 * z1)) < 1e-5
+    # BGV: exact mod t
+    prb = scheme.Params(N, 60, 60, 257)
+    sb, _ = harness.keygen(prb, g, hwt=None)
+    m1 = [int(v) for v in g.integers(0, 257, size=N)]
+    m2 = [int(v) for v in g.integers(0, 257, size=N)]
+    c1 = harness.encrypt(prb, g, sb, m1)
+    assert harness.decrypt_bgv(scheme.add_plain(prb, c1, m2), sb, prb) == [(a + b) % 257 for a, b in zip(m1, m2)]
+    assert harness.decrypt_bgv(scheme.mult_scalar(prb, c1, 11), sb, prb) == [(a * 11) % 257 for a in m1]
+    assert harness.decrypt_bgv(scheme.mult_scalar(prb, c1, -3), sb, prb) == [(-3 * a) % 257 for a in m1]
+    assert scheme.mult_scalar(prb, c1, 3) == scheme.ct_add(prb, scheme.ct_add(prb, c1, c1), c1)
