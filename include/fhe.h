@@ -173,6 +173,18 @@ fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uin
 fhe_status fhe_mult_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
                           uint32_t group, void* d_ws, size_t ws_bytes, void* stream);
 
+/* ---- NEXT-3, constants (addconst / multconst with a scalar: names only; reading in DESIGN.md 3) ------
+ *   fhe_add_plain     out[i] = (c0_i + m_j, c1_i) mod Q, j = i / group (group = 1: pairwise, group = batch: broadcast).
+ *                     d_ct, d_out2 [B][2][L][N]; d_pt [ceil(B / group)][L][N] canonical in [0, Q).  In place
+ *                     (d_out2 == d_ct) is allowed.  CKKS and BGV.
+ *   fhe_mult_scalar   every coefficient of `npoly` polynomials [L][N] times the integer k mod Q, |k| < 2^31 (k = INT32_MIN is
+ *                     FHE_ERR_ARG); in place allowed.  CKKS and BGV (BGV: FHE_ERR_UNSUPPORTED when logQ < 66, where the
+ *                     single-word quotient estimate does not hold).
+ * One streaming kernel each, a thread per coefficient; no workspace. */
+fhe_status fhe_add_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                         uint32_t group, void* stream);
+fhe_status fhe_mult_scalar(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, void* stream);
+
 /* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
 
 /* Host copies of the first `count` NTT primes and the primitive 2N-th roots psi_j the tables were built from. */

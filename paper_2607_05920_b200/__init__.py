@@ -25,6 +25,7 @@ EXPORTS = [
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
     "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_mul_monomial", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
+    "fhe_add_plain", "fhe_mult_scalar",
 ]
 
 
@@ -99,6 +100,10 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_mul_monomial.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
     lib.fhe_mul_monomial.restype = c_int
     lib.fhe_add.restype = lib.fhe_sub.restype = lib.fhe_negate.restype = lib.fhe_moddown.restype = c_int
+    lib.fhe_add_plain.argtypes = [vp, vp, vp, vp, c_uint32, c_uint32, vp]
+    lib.fhe_add_plain.restype = c_int
+    lib.fhe_mult_scalar.argtypes = [vp, vp, vp, ctypes.c_int32, c_uint32, vp]
+    lib.fhe_mult_scalar.restype = c_int
     lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
     lib.fhe_debug_crt_ambiguity.restype = c_int
     lib.fhe_debug_int_peak.argtypes = [vp, c_int, POINTER(ctypes.c_double), vp]
@@ -353,6 +358,21 @@ class Context:
 
     def fhe_moddown(self, a, new_logq: int, out=None):
         return self._elem(self._lib.fhe_moddown, a, None, out, extra=(new_logq,))
+
+    # ---- NEXT-3, constants ----
+    def fhe_add_plain(self, ct, pt, group: int = 1, out=None):
+        B = ct.shape[0]
+        npt = (B + group - 1) // group if group else 0
+        out = self._torch_empty_like(ct) if out is None else out
+        n = B * 2 * self.L * self.N
+        self._check(self._lib.fhe_add_plain(self._h, _dev_ptr(out, n, "out"), _dev_ptr(ct, n, "ct"),
+                                            _dev_ptr(pt, npt * self.L * self.N, "pt"), B, group, self._stream(None)))
+        return out
+
+    def fhe_mult_scalar(self, a, k: int, out=None):
+        if not -2 ** 31 <= k < 2 ** 31:
+            raise ValueError("k must fit a signed 32-bit integer")
+        return self._elem(self._lib.fhe_mult_scalar, a, None, out, extra=(k,))
 
     # ---- debug entry points --------------------------------------------------------------------------------------
     def fhe_debug_decompose(self, limbs, K: int, mask_bits: int = 0, stream=None):

@@ -310,6 +310,37 @@ fhe_status fhe_mul_monomial(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in,
   CK(launch_monomial(c, d_out, d_in, k, npoly, (cudaStream_t)stream), "monomial");
   return FHE_OK;
 }
+// ---- NEXT-3: constants ----------------------------------------------------------------------------------------------------
+fhe_status fhe_add_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                         uint32_t group, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (batch == 0) return FHE_OK;
+  if (!d_out2 || !d_ct || !d_pt) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out2, 16) || misaligned(d_ct, 16) || misaligned(d_pt, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (group == 0) return err(c, FHE_ERR_ARG, "group must be at least 1");
+  if (c->N < 256) return err(c, FHE_ERR_UNSUPPORTED, "N < 256");
+  CK(launch_add_plain(c, d_out2, d_ct, d_pt, batch, group, (cudaStream_t)stream), "add_plain");
+  return FHE_OK;
+}
+fhe_status fhe_mult_scalar(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (npoly == 0) return FHE_OK;
+  if (!d_out || !d_in) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out, 16) || misaligned(d_in, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (k == INT32_MIN) return err(c, FHE_ERR_ARG, "|k| must be below 2^31");
+  if (c->N < 256) return err(c, FHE_ERR_UNSUPPORTED, "N < 256");
+  if (c->t != 0) {   // the quotient estimate needs Q = 2^logQ + e with e < 2^(logQ - 33) (kernels_elem.cu)
+    std::vector<uint32_t> e(c->h_Q.begin(), c->h_Q.begin() + c->L);
+    e[c->logQ >> 5] &= ~(1u << (c->logQ & 31));
+    bool ok = c->logQ >= 34 + 32;
+    for (uint32_t l = 1; l < c->L; ++l) ok = ok && e[l] == 0;       // e below 2^32 <= 2^(logQ - 33) - 1 then
+    if (!ok) return err(c, FHE_ERR_UNSUPPORTED, "mult_scalar (BGV): Q - 2^logQ too large for this logQ");
+  }
+  CK(launch_mult_scalar(c, d_out, d_in, k, npoly, (cudaStream_t)stream), "mult_scalar");
+  return FHE_OK;
+}
 fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);

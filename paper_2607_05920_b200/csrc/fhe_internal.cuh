@@ -166,6 +166,9 @@ cudaError_t launch_elem(Context* c, int op, uint32_t* d_out, const uint32_t* d_a
 cudaError_t launch_automorphism(Context* c, uint32_t* d_out3, const uint32_t* d_in2, uint32_t k, uint32_t batch, cudaStream_t s);
 // out = X^k * in mod (X^N + 1, Q), 0 <= k < 2N, per polynomial (kernels_elem.cu); out must not alias in
 cudaError_t launch_monomial(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, cudaStream_t s);
+cudaError_t launch_add_plain(Context* c, uint32_t* d_out, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                             uint32_t group, cudaStream_t s);
+cudaError_t launch_mult_scalar(Context* c, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, cudaStream_t s);
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -181,6 +181,125 @@ monomial_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, con
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// NEXT-3, constants (addconst / multconst: names only; reading in DESIGN.md 3).
+//   add_plain:   out = (c0 + m, c1): ciphertext i gets plaintext polynomial i / group added to component 0; component 1 is
+//                copied (skipped in place).
+//   mult_scalar: every coefficient times the integer k, |k| < 2^31.  x |k| has L + 1 limbs.  CKKS: the low logQ bits,
+//                two's complement for k < 0.  BGV: Q = 2^logQ + e with 0 < e < 2^(logQ - 33) (the least odd integer above
+//                2^logQ that is 1 mod t, checked by the caller), so floor(x |k| / Q) is h = floor(x |k| / 2^logQ) or
+//                h - 1 (x |k| / 2^logQ - x |k| / Q < 2^31 e / 2^logQ < 1): r = x |k| - h Q, + Q when negative; Q - r for
+//                k < 0 and r != 0.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+add_plain_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ ct, const uint32_t* __restrict__ pt,
+                 const uint32_t* __restrict__ Q, uint32_t N, uint32_t L, uint32_t bits, uint32_t group, uint32_t ckks) {
+  const uint32_t bpp = N / 256;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
+  const size_t base = (size_t)poly * L * N + n;
+  if (poly & 1) {                                                   // component 1
+    if (out != ct)
+      for (uint32_t l = 0; l < L; ++l) out[base + (size_t)l * N] = ct[base + (size_t)l * N];
+    return;
+  }
+  const uint32_t* m = pt + (size_t)((poly >> 1) / group) * L * N + n;
+  uint32_t r[ELEM_MAX_LIMBS];
+  uint32_t carry = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    const uint64_t s = (uint64_t)ct[base + (size_t)l * N] + m[(size_t)l * N] + carry;
+    r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
+  }
+  if (ckks) {
+    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
+    for (uint32_t l = 0; l < L; ++l) out[base + (size_t)l * N] = l < Lb - 1 ? r[l] : (l == Lb - 1 ? r[l] & tm : 0u);
+    return;
+  }
+  bool ge = carry != 0;
+  if (!ge) {
+    ge = true;
+    for (uint32_t l = L; l-- > 0;) { const uint32_t q = __ldg(Q + l); if (r[l] != q) { ge = r[l] > q; break; } }
+  }
+  uint32_t borrow = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    uint32_t v = r[l];
+    if (ge) { const uint32_t q = __ldg(Q + l); const uint32_t d = v - q, d2 = d - borrow; borrow = (v < q) | (d < borrow); v = d2; }
+    out[base + (size_t)l * N] = v;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+mult_scalar_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, const uint32_t* __restrict__ Q, uint32_t N,
+                   uint32_t L, uint32_t bits, uint32_t kabs, uint32_t kneg, uint32_t ckks) {
+  const uint32_t bpp = N / 256;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
+  const size_t base = (size_t)poly * L * N + n;
+  uint32_t r[ELEM_MAX_LIMBS + 1];
+  uint32_t carry = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    const uint64_t s = (uint64_t)in[base + (size_t)l * N] * kabs + carry;
+    r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
+  }
+  r[L] = carry;
+  if (ckks) {
+    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
+    uint32_t c1 = kneg;                                             // -v = ~v + 1
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = 0;
+      if (l < Lb) {
+        v = r[l];
+        if (kneg) { const uint64_t s = (uint64_t)(~v) + c1; v = (uint32_t)s; c1 = (uint32_t)(s >> 32); }
+        if (l == Lb - 1) v &= tm;
+      }
+      out[base + (size_t)l * N] = v;
+    }
+    return;
+  }
+  const uint32_t w = bits >> 5, sh = bits & 31;                     // h = bits [logQ, logQ + 32) of the product
+  uint32_t h = r[w] >> sh;
+  if (sh && w + 1 <= L) h |= r[w + 1] << (32 - sh);
+  // r -= h Q over L + 1 limbs (Q has L limbs); the result is in (-Q, Q): its sign is the final borrow
+  uint64_t mc = 0;
+  uint32_t borrow = 0;
+  for (uint32_t l = 0; l <= L; ++l) {
+    const uint64_t pq = (l < L ? (uint64_t)__ldg(Q + l) * h : 0ull) + mc;
+    const uint32_t sub = (uint32_t)pq; mc = pq >> 32;
+    const uint32_t v = r[l], d = v - sub, d2 = d - borrow;
+    borrow = (v < sub) | (d < borrow);
+    r[l] = d2;
+  }
+  if (borrow) {                                                     // negative: add Q back once
+    uint32_t c2 = 0;
+    for (uint32_t l = 0; l < L; ++l) { const uint64_t s = (uint64_t)r[l] + __ldg(Q + l) + c2; r[l] = (uint32_t)s; c2 = (uint32_t)(s >> 32); }
+  }
+  uint32_t any = 0;
+  for (uint32_t l = 0; l < L; ++l) any |= r[l];
+  const bool flip = kneg && any;
+  uint32_t b2 = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    uint32_t v = r[l];
+    if (flip) { const uint32_t q = __ldg(Q + l); const uint32_t d = q - v, d2 = d - b2; b2 = (q < v) | (d < b2); v = d2; }
+    out[base + (size_t)l * N] = v;
+  }
+}
+
+cudaError_t launch_add_plain(Context* c, uint32_t* d_out, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
+                             uint32_t group, cudaStream_t s) {
+  if (!batch) return cudaSuccess;
+  if (c->L > ELEM_MAX_LIMBS) return cudaErrorInvalidValue;
+  LaunchTimer lt(c, KC_RESCALE, s);
+  add_plain_kernel<<<(c->N / 256) * 2 * batch, 256, 0, s>>>(d_out, d_ct, d_pt, c->d_Qlimbs, c->N, c->L, c->logQ, group, c->t == 0 ? 1u : 0u);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_mult_scalar(Context* c, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, cudaStream_t s) {
+  if (!npoly) return cudaSuccess;
+  if (c->L > ELEM_MAX_LIMBS) return cudaErrorInvalidValue;
+  const uint32_t kabs = k < 0 ? (uint32_t)(-(int64_t)k) : (uint32_t)k;
+  LaunchTimer lt(c, KC_RESCALE, s);
+  mult_scalar_kernel<<<(c->N / 256) * npoly, 256, 0, s>>>(d_out, d_in, c->d_Qlimbs, c->N, c->L, c->logQ, kabs, k < 0 ? 1u : 0u, c->t == 0 ? 1u : 0u);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_monomial(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, cudaStream_t s) {
   if (!npoly) return cudaSuccess;
   LaunchTimer lt(c, KC_RESCALE, s);

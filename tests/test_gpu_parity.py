@@ -569,3 +569,51 @@ def test_next1_mul_monomial_matches_the_oracle(N, logQ, t):
     d = polys_to_tensor([list(ct)], ctx.L)
     for k in (0, 1, N // 2, N - 1, N, 3 * N // 2, 2 * N - 1):
         assert tensor_to_polys(ctx.fhe_mul_monomial(d, k))[0] == [list(p) for p in scheme.mul_monomial(prm, ct, k)], k
+
+
+# ---- NEXT-3, constants: ct + plaintext (pairwise / broadcast) and ct x integer scalar -----------------------------------------
+@pytest.mark.parametrize("N,logQ,t,B,group", [(256, 128, 0, 3, 1), (1024, 218, 0, 5, 5), (256, 100, 257, 4, 2), (1024, 437, 65537, 3, 3)])
+def test_next3_add_plain_pairwise_and_broadcast(N, logQ, t, B, group):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logQ, t)
+    ctx = fhe.Context(N, logQ, logQ, t)
+    Q = prm.Q
+    rnd = np.random.default_rng(N + logQ + B)
+    def rand_poly():
+        p = [int.from_bytes(rnd.bytes((Q.bit_length() + 7) // 8 + 8), "little") % Q for _ in range(N)]
+        p[0], p[1], p[2] = 0, Q - 1, Q - 1
+        return p
+    npt = (B + group - 1) // group
+    cts = [(rand_poly(), rand_poly()) for _ in range(B)]
+    pts = [rand_poly() for _ in range(npt)]
+    for m in pts:
+        m[2] = 1                                               # (Q - 1) + 1 wraps to 0, (Q - 1) + (Q - 1) to Q - 2
+    d_ct = polys_to_tensor([list(c) for c in cts], ctx.L)
+    d_pt = polys_to_tensor(pts, ctx.L)
+    got = tensor_to_polys(ctx.fhe_add_plain(d_ct, d_pt, group))
+    for i in range(B):
+        want = scheme.add_plain(prm, cts[i], pts[i // group])
+        assert got[i] == [list(p) for p in want], i
+    # in place
+    ctx.fhe_add_plain(d_ct, d_pt, group, out=d_ct)
+    assert tensor_to_polys(d_ct) == got
+
+
+@pytest.mark.parametrize("N,logQ,t", [(256, 128, 0), (1024, 218, 0), (256, 100, 257), (1024, 437, 65537), (256, 96, 257)])
+def test_next3_mult_scalar_matches_the_oracle(N, logQ, t):
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logQ, t)
+    ctx = fhe.Context(N, logQ, logQ, t)
+    Q = prm.Q
+    rnd = np.random.default_rng(N + logQ + 5)
+    ct = tuple([int.from_bytes(rnd.bytes((Q.bit_length() + 7) // 8 + 8), "little") % Q for _ in range(N)] for _ in range(2))
+    ct[0][0], ct[0][1], ct[0][2], ct[1][0], ct[1][1] = 0, Q - 1, 1, Q - 1, (1 << logQ) - 1
+    d = polys_to_tensor([list(ct)], ctx.L)
+    for k in (0, 1, -1, 2, 3, -7, 65537, 2 ** 31 - 1, -(2 ** 31 - 1)):
+        assert tensor_to_polys(ctx.fhe_mult_scalar(d, k))[0] == [list(p) for p in scheme.mult_scalar(prm, ct, k)], k
+    keep = d.clone()
+    ctx.fhe_mult_scalar(d, -12345, out=d)                      # in place
+    assert tensor_to_polys(d)[0] == [list(p) for p in scheme.mult_scalar(prm, ct, -12345)]
+    assert torch.equal(ctx.fhe_add(ctx.fhe_mult_scalar(keep, 2), keep), ctx.fhe_mult_scalar(keep, 3))
+    with pytest.raises((fhe.FheError, ValueError)):
+        ctx.fhe_mult_scalar(keep, -2 ** 31)
