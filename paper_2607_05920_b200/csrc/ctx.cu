@@ -216,7 +216,7 @@ static cudaError_t build_target_top(Context* c, CrtTarget& tg, uint32_t K, uint3
   if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_Wfull, wfull)) != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_negMfull, negfull)) != cudaSuccess) return e;
-  std::vector<uint32_t> flags(1 + 3 * (size_t)TOP_MAX_FLAGS, 0u);
+  std::vector<uint32_t> flags((size_t)TOP_FLAGS_DONE + 1, 0u);
   if ((e = upload(c, &c->d_flags, flags)) != cudaSuccess) return e;
   return upload(c, &tg.d_scale, scale);
 }

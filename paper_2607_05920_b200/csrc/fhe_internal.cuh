@@ -37,7 +37,7 @@ struct CrtTarget {
   uint32_t* d_Wfull = nullptr;     // [K][Lfull]: (M/q_i) mod 2^(logP+logQ)
   uint32_t* d_negMfull = nullptr;  // [Lfull]
 };
-constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58, TOP_MAX_FLAGS = 65536;
+constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58, TOP_MAX_FLAGS = 65536, TOP_FLAGS_DONE = 1 + 3 * TOP_MAX_FLAGS;
 
 enum PostMode : int {
   POST_CKKS_MASK = 0,    // out = X mod 2^logQ
@@ -85,7 +85,7 @@ struct Context {
   bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
-  uint32_t* d_flags = nullptr;    // [1 + 3 TOP_MAX_FLAGS]: count, then (outer, inner, n) of the coefficients to recompute
+  uint32_t* d_flags = nullptr;    // [2 + 3 TOP_MAX_FLAGS]: count, (outer, inner, n) of the coefficients to recompute, blocks done
   uint32_t amb_bits = TOP_AMB;    // fhe_debug_crt_ambiguity lowers it so that tests reach the exact path
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
@@ -124,6 +124,28 @@ struct LaunchTimer {
   }
   ~LaunchTimer() { if (b) cudaEventRecord(b, s); }
 };
+
+// Programmatic dependent launch: the kernels of a step run back to back on one stream, each reading what the previous one
+// wrote.  A kernel launched with launch_pdl may have its blocks scheduled while the last wave of the previous kernel is
+// still running; pdl_sync() at its very top waits until that kernel has completed and its writes are visible
+// (griddepcontrol.wait), then lets the next kernel's blocks be scheduled behind its own (griddepcontrol.launch_dependents).
+// Nothing touches global memory before pdl_sync(); after an ordinary launch both instructions are no-ops.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_sync() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
 
 // ---- launchers (kernels_*.cu) --------------------------------------------------------------------------------------
 // Polynomials of a launch are indexed (o, i), o < nouter, i < ninner, and live at base + o * outer + i * inner (words).

@@ -445,7 +445,7 @@ __device__ void CrtEpi::post() {
 // ------------------------------------------------------------------------------------------------------------------
 constexpr uint32_t EXACT_MAX_LIMBS = 168;
 struct ExactArgs {
-  const uint32_t* flags;
+  uint32_t* flags;
   const uint32_t* res; size_t res_outer, res_inner;
   const uint32_t* add; size_t add_outer, add_inner;
   uint32_t* out; size_t out_outer, out_inner;
@@ -471,6 +471,7 @@ __device__ inline void big_shr_mask(uint32_t* x, uint32_t nin, uint32_t sh, uint
 
 __global__ void __launch_bounds__(64)
 crt_exact_kernel(ExactArgs a) {
+  pdl_sync();
   const uint32_t cnt = min(a.flags[0], TOP_MAX_FLAGS);
   uint32_t V[EXACT_MAX_LIMBS + 2];
   for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
@@ -519,6 +520,13 @@ crt_exact_kernel(ExactArgs a) {
     }
     uint32_t* dst = a.out + (size_t)o * a.out_outer + (size_t)i * a.out_inner + n;
     for (uint32_t l = 0; l < a.L; ++l) dst[(size_t)l * a.N] = V[l];
+  }
+  // the last block to finish clears the list for the next launch (every block has read the count by then), so that no
+  // memset sits between the kernels of a step
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(a.flags + TOP_FLAGS_DONE, 1u) == gridDim.x - 1) { a.flags[0] = 0; a.flags[TOP_FLAGS_DONE] = 0; }
   }
 }
 
@@ -571,11 +579,7 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   const uint32_t nb = pp.logQ - pb;
   ep.Lr = (nb + 31) / 32; ep.tm2 = top_mask(nb);
   ep.lend = ep.ws + pp.L + (pb ? ep.ws2 + 1 : 0);                 // last limb index the relin stream must see
-  if (tg.top) {
-    cudaError_t e = cudaMemsetAsync(c->d_flags, 0, sizeof(uint32_t), s);
-    if (e != cudaSuccess) return e;
-  }
-  cudaError_t e;
+  cudaError_t e;                                                  // the list count is zero here: crt_exact_kernel clears it
   {
     LaunchTimer lt(c, KC_CRT, s);
     e = pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
@@ -588,8 +592,8 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   x.out = d_out; x.out_outer = out_outer; x.out_inner = out_inner;
   x.W = tg.d_Wfull; x.negM = tg.d_negMfull; x.q = c->d_q;
   x.N = c->N; x.K = tg.K; x.Lfull = tg.Lfull; x.L = pp.L; x.logP = pp.logP; x.logQ = pp.logQ; x.rescale_bits = pp.rescale_bits;
-  crt_exact_kernel<<<32, 64, 0, s>>>(x);
-  return cudaGetLastError();
+  e = launch_pdl(crt_exact_kernel, 32, 64, 0, s, x);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------------------------

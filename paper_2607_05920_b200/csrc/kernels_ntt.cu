@@ -172,6 +172,7 @@ struct NttArgs {
 template <int LN, bool INV>
 __global__ void __launch_bounds__(256, 6)
 ntt_col_kernel(NttArgs a) {
+  pdl_sync();
   constexpr int LE = LN < 4 ? LN : 4, E = 1 << LE;   // points per thread
   constexpr int TPC = (1 << LN) / E;                 // threads per column
   constexpr int T = 256 / TPC;                       // columns per block
@@ -235,6 +236,7 @@ ntt_col_kernel(NttArgs a) {
 template <int LN, bool INV>
 __global__ void __launch_bounds__(256, 4)
 ntt_col2_kernel(NttArgs a) {
+  pdl_sync();
   static_assert(LN > 4 && LN <= 8, "paired column pass: 32..256-point columns");
   constexpr int TPC = (1 << LN) / 16;                // threads per column pair
   constexpr int T2 = 256 / TPC;                      // column pairs per block
@@ -326,6 +328,7 @@ __device__ __forceinline__ void load16(uint32_t (&x)[16], const uint32_t* __rest
 
 __global__ void __launch_bounds__(256)
 ntt_row_fwd_kernel(NttArgs a) {
+  pdl_sync();
   __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
   const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
   const uint32_t unit = blockIdx.x * 16 + rl;           // row of a transform: ((item * U + slot) * K + j) * N1 + r
@@ -348,6 +351,7 @@ ntt_row_fwd_kernel(NttArgs a) {
 template <bool FINAL>
 __global__ void __launch_bounds__(256)
 ntt_row_inv_kernel(NttArgs a) {
+  pdl_sync();
   __shared__ __align__(16) uint32_t sm[16 * ROW_SM];
   const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
   const uint32_t unit = blockIdx.x * 16 + rl;           // row of a transform, as in the forward row pass
@@ -388,6 +392,7 @@ constexpr int FUSED_ROWS = 2;   // units (half-warps) per block: one warp; measu
 template <int PW, bool FINAL>
 __global__ void __launch_bounds__(16 * FUSED_ROWS, 512 / (16 * FUSED_ROWS))
 ntt_row_fused_kernel(NttArgs a) {
+  pdl_sync();
   __shared__ __align__(16) uint32_t sm[FUSED_ROWS * ROW_SM];
   const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
   // unit = (j * N1 + r) * nitems + item: the half-warps of a block that share (j, r) share every twiddle of both
@@ -552,16 +557,17 @@ template <bool INV>
 static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaStream_t s) {
   const uint32_t ln1 = c->logN - 8;
   LaunchTimer lt(c, INV ? KC_NTT_INV : KC_NTT_FWD, s);
+  cudaError_t e = cudaSuccess;
 #define COL_CASE(LN)                                                                           \
   case LN: {                                                                                   \
     constexpr int TPC = (1 << LN) / ((LN) < 4 ? (1 << (LN)) : 16);                             \
-    ntt_col_kernel<LN, INV><<<ntr * TPC, 256, 0, s>>>(a);                                      \
+    e = launch_pdl(ntt_col_kernel<LN, INV>, ntr * TPC, 256, 0, s, a);                          \
     break;                                                                                     \
   }
 #define COL2_CASE(LN)                                                                          \
   case LN: {                                                                                   \
     constexpr int TPC = (1 << LN) / 16;                                                        \
-    ntt_col2_kernel<LN, INV><<<ntr * (256 / (2 * (256 / TPC))), 256, 0, s>>>(a);               \
+    e = launch_pdl(ntt_col2_kernel<LN, INV>, ntr * (256 / (2 * (256 / TPC))), 256, 0, s, a);   \
     break;                                                                                     \
   }
   switch (ln1) {   // blocks per transform = 256 / T = TPC (single columns) or TPC / 2 (column pairs)
@@ -570,7 +576,7 @@ static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaSt
   }
 #undef COL_CASE
 #undef COL2_CASE
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s) {
@@ -585,8 +591,8 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
     if (e != cudaSuccess) return e;
   }
   LaunchTimer lt(c, KC_NTT_FWD, s);
-  ntt_row_fwd_kernel<<<(a.units + 15) / 16, 256, 0, s>>>(a);
-  return cudaGetLastError();
+  const cudaError_t e = launch_pdl(ntt_row_fwd_kernel, (a.units + 15) / 16, 256, 0, s, a);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K,
@@ -600,9 +606,10 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
   const uint32_t blocks = (a.units + 15) / 16;
   {
     LaunchTimer lt(c, KC_NTT_INV, s);
-    if (fin) ntt_row_inv_kernel<true><<<blocks, 256, 0, s>>>(a);
-    else ntt_row_inv_kernel<false><<<blocks, 256, 0, s>>>(a);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e;
+    if (fin) e = launch_pdl(ntt_row_inv_kernel<true>, blocks, 256, 0, s, a);
+    else e = launch_pdl(ntt_row_inv_kernel<false>, blocks, 256, 0, s, a);
+    if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) return e;
   }
   if (!fin) return launch_col<true>(c, a, nitems * U * K, s);
@@ -641,12 +648,13 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
     LaunchTimer lt(c, KC_POINTWISE, s);
 #define FUSED_CASE(PW)                                                                 \
   case PW:                                                                             \
-    if (fin) ntt_row_fused_kernel<PW, true><<<blocks, 16 * FUSED_ROWS, 0, s>>>(a);     \
-    else ntt_row_fused_kernel<PW, false><<<blocks, 16 * FUSED_ROWS, 0, s>>>(a);        \
+    if (fin) e = launch_pdl(ntt_row_fused_kernel<PW, true>, blocks, 16 * FUSED_ROWS, 0, s, a);     \
+    else e = launch_pdl(ntt_row_fused_kernel<PW, false>, blocks, 16 * FUSED_ROWS, 0, s, a);        \
     break;
-    switch (pw_mode) { FUSED_CASE(PW_POLYMUL) FUSED_CASE(PW_TENSOR) FUSED_CASE(PW_RELIN) }
+    switch (pw_mode) { FUSED_CASE(PW_POLYMUL) FUSED_CASE(PW_TENSOR) FUSED_CASE(PW_RELIN) default: e = cudaErrorInvalidValue; }
 #undef FUSED_CASE
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
   }
   if (!fin) return launch_col<true>(c, a, nitems * Uout * K, s);
   return cudaSuccess;

@@ -245,6 +245,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  pdl_sync();   // barriers and TMEM are set up while the previous kernel drains; global memory is touched only after this
   const uint32_t tmem_a = ctl->tmem_base;                          // A buffers: columns [0, nA * a_cols)
   const uint32_t tmem_d = tmem_a + a.nA * a_cols;                  // chunk c of the pass: columns [c * NC, c * NC + NC)
 
@@ -421,8 +422,8 @@ inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params&
   PipeArgs a = a_in;
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);
   const uint32_t grid = ntiles < (uint32_t)n_sm ? ntiles : (uint32_t)n_sm;
-  pipe_kernel<Epi><<<grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s>>>(a, ep);
-  return cudaGetLastError();
+  const cudaError_t e = launch_pdl(pipe_kernel<Epi>, grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s, a, ep);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 #endif  // __CUDACC__
 
