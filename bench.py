@@ -413,8 +413,11 @@ def run_sweep(args):
     x1 = torch.from_numpy(synth.uniform_limbs(g, (1, 2), 1 << 16, 1240).view(np.int32)).to(dev).expand(64, 2, ctx.L, 1 << 16).contiguous()
     x2 = x1.clone()
     y = torch.empty_like(x1)
+    pt = x2[:, 0].contiguous()                                   # one plaintext polynomial per ciphertext
     for name, fn, nbuf in (("fhe_add", lambda: ctx.fhe_add(x1, x2, out=y), 3), ("fhe_sub", lambda: ctx.fhe_sub(x1, x2, out=y), 3),
-                           ("fhe_negate", lambda: ctx.fhe_negate(x1, out=y), 2), ("fhe_moddown", lambda: ctx.fhe_moddown(x1, 1200, out=y), 2)):
+                           ("fhe_negate", lambda: ctx.fhe_negate(x1, out=y), 2), ("fhe_moddown", lambda: ctx.fhe_moddown(x1, 1200, out=y), 2),
+                           ("fhe_mult_scalar", lambda: ctx.fhe_mult_scalar(x1, -12345, out=y), 2),
+                           ("fhe_add_plain", lambda: ctx.fhe_add_plain(x1, pt, 1, out=y), 2.5)):
         for _ in range(2):
             fn()
         torch.cuda.synchronize()

@@ -25,7 +25,7 @@ elem_ckks_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, con
   const size_t base = (size_t)poly * L * N + n;
   const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);     // limbs that hold bits; the rest of the L limbs are zero
   uint32_t carry = OP == EL_NEG ? 1u : 0u;                          // -a = ~a + 1
-  for (uint32_t l = 0; l < L; ++l) {
+  auto limb = [&](uint32_t l) {
     uint32_t v = 0;
     if (l < Lb) {
       const uint32_t x = a[base + (size_t)l * N];
@@ -44,6 +44,12 @@ elem_ckks_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ a, con
       if (l == Lb - 1) v &= tm;
     }
     out[base + (size_t)l * N] = v;
+  };
+  if constexpr (OP == EL_MODDOWN) {                                 // measured: a deeper unroll helps the copy, hurts add / sub
+#pragma unroll 8
+    for (uint32_t l = 0; l < L; ++l) limb(l);
+  } else {
+    for (uint32_t l = 0; l < L; ++l) limb(l);
   }
 }
 
@@ -203,16 +209,25 @@ add_plain_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ ct, co
     return;
   }
   const uint32_t* m = pt + (size_t)((poly >> 1) / group) * L * N + n;
-  uint32_t r[ELEM_MAX_LIMBS];
   uint32_t carry = 0;
+  if (ckks) {                                                       // streams: the sum wraps mod 2^(32 L), the top limb is masked
+    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
+#pragma unroll 8
+    for (uint32_t l = 0; l < L; ++l) {
+      uint32_t v = 0;
+      if (l < Lb) {
+        const uint64_t s = (uint64_t)ct[base + (size_t)l * N] + m[(size_t)l * N] + carry;
+        v = (uint32_t)s; carry = (uint32_t)(s >> 32);
+        if (l == Lb - 1) v &= tm;
+      }
+      out[base + (size_t)l * N] = v;
+    }
+    return;
+  }
+  uint32_t r[ELEM_MAX_LIMBS];
   for (uint32_t l = 0; l < L; ++l) {
     const uint64_t s = (uint64_t)ct[base + (size_t)l * N] + m[(size_t)l * N] + carry;
     r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
-  }
-  if (ckks) {
-    const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
-    for (uint32_t l = 0; l < L; ++l) out[base + (size_t)l * N] = l < Lb - 1 ? r[l] : (l == Lb - 1 ? r[l] & tm : 0u);
-    return;
   }
   bool ge = carry != 0;
   if (!ge) {
@@ -233,20 +248,16 @@ mult_scalar_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, 
   const uint32_t bpp = N / 256;
   const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 256 + threadIdx.x;
   const size_t base = (size_t)poly * L * N + n;
-  uint32_t r[ELEM_MAX_LIMBS + 1];
   uint32_t carry = 0;
-  for (uint32_t l = 0; l < L; ++l) {
-    const uint64_t s = (uint64_t)in[base + (size_t)l * N] * kabs + carry;
-    r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
-  }
-  r[L] = carry;
-  if (ckks) {
+  if (ckks) {                                                       // streams: product limb, two's complement, mask
     const uint32_t Lb = (bits + 31) / 32, tm = top_mask32(bits);
     uint32_t c1 = kneg;                                             // -v = ~v + 1
+#pragma unroll 8
     for (uint32_t l = 0; l < L; ++l) {
       uint32_t v = 0;
       if (l < Lb) {
-        v = r[l];
+        const uint64_t pr = (uint64_t)in[base + (size_t)l * N] * kabs + carry;
+        v = (uint32_t)pr; carry = (uint32_t)(pr >> 32);
         if (kneg) { const uint64_t s = (uint64_t)(~v) + c1; v = (uint32_t)s; c1 = (uint32_t)(s >> 32); }
         if (l == Lb - 1) v &= tm;
       }
@@ -254,6 +265,12 @@ mult_scalar_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, 
     }
     return;
   }
+  uint32_t r[ELEM_MAX_LIMBS + 1];
+  for (uint32_t l = 0; l < L; ++l) {
+    const uint64_t s = (uint64_t)in[base + (size_t)l * N] * kabs + carry;
+    r[l] = (uint32_t)s; carry = (uint32_t)(s >> 32);
+  }
+  r[L] = carry;
   const uint32_t w = bits >> 5, sh = bits & 31;                     // h = bits [logQ, logQ + 32) of the product
   uint32_t h = r[w] >> sh;
   if (sh && w + 1 <= L) h |= r[w + 1] << (32 - sh);
