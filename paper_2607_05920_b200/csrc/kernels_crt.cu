@@ -593,7 +593,9 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   x.W = tg.d_Wfull; x.negM = tg.d_negMfull; x.q = c->d_q;
   x.N = c->N; x.K = tg.K; x.Lfull = tg.Lfull; x.L = pp.L; x.logP = pp.logP; x.logQ = pp.logQ; x.rescale_bits = pp.rescale_bits;
   e = launch_pdl(crt_exact_kernel, 32, 64, 0, s, x);
-  return e != cudaSuccess ? e : cudaGetLastError();
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) cudaMemsetAsync(c->d_flags, 0, sizeof(uint32_t), s);   // nothing cleared the list: do not leave it to the next call
+  return e;
 }
 
 // ------------------------------------------------------------------------------------------------------------------
