@@ -160,6 +160,24 @@ def moddown(prm: Params, ct, new_logq: int):
     return tuple([x % m for x in a] for a in ct)
 
 
+# ---- NEXT-4: BGV modulus switching ----------------------------------------------------------------------
+# The paper names a "CKKS-BGV scheme" and lists one level-reducing operation (moddownBy_pairwise_into,
+# "modulus switching operation to reduce ciphertext level") without a BGV formula: PARITY UNPINNED by the
+# paper.  Reading (A20): the switch goes from Q to Q' = make_modulus(new_logQ, t), a modulus of the same
+# construction (odd, 1 mod t), and each coefficient c in [0, Q) becomes the integer nearest to c Q'/Q, corrected by the
+# same centred multiple of t as in the divide-by-P of the key switch (step 6 of SURVEY.md 8c): with x = c Q' in [0, Q Q'),
+#     r = x mod Q centred,  k = (-r Q^-1) mod t centred,  c' = ((x - r)/Q - k) mod Q'.
+# The removed quantity delta = r + Q k is 0 (mod Q-multiples aside) mod t and |delta| <= Q (1 + t)/2, so with
+# Q = Q' = 1 (mod t) the plaintext m + t e decrypts to the same m under Q' while the noise shrinks by Q'/Q.
+def modswitch_bgv(prm: Params, ct, new_logQ: int):
+    """BGV ciphertext mod Q -> the same plaintext mod Q' = make_modulus(new_logQ, t), every component."""
+    assert not prm.is_ckks and 1 <= new_logQ < prm.logQ
+    Q, t = prm.Q, prm.t
+    Q2 = make_modulus(new_logQ, t)
+    Qinv_t = pow(Q % t, -1, t)
+    return tuple([_div_p_bgv(int(c) * Q2, Q, Q2, t, Qinv_t) for c in comp] for comp in ct)
+
+
 # ---- NEXT-2 (SURVEY.md 8f): slot rotation / conjugation --------------------------------------------------------------------
 # The paper names the operations (conjugate_pairwise_into, leftrotate_broadcast_into with "precomputed Galois / rotation
 # keys", PAPER.md:656, 678-681) and gives no formula.  Reading: the Galois automorphism sigma_k: a(X) -> a(X^k) on both

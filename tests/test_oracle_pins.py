@@ -502,3 +502,87 @@ def test_next3_add_plain_and_mult_scalar_are_linear_under_decryption():
     assert harness.decrypt_bgv(scheme.mult_scalar(prb, c1, 11), sb, prb) == [(a * 11) % 257 for a in m1]
     assert harness.decrypt_bgv(scheme.mult_scalar(prb, c1, -3), sb, prb) == [(-3 * a) % 257 for a in m1]
     assert scheme.mult_scalar(prb, c1, 3) == scheme.ct_add(prb, scheme.ct_add(prb, c1, c1), c1)
+
+
+# ---- hand-worked pins of the rounding readings (tests/golden/relin_hand.txt) ---------------------------------------------
+# The paper prints no formula for the divide-by-P of the key switch or for the BGV level drop;
+# the readings are DESIGN.md 3 A3 / A10 / A20.  These values are worked out by hand in the golden file's comments, and a
+# plausible mistake in each reading (truncation instead of round-half-up; r or k left un-centred) fails one of them.
+def test_hand_ckks_divide_by_p_rounds_half_up():
+    gold = _read_golden("relin_hand.txt")
+    N, logQ, logP = gold["ckks_relin_params"]
+    prm = scheme.Params(N, logQ, logP)
+    zero, one = [0] * N, [1] + [0] * (N - 1)
+    out = scheme.relinearize_ckks(prm, (zero, zero, one), (gold["ckks_relin_evk_b"], zero))   # x_b = b' itself
+    assert out == (gold["ckks_relin_k_b"], zero)
+    # the same through relinearize(), with d0 / d1 carried along mod Q
+    d0, d1 = [15, 15, 1, 3], [2, 0, 9, 15]
+    want0 = [(a + b) % prm.Q for a, b in zip(d0, gold["ckks_relin_k_b"])]
+    assert scheme.relinearize(prm, (d0, d1, one), (gold["ckks_relin_evk_b"], zero)) == (want0, d1)
+
+
+def test_hand_bgv_divide_by_p_centres_r_and_k():
+    gold = _read_golden("relin_hand.txt")
+    t, P, Q = gold["bgv_div_params"]
+    assert scheme.make_modulus(4, t) == P == Q
+    Pinv_t = pow(P % t, -1, t)
+    got = [scheme._div_p_bgv(x, P, Q, t, Pinv_t) for x in gold["bgv_div_x"]]
+    assert got == gold["bgv_div_out"]
+    # through relinearize_bgv: N = 4, d2 = 1, so x_b = b', x_a = a' coefficient by coefficient
+    prm = scheme.Params(4, 4, 4, t)
+    xs, outs = gold["bgv_div_x"], gold["bgv_div_out"]
+    zero, one = [0] * 4, [1, 0, 0, 0]
+    assert scheme.relinearize_bgv(prm, (zero, zero, one), (xs[:4], xs[4:])) == (outs[:4], outs[4:])
+
+
+def test_hand_bgv_modswitch_and_its_invariants():
+    gold = _read_golden("relin_hand.txt")
+    t, logQ, new_logQ = gold["bgv_modswitch_params"]
+    prm = scheme.Params(4, logQ, logQ, t)
+    cs, outs = gold["bgv_modswitch_c"], gold["bgv_modswitch_out"]
+    for i in range(0, len(cs) - 3, 4):
+        assert scheme.modswitch_bgv(prm, (cs[i:i + 4], cs[i:i + 4]), new_logQ) == (outs[i:i + 4], outs[i:i + 4])
+    assert scheme.modswitch_bgv(prm, ([cs[-1]] * 4, [0] * 4), new_logQ) == ([outs[-1]] * 4, [0] * 4)
+    # invariants at a larger size, every c: some representative c' + j Q' (|j| <= 1) is within (1 + t)/2 of c Q'/Q and is
+    # = c (mod t) (Q = Q' = 1 mod t and the removed delta is a multiple of t)
+    t, logQ, new_logQ = 257, 20, 13
+    prm = scheme.Params(4, logQ, logQ, t)
+    Q, Q2 = prm.Q, scheme.make_modulus(new_logQ, t)
+    rnd = random.Random(4)
+    for c in [0, 1, Q - 1, Q // 2, Q // 2 + 1] + [rnd.randrange(Q) for _ in range(300)]:
+        cp = scheme.modswitch_bgv(prm, ([c] * 4, [c] * 4), new_logQ)[0][0]
+        assert 0 <= cp < Q2
+        assert any((cp + j * Q2 - c) % t == 0 and abs((cp + j * Q2) * Q - c * Q2) <= Q * (1 + t) // 2 for j in (-1, 0, 1))
+
+
+@pytest.mark.parametrize("N,logQ,new_logQ,t,hwt", [(64, 120, 80, 257, 16), (256, 200, 120, 65537, None)])
+def test_next4_modswitch_keeps_the_plaintext_and_shrinks_the_noise(N, logQ, new_logQ, t, hwt):
+    """R4 for the level drop: Dec_Q'(modswitch(ct)) = m exactly mod t, the noise drops by about Q/Q', and a product formed
+    and relinearised at the lower level still decrypts exactly (the evk there is generated for Q')."""
+    prm = scheme.Params(N, logQ, logQ, t)
+    g = synth.rng(N + t)
+    s, evk = harness.keygen(prm, g, hwt=hwt)
+    m1 = [int(v) for v in synth.uniform_mod(g, N, t)]
+    m2 = [int(v) for v in synth.uniform_mod(g, N, t)]
+    ct1, ct2 = harness.encrypt(prm, g, s, m1), harness.encrypt(prm, g, s, m2)
+    prod = scheme.relinearize(prm, scheme.he_mult(prm, ct1, ct2), evk)
+    assert harness.decrypt_bgv(prod, s, prm) == ring.pm(m1, m2, t)
+    noise_hi = max(abs(v) for v in harness.decrypt(prod, s, prm.Q))
+    low = scheme.modswitch_bgv(prm, prod, new_logQ)
+    prm2 = scheme.Params(N, new_logQ, new_logQ, t)
+    assert all(0 <= c < prm2.Q for comp in low for c in comp)
+    assert harness.decrypt_bgv(low, s, prm2) == ring.pm(m1, m2, t)
+    noise_lo = max(abs(v) for v in harness.decrypt(low, s, prm2.Q))
+    assert noise_lo < (noise_hi >> (logQ - new_logQ - 1)) + t * (N + 1)
+    # continue at the lower level: fresh key for Q', multiply by a switched fresh ciphertext
+    g2 = synth.rng(N + t + 1)
+    e2 = synth.gaussian_error(g2, N)
+    a2 = synth.uniform_big(g2, N, (prm2.PQ - 1).bit_length() - 1)
+    s2 = ring.pm([v % prm2.PQ for v in s], [v % prm2.PQ for v in s], prm2.PQ)
+    a_s = harness.pm_secret(a2, s, prm2.PQ)
+    evk2 = ([(-x + t * int(e) + prm2.P * y) % prm2.PQ for x, e, y in zip(a_s, e2, s2)], a2)
+    m3 = [int(v) for v in synth.uniform_mod(g2, N, t)]
+    ct3 = scheme.modswitch_bgv(prm, harness.encrypt(prm, g2, s, m3), new_logQ)
+    assert harness.decrypt_bgv(ct3, s, prm2) == m3
+    out = scheme.relinearize(prm2, scheme.he_mult(prm2, low, ct3), evk2)
+    assert harness.decrypt_bgv(out, s, prm2) == ring.pm(ring.pm(m1, m2, t), m3, t)
