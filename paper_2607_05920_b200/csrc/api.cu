@@ -15,13 +15,21 @@ fhe_status cuda_fail(Context* c, cudaError_t e, const char* where) {
   c->err = std::string(where) + ": " + cudaGetErrorString(e);
   return FHE_ERR_CUDA;
 }
+// Tables, keys, copy streams and the launch configuration all belong to the device the context was created on.
+fhe_status check_device(Context* c) {
+  int d = -1;
+  if (cudaGetDevice(&d) != cudaSuccess || d != c->device) return err(c, FHE_ERR_STATE, "the context's CUDA device is not the current device");
+  return FHE_OK;
+}
 #define CK(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, where); } while (0)
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 size_t ws_polymul(const Context* c, uint32_t b) { return align256((size_t)b * 2 * c->K_pm * c->N * 4); }
 size_t ws_tensor(const Context* c, uint32_t b) { return align256((size_t)b * 4 * c->K1 * c->N * 4); }
-size_t ws_relin(const Context* c, uint32_t b) { return align256((size_t)b * 2 * c->K2 * c->N * 4); }
+// residues [B][2][K2][N], then the flag bitmap of the exact CRT path, one bit per output coefficient (kernels_crt.cu)
+size_t ws_relin_res(const Context* c, uint32_t b) { return align256((size_t)b * 2 * c->K2 * c->N * 4); }
+size_t ws_relin(const Context* c, uint32_t b) { return ws_relin_res(c, b) + align256((size_t)b * 2 * (c->N / 32) * 4); }
 size_t ws_d3(const Context* c, uint32_t b) { return align256((size_t)b * 3 * c->L * c->N * 4); }
 size_t ws_evk(const Context* c) { return 0; }   // evk-hat is transformed in place inside the context
 
@@ -53,8 +61,9 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
   pp.amb_bits = c->amb_bits;
+  uint32_t* flags = (uint32_t*)((char*)ws + ws_relin_res(c, B));
   CK(launch_crt(c, c->tgt_relin, pp, d_out2, (size_t)2 * L * N, (size_t)L * N, ws, 2 * rp, rp, d_in3, (size_t)3 * L * N,
-                (size_t)L * N, B, 2, s), "crt relin");
+                (size_t)L * N, B, 2, s, flags), "crt relin");
   return FHE_OK;
 }
 
@@ -98,6 +107,7 @@ static fhe_status install_key(Context* c, uint32_t** slot, const uint32_t* d_key
 fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   (void)d_ws; (void)ws_bytes;
   if (!d_evk || misaligned(d_evk, 16)) return err(c, FHE_ERR_ARG, "d_evk NULL or misaligned");
   c->have_evk = false;
@@ -110,6 +120,7 @@ fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t w
 fhe_status fhe_set_rotation_key(fhe_ctx* ctx, uint32_t slot, uint32_t k, const uint32_t* d_key, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (slot >= (uint32_t)Context::MAX_ROT_KEYS) return err(c, FHE_ERR_ARG, "key slot out of range");
   if (!(k & 1) || k >= 2 * c->N) return err(c, FHE_ERR_ARG, "Galois element must be odd and below 2N");
   if (!d_key || misaligned(d_key, 16)) return err(c, FHE_ERR_ARG, "d_key NULL or misaligned");
@@ -124,6 +135,7 @@ fhe_status fhe_rotate(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, uin
                       size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_in2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out2, 16) || misaligned(d_in2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -157,6 +169,7 @@ fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const
                        void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out || !d_a || !d_b || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out, 16) || misaligned(d_a, 16) || misaligned(d_b, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -168,6 +181,7 @@ fhe_status fhe_mult_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, 
                           uint32_t group, void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_ct || !d_pt || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out2, 16) || misaligned(d_ct, 16) || misaligned(d_pt, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -181,6 +195,7 @@ fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, co
                        void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out3 || !d_ct1 || !d_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out3, 16) || misaligned(d_ct1, 16) || misaligned(d_ct2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -193,6 +208,7 @@ fhe_status fhe_relinearize(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in3
                            size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_in3 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out2, 16) || misaligned(d_in3, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -206,6 +222,7 @@ fhe_status fhe_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_in2, ui
                        void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (c->t != 0) return err(c, FHE_ERR_UNSUPPORTED, "rescale is CKKS-only");
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_in2) return err(c, FHE_ERR_ARG, "NULL pointer");
@@ -219,6 +236,7 @@ fhe_status fhe_mult_relin_rescale(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t
                                   uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_ct1 || !d_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out2, 16) || misaligned(d_ct1, 16) || misaligned(d_ct2, 16) || misaligned(d_ws, 256)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -239,6 +257,7 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
                                        uint32_t p_bits, uint32_t batch, void* d_ws, size_t ws_bytes, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!h_out2 || !h_ct1 || !h_ct2 || !d_ws) return err(c, FHE_ERR_ARG, "NULL pointer");
   const size_t ctb = align256((size_t)batch * 2 * c->L * c->N * 4);
@@ -253,28 +272,33 @@ fhe_status fhe_mult_relin_rescale_host(fhe_ctx* ctx, uint32_t* h_out2, const uin
   const uint32_t per = (batch + Context::HOST_PIECES - 1) / Context::HOST_PIECES;
   const uint32_t pieces = (batch + per - 1) / per;
   const size_t item_words = (size_t)2 * c->L * c->N;
-  CK(cudaEventRecord(c->ev_start, s), "event");
-  CK(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0), "wait");          // the staging buffers are free once `s` gets here
-  CK(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0), "wait");
+  // An error in the middle must not leave copies into / out of the caller's host buffers in flight behind the return:
+  // every exit drains the three streams first.
+  auto drain = [&]() { cudaStreamSynchronize(c->s_h2d); cudaStreamSynchronize(s); cudaStreamSynchronize(c->s_d2h); };
+#define CKH(call, where) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { drain(); return cuda_fail(c, e_, where); } } while (0)
+  CKH(cudaEventRecord(c->ev_start, s), "event");
+  CKH(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0), "wait");         // the staging buffers are free once `s` gets here
+  CKH(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0), "wait");
   for (uint32_t i = 0; i < pieces; ++i) {
     const uint32_t b0 = i * per, nb = batch - b0 < per ? batch - b0 : per;
     const size_t off = (size_t)b0 * item_words, bytes = (size_t)nb * item_words * 4;
-    CK(cudaMemcpyAsync(d1 + off, h_ct1 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct1");
-    CK(cudaMemcpyAsync(d2 + off, h_ct2 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct2");
-    CK(cudaEventRecord(c->ev_in[i], c->s_h2d), "event");
+    CKH(cudaMemcpyAsync(d1 + off, h_ct1 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct1");
+    CKH(cudaMemcpyAsync(d2 + off, h_ct2 + off, bytes, cudaMemcpyHostToDevice, c->s_h2d), "H2D ct2");
+    CKH(cudaEventRecord(c->ev_in[i], c->s_h2d), "event");
   }
   for (uint32_t i = 0; i < pieces; ++i) {
     const uint32_t b0 = i * per, nb = batch - b0 < per ? batch - b0 : per;
     const size_t off = (size_t)b0 * item_words, bytes = (size_t)nb * item_words * 4;
-    CK(cudaStreamWaitEvent(s, c->ev_in[i], 0), "wait");
+    CKH(cudaStreamWaitEvent(s, c->ev_in[i], 0), "wait");
     fhe_status st = fhe_mult_relin_rescale(ctx, d_o + off, d1 + off, d2 + off, p_bits, nb, d_ws, inner, stream);
-    if (st != FHE_OK) return st;
-    CK(cudaEventRecord(c->ev_done[i], s), "event");
-    CK(cudaStreamWaitEvent(c->s_d2h, c->ev_done[i], 0), "wait");
-    CK(cudaMemcpyAsync(h_out2 + off, d_o + off, bytes, cudaMemcpyDeviceToHost, c->s_d2h), "D2H out");
+    if (st != FHE_OK) { drain(); return st; }
+    CKH(cudaEventRecord(c->ev_done[i], s), "event");
+    CKH(cudaStreamWaitEvent(c->s_d2h, c->ev_done[i], 0), "wait");
+    CKH(cudaMemcpyAsync(h_out2 + off, d_o + off, bytes, cudaMemcpyDeviceToHost, c->s_d2h), "D2H out");
   }
-  CK(cudaStreamSynchronize(c->s_d2h), "sync");
-  CK(cudaStreamSynchronize(s), "sync");
+  CKH(cudaStreamSynchronize(c->s_d2h), "sync");
+  CKH(cudaStreamSynchronize(s), "sync");
+#undef CKH
   return FHE_OK;
 }
 
@@ -283,6 +307,7 @@ static fhe_status elem_call(fhe_ctx* ctx, int op, uint32_t* d_out, const uint32_
                             uint32_t bits, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (npoly == 0) return FHE_OK;
   if (!d_out || !d_a || (op <= 1 && !d_b)) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out, 16) || misaligned(d_a, 16) || (op <= 1 && misaligned(d_b, 16))) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -302,6 +327,7 @@ fhe_status fhe_negate(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, uint32
 fhe_status fhe_mul_monomial(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t k, uint32_t npoly, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (npoly == 0) return FHE_OK;
   if (!d_out || !d_in || d_out == d_in) return err(c, FHE_ERR_ARG, "NULL or aliasing pointer");
   if (misaligned(d_out, 16) || misaligned(d_in, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -315,6 +341,7 @@ fhe_status fhe_add_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, c
                          uint32_t group, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (batch == 0) return FHE_OK;
   if (!d_out2 || !d_ct || !d_pt) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out2, 16) || misaligned(d_ct, 16) || misaligned(d_pt, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -326,6 +353,7 @@ fhe_status fhe_add_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, c
 fhe_status fhe_mult_scalar(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (npoly == 0) return FHE_OK;
   if (!d_out || !d_in) return err(c, FHE_ERR_ARG, "NULL pointer");
   if (misaligned(d_out, 16) || misaligned(d_in, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
@@ -344,6 +372,7 @@ fhe_status fhe_mult_scalar(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, 
 fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logq, uint32_t npoly, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (c->t != 0) return err(c, FHE_ERR_UNSUPPORTED, "moddown is CKKS-only");
   if (new_logq < 1 || new_logq > c->logQ) return err(c, FHE_ERR_ARG, "new_logq out of range");
   return elem_call(ctx, 3, d_out, d_in, nullptr, npoly, new_logq, stream);
@@ -352,6 +381,7 @@ fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (bits < 1 || bits > TOP_AMB) return err(c, FHE_ERR_ARG, "bits out of range");
   c->amb_bits = bits;
   return FHE_OK;
@@ -360,6 +390,7 @@ fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
 fhe_status fhe_debug_int_peak(fhe_ctx* ctx, int mode, double* per_second, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (!per_second || mode < 0 || mode > 2) return err(c, FHE_ERR_ARG, "bad argument");
   CK(measure_int_peak(c, mode, per_second, (cudaStream_t)stream), "int peak");
   return FHE_OK;
@@ -369,6 +400,7 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
                                uint32_t K, uint32_t mask_bits, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (!d_res || !d_limbs || K == 0 || K > c->Kmax || Lin == 0 || Lin > MAX_LIMBS_IN) return err(c, FHE_ERR_ARG, "bad argument");
   CK(launch_decompose(c, d_res, 0, (size_t)K * c->N, d_limbs, 0, (size_t)Lin * c->N, 1, npoly, Lin, K, mask_bits, (cudaStream_t)stream), "decompose");
   return FHE_OK;
@@ -377,6 +409,7 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
 fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t K, int inverse, void* stream) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
   if (!d_res || K == 0 || K > c->Kmax) return err(c, FHE_ERR_ARG, "bad argument");
   if (inverse) CK(launch_ntt_inv(c, d_res, npoly, 1, 1, K, c->d_scale_plain, (cudaStream_t)stream), "ntt inv");
   else CK(launch_ntt_fwd(c, d_res, npoly, 1, 1, K, (cudaStream_t)stream), "ntt fwd");

@@ -216,8 +216,6 @@ static cudaError_t build_target_top(Context* c, CrtTarget& tg, uint32_t K, uint3
   if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_Wfull, wfull)) != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_negMfull, negfull)) != cudaSuccess) return e;
-  std::vector<uint32_t> flags((size_t)TOP_FLAGS_DONE + 1, 0u);
-  if ((e = upload(c, &c->d_flags, flags)) != cudaSuccess) return e;
   return upload(c, &tg.d_scale, scale);
 }
 
@@ -262,6 +260,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   while ((1u << c->logN) < N) ++c->logN;
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
+  c->device = dev;
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
   if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking);
   if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking);

@@ -31,13 +31,14 @@ struct CrtTarget {
   // mod 2^logQ only, i.e. the high logQ bits of W_i exactly and ONE carry out of the low logP bits.  That carry is taken
   // from the top TOP_BITS bits of the low parts (columns 8..31 of the image, then 4 L columns of the high parts); the
   // truncation can change it only when the TOP_AMB fractional bits below it are all ones, in which case the coefficient
-  // is flagged and recomputed exactly from the full constants by crt_exact_kernel.
+  // is flagged (one bit per coefficient in a bitmap kept in the caller's workspace, written in full by every launch) and
+  // recomputed exactly from the full constants by crt_exact_kernel.
   bool top = false;
   uint32_t Lfull = 0;              // limbs of the full constants: ceil((logP + logQ) / 32)
   uint32_t* d_Wfull = nullptr;     // [K][Lfull]: (M/q_i) mod 2^(logP+logQ)
   uint32_t* d_negMfull = nullptr;  // [Lfull]
 };
-constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58, TOP_MAX_FLAGS = 65536, TOP_FLAGS_DONE = 1 + 3 * TOP_MAX_FLAGS;
+constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58;
 
 enum PostMode : int {
   POST_CKKS_MASK = 0,    // out = X mod 2^logQ
@@ -69,6 +70,7 @@ struct Context {
   uint32_t bitsQ = 0, bitsP = 0, bitsPQ = 0, L = 0, L_P = 0, L_PQ = 0;
   uint32_t K_pm = 0, K1 = 0, K2 = 0, Kmax = 0;
   int n_sm = 0;
+  int device = 0;                 // the CUDA device the context was created on: every call must run with it current
   std::vector<uint32_t> h_q, h_psi;
   std::vector<uint32_t> h_Q, h_P, h_PQ;   // limbs
   // device tables (all primes 0..Kmax-1)
@@ -85,7 +87,6 @@ struct Context {
   bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
-  uint32_t* d_flags = nullptr;    // [2 + 3 TOP_MAX_FLAGS]: count, (outer, inner, n) of the coefficients to recompute, blocks done
   uint32_t amb_bits = TOP_AMB;    // fhe_debug_crt_ambiguity lowers it so that tests reach the exact path
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
@@ -172,10 +173,11 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
                                const uint2* d_scale, cudaStream_t s, uint32_t aux_group = 1);
 // CRT + post: residues [K][N] -> limbs [L][N] per polynomial (o, i); d_add: for the relin modes, the polynomial added
-// at the end, else nullptr
+// at the end, else nullptr.  d_flags: top-form targets only, nouter * ninner * N / 32 words of workspace for the bitmap of the
+// coefficients the exact path recomputes (written in full by the launch: no initialisation needed)
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
                        const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
-                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s);
+                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s, uint32_t* d_flags = nullptr);
 // register-only throughput of the NTT butterfly (mode 0), mad.lo.u32 (1), mul.hi.u32 (2) on this device, per second
 cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s);
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the pipeline have the TMEM / shared memory for it

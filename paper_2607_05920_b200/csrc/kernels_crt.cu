@@ -128,14 +128,14 @@ struct CrtEpi {
     const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
     const uint32_t* negM;                               // [Lraw]
     uint32_t Lraw, Lx, nl, ntab;                        // nl = limbs of V the chunks cover; ntab = entries of the negM table
-    uint32_t top, amb_bits; uint32_t* flags;             // top-form relin target (fhe_internal.cuh): flag list of the exact path
+    uint32_t top, amb_bits; uint32_t* flags;             // top-form relin target (fhe_internal.cuh): flag bitmap of the exact path
     uint32_t xs_off, adds_off, scratch_off;             // word offsets inside the scratch: negM table at 0, then the columns
     // CKKS relin streaming constants: shift by logP = 32 ws + bs, rounding bit rbit in limb rb; rescale likewise (.2)
     uint32_t ws, bs, rb, rbit, ws2, bs2, rb2, rbit2, Lr, tm2, tmq, lend;
     PostParams pp;
   };
   const Params& p;
-  const uint32_t N, etid;
+  const uint32_t N, etid, inner;
   const uint32_t* negm;  // [nl + 2] in shared memory, zero beyond Lraw
   uint32_t* xs;          // [Lx][TC]   (BGV)
   uint32_t* adds;        // [L][TC]    (relin modes)
@@ -145,10 +145,10 @@ struct CrtEpi {
   const uint32_t* aptr = nullptr;
   uint32_t alpha = 0, yprev = 0, cy = 0, zprev = 0, cz = 0;
   uint64_t carry = 0;
-  uint32_t cur_o = 0, cur_i = 0, cur_n = 0;
+  uint32_t flag_word = 0;   // word of the flag bitmap this warp's 32 coefficients own: bit = lane
 
   __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t, uint32_t bar)
-      : p(p_), N(a.N), etid(etid_), negm(reinterpret_cast<const uint32_t*>(sm)),
+      : p(p_), N(a.N), etid(etid_), inner(a.inner), negm(reinterpret_cast<const uint32_t*>(sm)),
         xs(reinterpret_cast<uint32_t*>(sm) + p_.xs_off), adds(reinterpret_cast<uint32_t*>(sm) + p_.adds_off),
         scratch(reinterpret_cast<uint32_t*>(sm) + p_.scratch_off) {
     uint32_t* w = reinterpret_cast<uint32_t*>(sm);
@@ -160,7 +160,7 @@ struct CrtEpi {
     out = p.out + (size_t)o * p.out_outer + (size_t)i * p.out_inner + n0 + etid;
     optr = out; aptr = adds + etid;
     carry = 0; yprev = 0; cy = 0; zprev = 0; cz = 0;
-    cur_o = o; cur_i = i; cur_n = n0 + etid;
+    flag_word = (o * inner + i) * (N >> 5) + ((n0 + etid) >> 5);
     if (p.add) {
       const uint32_t* src = p.add + (size_t)o * p.add_outer + (size_t)i * p.add_inner + n0 + etid;
       const uint32_t dst = umma::smem_u32(adds + etid);
@@ -207,7 +207,7 @@ struct CrtEpi {
   // Top-form relin target, first 32 columns of a tile: P[2..8) are the six limbs of S_t = sum_i y_i Wt_i + alpha Nt, the
   // low part of V cut down to its top TOP_BITS bits.  The carry into the high part is round(S_t / 2^96); the cut-off
   // bits can add less than 2^-58 to S_t / 2^96, so the rounding is certain unless the amb_bits fractional bits below the
-  // rounding position are all ones -- then the coefficient is put on the list crt_exact_kernel works off.
+  // rounding position are all ones -- then the coefficient's bit is set in the bitmap crt_exact_kernel works off.
   __device__ __forceinline__ void top_carry(const uint64_t* P) {
     uint32_t sl[TOP_LIMBS];
     uint64_t cr = 0;
@@ -222,12 +222,11 @@ struct CrtEpi {
     const uint64_t r4 = (uint64_t)sl[4] + (r3 >> 32);
     carry = (r3 & 0xFFFFFFFFu) | (r4 << 32);                      // bits 96.. of S_t + 2^95 (S_t < 2^134)
     const uint64_t frac = ((uint64_t)(uint32_t)r2 << 32) | sl[1];  // fractional bits 32..95
-    if ((frac >> (64 - p.amb_bits)) == (~0ull >> (64 - p.amb_bits))) {
-      const uint32_t idx = atomicAdd(p.flags, 1u);
-      if (idx < TOP_MAX_FLAGS) {
-        p.flags[1 + 3 * idx] = cur_o; p.flags[2 + 3 * idx] = cur_i; p.flags[3 + 3 * idx] = cur_n;
-      }
-    }
+    // One bit per coefficient, [polynomial][N / 32] words: the 32 lanes of a warp own consecutive coefficients, i.e. one
+    // word, which the warp writes whole (zero or not) -- no atomics, nothing to clear, no coefficient can be dropped.
+    const bool amb = (frac >> (64 - p.amb_bits)) == (~0ull >> (64 - p.amb_bits));
+    const uint32_t m = __ballot_sync(0xFFFFFFFFu, amb);
+    if ((etid & 31) == 0) p.flags[flag_word] = m;
   }
 
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
@@ -441,7 +440,9 @@ __device__ void CrtEpi::post() {
 // The exact path of the top-form relin target: one thread per flagged coefficient recomputes the whole output
 // coefficient from the full constants -- V = sum_i y_i W_i + alpha negM mod 2^(logP+logQ) limb by limb, divide by P with
 // rounding, add d, optional rescale (the formulas of DESIGN.md 3, A3/A4) -- and overwrites what the pipeline stored.
-// Expected work: 2^-58 of the coefficients; the launch costs a few microseconds when the list is empty.
+// The flagged coefficients are the set bits of a bitmap [polynomial][N / 32] that the pipeline writes in full on every
+// launch (kernels_crt.cu, top_carry), so no coefficient can be dropped and nothing needs clearing.  Expected work: 2^-58 of
+// the coefficients; the launch costs a few microseconds when no bit is set.
 // ------------------------------------------------------------------------------------------------------------------
 constexpr uint32_t EXACT_MAX_LIMBS = 168;
 struct ExactArgs {
@@ -450,7 +451,7 @@ struct ExactArgs {
   const uint32_t* add; size_t add_outer, add_inner;
   uint32_t* out; size_t out_outer, out_inner;
   const uint32_t* W; const uint32_t* negM; const uint32_t* q;
-  uint32_t N, K, Lfull, L, logP, logQ, rescale_bits;
+  uint32_t N, K, Lfull, L, logP, logQ, rescale_bits, inner, nwords;
 };
 
 // x[0..n) += 2^bit
@@ -472,61 +473,60 @@ __device__ inline void big_shr_mask(uint32_t* x, uint32_t nin, uint32_t sh, uint
 __global__ void __launch_bounds__(64)
 crt_exact_kernel(ExactArgs a) {
   pdl_sync();
-  const uint32_t cnt = min(a.flags[0], TOP_MAX_FLAGS);
   uint32_t V[EXACT_MAX_LIMBS + 2];
-  for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
-    const uint32_t o = a.flags[1 + 3 * e], i = a.flags[2 + 3 * e], n = a.flags[3 + 3 * e];
-    const uint32_t* y = a.res + (size_t)o * a.res_outer + (size_t)i * a.res_inner + n;
-    const uint32_t nl = a.Lfull + 2;
-    for (uint32_t l = 0; l < nl; ++l) V[l] = 0;
-    uint64_t asum = 0;
-    for (uint32_t j = 0; j < a.K; ++j) {
-      const uint32_t yj = y[(size_t)j * a.N];
-      asum += (uint64_t)yj * ((1ull << ALPHA_SHIFT) / a.q[j]);
-      uint64_t cr = 0;
-      const uint32_t* w = a.W + (size_t)j * a.Lfull;
-      for (uint32_t l = 0; l < a.Lfull; ++l) {
-        const uint64_t t = (uint64_t)yj * w[l] + V[l] + cr;
-        V[l] = (uint32_t)t; cr = t >> 32;
+  const uint32_t wpp = a.N >> 5;                                   // bitmap words per polynomial
+  for (uint32_t w = blockIdx.x * blockDim.x + threadIdx.x; w < a.nwords; w += gridDim.x * blockDim.x) {
+    uint32_t bits = a.flags[w];
+    const uint32_t poly = w / wpp, o = poly / a.inner, i = poly % a.inner;
+    while (bits) {
+      const uint32_t b = __ffs(bits) - 1;
+      bits &= bits - 1;
+      const uint32_t n = (w % wpp) * 32 + b;
+      const uint32_t* y = a.res + (size_t)o * a.res_outer + (size_t)i * a.res_inner + n;
+      const uint32_t nl = a.Lfull + 2;
+      for (uint32_t l = 0; l < nl; ++l) V[l] = 0;
+      uint64_t asum = 0;
+      for (uint32_t j = 0; j < a.K; ++j) {
+        const uint32_t yj = y[(size_t)j * a.N];
+        asum += (uint64_t)yj * ((1ull << ALPHA_SHIFT) / a.q[j]);
+        uint64_t cr = 0;
+        const uint32_t* wj = a.W + (size_t)j * a.Lfull;
+        for (uint32_t l = 0; l < a.Lfull; ++l) {
+          const uint64_t t = (uint64_t)yj * wj[l] + V[l] + cr;
+          V[l] = (uint32_t)t; cr = t >> 32;
+        }
+        for (uint32_t l = a.Lfull; l < nl && cr; ++l) { const uint64_t t = (uint64_t)V[l] + cr; V[l] = (uint32_t)t; cr = t >> 32; }
       }
-      for (uint32_t l = a.Lfull; l < nl && cr; ++l) { const uint64_t t = (uint64_t)V[l] + cr; V[l] = (uint32_t)t; cr = t >> 32; }
-    }
-    const uint32_t alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
-    {
-      uint64_t cr = 0;
-      for (uint32_t l = 0; l < a.Lfull; ++l) {
-        const uint64_t t = (uint64_t)alpha * a.negM[l] + V[l] + cr;
-        V[l] = (uint32_t)t; cr = t >> 32;
+      const uint32_t alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
+      {
+        uint64_t cr = 0;
+        for (uint32_t l = 0; l < a.Lfull; ++l) {
+          const uint64_t t = (uint64_t)alpha * a.negM[l] + V[l] + cr;
+          V[l] = (uint32_t)t; cr = t >> 32;
+        }
       }
+      // x = V mod 2^(logP+logQ); k = ((x + 2^(logP-1)) >> logP) mod 2^logQ
+      big_shr_mask(V, a.Lfull, 0, a.logP + a.logQ, a.Lfull);
+      V[a.Lfull] = V[a.Lfull + 1] = 0;
+      big_add_pow2(V, a.Lfull + 1, a.logP - 1);
+      big_shr_mask(V, a.Lfull + 1, a.logP, a.logQ, a.L);
+      // z = (d + k) mod 2^logQ
+      const uint32_t* d = a.add + (size_t)o * a.add_outer + (size_t)i * a.add_inner + n;
+      uint32_t cy = 0;
+      for (uint32_t l = 0; l < a.L; ++l) {
+        const uint64_t t = (uint64_t)V[l] + d[(size_t)l * a.N] + cy;
+        V[l] = (uint32_t)t; cy = (uint32_t)(t >> 32);
+      }
+      V[a.L] = 0;                                                  // the carry out of 2^(32 L) is dropped by the mask below
+      big_shr_mask(V, a.L, 0, a.logQ, a.L);
+      if (a.rescale_bits) {
+        V[a.L] = 0;
+        big_add_pow2(V, a.L + 1, a.rescale_bits - 1);
+        big_shr_mask(V, a.L + 1, a.rescale_bits, a.logQ - a.rescale_bits, a.L);
+      }
+      uint32_t* dst = a.out + (size_t)o * a.out_outer + (size_t)i * a.out_inner + n;
+      for (uint32_t l = 0; l < a.L; ++l) dst[(size_t)l * a.N] = V[l];
     }
-    // x = V mod 2^(logP+logQ); k = ((x + 2^(logP-1)) >> logP) mod 2^logQ
-    big_shr_mask(V, a.Lfull, 0, a.logP + a.logQ, a.Lfull);
-    V[a.Lfull] = V[a.Lfull + 1] = 0;
-    big_add_pow2(V, a.Lfull + 1, a.logP - 1);
-    big_shr_mask(V, a.Lfull + 1, a.logP, a.logQ, a.L);
-    // z = (d + k) mod 2^logQ
-    const uint32_t* d = a.add + (size_t)o * a.add_outer + (size_t)i * a.add_inner + n;
-    uint32_t cy = 0;
-    for (uint32_t l = 0; l < a.L; ++l) {
-      const uint64_t t = (uint64_t)V[l] + d[(size_t)l * a.N] + cy;
-      V[l] = (uint32_t)t; cy = (uint32_t)(t >> 32);
-    }
-    V[a.L] = 0;                                                    // the carry out of 2^(32 L) is dropped by the mask below
-    big_shr_mask(V, a.L, 0, a.logQ, a.L);
-    if (a.rescale_bits) {
-      V[a.L] = 0;
-      big_add_pow2(V, a.L + 1, a.rescale_bits - 1);
-      big_shr_mask(V, a.L + 1, a.rescale_bits, a.logQ - a.rescale_bits, a.L);
-    }
-    uint32_t* dst = a.out + (size_t)o * a.out_outer + (size_t)i * a.out_inner + n;
-    for (uint32_t l = 0; l < a.L; ++l) dst[(size_t)l * a.N] = V[l];
-  }
-  // the last block to finish clears the list for the next launch (every block has read the count by then), so that no
-  // memset sits between the kernels of a step
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    __threadfence();
-    if (atomicAdd(a.flags + TOP_FLAGS_DONE, 1u) == gridDim.x - 1) { a.flags[0] = 0; a.flags[TOP_FLAGS_DONE] = 0; }
   }
 }
 
@@ -551,8 +551,9 @@ bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
 
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
                        const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
-                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s) {
+                       size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s, uint32_t* d_flags) {
   if (nouter * ninner == 0) return cudaSuccess;
+  if (tg.top && !d_flags) return cudaErrorInvalidValue;
   CrtEpi::Params ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);
@@ -572,14 +573,14 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   const uint32_t shiftP = tg.top ? 0 : pp.logP;                  // the top form hands the epilogue V >> logP directly
   ep.ws = shiftP >> 5; ep.bs = shiftP & 31;
   ep.rb = shiftP ? (shiftP - 1) >> 5 : 0; ep.rbit = shiftP ? 1u << ((shiftP - 1) & 31) : 0;
-  ep.top = tg.top ? 1 : 0; ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = c->d_flags;
+  ep.top = tg.top ? 1 : 0; ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = d_flags;
   const uint32_t pb = pp.rescale_bits;
   ep.ws2 = pb >> 5; ep.bs2 = pb & 31;
   ep.rb2 = pb ? (pb - 1) >> 5 : 0; ep.rbit2 = pb ? 1u << ((pb - 1) & 31) : 0;
   const uint32_t nb = pp.logQ - pb;
   ep.Lr = (nb + 31) / 32; ep.tm2 = top_mask(nb);
   ep.lend = ep.ws + pp.L + (pb ? ep.ws2 + 1 : 0);                 // last limb index the relin stream must see
-  cudaError_t e;                                                  // the list count is zero here: crt_exact_kernel clears it
+  cudaError_t e;
   {
     LaunchTimer lt(c, KC_CRT, s);
     e = pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
@@ -587,15 +588,15 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   if (e != cudaSuccess || !tg.top) return e;
   LaunchTimer lt(c, KC_CRT, s);
   ExactArgs x;
-  x.flags = c->d_flags; x.res = d_res; x.res_outer = res_outer; x.res_inner = res_inner;
+  x.flags = d_flags; x.res = d_res; x.res_outer = res_outer; x.res_inner = res_inner;
   x.add = d_add; x.add_outer = add_outer; x.add_inner = add_inner;
   x.out = d_out; x.out_outer = out_outer; x.out_inner = out_inner;
   x.W = tg.d_Wfull; x.negM = tg.d_negMfull; x.q = c->d_q;
   x.N = c->N; x.K = tg.K; x.Lfull = tg.Lfull; x.L = pp.L; x.logP = pp.logP; x.logQ = pp.logQ; x.rescale_bits = pp.rescale_bits;
-  e = launch_pdl(crt_exact_kernel, 32, 64, 0, s, x);
-  if (e == cudaSuccess) e = cudaGetLastError();
-  if (e != cudaSuccess) cudaMemsetAsync(c->d_flags, 0, sizeof(uint32_t), s);   // nothing cleared the list: do not leave it to the next call
-  return e;
+  x.inner = ninner; x.nwords = nouter * ninner * (c->N >> 5);
+  const uint32_t blocks = std::min<uint32_t>((x.nwords + 63) / 64, 4u * (uint32_t)c->n_sm);
+  e = launch_pdl(crt_exact_kernel, blocks, 64, 0, s, x);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------------------------

@@ -413,11 +413,16 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
 
 template <class Epi>
 inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params& ep, size_t smem, int n_sm, cudaStream_t s) {
-  static size_t configured = 0;
-  if (smem > configured) {
+  // the attribute belongs to the (kernel, device) pair: one high-water mark per device
+  constexpr int MAX_DEV = 64;
+  static size_t configured[MAX_DEV] = {};
+  int dev = 0;
+  cudaError_t e0 = cudaGetDevice(&dev);
+  if (e0 != cudaSuccess) return e0;
+  if (dev < 0 || dev >= MAX_DEV || smem > configured[dev]) {
     cudaError_t e = cudaFuncSetAttribute(pipe_kernel<Epi>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = smem;
+    if (dev >= 0 && dev < MAX_DEV) configured[dev] = smem;
   }
   PipeArgs a = a_in;
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);

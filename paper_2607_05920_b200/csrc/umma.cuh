@@ -27,11 +27,20 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-// Blocks until the phase with the given parity has completed.  A wait that does not complete within ~2^26 polls can
-// only mean a programming error in this file: trap (launch failure) instead of hanging the device.
+// Blocks until the phase with the given parity has completed.  A wait that does not complete can only mean a programming
+// error in this file; it traps (launch failure) instead of hanging the device -- but by wall clock, not by poll count:
+// under compute-sanitizer, an ncu replay or time-slicing a correct kernel can poll millions of times.  The timer is read
+// once per 2^16 unsuccessful polls (each try_wait already suspends the thread for a hardware-defined interval).
+constexpr uint64_t MBAR_TIMEOUT_NS = 60ull * 1000 * 1000 * 1000;
+__device__ __forceinline__ uint64_t global_ns() {
+  uint64_t t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t done = 0;
   uint32_t polls = 0;
+  uint64_t t0 = 0;
   while (true) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -41,7 +50,11 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
     if (done) break;
-    if (++polls > (1u << 26)) __trap();
+    if ((++polls & 0xFFFFu) == 0) {
+      const uint64_t now = global_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > MBAR_TIMEOUT_NS) __trap();
+    }
   }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }

@@ -192,8 +192,8 @@ def _check_he_mult_samples(out3, ct1, ct2, Q, ks):
         assert coeff_from_limbs(out3[2], k) == ring.pm_coeff(c1, e1, k, Q), ("d2", k)
 
 
-def _relin_coeff_ckks(prm, d3, evk_polys, k):
-    d2 = from_limbs(d3[2])
+def _relin_coeff_ckks(prm, d3, evk_polys, k, d2=None):
+    d2 = from_limbs(d3[2]) if d2 is None else d2
     out = []
     for comp in range(2):
         x = ring.pm_coeff(d2, evk_polys[comp], k, prm.PQ)
@@ -213,65 +213,116 @@ def _relin_coeff_bgv(prm, d3, evk_polys, k):
     return out
 
 
+def _structured_ks(N, item, n_items, polys_per_item, n_sm, per_item=72):
+    """Coefficient positions chosen by the structure of the conversion pipeline, not by an RNG: the CRT launch walks the
+    128-coefficient tiles of polynomial p = item * polys_per_item + comp, tile = p * N/128 + k/128, CTA = tile mod grid,
+    and the CTA's tiles alternate between its two epilogue groups / accumulator sets.  Returned for one item: per_item
+    residues k mod 128 (items take them in turn, so that the items of a batch together cover every k mod 128; each in a
+    different tile), the first and last coefficient of the polynomial and of its first / last 256-point rows, and the
+    tiles that are the first and the last tile CTA 0 and CTA grid-1 see in this item."""
+    tpp = N // 128
+    grid = min(n_items * polys_per_item * tpp, n_sm)
+    ks = {0, 127, 128, 255, 256, N - 256, N - 129, N - 128, N - 1}
+    for r in range(item * per_item, (item + 1) * per_item):
+        ks.add(((r * 131 + item * 17) % tpp) * 128 + r % 128)
+    for comp in range(polys_per_item):
+        tiles = range((item * polys_per_item + comp) * tpp, (item * polys_per_item + comp + 1) * tpp)
+        for cta in (0, grid - 1):
+            mine = [t for t in tiles if t % grid == cta]
+            for t, r in ((mine[0], 0), (mine[-1], 127)):
+                ks.add((t % tpp) * 128 + r)
+    return sorted(ks)
+
+
+def _groups_hit(N, item, polys_per_item, n_items, n_sm, ks):
+    """Which (epilogue group, k mod 128 half) combinations the positions reach, over the polynomials of the item."""
+    tpp = N // 128
+    grid = min(n_items * polys_per_item * tpp, n_sm)
+    hit = set()
+    for comp in range(polys_per_item):
+        for k in ks:
+            tile = (item * polys_per_item + comp) * tpp + k // 128
+            hit.add(((tile // grid) & 1, tile % grid in (0, grid - 1)))
+    return hit
+
+
 @pytest.mark.parametrize("N,logQ,logP,B", [(1 << 15, 620, 620, 8), (1 << 16, 1240, 1240, 4)])
-def test_ckks_full_size_sampled(N, logQ, logP, B):
-    """configs[2] and configs[4]: uniform random ciphertexts and key of the configured shape (parity does not need
-    real encryptions); each call checked on sampled coefficients; the fused call must equal the three calls."""
+def test_ckks_full_size_every_limb_of_one_pair_and_structured_samples(N, logQ, logP, B):
+    """configs[2] and configs[4] (the benchmarked shape, in the launch configuration bench.py times: the whole batch in one
+    call).  Item 0 is a REAL encryption (HWT-64 secret, sigma = 3.2, Delta = 2^40) and is compared on every limb of every
+    coefficient against the oracle's own NTT route for he_mult (d0, d1, d2), relinearize and rescale, then decrypted:
+    the slot product within 2^-20.  The other items are uniform ciphertexts checked on positions chosen by the structure
+    of the kernels (every k mod 128 over the batch, both CRT epilogue groups, first / last tiles of the first / last CTA,
+    row boundaries; >= 512 in all), from the definition Eq. 5-6 one coefficient at a time.  The fused call must equal the
+    three calls."""
     fhe = _lib()
-    prm = scheme.Params(N, logQ, logP, 0)
+    prm, s, evk, cts1, cts2, zs = _ckks_setup(N, logQ, logP, 1, seed=N)
     ctx = fhe.Context(N, logQ, logP)
     g = synth.rng(N + logQ)
     ct1 = synth.uniform_limbs(g, (B, 2), N, logQ)
     ct2 = synth.uniform_limbs(g, (B, 2), N, logQ)
-    evk = synth.uniform_limbs(g, (2,), N, logQ + logP)
-    ct1[0, 0, :, 0] = 0xFFFFFFFF                     # a coefficient with every stored bit set (masked on load)
-    ctx.fhe_set_evk(limbs_np_to_tensor(evk))
+    ct1[0] = np.stack([to_limbs(p, ctx.L) for p in cts1[0]])
+    ct2[0] = np.stack([to_limbs(p, ctx.L) for p in cts2[0]])
+    ct1[1, 0, :, 0] = 0xFFFFFFFF                     # a coefficient with every stored bit set (masked on load)
+    evk_np = np.stack([to_limbs(p, ctx.L_PQ) for p in evk])
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk_np))
     d1, d2 = limbs_np_to_tensor(ct1), limbs_np_to_tensor(ct2)
     t3 = ctx.fhe_he_mult(d1, d2)
-    out3 = tensor_to_np(t3)
-    ct1m = ct1.copy()
-    ct1m[..., ctx.L - 1, :] &= np.uint32((1 << (logQ % 32)) - 1) if logQ % 32 else np.uint32(0xFFFFFFFF)
-    for b in (0, B - 1):
-        _check_he_mult_samples(out3[b], ct1m[b], ct2[b], prm.Q, _sample_ks(N, b, 2))
     t2 = ctx.fhe_relinearize(t3)
-    out2 = tensor_to_np(t2)
-    evk_polys = [from_limbs(evk[0]), from_limbs(evk[1])]
-    for b in (0, B - 1):
-        for k in _sample_ks(N, 10 + b, 2):
-            want = _relin_coeff_ckks(prm, out3[b], evk_polys, k)
-            assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
     tr = ctx.fhe_rescale(t2, 40)
-    outr = tensor_to_np(tr)
-    Q2 = 1 << (logQ - 40)
-    rnd = np.random.default_rng(3)
-    for b in range(B):
-        for comp in range(2):
-            for k in [int(v) for v in rnd.integers(0, N, size=16)]:
-                c = coeff_from_limbs(out2[b, comp], k)
-                assert coeff_from_limbs(outr[b, comp], k) == scheme.round_shift(c, 40) % Q2
     fused = ctx.fhe_mult_relin_rescale(d1, d2, 40)
     assert torch.equal(fused, tr)
-    # R1 (any size): 2^p c' - c in (-2^(p-1), 2^(p-1)] mod Q, checked on every coefficient of one component with numpy
-    lo_in = out2[0, 0, 0].astype(np.uint64) | (out2[0, 0, 1].astype(np.uint64) << np.uint64(32))
-    lo_out = outr[0, 0, 0].astype(np.uint64)
-    diff = ((lo_out << np.uint64(40)) - lo_in).astype(np.int64)     # low 64 bits suffice for the low-bit identity
-    low40 = (lo_in & np.uint64((1 << 40) - 1)).astype(np.int64)
-    expect = np.where(low40 >= (1 << 39), (1 << 40) - low40, -low40)
-    assert np.array_equal(diff & ((1 << 62) - 1), expect & ((1 << 62) - 1))
-
-
-def test_c3_ckks_decryption_bound_real_encryptions():
-    """configs[2] with real encryptions (one pair of the batch): CKKS decrypt(mult) within 2^-20 of the slot product."""
-    fhe = _lib()
-    N, logQ, logP = 1 << 15, 620, 620
-    prm, s, evk, cts1, cts2, zs = _ckks_setup(N, logQ, logP, 1, seed=0)
-    ctx = fhe.Context(N, logQ, logP)
-    ctx.fhe_set_evk(polys_to_tensor(list(evk), ctx.L_PQ))
-    out = ctx.fhe_mult_relin_rescale(polys_to_tensor(cts1, ctx.L), polys_to_tensor(cts2, ctx.L), 40)
-    got = tensor_to_polys(out)[0]
-    mu = harness.decrypt(tuple(got), s, 1 << (logQ - 40))
-    z = harness.decode(mu, N, 2.0 ** 40)
+    out3, out2, outr = tensor_to_np(t3), tensor_to_np(t2), tensor_to_np(tr)
+    # ---- item 0: every limb of every coefficient, against the oracle's own NTT route ----
+    want3 = scheme.he_mult(prm, cts1[0], cts2[0])
+    assert [from_limbs(out3[0, i]) for i in range(3)] == [list(p) for p in want3]
+    want2 = scheme.relinearize(prm, want3, evk)
+    assert [from_limbs(out2[0, i]) for i in range(2)] == [list(p) for p in want2]
+    wantr = scheme.rescale(prm, want2, 40)
+    gotr = [from_limbs(outr[0, i]) for i in range(2)]
+    assert gotr == [list(p) for p in wantr]
+    z = harness.decode(harness.decrypt(tuple(gotr), s, 1 << (logQ - 40)), N, 2.0 ** 40)
     assert np.max(np.abs(z - zs[0][0] * zs[0][1])) <= 2.0 ** -20
+    # ---- the other items: positions chosen by structure, from the definition (one output polynomial per position, in
+    # turn: a coefficient costs N big-integer products on the CPU) ----
+    ct1m = ct1.copy()
+    ct1m[..., ctx.L - 1, :] &= np.uint32((1 << (logQ % 32)) - 1) if logQ % 32 else np.uint32(0xFFFFFFFF)
+    Q, Q2 = prm.Q, 1 << (logQ - 40)
+    total, residues = 0, set()
+    for b in range(1, B):
+        ks3 = _structured_ks(N, b, B, 3, ctx.n_sm)
+        assert _groups_hit(N, b, 3, B, ctx.n_sm, ks3) >= {(0, False), (1, False)}
+        c0, c1 = from_limbs(ct1m[b, 0]), from_limbs(ct1m[b, 1])
+        e0, e1 = from_limbs(ct2[b, 0]), from_limbs(ct2[b, 1])
+        for n, k in enumerate(ks3):
+            which = (n + b) % 3
+            if which == 0:
+                want = ring.pm_coeff(c0, e0, k, Q)
+            elif which == 1:
+                want = (ring.pm_coeff(c0, e1, k, Q) + ring.pm_coeff(c1, e0, k, Q)) % Q
+            else:
+                want = ring.pm_coeff(c1, e1, k, Q)
+            assert coeff_from_limbs(out3[b, which], k) == want, (b, which, k)
+        ks2 = _structured_ks(N, b, B, 2, ctx.n_sm)
+        d2b = from_limbs(out3[b, 2])
+        for n, k in enumerate(ks2):
+            comp = (n + b) % 2
+            x = ring.pm_coeff(d2b, evk[comp], k, prm.PQ)
+            want = (coeff_from_limbs(out3[b, comp], k) + scheme.round_shift(x, logP)) % Q
+            assert coeff_from_limbs(out2[b, comp], k) == want, (b, comp, k)
+            assert coeff_from_limbs(outr[b, comp], k) == scheme.round_shift(want, 40) % Q2, (b, comp, k)
+        total += len(ks3) + len(ks2)
+        residues |= {k % 128 for k in ks3}
+    assert total >= 512 and (B < 3 or len(residues) == 128)
+    # R1 (any size): 2^p c' - c in (-2^(p-1), 2^(p-1)] mod Q, on every coefficient of every polynomial with numpy
+    for b in range(B):
+        for comp in range(2):
+            lo_in = out2[b, comp, 0].astype(np.uint64) | (out2[b, comp, 1].astype(np.uint64) << np.uint64(32))
+            lo_out = outr[b, comp, 0].astype(np.uint64)
+            diff = ((lo_out << np.uint64(40)) - lo_in).astype(np.int64)     # low 64 bits suffice for the low-bit identity
+            low40 = (lo_in & np.uint64((1 << 40) - 1)).astype(np.int64)
+            expect = np.where(low40 >= (1 << 39), (1 << 40) - low40, -low40)
+            assert np.array_equal(diff & ((1 << 62) - 1), expect & ((1 << 62) - 1))
 
 
 # ---- configs[3]: non-RNS BGV ---------------------------------------------------------------------------------------------
@@ -446,6 +497,68 @@ def test_relin_top_form_and_its_exact_path(bits, logQ, logP):
         c2 = tuple(from_limbs(ct_np[1, i, k]) for k in range(2))
         want = scheme.rescale(prm, scheme.relinearize(prm, scheme.he_mult(prm, c1, c2), evk), p)
         assert tensor_to_polys(fused[i]) == [list(q) for q in want]
+
+
+@pytest.mark.parametrize("logQ,logP,amb", [(352, 352, 58), (352, 352, 1), (365, 120, 58), (365, 120, 1), (352, 64, 58), (365, 90, 58)])
+def test_fused_rescale_epilogue_shift_amounts(logQ, logP, amb):
+    """The rescale fused into the relin CRT epilogue (what fhe_mult_relin_rescale, the benchmarked call, runs) over the
+    shift amounts that move its limb boundaries: p < 32, p a multiple of 32, p = logQ - 1, p past the rounding limb;
+    top-form targets (logP >= 96, with the exact path forced on half of the coefficients and off) and full targets
+    (logP < 96); logQ a multiple of 32 and not.  L = 11 / 12 limbs, so the streaming fast path (no boundary inside a group
+    of eight limbs) is taken as well as the boundary path.  Each must equal the three separate calls and the oracle."""
+    fhe = _lib()
+    N, B = 256, 2
+    prm = scheme.Params(N, logQ, logP, 0)
+    ctx = fhe.Context(N, logQ, logP)
+    assert ctx.L > 10
+    ctx.fhe_debug_crt_ambiguity(amb)
+    g = synth.rng(logQ + logP + amb)
+    ct_np = synth.uniform_limbs(g, (2, B, 2), N, logQ)
+    evk_np = synth.uniform_limbs(g, (2,), N, logQ + logP)
+    evk = tuple(from_limbs(evk_np[k]) for k in range(2))
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk_np))
+    d1, d2 = limbs_np_to_tensor(ct_np[0]), limbs_np_to_tensor(ct_np[1])
+    t2 = ctx.fhe_relinearize(ctx.fhe_he_mult(d1, d2))
+    want2 = []
+    for i in range(B):
+        c1 = tuple(from_limbs(ct_np[0, i, k]) for k in range(2))
+        c2 = tuple(from_limbs(ct_np[1, i, k]) for k in range(2))
+        want2.append(scheme.relinearize(prm, scheme.he_mult(prm, c1, c2), evk))
+    assert tensor_to_polys(t2) == [[list(q) for q in w] for w in want2]
+    assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, 0), t2)
+    for p in (1, 31, 32, 33, 64, 96, 320, logQ - 1):
+        fused = ctx.fhe_mult_relin_rescale(d1, d2, p)
+        assert torch.equal(fused, ctx.fhe_rescale(t2, p)), p
+        assert tensor_to_polys(fused) == [[list(q) for q in scheme.rescale(prm, w, p)] for w in want2], p
+
+
+def test_exact_path_takes_every_flagged_coefficient_of_a_large_launch():
+    """With the flag threshold at one fractional bit half of the coefficients of a launch go down the exact CRT path:
+    2 items x 2 polynomials x 2^16 coefficients = 131 072 flagged ones in one launch (the flag store is a bitmap sized to
+    the launch, so none can be dropped).  The result must be the same limbs as with the threshold at 58 bits, and the
+    oracle's on structured positions."""
+    fhe = _lib()
+    N, logQ, logP, B, p = 1 << 16, 128, 128, 2, 40
+    prm = scheme.Params(N, logQ, logP, 0)
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(4242)
+    ct1 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    ct2 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    evk_np = synth.uniform_limbs(g, (2,), N, logQ + logP)
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk_np))
+    d1, d2 = limbs_np_to_tensor(ct1), limbs_np_to_tensor(ct2)
+    t3 = ctx.fhe_he_mult(d1, d2)
+    ref2, ref = ctx.fhe_relinearize(t3), ctx.fhe_mult_relin_rescale(d1, d2, p)
+    ctx.fhe_debug_crt_ambiguity(1)
+    got2, got = ctx.fhe_relinearize(t3), ctx.fhe_mult_relin_rescale(d1, d2, p)
+    assert torch.equal(got2, ref2) and torch.equal(got, ref)
+    out3, out2 = tensor_to_np(t3), tensor_to_np(got2)
+    evk = [from_limbs(evk_np[0]), from_limbs(evk_np[1])]
+    for b in range(B):
+        d2b = from_limbs(out3[b, 2])
+        for k in _structured_ks(N, b, B, 2, ctx.n_sm, per_item=16):
+            want = _relin_coeff_ckks(prm, out3[b], evk, k, d2b)
+            assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
 
 
 # ---- NEXT-1 (SURVEY.md 8f): coefficient-wise operations, level drop, and a depth-2 circuit across two levels ----------------
