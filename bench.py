@@ -8,7 +8,8 @@ inverse NTT, CRT + mod Q, relinearise with evk mod PQ + divide by P, rescale by 
 synthetic ciphertext pairs per GPU (BASELINE.json configs[4]).  Prints ONE JSON line (rank 0).
 Multi-GPU: the batch dimension shards with no data-path collective -> weak scaling, evk replicated.
 `--impl reference` times the CPU oracle (oracle/, test infrastructure) on a bounded sample (one ring product of the
-workload's shape per step) on the host cores.
+workload's shape per step, mod Q and mod PQ in the 4 : 2 mix of an op) on the host cores.
+`python bench.py --gpus N` without a launcher re-executes itself under torch.distributed.run with N ranks.
 """
 from __future__ import annotations
 
@@ -32,12 +33,44 @@ WORKLOADS = {
     "c3": (1 << 15, 620, 620, 8, 40),
     "c1": (1 << 10, 128, 128, 1, 40),
 }
-# one op at C5 on the oracle = 4 ring products mod Q + 2 mod PQ; a mod-PQ product costs 2.06x a mod-Q product
-# (measured once on the dev box: 61.7 s vs 29.9 s); used only to scale the timed CPU sample to ops/s.
-ORACLE_PRODUCTS_PER_OP = 4 + 2 * 2.06
-# DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/, same command as the
-# timed run): dram__bytes_read.sum + dram__bytes_write.sum, averaged over that class's launches of one step.
-NCU_TRAFFIC = {"pointwise": 605.3e6}   # profiles/r1y_launches_and_captures.md: (440.2 + 218.6 + 329.8 + 221.9) MB / 2 launches
+# DRAM bytes per launch of each kernel class come from a committed `ncu --set full` capture of this same command
+# (profiles/dram_traffic.csv: class, launches per step, dram__bytes_read.sum + dram__bytes_write.sum per launch, the sha256
+# of the kernel sources the capture was taken with, the capture's file name).  A capture taken with other kernel sources
+# than the ones that are running is refused: `traffic` is then null and `traffic_source` says why.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+CSRC = os.path.join(ROOT, "paper_2607_05920_b200", "csrc")
+
+
+def kernel_source_hash() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name.endswith((".cu", ".cuh", ".hpp")):
+            with open(os.path.join(CSRC, name), "rb") as f:
+                h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(kernel_class: str):
+    """(bytes per launch or None, source string) for one kernel class from profiles/dram_traffic.csv."""
+    try:
+        with open(TRAFFIC_CSV) as f:
+            rows = [r.strip().split(",") for r in f if r.strip() and not r.startswith("#")]
+    except OSError:
+        return None, "no committed capture (profiles/dram_traffic.csv missing)"
+    head = kernel_source_hash()
+    for r in rows[1:]:
+        if len(r) >= 5 and r[0] == kernel_class:
+            if r[3] != head:
+                return None, f"stale: {r[4]} was captured with kernel sources {r[3]}, running {head}"
+            return float(r[2]), f"{r[4]} (ncu --set full, same command, kernel sources {r[3]})"
+    return None, f"no row for {kernel_class} in profiles/dram_traffic.csv"
+
+
+def workload_string(name: str) -> str:
+    N, logQ, logP, B, p_bits = WORKLOADS[name]
+    tag = " (BASELINE.json configs[4])" if name == "c5" else ""
+    return f"{name}: CKKS N={N} logQ={logQ} logP={logP} batch={B}/GPU rescale={p_bits}{tag}"
 
 
 def _peaks():
@@ -199,43 +232,56 @@ def shard_units(per_gpu_batch: int, world: int):
 
 
 # ---- the CPU oracle arm ---------------------------------------------------------------------------------------------------
-def oracle_sample_product(N, logQ, seed=0):
-    """Time ONE ring product mod Q of the workload's shape on the oracle (its own NTT route). Returns seconds."""
+# One op on the oracle = 4 ring products mod Q (the tensor product) + 2 mod PQ (the key switch); the divide-by-P, the
+# additions and the rescale are a fraction of a percent beside them.  Both kinds of product are timed in the run.
+def oracle_sample_product(N, logQ, logP=0, seed=0):
+    """Time ONE ring product of the workload's shape on the oracle (its own NTT route): a (< Q) times b (< Q when
+    logP == 0: a tensor-product term; < PQ = 2^(logP + logQ) else: a key-switch term, reduced mod PQ).  Seconds."""
     import synth
     from oracle import ring
     from oracle.limbs import from_limbs
     g = synth.rng(seed)
     a = from_limbs(synth.uniform_limbs(g, (), N, logQ))
-    b = from_limbs(synth.uniform_limbs(g, (), N, logQ))
+    b = from_limbs(synth.uniform_limbs(g, (), N, logQ + logP))
     t0 = time.perf_counter()
-    ring.pm(a, b, 1 << logQ)
+    ring.pm(a, b, 1 << (logQ + logP))
     return time.perf_counter() - t0
+
+
+def oracle_ops_per_s(t_q: float, t_pq: float) -> float:
+    return 1.0 / (4.0 * t_q + 2.0 * t_pq)
 
 
 def run_reference(args):
     """The oracle as it stands on the host cores: at this size its ring product goes through its own NTT route
-    (oracle.ring.pm).  A step times ONE ring product mod Q of one pair of the workload's shape (about 14 s on one core)
-    and converts it to ops/s with the 4 + 2 * 2.06 products an op costs -- the same bounded sample as `cpu_baseline`."""
+    (oracle.ring.pm).  A step times ONE ring product of one pair of the workload's shape -- mod Q in two steps out of three,
+    mod PQ in the third, the 4 : 2 mix of an op -- and the line converts the two measured means to ops/s."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
     N, logQ, logP, B, p_bits = WORKLOADS[args.workload]
     for i in range(args.warmup):
-        oracle_sample_product(N, logQ, seed=100 + i)
+        oracle_sample_product(N, logQ, logP if i % 3 == 2 else 0, seed=100 + i)
+    tq, tpq = [], []
     t0 = time.perf_counter()
     for i in range(args.steps):
-        oracle_sample_product(N, logQ, seed=i)
+        if i % 3 == 2:
+            tpq.append(oracle_sample_product(N, logQ, logP, seed=i))
+        else:
+            tq.append(oracle_sample_product(N, logQ, 0, seed=i))
     dt = time.perf_counter() - t0
-    t_prod = dt / args.steps
-    value = 1.0 / (t_prod * ORACLE_PRODUCTS_PER_OP)
-    sample = (f"per step 1 ring product mod Q of 1 pair (oracle.ring.pm, own NTT route) = {t_prod:.1f} s; "
-              f"an op = 4 products mod Q + 2 mod PQ = {ORACLE_PRODUCTS_PER_OP:.2f} such products")
+    t_q = sum(tq) / len(tq)
+    t_pq = sum(tpq) / len(tpq) if tpq else 2.0 * t_q          # fewer than three steps: no mod-PQ sample, assume twice
+    value = oracle_ops_per_s(t_q, t_pq)
+    sample = (f"per step 1 ring product of 1 pair (oracle.ring.pm, own NTT route): {len(tq)} mod Q = {t_q:.1f} s each, "
+              f"{len(tpq)} mod PQ = {t_pq:.1f} s each; an op = 4 mod Q + 2 mod PQ = {4 * t_q + 2 * t_pq:.1f} s")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int (python big integers, numpy uint64 NTT)", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: CKKS N={N} logQ={logQ} logP={logP} batch={B} rescale={p_bits}"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(), "sample": sample},
+        "config": {"workload": workload_string(args.workload)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle (python, 1 core, extrapolated from single ring products)",
+                         "host_cores": os.cpu_count(), "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
     print(json.dumps(line), flush=True)
@@ -343,15 +389,20 @@ def run_ours(args):
     n_launch_top = max(1, per_class[top][1])
     avg_launch_s = per_class[top][0] / 1e3 / n_launch_top
     t_hbm = byt[top] / (hbm_gbs * 1e9)
+    # a second, mix-independent integer ceiling for the butterfly: one mul.hi and two mad.lo per butterfly at the measured
+    # instruction rates -- it cannot move when the kernels' own butterfly code changes
+    bf_peak_instr = 1.0 / (1.0 / mulhi_peak + 2.0 / mad_peak)
     if t_int(top) >= t_hbm and bf[top] > 0:
-        roof = {"bound": "alu", "kernel": top, "achieved": bf[top] * args.steps / n_launch_top / avg_launch_s / 1e9,
-                "peak": bf_peak / 1e9, "unit": "Gbutterfly/s",
-                "peak_kind": "measured in this run: the kernels' own forward butterfly, register-only (fhe_debug_int_peak; DESIGN.md 7)"}
+        ach = bf[top] * args.steps / n_launch_top / avg_launch_s
+        roof = {"bound": "alu", "kernel": top, "achieved": ach / 1e9, "peak": bf_peak / 1e9, "unit": "Gbutterfly/s",
+                "peak_kind": "measured in this run: the kernels' own forward butterfly, register-only (fhe_debug_int_peak; DESIGN.md 7)",
+                "frac_vs_instruction_peak": ach / bf_peak_instr, "instruction_peak": bf_peak_instr / 1e9,
+                "instruction_peak_kind": "1 mul.hi.u32 + 2 mad.lo.u32 per butterfly at the rates measured in this run"}
     else:
         roof = {"bound": "hbm", "kernel": top, "achieved": byt[top] * args.steps / n_launch_top / avg_launch_s / 1e9,
                 "peak": hbm_gbs, "unit": "GB/s", "peak_kind": peak_kind}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = NCU_TRAFFIC.get(top) if args.workload == "c5" else None
+    roof["traffic"], roof["traffic_source"] = committed_traffic(top) if args.workload == "c5" else (None, "captures exist for c5 only")
     roof["algorithmic_bytes_per_launch"] = byt[top] * args.steps / n_launch_top
     roof["avg_launch_ms"] = avg_launch_s * 1e3
     roof["hbm_frac"] = byt[top] * args.steps / n_launch_top / avg_launch_s / 1e9 / hbm_gbs
@@ -363,22 +414,23 @@ def run_ours(args):
     path = {"t_int_ms": t_path_alu * 1e3, "t_hbm_ms": t_path_hbm * 1e3, "t_measured_ms": t_step * 1e3,
             "frac": max(t_path_alu, t_path_hbm) / t_step, "gbutterfly_per_step": sum(bf.values()) / 1e9,
             "compulsory_mb_per_step": compulsory / 1e6,
-            "int_peaks": {"gbutterfly_per_s": bf_peak / 1e9, "gmadlo_per_s": mad_peak / 1e9, "gmulhi_per_s": mulhi_peak / 1e9}}
+            "frac_vs_instruction_peak": max(sum(bf[k] / bf_peak_instr + units[k] / mad_peak for k in bf), t_path_hbm) / t_step,
+            "int_peaks": {"gbutterfly_per_s": bf_peak / 1e9, "gbutterfly_per_s_from_instruction_rates": bf_peak_instr / 1e9,
+                          "gmadlo_per_s": mad_peak / 1e9, "gmulhi_per_s": mulhi_peak / 1e9}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        t_prod = oracle_sample_product(N, logQ)
-        cpu = {"value": 1.0 / (t_prod * ORACLE_PRODUCTS_PER_OP), "unit": UNIT, "cores": 1, "kind": "oracle",
-               "host_cores": os.cpu_count(),
-               "sample": (f"1 ring product mod Q of 1 pair (oracle.ring.pm, own NTT route) = {t_prod:.1f} s; "
-                          f"an op = 4 products mod Q + 2 mod PQ = {ORACLE_PRODUCTS_PER_OP:.2f} such products")}
+        t_q, t_pq = oracle_sample_product(N, logQ, 0), oracle_sample_product(N, logQ, logP)
+        cpu = {"value": oracle_ops_per_s(t_q, t_pq), "unit": UNIT, "cores": 1,
+               "kind": "oracle (python, 1 core, extrapolated from single ring products)", "host_cores": os.cpu_count(),
+               "sample": (f"1 ring product mod Q ({t_q:.1f} s) and 1 mod PQ ({t_pq:.1f} s) of 1 pair (oracle.ring.pm, own NTT "
+                          f"route), both timed in this run; an op = 4 mod Q + 2 mod PQ = {4 * t_q + 2 * t_pq:.1f} s")}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "u32 (exact integer)", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: CKKS N={N} logQ={logQ} logP={logP} batch={B}/GPU rescale={p_bits} "
-                               f"(BASELINE.json configs[4])" if args.workload == "c5" else args.workload,
+        "config": {"workload": workload_string(args.workload),
                    "L": ctx.L, "K1": ctx.K1, "K2": ctx.K2, "global_batch": total_units, "parallelism": f"batch-sharded x{world}, no collective",
                    "l2": "inputs + workspace per step (~0.9 GB) exceed the 126 MB L2; no explicit flush"},
         "clocks": clocks, "gpu_launches": int(launches),
@@ -477,11 +529,22 @@ def run_sweep(args):
             ms = e0.elapsed_time(e1) / reps
             w = 4
             alg = batch * N * w * (2 * L + 2 * K) + batch * N * w * (2 * 2 * K + 2 * K + K + 2 * K) + batch * N * w * (K + L)
+            cpu = None
+            if N <= (1 << 14) and not args.no_cpu_baseline:
+                # the oracle beside it: one pair per cell, cells with N <= 2^14 only, one host core
+                from oracle import ring
+                from oracle.limbs import from_limbs
+                ha, hb = from_limbs(a1[0].cpu().numpy().view(np.uint32)), from_limbs(b1[0].cpu().numpy().view(np.uint32))
+                t0 = time.perf_counter()
+                ring.pm(ha, hb, 1 << logQ)
+                t_or = time.perf_counter() - t0
+                cpu = {"value": 1.0 / t_or, "unit": "polymuls/s", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+                       "sample": f"1 pair of this cell (oracle.ring.pm) = {t_or:.2f} s; cells with N <= 2^14 only"}
             print(json.dumps({"sweep": True, "metric": "polymuls/s", "value": batch / (ms / 1e3), "unit": "polymuls/s",
                               "N": N, "logQ": logQ, "L": L, "K": K, "batch": batch, "ms_per_call": ms,
                               "us_per_polymul": ms * 1e3 / batch, "algorithmic_gb_per_s": alg / (ms / 1e3) / 1e9,
                               "hbm_frac_of_plan": alg / (ms / 1e3) / 1e9 / hbm_gbs, "dtype": "u32 (exact integer)",
-                              "data": "synthetic"}), flush=True)
+                              "data": "synthetic", "cpu_baseline": cpu}), flush=True)
             del ctx, a, b, out
             torch.cuda.empty_cache()
     return 0
@@ -498,6 +561,12 @@ def main():
     ap.add_argument("--sweep", action="store_true",
                     help="standalone polymul sweep N = 2^12..2^16 x logQ in {64, 256, 620, 1240, 2480}: one JSON line per cell")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not args.sweep:
+        # plain `python bench.py --gpus N`: become the N-rank launch the contract describes (one process per GPU)
+        port = os.environ.get("MASTER_PORT", "29511")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", port, os.path.abspath(__file__)] + sys.argv[1:]
+        os.execv(sys.executable, cmd)
     if args.impl == "reference":
         return run_reference(args)
     if args.sweep:

@@ -402,7 +402,7 @@ fhe_status fhe_debug_decompose(fhe_ctx* ctx, uint32_t* d_res, const uint32_t* d_
   Context* c = C(ctx);
   if (fhe_status ds = check_device(c)) return ds;
   if (!d_res || !d_limbs || K == 0 || K > c->Kmax || Lin == 0 || Lin > MAX_LIMBS_IN) return err(c, FHE_ERR_ARG, "bad argument");
-  CK(launch_decompose(c, d_res, 0, (size_t)K * c->N, d_limbs, 0, (size_t)Lin * c->N, 1, npoly, Lin, K, mask_bits, (cudaStream_t)stream), "decompose");
+  CK(launch_decompose(c, d_res, 0, (size_t)K * c->N, d_limbs, 0, (size_t)Lin * c->N, 1, npoly, Lin, K, mask_bits, (cudaStream_t)stream, false), "decompose");
   return FHE_OK;
 }
 

@@ -150,10 +150,11 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 
 // ---- launchers (kernels_*.cu) --------------------------------------------------------------------------------------
 // Polynomials of a launch are indexed (o, i), o < nouter, i < ninner, and live at base + o * outer + i * inner (words).
-// decompose: limbs [Lin][N] -> residues [K][N] per polynomial; mask_bits > 0 reduces the input mod 2^mask_bits first
+// decompose: limbs [Lin][N] -> residues [K][N] per polynomial; mask_bits > 0 reduces the input mod 2^mask_bits first;
+// lazy: residues in [0, 2q) instead of [0, q) (what the forward transforms accept)
 cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                              size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin,
-                             uint32_t K, uint32_t mask_bits, cudaStream_t s);
+                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy = true);
 // Transforms live in an item-major residue buffer [nitems][S][K][N] (S slots per item); slots 0..U-1 of every item
 // are transformed in place.  Forward output is in bit-reversed order and canonical ([0, q)).
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s);

@@ -109,31 +109,51 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
 // CRT epilogue of the conversion pipeline (pipe.cuh).  The loaders stage the residues y[i][n] as the A operand (word i =
 // column i), the tensor cores contract them with the constant image B: column 8 + e receives
 // S_e = sum_{i,b} y_ib * byte_{e-b}(W_i), columns 0..5 the byte sums of sum_i y_i floor(2^48 / q_i) (-> alpha).  Here:
-//   carry pass   V = sum_e S_e 2^(8 e) + alpha * negM, four columns (one limb) at a time as the accumulator chunks
-//                arrive; everything but the two-instruction carry chain is independent across the limbs of a group
-//   post         CKKS: streamed, in registers -- mask (tensor / polymul), or shift by logP with rounding + add (d0, d1)
-//                [+ shift by the rescale bits with rounding] through one-limb delay lines, coalesced stores as the limbs
-//                come out.  BGV: the limbs go to this thread's column xs[.][etid] in shared memory and the multi-limb
-//                Barrett reductions run on the column (post()).
-//                The polynomial added by the relin modes is prefetched into a second column with cp.async while the
-//                tile's MMAs run.
+//   column sums  P_l = S_4l + 2^8 S_4l+1 + 2^16 S_4l+2 + 2^24 S_4l+3 + alpha negM_l  (< 2^52): four mad.wide per limb,
+//                independent across the eight limbs of a call
+//   CKKS relin   everything that is ADDED to V before the shifts is added to the column sums first -- the polynomial d
+//                (d0 or d1) at bit position s1, the rounding 2^(logP-1) of the divide by P, the rounding 2^(s1+p-1) of the
+//                rescale (s1 = logP, or 0 for the top form, which hands V >> logP over directly) -- so that ONE carry chain
+//                (two dependent instructions per limb) yields the limbs of  total = V + 2^(logP-1) + (d << s1) + 2^(s1+p-1)
+//                and the output limb m is bits [s1 + p + 32 m, +32) of it, one funnel shift.  Carries out of bit
+//                s1 + logQ only reach bits the final reduction mod 2^(logQ-p) drops, so (d + k) needs no reduction mod
+//                2^logQ between the two roundings: the result is the one of the three separate steps (A3/A4).
+//   CKKS mask    the limbs of V below logQ, top limb masked (tensor / polymul)
+//   BGV          the limbs go to this thread's column xs[.][etid] in shared memory and the multi-limb Barrett
+//                reductions run on the column (post()).
+// The polynomial added by the relin modes is prefetched into a shared-memory column with cp.async while the tile's
+// MMAs run.  MODE / TOP / RESC are template parameters: the hot loops carry no mode branches.
 // ------------------------------------------------------------------------------------------------------------------
+struct CrtParams {
+  uint32_t* out; size_t out_outer, out_inner;
+  const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
+  const uint32_t* negM;                               // [Lraw]
+  uint32_t Lraw, Lx, nl, ntab;                        // nl = limbs of V the chunks cover; ntab = entries of the negM table
+  uint32_t amb_bits; uint32_t* flags;                 // top-form relin target (fhe_internal.cuh): flag bitmap of the exact path
+  uint32_t xs_off, adds_off, scratch_off;             // word offsets inside the scratch: negM table at 0, then the columns
+  // CKKS relin: d enters at limb wd, bit bd (s1 = 32 wd + bd); the output starts at limb ws, bit bs of the total
+  // (s1 + p = 32 ws + bs); roundings rbit1 at limb rb1 (divide by P; full form only), rbit2 at limb rb2 (rescale);
+  // the result has Lr limbs, the top one masked with tm; lend = last limb of the total the stream must see
+  uint32_t wd, bd, ws, bs, rb1, rbit1, rb2, rbit2, Lr, tm, tmq, lend;
+  PostParams pp;
+};
+
+__device__ __forceinline__ uint64_t madw(uint32_t a, uint32_t b, uint64_t c) {
+  uint64_t d;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
+  return d;
+}
+
+template <int MODE, bool TOP, bool RESC>
 struct CrtEpi {
   static constexpr int LOAD_WORDS = 64, MAX_REGS = 96;     // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
   static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;
   static constexpr bool LOAD_ALT = false;
   static constexpr bool TILE_ALT = true;                   // two whole epilogues on alternate tiles: the epilogue bounds S5
-  struct Params {
-    uint32_t* out; size_t out_outer, out_inner;
-    const uint32_t* add; size_t add_outer, add_inner;   // relin modes; else nullptr
-    const uint32_t* negM;                               // [Lraw]
-    uint32_t Lraw, Lx, nl, ntab;                        // nl = limbs of V the chunks cover; ntab = entries of the negM table
-    uint32_t top, amb_bits; uint32_t* flags;             // top-form relin target (fhe_internal.cuh): flag bitmap of the exact path
-    uint32_t xs_off, adds_off, scratch_off;             // word offsets inside the scratch: negM table at 0, then the columns
-    // CKKS relin streaming constants: shift by logP = 32 ws + bs, rounding bit rbit in limb rb; rescale likewise (.2)
-    uint32_t ws, bs, rb, rbit, ws2, bs2, rb2, rbit2, Lr, tm2, tmq, lend;
-    PostParams pp;
-  };
+  static constexpr bool RELIN = MODE == POST_CKKS_RELIN || MODE == POST_BGV_RELIN;
+  static_assert(!TOP || MODE == POST_CKKS_RELIN, "the top form exists for the CKKS relin target only");
+  static_assert(!RESC || MODE == POST_CKKS_RELIN, "the fused rescale is CKKS-only");
+  using Params = CrtParams;
   const Params& p;
   const uint32_t N, etid, inner;
   const uint32_t* negm;  // [nl + 2] in shared memory, zero beyond Lraw
@@ -142,10 +162,10 @@ struct CrtEpi {
   uint32_t* scratch;     // [scratch_limbs][TC]  (BGV relin)
   uint32_t* out = nullptr;
   uint32_t* optr = nullptr;
-  const uint32_t* aptr = nullptr;
-  uint32_t alpha = 0, yprev = 0, cy = 0, zprev = 0, cz = 0;
+  uint32_t alpha = 0, yprev = 0;
   uint64_t carry = 0;
   uint32_t flag_word = 0;   // word of the flag bitmap this warp's 32 coefficients own: bit = lane
+  bool d_ready = false;
 
   __device__ CrtEpi(const Params& p_, const pipe::PipeArgs&a, uint8_t* sm, uint32_t etid_, uint32_t, uint32_t bar)
       : p(p_), N(a.N), etid(etid_), inner(a.inner), negm(reinterpret_cast<const uint32_t*>(sm)),
@@ -158,50 +178,17 @@ struct CrtEpi {
 
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.out + (size_t)o * p.out_outer + (size_t)i * p.out_inner + n0 + etid;
-    optr = out; aptr = adds + etid;
-    carry = 0; yprev = 0; cy = 0; zprev = 0; cz = 0;
-    flag_word = (o * inner + i) * (N >> 5) + ((n0 + etid) >> 5);
-    if (p.add) {
+    optr = out;
+    carry = 0; yprev = 0;
+    if constexpr (TOP) flag_word = (o * inner + i) * (N >> 5) + ((n0 + etid) >> 5);
+    if constexpr (RELIN) {
       const uint32_t* src = p.add + (size_t)o * p.add_outer + (size_t)i * p.add_inner + n0 + etid;
       const uint32_t dst = umma::smem_u32(adds + etid);
       for (uint32_t k = 0; k < p.pp.L; ++k)
         asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + k * TC * 4), "l"(src + (size_t)k * N) : "memory");
       asm volatile("cp.async.commit_group;" ::: "memory");
+      d_ready = false;
     }
-  }
-
-  // One limb of the CKKS relin stream: y = limb lg of V + 2^(logP-1).  Emits limb lg - 1 - ws of
-  // z = (d + (V + 2^(logP-1)) >> logP) mod 2^logQ, and from that, with rescaling, limb lg - 2 - ws - ws2 of the result.
-  // IN: the caller guarantees that no boundary (first / top limb, rounding limb, mask) falls on this limb.
-  template <bool IN>
-  __device__ __forceinline__ void relin_step(uint32_t lg, uint32_t y) {
-    if (IN || lg > p.ws) {
-      const uint32_t kidx = lg - 1 - p.ws;
-      const bool rescale = p.pp.rescale_bits != 0;
-      uint32_t z = 0;
-      if (IN || kidx < p.pp.L) {
-        const uint32_t kk = __funnelshift_r(yprev, y, p.bs);
-        const uint64_t s = (uint64_t)kk + *aptr + cy;
-        aptr += TC;
-        cy = (uint32_t)(s >> 32);
-        z = (uint32_t)s;
-        if (!IN && kidx == p.pp.L - 1) z &= p.tmq;
-        if (!rescale) { *optr = z; optr += N; }
-      }
-      if (rescale && (IN || kidx <= p.pp.L + p.ws2)) {            // limbs >= L of z are virtual: the rounding carry, then zero
-        const uint64_t s2 = (uint64_t)z + cz + ((!IN && kidx == p.rb2) ? p.rbit2 : 0u);
-        const uint32_t zz = (uint32_t)s2;
-        cz = (uint32_t)(s2 >> 32);
-        if (IN || kidx > p.ws2) {
-          const uint32_t m = kidx - 1 - p.ws2;
-          uint32_t v = __funnelshift_r(zprev, zz, p.bs2);
-          if (!IN) { if (m == p.Lr - 1) v &= p.tm2; if (m >= p.Lr) v = 0; }
-          if (IN || m < p.pp.L) { *optr = v; optr += N; }
-        }
-        zprev = zz;
-      }
-    }
-    yprev = y;
   }
 
   // Top-form relin target, first 32 columns of a tile: P[2..8) are the six limbs of S_t = sum_i y_i Wt_i + alpha Nt, the
@@ -229,31 +216,56 @@ struct CrtEpi {
     if ((etid & 31) == 0) p.flags[flag_word] = m;
   }
 
+  // bits of (d << s1) that fall into limb lg of the total (any lg): the generic, bounds-checked form
+  __device__ __forceinline__ uint32_t d_limb(uint32_t lg) const {
+    const uint32_t j = lg - p.wd;                                  // wraps for lg < wd: both tests below then fail
+    const uint32_t hi = j < p.pp.L ? adds[j * TC + etid] : 0u;
+    if (p.bd == 0) return hi;
+    const uint32_t lo = j - 1 < p.pp.L ? adds[(j - 1) * TC + etid] : 0u;
+    return __funnelshift_l(lo, hi, p.bd);
+  }
+  // One limb of the CKKS relin stream with every boundary checked: P = column sum of limb lg of the total.
+  __device__ __forceinline__ void relin_step(uint32_t lg, uint64_t P) {
+    P += d_limb(lg);
+    if (!TOP && lg == p.rb1) P += p.rbit1;
+    if (RESC && lg == p.rb2) P += p.rbit2;
+    const uint64_t v = carry + P;
+    carry = v >> 32;
+    const uint32_t y = (uint32_t)v;
+    if (lg > p.ws) {
+      const uint32_t m = lg - 1 - p.ws;
+      if (m < p.pp.L) {
+        uint32_t o = __funnelshift_r(yprev, y, p.bs);
+        if (m == p.Lr - 1) o &= p.tm;
+        if (m >= p.Lr) o = 0;
+        *optr = o; optr += N;
+      }
+    }
+    yprev = y;
+  }
+
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     int g0 = 0;
     if (col0 == 0) {
-      uint64_t asum = 0;
-#pragma unroll
-      for (int e = 0; e < 6; ++e) asum += (uint64_t)t[e] << (8 * e);
+      uint64_t asum = madw(t[3], 1u << 24, madw(t[2], 1u << 16, madw(t[1], 256u, (uint64_t)t[0])));
+      asum += ((uint64_t)t[4] << 32) + ((uint64_t)t[5] << 40);
       alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
       g0 = CRT_ALPHA_COLS / 4;
     }
-    uint32_t l0 = col0 / 4 - CRT_ALPHA_COLS / 4;                   // limb of group element 0 (wraps for col0 = 0; elements 0, 1 unused)
+    const uint32_t tb = col0 / 4 - CRT_ALPHA_COLS / 4;             // table / limb index of group element 0 (wraps for col0 = 0; elements 0, 1 unused)
     uint64_t P[8];                                                 // the limb's column sum + alpha * negM: independent of the carry
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
       if (g < g0) { P[g] = 0; continue; }
-      const uint64_t s01 = (uint64_t)t[4 * g + 1] * 256u + t[4 * g];
-      const uint64_t s23 = (uint64_t)t[4 * g + 3] * 256u + t[4 * g + 2];
-      P[g] = (uint64_t)alpha * negm[l0 + g] + s01 + (s23 << 16);
+      P[g] = madw(alpha, negm[tb + g], madw(t[4 * g + 3], 1u << 24, madw(t[4 * g + 2], 1u << 16, madw(t[4 * g + 1], 256u, (uint64_t)t[4 * g]))));
     }
-    if (p.top) {
+    uint32_t l0 = tb;
+    if constexpr (TOP) {
       if (col0 == 0) { top_carry(P); return; }
       l0 -= TOP_LIMBS;                                             // from here on l0 counts limbs of the high part
     }
-    const int mode = p.pp.mode;
     const uint32_t L = p.pp.L;
-    if (mode == POST_CKKS_MASK) {
+    if constexpr (MODE == POST_CKKS_MASK) {
       if (g0 == 0 && l0 + 8 < L) {
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
@@ -271,11 +283,40 @@ struct CrtEpi {
           if (lg < L) { *optr = lg == L - 1 ? ((uint32_t)v & p.tmq) : (uint32_t)v; optr += N; }
         }
       }
-    } else if (mode == POST_CKKS_RELIN) {
-      const uint32_t k0 = l0 - 1 - p.ws;                           // first z limb this group emits (when l0 > ws)
-      const bool rescale = p.pp.rescale_bits != 0;
-      if (l0 + 8 > p.rb) asm volatile("cp.async.wait_group 0;" ::: "memory");   // the add column is read from here on
-      if (l0 + 8 <= p.rb) {                                        // far below the shift: only the carry matters
+    } else if constexpr (MODE == POST_CKKS_RELIN) {
+      if (!d_ready && l0 + 8 > p.wd) {                             // the add column is read from here on
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        d_ready = true;
+      }
+      if (g0 == 0 && l0 > p.ws && l0 + 7 - p.wd < L && l0 + 7 - p.ws < p.Lr) {
+        // interior group: d_{j-1}, d_j exist for all eight limbs, no rounding limb (rb1 <= wd, rb2 <= ws < l0), every
+        // output limb below the masked top limb
+        const uint32_t* ap = adds + (l0 - p.wd) * TC + etid;
+        if (p.bd == 0) {
+#pragma unroll
+          for (int g = 0; g < 8; ++g) P[g] += ap[g * TC];
+        } else {
+          uint32_t dlo = ap[-TC];
+#pragma unroll
+          for (int g = 0; g < 8; ++g) {
+            const uint32_t dhi = ap[g * TC];
+            P[g] += __funnelshift_l(dlo, dhi, p.bd);
+            dlo = dhi;
+          }
+        }
+        uint32_t y[9];
+        y[0] = yprev;
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          const uint64_t v = carry + P[g];
+          carry = v >> 32;
+          y[g + 1] = (uint32_t)v;
+        }
+        yprev = y[8];
+#pragma unroll
+        for (int g = 0; g < 8; ++g) { *optr = __funnelshift_r(y[g], y[g + 1], p.bs); optr += N; }
+      } else if (l0 + 8 <= p.wd && l0 + 8 <= p.ws && (TOP || l0 + 8 <= p.rb1) && (!RESC || l0 + 8 <= p.rb2)) {
+        // far below everything: only the carry matters
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
           if (g < g0) continue;
@@ -283,22 +324,11 @@ struct CrtEpi {
           carry = v >> 32;
           yprev = (uint32_t)v;
         }
-      } else if (g0 == 0 && l0 > p.ws && k0 + 8 < L &&
-                 (!rescale || (k0 > p.rb2 && k0 > p.ws2 && k0 + 8 - 1 - p.ws2 < p.Lr - 1))) {
-#pragma unroll
-        for (int g = 0; g < 8; ++g) {
-          const uint64_t v = carry + P[g];
-          carry = v >> 32;
-          relin_step<true>(l0 + g, (uint32_t)v);
-        }
       } else {
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
           if (g < g0) continue;
-          const uint32_t lg = l0 + g;
-          const uint64_t v = carry + P[g] + (lg == p.rb ? p.rbit : 0u);
-          carry = v >> 32;
-          relin_step<false>(lg, (uint32_t)v);
+          relin_step(l0 + g, P[g]);
         }
       }
     } else {                                                       // BGV: the column in shared memory
@@ -314,36 +344,36 @@ struct CrtEpi {
   }
 
   __device__ void end_tile() {
-    const int mode = p.pp.mode;
-    if (mode == POST_CKKS_MASK) return;                            // the chunks cover all L limbs
-    if (p.add) asm volatile("cp.async.wait_group 0;" ::: "memory");
-    if (mode == POST_CKKS_RELIN) {
-      for (uint32_t lg = p.nl; lg <= p.lend; ++lg) {               // limbs past the last chunk: the carry, then zeros
-        const uint64_t v = carry + (lg == p.rb ? p.rbit : 0u);
-        carry = v >> 32;
-        relin_step<false>(lg, (uint32_t)v);
-      }
+    if constexpr (MODE == POST_CKKS_MASK) return;                  // the chunks cover all L limbs
+    if constexpr (RELIN) {
+      if (!d_ready) { asm volatile("cp.async.wait_group 0;" ::: "memory"); d_ready = true; }
+    }
+    if constexpr (MODE == POST_CKKS_RELIN) {
+      for (uint32_t lg = p.nl; lg <= p.lend; ++lg) relin_step(lg, 0);   // limbs past the last chunk: carry and d only
       return;
     }
-    for (uint32_t lg = p.nl; lg < p.Lx; ++lg) { xs[lg * TC + etid] = (uint32_t)carry; carry = 0; }
-    post();
+    if constexpr (MODE == POST_BGV_MODQ || MODE == POST_BGV_RELIN) {
+      for (uint32_t lg = p.nl; lg < p.Lx; ++lg) { xs[lg * TC + etid] = (uint32_t)carry; carry = 0; }
+      post();
+    }
   }
   __device__ void post();
 };
 
-__device__ void CrtEpi::post() {
+template <int MODE, bool TOP, bool RESC>
+__device__ void CrtEpi<MODE, TOP, RESC>::post() {
   const PostParams& pp = p.pp;
   const uint32_t Lx = p.Lx;
   Col x{xs + etid};
   Col ad{adds + etid};
   const uint32_t L = pp.L;
-  if (pp.mode == POST_BGV_MODQ) {
+  if constexpr (MODE == POST_BGV_MODQ) {
     col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
     for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     return;
   }
   // POST_BGV_RELIN: V -> xc = V mod PQ -> (q3, rem) = divmod(xc, P) -> centred r, kk -> (hi - kk + d) mod Q
-  {
+  if constexpr (MODE == POST_BGV_RELIN) {
     const uint32_t LP = pp.L_P, LPQ = pp.L_PQ, g = pp.g_limbs;   // g = LPQ - LP
     col_barrett1(x, Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);     // x[0..LPQ) = xc
     // Barrett quotient estimate (HAC 14.42 generalised): q1 = xc >> 32(LP-1)  (g+1 limbs),
@@ -532,7 +562,7 @@ crt_exact_kernel(ExactArgs a) {
 
 // scratch layout of CrtEpi (words): negM table [nl + 2] | xs [Lx][TC] (BGV) | adds [L][TC] (relin modes) |
 // BGV divide-by-P scratch [scratch_limbs][TC]
-static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi::Params& ep, size_t& bytes) {
+static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtParams& ep, size_t& bytes) {
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   const bool bgv = pp.mode == POST_BGV_MODQ || pp.mode == POST_BGV_RELIN;
   ep.ntab = tg.nchunks * (pipe::NC / 4);
@@ -543,10 +573,12 @@ static void crt_scratch_layout(const CrtTarget& tg, const PostParams& pp, CrtEpi
   bytes = ((size_t)ep.scratch_off + (pp.mode == POST_BGV_RELIN ? pp.scratch_limbs * TC : 0)) * 4;
 }
 
+using CrtEpiAny = CrtEpi<POST_CKKS_MASK, false, false>;   // the pipeline shape (warps, groups, tile alternation) is the same for all
+
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp) {
-  CrtEpi::Params ep; size_t bytes;
+  CrtParams ep; size_t bytes;
   crt_scratch_layout(tg, pp, ep, bytes);
-  return pipe::make_plan(tg.KB, tg.nchunks, bytes, true, CrtEpi::TILE_ALT).ok;
+  return pipe::make_plan(tg.KB, tg.nchunks, bytes, true, CrtEpiAny::TILE_ALT).ok;
 }
 
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
@@ -554,10 +586,10 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
                        size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s, uint32_t* d_flags) {
   if (nouter * ninner == 0) return cudaSuccess;
   if (tg.top && !d_flags) return cudaErrorInvalidValue;
-  CrtEpi::Params ep;
+  CrtParams ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);
-  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true, CrtEpi::TILE_ALT);
+  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true, CrtEpiAny::TILE_ALT);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   if (relin && !d_add) return cudaErrorInvalidValue;
@@ -570,20 +602,32 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;
   ep.negM = tg.d_negM; ep.Lraw = tg.Lraw; ep.Lx = tg.Lx; ep.pp = pp;
   ep.tmq = top_mask(pp.logQ);
-  const uint32_t shiftP = tg.top ? 0 : pp.logP;                  // the top form hands the epilogue V >> logP directly
-  ep.ws = shiftP >> 5; ep.bs = shiftP & 31;
-  ep.rb = shiftP ? (shiftP - 1) >> 5 : 0; ep.rbit = shiftP ? 1u << ((shiftP - 1) & 31) : 0;
-  ep.top = tg.top ? 1 : 0; ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = d_flags;
-  const uint32_t pb = pp.rescale_bits;
-  ep.ws2 = pb >> 5; ep.bs2 = pb & 31;
-  ep.rb2 = pb ? (pb - 1) >> 5 : 0; ep.rbit2 = pb ? 1u << ((pb - 1) & 31) : 0;
+  // CKKS relin stream (CrtEpi): total = V + 2^(logP-1) + (d << s1) + 2^(s1+p-1), output = bits [s1 + p, ...) of it
+  const uint32_t s1 = tg.top ? 0 : pp.logP;                      // the top form hands the epilogue V >> logP directly
+  const uint32_t pb = pp.mode == POST_CKKS_RELIN ? pp.rescale_bits : 0, sh = s1 + pb;
+  ep.wd = s1 >> 5; ep.bd = s1 & 31;
+  ep.ws = sh >> 5; ep.bs = sh & 31;
+  ep.rb1 = s1 ? (s1 - 1) >> 5 : 0; ep.rbit1 = s1 ? 1u << ((s1 - 1) & 31) : 0;
+  ep.rb2 = pb ? (sh - 1) >> 5 : 0; ep.rbit2 = pb ? 1u << ((sh - 1) & 31) : 0;
   const uint32_t nb = pp.logQ - pb;
-  ep.Lr = (nb + 31) / 32; ep.tm2 = top_mask(nb);
-  ep.lend = ep.ws + pp.L + (pb ? ep.ws2 + 1 : 0);                 // last limb index the relin stream must see
+  ep.Lr = (nb + 31) / 32; ep.tm = top_mask(nb);
+  ep.lend = ep.ws + pp.L;                                        // output limb m needs limbs ws + m and ws + m + 1 of the total
+  ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = d_flags;
   cudaError_t e;
   {
     LaunchTimer lt(c, KC_CRT, s);
-    e = pipe::launch_pipe<CrtEpi>(a, ep, plan.smem, c->n_sm, s);
+    switch (pp.mode) {
+      case POST_CKKS_MASK: e = pipe::launch_pipe<CrtEpi<POST_CKKS_MASK, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
+      case POST_BGV_MODQ: e = pipe::launch_pipe<CrtEpi<POST_BGV_MODQ, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
+      case POST_BGV_RELIN: e = pipe::launch_pipe<CrtEpi<POST_BGV_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
+      case POST_CKKS_RELIN:
+        if (tg.top) e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, true>>(a, ep, plan.smem, c->n_sm, s)
+                           : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, false>>(a, ep, plan.smem, c->n_sm, s);
+        else e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, true>>(a, ep, plan.smem, c->n_sm, s)
+                    : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s);
+        break;
+      default: e = cudaErrorInvalidValue;
+    }
   }
   if (e != cudaSuccess || !tg.top) return e;
   LaunchTimer lt(c, KC_CRT, s);

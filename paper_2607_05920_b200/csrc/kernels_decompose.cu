@@ -16,17 +16,21 @@ namespace fhe {
 // Per residue: the low word of v = T0 + 2^8 T1 + 2^16 T2 + 2^24 T3 (< 2^49) exactly, an estimate vh <= v >> 21 that
 // is at most 20 short (the shifted-out bits of T1, T2 and T0 >> 21 < 16), and one Barrett step: qh = mulhi(vh, mu) is
 // floor(v / q) or one less (20 * 2^21 / q < 0.16 for q > 2^28), so the 32-bit remainder lies in [0, 2q).
+struct DecParams {
+  uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
+  const uint2* qmu;                             // (q_j, floor(2^53 / q_j))
+  uint32_t K;
+};
+// LAZY: the residues leave in [0, 2q) (no final conditional subtraction) -- what the forward transform's lazy butterflies
+// accept (kernels_ntt.cu); the debug entry point asks for canonical ones.
+template <bool LAZY>
 struct DecEpi {
   static constexpr int LOAD_WORDS = 40, MAX_REGS = 96;   // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
   static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;   // measured: 1 group 0.229 ms, 2 groups 0.202 ms, 4 groups 0.215 ms per C5 step
   static constexpr bool TILE_ALT = false;
   static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: the loaders' round trip bounds S1
   static constexpr int PPG = GROUPS == 1 ? 8 : 16 / GROUPS;   // primes per consume call (GROUPS = 1: two calls per chunk)
-  struct Params {
-    uint32_t* res; size_t res_outer, res_inner;   // residues of polynomial (o, i) at res + o * res_outer + i * res_inner, [K][N]
-    const uint2* qmu;                             // (q_j, floor(2^53 / q_j))
-    uint32_t K;
-  };
+  using Params = DecParams;
   const Params& p;
   const uint32_t N, etid;
   const uint2* tab;
@@ -44,7 +48,8 @@ struct DecEpi {
     const uint32_t lo = t[0] + (t[1] << 8) + (t[2] << 16) + (t[3] << 24);
     const uint32_t vh = (t[3] << 3) + (t[2] >> 5) + (t[1] >> 13);
     const uint32_t qh = __umulhi(vh, qm.y);
-    return csub(lo - qh * qm.x, qm.x);
+    const uint32_t r = lo - qh * qm.x;
+    return LAZY ? r : csub(r, qm.x);
   }
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     const uint32_t j0 = col0 / 4;
@@ -65,7 +70,7 @@ struct DecEpi {
 
 cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                              size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin,
-                             uint32_t K, uint32_t mask_bits, cudaStream_t s) {
+                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy) {
   if (nouter * ninner == 0) return cudaSuccess;
   uint32_t eff = Lin;
   if (mask_bits && (mask_bits + 31) / 32 < eff) eff = (mask_bits + 31) / 32;
@@ -78,10 +83,11 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = eff; a.mask_bits = mask_bits;
   a.B = c->d_decB; a.b_cols = c->dec_cols;
   pipe::fill_args(a, plan);
-  DecEpi::Params ep;
+  DecParams ep;
   ep.res = d_res; ep.res_outer = res_outer; ep.res_inner = res_inner; ep.qmu = c->d_qmu; ep.K = K;
   LaunchTimer lt(c, KC_DECOMPOSE, s);
-  return pipe::launch_pipe<DecEpi>(a, ep, plan.smem, c->n_sm, s);
+  return lazy ? pipe::launch_pipe<DecEpi<true>>(a, ep, plan.smem, c->n_sm, s)
+              : pipe::launch_pipe<DecEpi<false>>(a, ep, plan.smem, c->n_sm, s);
 }
 
 }  // namespace fhe

@@ -147,23 +147,22 @@ __device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
   asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
   return v;
 }
-// One batch of LR words (A columns [w0, w0 + LR)) of this thread's row: issue the loads ...
+// One batch of LR words (A columns [w0, w0 + LR)) of this thread's row, word w at q + w * N.  The common case -- every
+// word of the batch exists -- is one load and one pointer step per word; only the last batch of a row pays for the
+// per-word bound (words past `nvalid` read as zero: the padding of the contraction dimension).
 template <int LR>
-__device__ __forceinline__ void load_batch(uint32_t (&w)[LR], const uint32_t* __restrict__ p, size_t N, uint32_t w0,
-                                           uint32_t nwords) {
+__device__ __forceinline__ void load_full(uint32_t (&w)[LR], const uint32_t* __restrict__ q, size_t N) {
 #pragma unroll
-  for (int i = 0; i < LR; ++i) {
-    const uint32_t wi = w0 + i;
-    w[i] = wi < nwords ? ld_stream(p + (size_t)wi * N) : 0u;    // warp-uniform predicate
-  }
+  for (int i = 0; i < LR; ++i) { w[i] = ld_stream(q); q += N; }
 }
-// ... then mask the top word and write the batch to TMEM columns [w0, min(w0 + LR, a_cols)).
 template <int LR>
-__device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a, uint32_t w0, uint32_t a_cols,
-                                            uint32_t mask_bits) {
+__device__ __forceinline__ void load_tail(uint32_t (&w)[LR], const uint32_t* __restrict__ q, size_t N, uint32_t nvalid) {
 #pragma unroll
-  for (int i = 0; i < LR; ++i)
-    if ((mask_bits & 31) && w0 + i == (mask_bits >> 5)) w[i] &= (1u << (mask_bits & 31)) - 1u;
+  for (int i = 0; i < LR; ++i) { w[i] = (uint32_t)i < nvalid ? ld_stream(q) : 0u; q += N; }   // warp-uniform predicate
+}
+// ... then write the batch to TMEM columns [w0, min(w0 + LR, a_cols)), eight at a time.
+template <int LR>
+__device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a, uint32_t w0, uint32_t a_cols) {
 #pragma unroll
   for (int c = 0; c < LR / 8; ++c)
     if (w0 + c * 8 < a_cols) tmem_st8(taddr_a + w0 + c * 8, &w[c * 8]);
@@ -304,6 +303,8 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
     // ===== loaders =====
     const uint32_t lw = warp - EPIW, quarter = lw & 3, half = lw >> 2;
     const uint32_t row = quarter * 32 + lane;
+    // mask_bits != 0 reduces the row mod 2^mask_bits: its top word is cut (the words above are not loaded at all)
+    const uint32_t mask_w = a.mask_bits >> 5, mask_m = (a.mask_bits & 31) ? (1u << (a.mask_bits & 31)) - 1u : 0u;
     uint32_t wi = 0;
     for (uint32_t ps = 0; ps < a.npass; ++ps) {
       for (uint32_t k = 0; k < mine; ++k, ++wi) {
@@ -318,15 +319,23 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         // the warps of a lane quarter share the row: contiguous, equal ranges of its words (multiples of 8), LR at a time
         const uint32_t wph = ALT ? a_cols : ((a_cols + HALVES - 1) / HALVES + 7) / 8 * 8;
         const uint32_t w_lo = ALT ? 0 : half * wph, w_hi = w_lo + wph < a_cols ? w_lo + wph : a_cols;
+        const uint32_t lim = w_hi < a.nwords ? w_hi : a.nwords;   // words of this warp's range that exist
         for (uint32_t w0 = w_lo; w0 < w_hi; w0 += LR) {
           uint32_t w[LR];
-          load_batch<LR>(w, p, a.N, w0, w_hi < a.nwords ? w_hi : a.nwords);
+          const uint32_t* q = p + (size_t)w0 * a.N;
+          if (w0 + LR <= lim) load_full<LR>(w, q, a.N);
+          else load_tail<LR>(w, q, a.N, lim > w0 ? lim - w0 : 0u);
           if (!waited) {                                           // loads are in flight while the buffer is still being read
             mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
             tc_fence_after();
             waited = true;
           }
-          store_batch<LR>(w, taddr, w0, w_hi, a.mask_bits);
+          if (mask_m && mask_w - w0 < (uint32_t)LR) {              // the batch holding the top word of a masked input
+#pragma unroll
+            for (int i = 0; i < LR; ++i)
+              if (w0 + i == mask_w) w[i] &= mask_m;
+          }
+          store_batch<LR>(w, taddr, w0, w_hi);
         }
         if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);   // a warp without batches still keeps in step
         tmem_st_wait();

@@ -30,8 +30,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 // Blocks until the phase with the given parity has completed.  A wait that does not complete can only mean a programming
 // error in this file; it traps (launch failure) instead of hanging the device -- but by wall clock, not by poll count:
 // under compute-sanitizer, an ncu replay or time-slicing a correct kernel can poll millions of times.  The timer is read
-// once per 2^16 unsuccessful polls (each try_wait already suspends the thread for a hardware-defined interval).
+// once per 2^10 unsuccessful polls (each try_wait suspends the thread until the phase completes or the hint runs out).
 constexpr uint64_t MBAR_TIMEOUT_NS = 60ull * 1000 * 1000 * 1000;
+// upper bound of one hardware suspension of try_wait: a waiting warp sleeps instead of spending issue slots on polling
+constexpr uint32_t MBAR_SUSPEND_HINT_NS = 10u * 1000 * 1000;
 __device__ __forceinline__ uint64_t global_ns() {
   uint64_t t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -44,13 +46,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (true) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}\n"
         : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(MBAR_SUSPEND_HINT_NS)
         : "memory");
     if (done) break;
-    if ((++polls & 0xFFFFu) == 0) {
+    if ((++polls & 0x3FFu) == 0) {
       const uint64_t now = global_ns();
       if (t0 == 0) t0 = now;
       else if (now - t0 > MBAR_TIMEOUT_NS) __trap();
