@@ -150,6 +150,7 @@ struct CrtEpi {
   static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;
   static constexpr bool LOAD_ALT = false;
   static constexpr bool TILE_ALT = true;                   // two whole epilogues on alternate tiles: the epilogue bounds S5
+  static constexpr bool CHUNK_ALT = false;
   static constexpr bool RELIN = MODE == POST_CKKS_RELIN || MODE == POST_BGV_RELIN;
   static_assert(!TOP || MODE == POST_CKKS_RELIN, "the top form exists for the CKKS relin target only");
   static_assert(!RESC || MODE == POST_CKKS_RELIN, "the fused rescale is CKKS-only");

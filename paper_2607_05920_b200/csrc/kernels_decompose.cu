@@ -25,11 +25,16 @@ struct DecParams {
 // accept (kernels_ntt.cu); the debug entry point asks for canonical ones.
 template <bool LAZY>
 struct DecEpi {
-  static constexpr int LOAD_WORDS = 40, MAX_REGS = 96;   // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
-  static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;   // measured: 1 group 0.229 ms, 2 groups 0.202 ms, 4 groups 0.215 ms per C5 step
-  static constexpr bool TILE_ALT = false;
-  static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: the loaders' round trip bounds S1
-  static constexpr int PPG = GROUPS == 1 ? 8 : 16 / GROUPS;   // primes per consume call (GROUPS = 1: two calls per chunk)
+  // Measured on the role timers (C5, 28 tiles per CTA): with two groups splitting every chunk's columns, the chunks of a span
+  // were drained one after the other, the span's columns came back 1800 cycles after the MMAs had finished and the next
+  // tile's MMA chain (2100 cycles from first issue to commit) could not start before: 4500 cycles per tile with neither the
+  // tensor pipe nor the epilogue busy.  Four groups taking whole chunks side by side hand a span back within a few hundred.
+  static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
+  static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
+  static constexpr bool TILE_ALT = false, CHUNK_ALT = true;
+  static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: with four loader warps (one tile) the
+                                                         // MMA thread waited 1400 cycles per tile for its A operand
+  static constexpr int PPG = 8;                          // primes per consume call: half a chunk
   using Params = DecParams;
   const Params& p;
   const uint32_t N, etid;
@@ -51,16 +56,25 @@ struct DecEpi {
     const uint32_t r = lo - qh * qm.x;
     return LAZY ? r : csub(r, qm.x);
   }
+  // The constants are read and all residues of the call computed before the first store: a store through `out` may alias
+  // the table as far as the compiler knows, and interleaved they run one residue at a time (LDS -> chain -> STG: 65 cycles
+  // per residue measured) instead of PPG independent chains.
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     const uint32_t j0 = col0 / 4;
+    uint2 qm[PPG];
+#pragma unroll
+    for (int e = 0; e < PPG; ++e) qm[e] = tab[j0 + e];
+    uint32_t r[PPG];
+#pragma unroll
+    for (int e = 0; e < PPG; ++e) r[e] = reduce(t + 4 * e, qm[e]);
     uint32_t* o = out + (size_t)j0 * N;
     if (j0 + PPG <= p.K) {
 #pragma unroll
-      for (int e = 0; e < PPG; ++e) { *o = reduce(t + 4 * e, tab[j0 + e]); o += N; }
+      for (int e = 0; e < PPG; ++e) { *o = r[e]; o += N; }
     } else {
 #pragma unroll
       for (int e = 0; e < PPG; ++e) {
-        if (j0 + e < p.K) *o = reduce(t + 4 * e, tab[j0 + e]);
+        if (j0 + e < p.K) *o = r[e];
         o += N;
       }
     }

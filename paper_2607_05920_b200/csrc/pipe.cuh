@@ -181,6 +181,11 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 //   struct Params;                                                    by-value kernel argument
 //   static constexpr bool TILE_ALT;                                   GROUPS = 2 only: the groups are two whole epilogues on
 //                                                                     alternate tiles (own accumulator set, scratch, Epi object)
+//   static constexpr bool CHUNK_ALT;                                  the groups take WHOLE chunks in rotation (chunk c of work item
+//                                                                     wi goes to group (c + wi) mod GROUPS), so the chunks of a span
+//                                                                     are drained side by side and handed back within one chunk time:
+//                                                                     the next tile's MMAs overlap this tile's arithmetic.  For
+//                                                                     epilogues without state across chunks (S1)
 //   __device__ Epi(const Params&, const PipeArgs&, uint8_t* scratch, uint32_t etid, uint32_t grp, uint32_t bar);
 //                                                                     bar: named barrier of the threads sharing this scratch (epi_sync)
 //   __device__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0);  polynomial (o, i), first coefficient of the tile
@@ -234,8 +239,8 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
     // one arrival per WARP (its lane 0, after the warp-collective tcgen05.wait): hundreds of per-thread arrivals on one
     // mbarrier serialise in shared memory and were a quarter of the epilogue's time
     for (uint32_t i = 0; i < MAX_CHUNKS; ++i) {
-      mbar_init(&ctl->d_free[0][i], Epi::TILE_ALT ? 4 : EPIW);
-      mbar_init(&ctl->d_free[1][i], Epi::TILE_ALT ? 4 : EPIW);
+      mbar_init(&ctl->d_free[0][i], (Epi::TILE_ALT || Epi::CHUNK_ALT) ? 4 : EPIW);
+      mbar_init(&ctl->d_free[1][i], (Epi::TILE_ALT || Epi::CHUNK_ALT) ? 4 : EPIW);
     }
     mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
     fence_barrier_init();
@@ -377,6 +382,37 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
           epi.end_tile();
         }
       }
+    } else if constexpr (Epi::CHUNK_ALT) {
+      // whole chunks in rotation: every chunk of a span has its own group (GROUPS >= chunks per span), so the span's
+      // accumulator columns are back with the MMA thread one half-chunk of arithmetic after they were finished
+      Epi epi(ep, a, smem + a.epi_off, etid, grp, 1);
+      uint32_t wi = 0;
+      for (uint32_t ps = 0; ps < a.npass; ++ps) {
+        const uint32_t c0 = ps * a.cpp;
+        const uint32_t nc = a.nchunks - c0 < a.cpp ? a.nchunks - c0 : a.cpp;
+        for (uint32_t k = 0; k < mine; ++k, ++wi) {
+          const uint32_t tile = blockIdx.x + k * gridDim.x;
+          const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
+          epi.begin_tile(poly / a.inner, poly % a.inner, n0);
+          for (uint32_t c = (grp + GROUPS - wi % GROUPS) % GROUPS; c < nc; c += GROUPS) {
+            mbar_wait(&ctl->d_full[0][c / SPAN], wi & 1);          // completes once per work item; see the note on parity below
+            tc_fence_after();
+            uint32_t t[32];
+            tmem_ld32_nowait(tmem_d + c * NC + lane_off, t);
+            tmem_ld_wait();
+            epi.consume((c0 + c) * NC, t);
+            tmem_ld32_nowait(tmem_d + c * NC + 32 + lane_off, t);
+            tmem_ld_wait();
+            tc_fence_before();
+            if (lane == 0) mbar_arrive(&ctl->d_free[0][c]);        // the whole chunk has been read: hand it back
+            epi.consume((c0 + c) * NC + 32, t);
+          }
+          epi.end_tile();
+        }
+      }
+      // Parity: a group waits on d_full[span] only in the work items in which it owns a chunk of that span.  The barrier
+      // cannot run ahead of it by a whole phase: the span's next MMAs need every chunk of the span handed back, the
+      // group's own included.
     } else {
     Epi epi(ep, a, smem + a.epi_off, etid, grp, 1);
     uint32_t wi = 0;
