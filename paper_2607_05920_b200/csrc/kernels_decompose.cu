@@ -43,18 +43,19 @@ struct DecEpi {
   __device__ DecEpi(const Params& p_, const pipe::PipeArgs& a, uint8_t* sm, uint32_t etid_, uint32_t grp, uint32_t bar)
       : p(p_), N(a.N), etid(etid_), tab(reinterpret_cast<const uint2*>(sm)) {
     uint2* w = reinterpret_cast<uint2*>(sm);
-    for (uint32_t j = grp * 128 + etid; j < a.nchunks * 16; j += 128 * GROUPS) w[j] = j < p.K ? __ldg(p.qmu + j) : make_uint2(1u, 0u);
+    for (uint32_t j = grp * 128 + etid; j < a.nchunks * 16; j += 128 * GROUPS) w[j] = j < p.K ? make_uint2(0u - __ldg(p.qmu + j).x, __ldg(p.qmu + j).y) : make_uint2(0u, 0u);
     pipe::epi_sync(bar, 128 * GROUPS);
   }
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.res + (size_t)o * p.res_outer + (size_t)i * p.res_inner + n0 + etid;
   }
+  // qm = (2^32 - q, floor(2^53 / q)): with -q in the table the remainder is one multiply-add, lo + qh * (-q)
   __device__ __forceinline__ uint32_t reduce(const uint32_t* t, const uint2 qm) const {
     const uint32_t lo = t[0] + (t[1] << 8) + (t[2] << 16) + (t[3] << 24);
     const uint32_t vh = (t[3] << 3) + (t[2] >> 5) + (t[1] >> 13);
     const uint32_t qh = __umulhi(vh, qm.y);
-    const uint32_t r = lo - qh * qm.x;
-    return LAZY ? r : csub(r, qm.x);
+    const uint32_t r = lo + qh * qm.x;
+    return LAZY ? r : csub(r, 0u - qm.x);
   }
   // The constants are read and all residues of the call computed before the first store: a store through `out` may alias
   // the table as far as the compiler knows, and interleaved they run one residue at a time (LDS -> chain -> STG: 65 cycles

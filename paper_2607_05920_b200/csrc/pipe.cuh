@@ -41,6 +41,7 @@ struct Ctrl {
   uint64_t a_full[MAX_A], a_free[MAX_A];      // A buffer written (one arrival per loader warp) / consumed (MMA commit)
   uint64_t d_full[2][MAX_SPANS];              // [accumulator set] the span's accumulators finished (MMA commit)
   uint64_t d_free[2][MAX_CHUNKS];                // the chunk's accumulators are in registers (one arrival per epilogue warp)
+  uint64_t g_full[MAX_SPANS][4];              // CHUNK_ALT: the span finished, barrier [wi mod 4] for work item wi
   uint64_t b_full, mma_done;                  // B of the pass landed (bulk copies) / every MMA of the pass finished
   uint32_t tmem_base;
 };
@@ -235,7 +236,10 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
 
   if (tid == 0) {
     for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], ALT ? 4 : LOAD_WARPS); mbar_init(&ctl->a_free[i], 1); }
-    for (uint32_t i = 0; i < MAX_SPANS; ++i) { mbar_init(&ctl->d_full[0][i], 1); mbar_init(&ctl->d_full[1][i], 1); }
+    for (uint32_t i = 0; i < MAX_SPANS; ++i) {
+      mbar_init(&ctl->d_full[0][i], 1); mbar_init(&ctl->d_full[1][i], 1);
+      for (uint32_t g = 0; g < 4; ++g) mbar_init(&ctl->g_full[i][g], 1);
+    }
     // one arrival per WARP (its lane 0, after the warp-collective tcgen05.wait): hundreds of per-thread arrivals on one
     // mbarrier serialise in shared memory and were a quarter of the epilogue's time
     for (uint32_t i = 0; i < MAX_CHUNKS; ++i) {
@@ -297,7 +301,11 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
               const uint64_t db = smem_desc(baddr + ks * 2 * lbo, lbo, 128);
               mma_i8_ts(tmem_d + (dset * a.cpp + cs) * NC, tmem_a + abuf * a_cols + ks * (KSTEP / 4), db, idesc, ks > 0);
             }
-            mma_commit(&ctl->d_full[dset][sp]);
+            if constexpr (Epi::CHUNK_ALT) {
+              mma_commit(&ctl->g_full[sp][wi % GROUPS]);
+            } else {
+              mma_commit(&ctl->d_full[dset][sp]);
+            }
           }
           mma_commit(&ctl->a_free[abuf]);
         }
@@ -383,8 +391,13 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
         }
       }
     } else if constexpr (Epi::CHUNK_ALT) {
-      // whole chunks in rotation: every chunk of a span has its own group (GROUPS >= chunks per span), so the span's
-      // accumulator columns are back with the MMA thread one half-chunk of arithmetic after they were finished
+      // Whole chunks in rotation: chunk c of work item wi belongs to group (c + wi) mod GROUPS, so the chunks of a span sit
+      // with several groups at once and the span's accumulator columns are back with the MMA thread within one half chunk
+      // of arithmetic.  mbarrier waits only see the phase parity, so a waiter must see every completion of its barrier:
+      // "span finished" is signalled on barrier [wi mod GROUPS], and since ownership depends on wi only through wi mod
+      // GROUPS, a group either waits on every completion of a given barrier or on none (parity (wi / GROUPS) & 1).  (With
+      // one barrier, a group without a chunk in some work item took the completion of phase wi - 1 for that of wi + 1.)
+      static_assert(GROUPS == 4 && SPAN == 4, "rotation laid out for four groups and spans of four chunks");
       Epi epi(ep, a, smem + a.epi_off, etid, grp, 1);
       uint32_t wi = 0;
       for (uint32_t ps = 0; ps < a.npass; ++ps) {
@@ -394,8 +407,10 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
           const uint32_t tile = blockIdx.x + k * gridDim.x;
           const uint32_t poly = tile / tpp, n0 = (tile % tpp) * TILE_M;
           epi.begin_tile(poly / a.inner, poly % a.inner, n0);
+          // spans hold GROUPS chunks, so a group owns at most one chunk per span
           for (uint32_t c = (grp + GROUPS - wi % GROUPS) % GROUPS; c < nc; c += GROUPS) {
-            mbar_wait(&ctl->d_full[0][c / SPAN], wi & 1);          // completes once per work item; see the note on parity below
+            const uint32_t sp = c / SPAN;
+            mbar_wait(&ctl->g_full[sp][wi % GROUPS], (wi / GROUPS) & 1);
             tc_fence_after();
             uint32_t t[32];
             tmem_ld32_nowait(tmem_d + c * NC + lane_off, t);
@@ -410,9 +425,6 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
           epi.end_tile();
         }
       }
-      // Parity: a group waits on d_full[span] only in the work items in which it owns a chunk of that span.  The barrier
-      // cannot run ahead of it by a whole phase: the span's next MMAs need every chunk of the span handed back, the
-      // group's own included.
     } else {
     Epi epi(ep, a, smem + a.epi_off, etid, grp, 1);
     uint32_t wi = 0;
