@@ -185,6 +185,15 @@ fhe_status fhe_add_plain(fhe_ctx* ctx, uint32_t* d_out2, const uint32_t* d_ct, c
                          uint32_t group, void* stream);
 fhe_status fhe_mult_scalar(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, void* stream);
 
+/* ---- NEXT-4: BGV modulus switching (named only; reading DESIGN.md 3, A20) ---------------
+ * Every coefficient c in [0, Q) of `npoly` polynomials [L][N] becomes c' in [0, Q'), Q' = the modulus of the same construction
+ * above 2^new_logQ (least odd integer that is 1 mod t):  x = c Q',  r = x mod Q centred,  k = (-r Q^-1) mod t centred,
+ * c' = ((x - r)/Q - k) mod Q'  -- the integer nearest to c Q'/Q that keeps the plaintext exact, the noise shrinks by Q'/Q.
+ * Output in the same L-limb stride (limbs above Q' are zero); a ciphertext at the lower level is then used with a context
+ * created for logQ = new_logQ.  In place allowed.  BGV only (FHE_ERR_UNSUPPORTED on CKKS, and when logQ < 96 or
+ * new_logQ < 34, where the kernel's shortcuts for Q = 2^logQ + e do not hold); 34 <= new_logQ < logQ. */
+fhe_status fhe_modswitch(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logQ, uint32_t npoly, void* stream);
+
 /* ---- debug / unit-parity entry points (same kernels as the hot path, one step at a time) ------------------- */
 
 /* Host copies of the first `count` NTT primes and the primitive 2N-th roots psi_j the tables were built from. */

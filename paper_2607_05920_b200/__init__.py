@@ -25,7 +25,7 @@ EXPORTS = [
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
     "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_mul_monomial", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
-    "fhe_add_plain", "fhe_mult_scalar",
+    "fhe_add_plain", "fhe_mult_scalar", "fhe_modswitch",
 ]
 
 
@@ -104,6 +104,8 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_add_plain.restype = c_int
     lib.fhe_mult_scalar.argtypes = [vp, vp, vp, ctypes.c_int32, c_uint32, vp]
     lib.fhe_mult_scalar.restype = c_int
+    lib.fhe_modswitch.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
+    lib.fhe_modswitch.restype = c_int
     lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
     lib.fhe_debug_crt_ambiguity.restype = c_int
     lib.fhe_debug_int_peak.argtypes = [vp, c_int, POINTER(ctypes.c_double), vp]
@@ -358,6 +360,10 @@ class Context:
 
     def fhe_moddown(self, a, new_logq: int, out=None):
         return self._elem(self._lib.fhe_moddown, a, None, out, extra=(new_logq,))
+
+    # ---- NEXT-4: BGV modulus switch ----
+    def fhe_modswitch(self, a, new_logQ: int, out=None):
+        return self._elem(self._lib.fhe_modswitch, a, None, out, extra=(new_logQ,))
 
     # ---- NEXT-3, constants ----
     def fhe_add_plain(self, ct, pt, group: int = 1, out=None):

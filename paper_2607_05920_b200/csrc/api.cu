@@ -378,6 +378,22 @@ fhe_status fhe_moddown(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint
   return elem_call(ctx, 3, d_out, d_in, nullptr, npoly, new_logq, stream);
 }
 
+// ---- NEXT-4: BGV modulus switch ----------------------------------------------------------------------------------------------
+fhe_status fhe_modswitch(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logQ, uint32_t npoly, void* stream) {
+  if (!ctx) return FHE_ERR_ARG;
+  Context* c = C(ctx);
+  if (fhe_status ds = check_device(c)) return ds;
+  if (c->t == 0) return err(c, FHE_ERR_UNSUPPORTED, "modswitch is BGV-only (CKKS: fhe_rescale / fhe_moddown)");
+  if (npoly == 0) return FHE_OK;
+  if (!d_out || !d_in) return err(c, FHE_ERR_ARG, "NULL pointer");
+  if (misaligned(d_out, 16) || misaligned(d_in, 16)) return err(c, FHE_ERR_ARG, "misaligned pointer");
+  if (new_logQ >= c->logQ) return err(c, FHE_ERR_ARG, "new_logQ must be below logQ");
+  if (c->logQ < 96 || new_logQ < 34) return err(c, FHE_ERR_UNSUPPORTED, "modswitch needs logQ >= 96 and new_logQ >= 34");
+  const uint64_t e = modulus_offset(c->logQ, c->t), e2 = modulus_offset(new_logQ, c->t);   // both < 2 t < 2^32
+  CK(launch_modswitch(c, d_out, d_in, new_logQ, (uint32_t)e, (uint32_t)e2, npoly, (cudaStream_t)stream), "modswitch");
+  return FHE_OK;
+}
+
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);

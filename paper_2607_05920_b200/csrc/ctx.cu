@@ -60,16 +60,20 @@ static cudaError_t upload(Context* c, T** dptr, const std::vector<T>& h) {
   return e;
 }
 
-// modulus 2^log (t == 0) or the least odd integer > 2^log that is 1 mod t
-static BigU make_modulus(uint32_t log, uint64_t t) {
-  BigU m = BigU::pow2(log);
-  if (t == 0) return m;
+// modulus 2^log (t == 0) or the least odd integer > 2^log that is 1 mod t: 2^log + modulus_offset(log, t)
+uint64_t modulus_offset(uint32_t log, uint64_t t) {
+  if (t == 0) return 0;
   uint32_t tt = (uint32_t)t;
   uint32_t two = powmod(2, log, tt);
   uint32_t c0 = (uint32_t)(((uint64_t)1 + tt - two) % tt);   // (1 - 2^log) mod t
   uint64_t c = c0 == 0 ? tt : c0;
   if ((c & 1) == 0) c += tt;                                  // t odd: flips parity
-  m.add(BigU(c));
+  return c;
+}
+static BigU make_modulus(uint32_t log, uint64_t t) {
+  BigU m = BigU::pow2(log);
+  if (t == 0) return m;
+  m.add(BigU(modulus_offset(log, t)));
   return m;
 }
 

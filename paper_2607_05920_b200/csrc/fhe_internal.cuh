@@ -194,6 +194,11 @@ cudaError_t launch_monomial(Context* c, uint32_t* d_out, const uint32_t* d_in, u
 cudaError_t launch_add_plain(Context* c, uint32_t* d_out, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
                              uint32_t group, cudaStream_t s);
 cudaError_t launch_mult_scalar(Context* c, uint32_t* d_out, const uint32_t* d_in, int32_t k, uint32_t npoly, cudaStream_t s);
+// BGV modulus switch from Q = 2^logQ + e to Q' = 2^new_logQ + e2 (kernels_elem.cu), per coefficient of npoly polynomials [L][N]
+cudaError_t launch_modswitch(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logQ, uint32_t e, uint32_t e2,
+                             uint32_t npoly, cudaStream_t s);
+// offset of the modulus above its power of two: 0 (t == 0), else the least odd c with 2^log + c = 1 (mod t)   (ctx.cu)
+uint64_t modulus_offset(uint32_t log, uint64_t t);
 cudaError_t launch_rescale(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t npoly, uint32_t p_bits,
                            cudaStream_t s);
 

@@ -299,6 +299,161 @@ mult_scalar_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, 
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// NEXT-4: BGV modulus switch (named only; reading DESIGN.md 3, A20).  Q = 2^logQ + e, Q' = 2^b + e'
+// (both the least odd integer above the power of two that is 1 mod t, so e, e' < 2 t < 2^32).  Per coefficient c in [0, Q):
+//     x = c Q',   r = x mod Q centred,   k = (-r Q^-1) mod t centred = (-r) mod t centred (Q = 1 mod t),
+//     c' = ((x - r)/Q - k) mod Q'.
+// The division by Q uses its shape instead of a general Barrett step:  x = h0 2^logQ + xl  gives  x = h0 Q + (xl - h0 e),
+// and when z = xl - h0 e is negative, y = -z = j 2^logQ + yl = j Q + (yl - j e) moves j (< 2^35) or j + 1 more multiples of Q
+// across; |j e| < 2^67 < Q (logQ >= 96 is required), so the remainder lands in [0, Q) without a loop.
+// One thread per coefficient with the numbers in local arrays: a level drop happens once per multiplication depth, the
+// kernel needs no tuning beyond coalesced limb accesses.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr uint32_t MS_H = ELEM_MAX_LIMBS + 2, MS_X = 2 * ELEM_MAX_LIMBS + 6;
+
+// acc * 2^32 + limb  mod t   (acc < t < 2^31; mu = floor(2^64 / t))
+__device__ __forceinline__ uint32_t horner_mod(uint32_t acc, uint32_t limb, uint32_t t, uint64_t mu) {
+  const uint64_t v = ((uint64_t)acc << 32) | limb;
+  uint64_t r = v - __umul64hi(v, mu) * t;                           // quotient estimate at most 1 short: r in [0, 2 t)
+  if (r >= t) r -= t;
+  return (uint32_t)r;
+}
+
+__global__ void __launch_bounds__(128)
+modswitch_bgv_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, uint32_t N, uint32_t L, uint32_t logQ,
+                     uint32_t e, uint32_t b, uint32_t e2, uint32_t t, uint64_t mu_t) {
+  const uint32_t bpp = N / 128;
+  const uint32_t poly = blockIdx.x / bpp, n = (blockIdx.x % bpp) * 128 + threadIdx.x;
+  const size_t base = (size_t)poly * L * N + n;
+  const uint32_t wq = logQ >> 5, bq = logQ & 31, Lq = (logQ + 31) / 32;     // Q's power of two: limb wq, bit bq
+  const uint32_t ws = b >> 5, bs = b & 31, L2 = b / 32 + 1;                 // Q' has b + 1 bits
+  const uint32_t nx = L + L2 + 2;
+  uint32_t x[MS_X], h[MS_H];
+  for (uint32_t l = 0; l < nx; ++l) x[l] = 0;
+  // ---- x = c e' + (c << b) ----
+  {
+    uint32_t carry = 0, cprev = 0, carry2 = 0;
+    for (uint32_t l = 0; l <= L; ++l) {
+      const uint32_t cl = l < L ? in[base + (size_t)l * N] : 0u;
+      const uint64_t pr = (uint64_t)cl * e2 + carry + x[l];       // x[l] may already hold a limb of the shifted copy
+      x[l] = (uint32_t)pr; carry = (uint32_t)(pr >> 32);
+      const uint32_t v = bs ? (cl << bs) | (cprev >> (32 - bs)) : cl;
+      cprev = cl;
+      const uint64_t s = (uint64_t)x[l + ws] + v + carry2;        // ws >= 1: never the limb the product has just written
+      x[l + ws] = (uint32_t)s; carry2 = (uint32_t)(s >> 32);
+    }
+    for (uint32_t l = L + 1; carry && l < nx; ++l) { const uint64_t s = (uint64_t)x[l] + carry; x[l] = (uint32_t)s; carry = (uint32_t)(s >> 32); }
+    for (uint32_t l = L + ws + 1; carry2 && l < nx; ++l) { const uint64_t s = (uint64_t)x[l] + carry2; x[l] = (uint32_t)s; carry2 = (uint32_t)(s >> 32); }
+  }
+  // ---- h0 = x >> logQ (b + 2 bits), xl = x mod 2^logQ (left in x[0 .. Lq)) ----
+  const uint32_t nh = (b + 2) / 32 + 1;
+  for (uint32_t i = 0; i < nh; ++i) {
+    const uint32_t lo = wq + i < nx ? x[wq + i] : 0u, hi = wq + i + 1 < nx ? x[wq + i + 1] : 0u;
+    h[i] = bq ? (lo >> bq) | (hi << (32 - bq)) : lo;
+  }
+  h[nh] = 0;
+  if (bq) x[Lq - 1] &= (1u << bq) - 1u;
+  const uint32_t nz = (Lq > nh + 1 ? Lq : nh + 1) + 1;             // limbs of z = xl - h0 e (signed)
+  for (uint32_t l = Lq; l < nz; ++l) x[l] = 0;
+  uint32_t borrow = 0;
+  {
+    uint32_t mc = 0;
+    for (uint32_t l = 0; l < nz; ++l) {
+      const uint64_t pr = (l < nh ? (uint64_t)h[l] * e : 0ull) + mc;
+      const uint32_t sub = (uint32_t)pr; mc = (uint32_t)(pr >> 32);
+      const uint32_t v = x[l], d = v - sub, d2 = d - borrow;
+      borrow = (v < sub) | (d < borrow);
+      x[l] = d2;
+    }
+  }
+  // ---- remainder in [0, Q) (x[0 .. Lq]) and quotient (h) ----
+  uint64_t hdec = 0;                                               // what comes off h0
+  if (borrow) {
+    uint32_t c1 = 1;                                               // y = -z
+    for (uint32_t l = 0; l < nz; ++l) { const uint64_t s = (uint64_t)(~x[l]) + c1; x[l] = (uint32_t)s; c1 = (uint32_t)(s >> 32); }
+    const uint32_t j0 = wq < nz ? x[wq] : 0u, j1 = wq + 1 < nz ? x[wq + 1] : 0u, j2 = wq + 2 < nz ? x[wq + 2] : 0u;
+    const uint64_t j = bq ? ((uint64_t)(j0 >> bq) | ((uint64_t)j1 << (32 - bq)) | ((uint64_t)j2 << (64 - bq))) : ((uint64_t)j0 | ((uint64_t)j1 << 32));
+    if (bq) x[Lq - 1] &= (1u << bq) - 1u;                          // yl
+    for (uint32_t l = Lq; l <= Lq; ++l) x[l] = 0;
+    // w = yl - j e over Lq + 1 limbs (j e < 2^67)
+    const uint64_t p0 = (uint64_t)(uint32_t)j * e, p1 = (j >> 32) * e + (p0 >> 32);
+    const uint32_t je[3] = {(uint32_t)p0, (uint32_t)p1, (uint32_t)(p1 >> 32)};
+    uint32_t bw = 0, any = 0;
+    for (uint32_t l = 0; l <= Lq; ++l) {
+      const uint32_t sub = l < 3 ? je[l] : 0u, v = x[l], d = v - sub, d2 = d - bw;
+      bw = (v < sub) | (d < bw);
+      x[l] = d2; any |= d2;
+    }
+    if (!bw && any) {                                              // w > 0: one more multiple, remainder Q - w
+      hdec = j + 1;
+      uint32_t b2 = 0;
+      for (uint32_t l = 0; l <= Lq; ++l) {
+        const uint32_t ql = (l == 0 ? e : 0u) + (l == wq ? 1u << bq : 0u), v = x[l], d = ql - v, d2 = d - b2;
+        b2 = (ql < v) | (d < b2);
+        x[l] = d2;
+      }
+    } else {                                                       // w <= 0: remainder -w
+      hdec = j;
+      uint32_t c2 = 1;
+      for (uint32_t l = 0; l <= Lq; ++l) { const uint64_t s = (uint64_t)(~x[l]) + c2; x[l] = (uint32_t)s; c2 = (uint32_t)(s >> 32); }
+    }
+  }
+  // ---- centre the remainder: r = rem - Q when 2 rem > Q (Q odd: no tie) ----
+  bool negr;
+  {
+    int cmp = 0;
+    for (uint32_t l = Lq + 1; l-- > 0 && cmp == 0;) {
+      const uint32_t two = (x[l] << 1) | (l ? x[l - 1] >> 31 : 0u);
+      const uint32_t ql = (l == 0 ? e : 0u) + (l == wq ? 1u << bq : 0u);
+      if (two != ql) cmp = two > ql ? 1 : -1;
+    }
+    // bit 32 (Lq + 1) of 2 rem: rem < Q < 2^(32 Lq + 32 - 1) so x[Lq] < 2^31 and nothing is shifted out
+    negr = cmp > 0;
+  }
+  uint32_t rt = 0;                                                 // rem mod t, then r mod t
+  for (uint32_t l = Lq + 1; l-- > 0;) rt = horner_mod(rt, x[l], t, mu_t);
+  if (negr) rt = rt ? rt - 1 : t - 1;                              // r = rem - Q, Q = 1 (mod t)
+  const uint32_t k = rt ? t - rt : 0u;                             // (-r) mod t
+  const bool kneg = k > t / 2;                                     // centred: k - t
+  const uint32_t kmag = kneg ? t - k : k;
+  // ---- v = h0 - hdec + [negr] - k_centred, then mod Q' ----
+  int64_t cc = (int64_t)(negr ? 1 : 0) + (kneg ? (int64_t)kmag : -(int64_t)kmag);
+  {
+    uint32_t bw = 0;
+    for (uint32_t l = 0; l <= nh; ++l) {                           // h -= hdec (hdec <= h0)
+      const uint32_t sub = l == 0 ? (uint32_t)hdec : l == 1 ? (uint32_t)(hdec >> 32) : 0u, v = h[l], d = v - sub, d2 = d - bw;
+      bw = (v < sub) | (d < bw);
+      h[l] = d2;
+    }
+    for (uint32_t l = 0; l <= nh; ++l) { const int64_t s = (int64_t)h[l] + cc; h[l] = (uint32_t)s; cc = s >> 32; }
+  }
+  auto q2limb = [&](uint32_t l) { return (l == 0 ? e2 : 0u) + (l == ws ? 1u << bs : 0u); };
+  if (cc < 0) {                                                    // negative: + Q'
+    uint32_t c3 = 0;
+    for (uint32_t l = 0; l <= nh; ++l) { const uint64_t s = (uint64_t)h[l] + q2limb(l) + c3; h[l] = (uint32_t)s; c3 = (uint32_t)(s >> 32); }
+  } else {
+    bool ge = true;                                                // v >= Q' ?
+    for (uint32_t l = nh + 1; l-- > 0;) { const uint32_t ql = q2limb(l); if (h[l] != ql) { ge = h[l] > ql; break; } }
+    if (ge) {
+      uint32_t b3 = 0;
+      for (uint32_t l = 0; l <= nh; ++l) { const uint32_t ql = q2limb(l), v = h[l], d = v - ql, d2 = d - b3; b3 = (v < ql) | (d < b3); h[l] = d2; }
+    }
+  }
+  for (uint32_t l = 0; l < L; ++l) out[base + (size_t)l * N] = l <= nh ? h[l] : 0u;
+}
+
+cudaError_t launch_modswitch(Context* c, uint32_t* d_out, const uint32_t* d_in, uint32_t new_logQ, uint32_t e, uint32_t e2,
+                             uint32_t npoly, cudaStream_t s) {
+  if (!npoly) return cudaSuccess;
+  if (c->L > ELEM_MAX_LIMBS) return cudaErrorInvalidValue;
+  const uint32_t t = (uint32_t)c->t;
+  const uint64_t mu_t = ~0ull / t;                                 // floor((2^64 - 1) / t): at most 1 below floor(2^64 / t)
+  LaunchTimer lt(c, KC_RESCALE, s);
+  modswitch_bgv_kernel<<<(c->N / 128) * npoly, 128, 0, s>>>(d_out, d_in, c->N, c->L, c->logQ, e, new_logQ, e2, t, mu_t);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_add_plain(Context* c, uint32_t* d_out, const uint32_t* d_ct, const uint32_t* d_pt, uint32_t batch,
                              uint32_t group, cudaStream_t s) {
   if (!batch) return cudaSuccess;

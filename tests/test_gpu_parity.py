@@ -730,3 +730,87 @@ def test_next3_mult_scalar_matches_the_oracle(N, logQ, t):
     assert torch.equal(ctx.fhe_add(ctx.fhe_mult_scalar(keep, 2), keep), ctx.fhe_mult_scalar(keep, 3))
     with pytest.raises((fhe.FheError, ValueError)):
         ctx.fhe_mult_scalar(keep, -2 ** 31)
+
+
+# ---- NEXT-4: BGV modulus switching -------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,logQ,t,news", [(256, 100, 257, (99, 92, 60, 34)), (1024, 437, 65537, (436, 429, 405, 300, 34)),
+                                           (256, 128, 3, (127, 96, 64)), (256, 160, 786433, (159, 140, 97, 40))])
+def test_next4_modswitch_matches_the_oracle(N, logQ, t, news):
+    """Every coefficient against scheme.modswitch_bgv, over drops of one bit (the quotient correction moves many multiples
+    of Q), a few bits, a limb, many limbs; the ends of the range, Q/2 and its neighbours (the centring of r), in place."""
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logQ, t)
+    ctx = fhe.Context(N, logQ, logQ, t)
+    Q = prm.Q
+    rnd = np.random.default_rng(N + logQ + t % 1000)
+    def rand_poly():
+        p = [int.from_bytes(rnd.bytes((Q.bit_length() + 7) // 8 + 8), "little") % Q for _ in range(N)]
+        p[:8] = [0, 1, Q - 1, Q - 2, Q // 2, Q // 2 + 1, Q // 2 - 1, (1 << logQ) - 1]
+        return p
+    ct = (rand_poly(), rand_poly())
+    d = polys_to_tensor([list(ct)], ctx.L)
+    for new_logQ in news:
+        want = scheme.modswitch_bgv(prm, ct, new_logQ)
+        got = tensor_to_polys(ctx.fhe_modswitch(d, new_logQ))[0]
+        assert got == [list(p) for p in want], new_logQ
+    keep = d.clone()
+    ctx.fhe_modswitch(d, news[-1], out=d)
+    assert torch.equal(d, ctx.fhe_modswitch(keep, news[-1]))
+    with pytest.raises(fhe.FheError):
+        ctx.fhe_modswitch(keep, logQ)
+    with pytest.raises(fhe.FheError):
+        fhe.Context(256, 128, 128).fhe_modswitch(torch.zeros((1, 2, 4, 256), dtype=torch.int32, device="cuda"), 64)   # CKKS
+
+
+def test_next4_bgv_depth_two_circuit_across_a_modulus_switch():
+    """(m1 m2) m3 on BGV at the C4 parameter shape (t = 65537, logQ = 437): multiply + relinearise at Q, switch the product
+    and a fresh ciphertext down to Q' (logQ' = 300) with fhe_modswitch, multiply + relinearise again with a context and a
+    key for Q'.  Every ciphertext equals the oracle's limb for limb; the final decryption is exact mod t."""
+    fhe = _lib()
+    N, logQ, new_logQ, t = 1 << 10, 437, 300, 65537
+    prm, s, evk, cts1, cts2, ms = _bgv_setup(N, logQ, logQ, t, 2, seed=9)
+    hi = fhe.Context(N, logQ, logQ, t)
+    hi.fhe_set_evk(polys_to_tensor(list(evk), hi.L_PQ))
+    prod = hi.fhe_mult_relin_rescale(polys_to_tensor([cts1[0]], hi.L), polys_to_tensor([cts2[0]], hi.L), 0)
+    want_prod = scheme.relinearize(prm, scheme.he_mult(prm, cts1[0], cts2[0]), evk)
+    assert tensor_to_polys(prod)[0] == [list(p) for p in want_prod]
+    low = hi.fhe_modswitch(prod, new_logQ)
+    third = hi.fhe_modswitch(polys_to_tensor([cts1[1]], hi.L), new_logQ)
+    want_low, want_third = scheme.modswitch_bgv(prm, want_prod, new_logQ), scheme.modswitch_bgv(prm, cts1[1], new_logQ)
+    assert tensor_to_polys(low)[0] == [list(p) for p in want_low]
+    assert tensor_to_polys(third)[0] == [list(p) for p in want_third]
+    prm2 = scheme.Params(N, new_logQ, new_logQ, t)
+    assert harness.decrypt_bgv(want_low, s, prm2) == ring.pm(ms[0][0], ms[0][1], t)
+    # key for the lower level: same secret, evk mod P'Q'
+    g2 = synth.rng(99)
+    e2 = synth.gaussian_error(g2, N)
+    a2 = synth.uniform_big(g2, N, (prm2.PQ - 1).bit_length() - 1)
+    s2 = ring.pm([v % prm2.PQ for v in s], [v % prm2.PQ for v in s], prm2.PQ)
+    a_s = harness.pm_secret(a2, s, prm2.PQ)
+    evk2 = ([(-x + t * int(e) + prm2.P * y) % prm2.PQ for x, e, y in zip(a_s, e2, s2)], a2)
+    lo = fhe.Context(N, new_logQ, new_logQ, t)
+    assert lo.modulus(0) == prm2.Q
+    lo.fhe_set_evk(polys_to_tensor(list(evk2), lo.L_PQ))
+    a = low[..., : lo.L, :].contiguous()
+    b = third[..., : lo.L, :].contiguous()
+    out = lo.fhe_mult_relin_rescale(a, b, 0)
+    want = scheme.relinearize(prm2, scheme.he_mult(prm2, want_low, want_third), evk2)
+    got = tensor_to_polys(out)[0]
+    assert got == [list(p) for p in want]
+    assert harness.decrypt_bgv(tuple(got), s, prm2) == ring.pm(ring.pm(ms[0][0], ms[0][1], t), ms[1][0], t)
+
+
+def test_repeated_runs_are_bit_identical():
+    """The pipeline kernels hand tiles between warp roles through mbarriers, tensor memory and shared memory; a race
+    would show as run-to-run differences.  (compute-sanitizer is closed on this pool.)  40 runs of the fused call on a
+    shape with several tiles per CTA and ragged last tiles must give one and the same result."""
+    fhe = _lib()
+    N, logQ, logP, B, p = 1 << 13, 218, 250, 5, 40
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(31337)
+    ct1 = limbs_np_to_tensor(synth.uniform_limbs(g, (B, 2), N, logQ))
+    ct2 = limbs_np_to_tensor(synth.uniform_limbs(g, (B, 2), N, logQ))
+    ctx.fhe_set_evk(limbs_np_to_tensor(synth.uniform_limbs(g, (2,), N, logQ + logP)))
+    ref = ctx.fhe_mult_relin_rescale(ct1, ct2, p).clone()
+    for _ in range(40):
+        assert torch.equal(ctx.fhe_mult_relin_rescale(ct1, ct2, p), ref)
