@@ -25,7 +25,7 @@ EXPORTS = [
     "fhe_mult_relin_rescale_host", "fhe_debug_primes", "fhe_debug_decompose", "fhe_debug_ntt",
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
     "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_mul_monomial", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
-    "fhe_add_plain", "fhe_mult_scalar", "fhe_modswitch",
+    "fhe_add_plain", "fhe_mult_scalar", "fhe_modswitch", "fhe_debug_force_pipeline",
 ]
 
 
@@ -106,6 +106,8 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_mult_scalar.restype = c_int
     lib.fhe_modswitch.argtypes = [vp, vp, vp, c_uint32, c_uint32, vp]
     lib.fhe_modswitch.restype = c_int
+    lib.fhe_debug_force_pipeline.argtypes = [vp, c_int]
+    lib.fhe_debug_force_pipeline.restype = c_int
     lib.fhe_debug_crt_ambiguity.argtypes = [vp, c_uint32]
     lib.fhe_debug_crt_ambiguity.restype = c_int
     lib.fhe_debug_int_peak.argtypes = [vp, c_int, POINTER(ctypes.c_double), vp]
@@ -208,6 +210,9 @@ class Context:
         return int(self._lib.fhe_debug_launch_count(self._h))
 
     KERNEL_CLASSES = ("decompose", "ntt_fwd", "ntt_inv", "pointwise", "crt", "rescale")
+
+    def fhe_debug_force_pipeline(self, on: bool):
+        self._check(self._lib.fhe_debug_force_pipeline(self._h, 1 if on else 0))
 
     def fhe_debug_crt_ambiguity(self, bits: int):
         self._check(self._lib.fhe_debug_crt_ambiguity(self._h, bits))

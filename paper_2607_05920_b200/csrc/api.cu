@@ -394,6 +394,12 @@ fhe_status fhe_modswitch(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, ui
   return FHE_OK;
 }
 
+fhe_status fhe_debug_force_pipeline(fhe_ctx* ctx, int on) {
+  if (!ctx) return FHE_ERR_ARG;
+  C(ctx)->force_pipe = on != 0;
+  return FHE_OK;
+}
+
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits) {
   if (!ctx) return FHE_ERR_ARG;
   Context* c = C(ctx);

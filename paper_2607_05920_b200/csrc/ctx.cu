@@ -151,6 +151,16 @@ static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2
   cudaError_t e = upload(c, &tg.d_B, img);
   if (e != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
+  if (pow2 && K <= SMALL_K && tg.Lraw <= SMALL_LIMBS) {                 // limb form of the constants for the CUDA-core CRT
+    std::vector<uint32_t> wl((size_t)(K + 1) * tg.Lraw, 0u);
+    for (uint32_t i = 0; i < K; ++i) {
+      BigU Mi = M;
+      Mi.divmod_small(c->h_q[i]);
+      Mi.low_bits(32 * tg.Lraw).to_limbs(wl.data() + (size_t)i * tg.Lraw, tg.Lraw);
+    }
+    for (uint32_t l = 0; l < tg.Lraw; ++l) wl[(size_t)K * tg.Lraw + l] = negM[l];
+    if ((e = upload(c, &tg.d_Wlimbs, wl)) != cudaSuccess) return e;
+  }
   return upload(c, &tg.d_scale, scale);
 }
 
@@ -300,6 +310,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   // ---- per-prime constants and twiddle tables ---------------------------------------------------------------------
   std::vector<uint32_t> qn(Kmax);
   std::vector<uint2> qmu(Kmax);
+  std::vector<uint4> qsmall(Kmax);
   std::vector<uint2> scale_plain(Kmax);
   // decompose constants: widest input is the evk (L_PQ limbs) or what fhe_debug_decompose may pass (MAX_LIMBS_IN)
   c->dec_KBimg = (4 * MAX_LIMBS_IN + 31) / 32 * 32;
@@ -314,6 +325,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     for (int it = 0; it < 5; ++it) inv *= 2u - q * inv;
     qn[j] = 0u - inv;
     qmu[j] = make_uint2(q, (uint32_t)((1ull << 53) / q));
+    qsmall[j] = make_uint4(q, (uint32_t)((1ull << 32) % q), (uint32_t)((1ull << 61) / q), (uint32_t)((1ull << ALPHA_SHIFT) / q));
     uint32_t psi = 0;
     for (uint32_t g = 2; g < 2000 && !psi; ++g) {
       uint32_t cand = powmod(g, (q - 1) / (2 * N), q);
@@ -341,7 +353,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
 #define UP(dst, vec)                                                                                   \
   if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
-  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
+  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_qsmall, qsmall) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
   UP(d_scale_plain, scale_plain) UP(d_decB, decB)
 
   // ---- CRT targets -------------------------------------------------------------------------------------------------

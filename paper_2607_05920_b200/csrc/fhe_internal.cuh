@@ -27,6 +27,7 @@ struct CrtTarget {
   uint8_t* d_B = nullptr;      // [KB/16][64 nchunks][16]: the constant matrix as K-major 16-byte core-matrix rows (pipe.cuh)
   uint32_t* d_negM = nullptr;  // [Lraw]
   uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
+  uint32_t* d_Wlimbs = nullptr; // small CKKS targets only (K <= SMALL_K, see kernels_small.cu): [K][Lraw] limbs of W_i, then [Lraw] negM
   // "Top" form of the CKKS relin target: the output needs floor((V mod 2^(logP+logQ) + 2^(logP-1)) >> logP)
   // mod 2^logQ only, i.e. the high logQ bits of W_i exactly and ONE carry out of the low logP bits.  That carry is taken
   // from the top TOP_BITS bits of the low parts (columns 8..31 of the image, then 4 L columns of the high parts); the
@@ -39,6 +40,9 @@ struct CrtTarget {
   uint32_t* d_negMfull = nullptr;  // [Lfull]
 };
 constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58;
+// Shapes below these bounds convert on the CUDA cores (kernels_small.cu): a 128-coefficient tile of the tensor-core pipeline
+// costs a few thousand cycles whatever its size, which two-limb coefficients cannot amortise.
+constexpr uint32_t SMALL_K = 32, SMALL_LIMBS = 16, SMALL_WORK = 48;   // K, limbs, K x limbs
 
 enum PostMode : int {
   POST_CKKS_MASK = 0,    // out = X mod 2^logQ
@@ -77,6 +81,7 @@ struct Context {
   uint32_t* d_q = nullptr;        // [Kmax]
   uint32_t* d_qinv_neg = nullptr; // [Kmax] -q^-1 mod 2^32 (Montgomery)
   uint2* d_qmu = nullptr;         // [Kmax] (q, floor(2^53 / q)): one-word Barrett pair of the decompose epilogue
+  uint4* d_qsmall = nullptr;      // [Kmax] (q, 2^32 mod q, floor(2^61 / q), floor(2^48 / q)): the CUDA-core conversions
   uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion
   uint2* d_tw_inv = nullptr;      // [Kmax][N]: psi^-bitrev(k) and Shoup companion
   uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
@@ -87,6 +92,7 @@ struct Context {
   bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
+  bool force_pipe = false;        // fhe_debug_force_pipeline: small shapes take the tensor-core pipeline too (tests)
   uint32_t amb_bits = TOP_AMB;    // fhe_debug_crt_ambiguity lowers it so that tests reach the exact path
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)
@@ -179,6 +185,14 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
 cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
                        const uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_add, size_t add_outer,
                        size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s, uint32_t* d_flags = nullptr);
+// CUDA-core conversions for small shapes (kernels_small.cu): same contracts as launch_decompose / launch_crt (CKKS mask mode)
+bool small_decompose_ok(const Context* c, uint32_t Lin_eff, uint32_t K);
+cudaError_t launch_decompose_small(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
+                                   size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin_eff,
+                                   uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy);
+bool small_crt_ok(const Context* c, const CrtTarget& tg, const PostParams& pp);
+cudaError_t launch_crt_small(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
+                             const uint32_t* d_res, size_t res_outer, size_t res_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s);
 // register-only throughput of the NTT butterfly (mode 0), mad.lo.u32 (1), mul.hi.u32 (2) on this device, per second
 cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s);
 bool crt_target_fits(const CrtTarget& tg, const PostParams& pp);   // does the pipeline have the TMEM / shared memory for it

@@ -587,6 +587,8 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
                        size_t add_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s, uint32_t* d_flags) {
   if (nouter * ninner == 0) return cudaSuccess;
   if (tg.top && !d_flags) return cudaErrorInvalidValue;
+  if (small_crt_ok(c, tg, pp))                                     // small shapes: one thread per coefficient (kernels_small.cu)
+    return launch_crt_small(c, tg, pp, d_out, out_outer, out_inner, d_res, res_outer, res_inner, nouter, ninner, s);
   CrtParams ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);

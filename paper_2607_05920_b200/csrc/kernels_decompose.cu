@@ -91,6 +91,8 @@ cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size
   if (mask_bits && (mask_bits + 31) / 32 < eff) eff = (mask_bits + 31) / 32;
   const uint32_t KB = (4 * eff + 31) / 32 * 32;
   if (KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
+  if (small_decompose_ok(c, eff, K))                               // small shapes: one thread per coefficient (kernels_small.cu)
+    return launch_decompose_small(c, d_res, res_outer, res_inner, d_limbs, limb_outer, limb_inner, nouter, ninner, eff, K, mask_bits, s, lazy);
   const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2), false);
   if (!plan.ok || plan.nA != 2) return cudaErrorInvalidConfiguration;
   pipe::PipeArgs a;

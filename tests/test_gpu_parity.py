@@ -32,10 +32,15 @@ def _bitrev(i, bits):
 
 
 # ---- S1: decompose ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N,logQ,Lin,mask", [(1024, 128, 4, 0), (1024, 128, 8, 0), (4096, 620, 20, 620), (256, 1240, 78, 0)])
-def test_decompose_matches_python_mod(N, logQ, Lin, mask):
+@pytest.mark.parametrize("pipeline", [False, True])
+@pytest.mark.parametrize("N,logQ,Lin,mask", [(1024, 128, 4, 0), (1024, 128, 8, 0), (4096, 620, 20, 620), (256, 1240, 78, 0),
+                                             (512, 64, 2, 61), (2048, 256, 8, 250)])
+def test_decompose_matches_python_mod(N, logQ, Lin, mask, pipeline):
+    """pipeline = False: small shapes convert on the CUDA cores (kernels_small.cu), the others on the tensor-core pipeline;
+    True: everything through the pipeline."""
     fhe = _lib()
     ctx = fhe.Context(N, logQ, logQ)
+    ctx.fhe_debug_force_pipeline(pipeline)
     g = synth.rng(11)
     limbs = synth.uniform_limbs(g, (2,), N, 32 * Lin)
     K = ctx.K2
@@ -72,10 +77,12 @@ def test_ntt_forward_is_eq8_bitreversed_and_inverse_roundtrips(N):
 
 
 # ---- fhe_polymul ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N,logQ,batch", [(256, 64, 3), (1024, 128, 2), (1024, 218, 2), (2048, 61, 1)])
-def test_polymul_small_full(N, logQ, batch):
+@pytest.mark.parametrize("pipeline", [False, True])
+@pytest.mark.parametrize("N,logQ,batch", [(256, 64, 3), (1024, 128, 2), (1024, 218, 2), (2048, 61, 1), (512, 256, 2), (256, 33, 2)])
+def test_polymul_small_full(N, logQ, batch, pipeline):
     fhe = _lib()
     ctx = fhe.Context(N, logQ, 32)
+    ctx.fhe_debug_force_pipeline(pipeline)
     g = synth.rng(100 + N + logQ)
     a = synth.uniform_limbs(g, (batch,), N, logQ)
     b = synth.uniform_limbs(g, (batch,), N, logQ)
@@ -99,12 +106,14 @@ def test_polymul_extremes_all_q_minus_1_and_zero():
     assert not out.any()
 
 
-def test_polymul_c2_shape():
+@pytest.mark.parametrize("pipeline", [False, True])
+def test_polymul_c2_shape(pipeline):
     """configs[1]: N = 2^13, 218-bit coefficients (7 limbs), a slice of the batch of 64 checked in full against the
     oracle's own NTT route, the rest on sampled coefficients from the definition."""
     fhe = _lib()
     N, logQ, batch = 1 << 13, 218, 64
     ctx = fhe.Context(N, logQ, 32)
+    ctx.fhe_debug_force_pipeline(pipeline)
     assert ctx.L == 7
     g = synth.rng(2)
     a = synth.uniform_limbs(g, (batch,), N, logQ)
