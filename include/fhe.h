@@ -211,10 +211,13 @@ fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t
  * and maximum 58: the truncation error is below 2^-58, so nothing else can be wrong).  A smaller value
  * only sends more coefficients down the exact path -- results are identical -- which is how the tests reach it. */
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits);
-/* Small shapes (K <= 32 primes, <= 16 limbs, K x limbs <= 48) convert on the CUDA cores, one thread per coefficient, because
- * a tile of the tensor-core pipeline costs more than it moves there.  on != 0 sends them through the pipeline as well --
- * results are identical -- which is how the tests keep the pipeline covered at small shapes. */
-fhe_status fhe_debug_force_pipeline(fhe_ctx* ctx, int on);
+/* Path selection by shape.  Small conversions (K <= 32 primes, <= 16 limbs, K x limbs <= 48) run on the CUDA cores, one
+ * thread per coefficient, because a tile of the tensor-core pipeline costs more than it moves there; N = 2^12 runs every
+ * product's transforms in ONE kernel (whole prime-polynomial in shared memory), larger N in three passes.  mode 0: that
+ * choice (by measurement); 1: the large-shape paths everywhere (tensor-core conversions, three-pass NTT); 2: the small-shape
+ * paths wherever they exist (the whole-transform NTT also at N = 2^13, where the three passes measure 8-13 % faster).
+ * Results are identical in every mode -- this is how the tests cover each path at the shapes where it is not the default. */
+fhe_status fhe_debug_force_pipeline(fhe_ctx* ctx, int mode);
 /* Calibration for the roofline report: register-only throughput, in operations per second over the
  * whole device, of mode 0: the forward NTT butterfly exactly as the kernels execute it (Eq. 8: one
  * Shoup modular multiplication, one add, one subtract, lazy corrections); 1: mad.lo.u32; 2: mul.hi.u32.  Allocates

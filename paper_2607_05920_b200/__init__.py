@@ -211,8 +211,9 @@ class Context:
 
     KERNEL_CLASSES = ("decompose", "ntt_fwd", "ntt_inv", "pointwise", "crt", "rescale")
 
-    def fhe_debug_force_pipeline(self, on: bool):
-        self._check(self._lib.fhe_debug_force_pipeline(self._h, 1 if on else 0))
+    def fhe_debug_force_pipeline(self, mode: int):
+        """0 auto, 1 large-shape paths everywhere, 2 small-shape paths wherever they exist (include/fhe.h)."""
+        self._check(self._lib.fhe_debug_force_pipeline(self._h, int(mode)))
 
     def fhe_debug_crt_ambiguity(self, bits: int):
         self._check(self._lib.fhe_debug_crt_ambiguity(self._h, bits))

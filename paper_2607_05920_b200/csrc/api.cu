@@ -394,9 +394,9 @@ fhe_status fhe_modswitch(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_in, ui
   return FHE_OK;
 }
 
-fhe_status fhe_debug_force_pipeline(fhe_ctx* ctx, int on) {
-  if (!ctx) return FHE_ERR_ARG;
-  C(ctx)->force_pipe = on != 0;
+fhe_status fhe_debug_force_pipeline(fhe_ctx* ctx, int mode) {
+  if (!ctx || mode < 0 || mode > 2) return FHE_ERR_ARG;
+  C(ctx)->force_pipe = mode;
   return FHE_OK;
 }
 

@@ -92,7 +92,8 @@ struct Context {
   bool fit_pm = false, fit_tensor = false, fit_relin = false;   // does the conversion pipeline hold the target (pipe.cuh)
   PostParams post_pm, post_tensor, post_relin;
   uint32_t *d_Qlimbs = nullptr, *d_Plimbs = nullptr, *d_PQlimbs = nullptr, *d_muP = nullptr, *d_pow32_t = nullptr;
-  bool force_pipe = false;        // fhe_debug_force_pipeline: small shapes take the tensor-core pipeline too (tests)
+  int force_pipe = 0;             // fhe_debug_force_pipeline: 0 auto; 1 the large-shape paths everywhere (tensor-core conversions,
+                                  // three-pass NTT); 2 the small-shape paths wherever they exist (whole-transform NTT at N = 2^13 too)
   uint32_t amb_bits = TOP_AMB;    // fhe_debug_crt_ambiguity lowers it so that tests reach the exact path
   // evk-hat
   uint32_t* d_evk_hat = nullptr;  // [2][K2][N], forward NTT of the evk residues (plain domain)

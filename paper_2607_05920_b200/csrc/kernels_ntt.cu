@@ -483,6 +483,157 @@ ntt_row_fused_kernel(NttArgs a) {
 }
 
 // ------------------------------------------------------------------------------------------------------------------
+// Whole transform in one kernel, N = 2^12 and 2^13 (north_star: "one fused kernel for N <= 2^13"; the paper's reason for two
+// passes is only that one block's shared memory cannot hold the polynomial at n >= 2^16).  One block per
+// (item, prime) of N / 16 threads keeps the prime-polynomial on chip: column phase (16- or 32-point transforms at stride
+// 256, in registers), transposition through a shared-memory tile, row phase (row_fwd_core), the pointwise products in
+// registers, and the same backwards -- forward transforms, S3 and inverse transforms with ONE read of the operands and ONE
+// write of the results (three words per point and product instead of nine in the three-pass plan).
+// The tile keeps rows at a stride of 336 words, so a row's region doubles as the exchange scratch of its row transform.
+// ------------------------------------------------------------------------------------------------------------------
+constexpr int WROW = ROW_SM;
+
+// the thread's 16 points of the column phase: g[N] (global) -> registers.  All operands of a block are loaded before the first
+// transform starts, so that their latency is paid once.
+template <int LN1>
+__device__ __forceinline__ void whole_load(uint32_t (&x)[16], const uint32_t* __restrict__ g, uint32_t tid) {
+  constexpr int TPC = (1 << LN1) / 16;                             // threads per column
+  const uint32_t cc = tid & 255, tc = tid >> 8;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = g[(i * TPC + tc) * 256 + cc];
+}
+// registers (whole_load) -> registers: thread (r = tid / 16, t = tid % 16) ends with 16 contiguous points of row r, in [0, 4q)
+template <int LN1>
+__device__ __forceinline__ void whole_fwd(uint32_t (&x)[16], uint32_t* tile, uint32_t tid, const uint2* __restrict__ tw,
+                                          uint32_t q, uint32_t q2) {
+  static_assert(LN1 == 4 || LN1 == 5, "whole transform: N = 2^12 or 2^13");
+  constexpr int TPC = (1 << LN1) / 16;
+  const uint32_t cc = tid & 255, tc = tid >> 8, r = tid >> 4, t = tid & 15;
+  if constexpr (LN1 == 4) {
+    phase_b<4, false>(x, tw, 1, 0, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) tile[i * WROW + cc] = x[i];
+  } else {
+    phase_a<false, 1>(x, tw, 1, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) tile[(i * TPC + tc) * WROW + cc] = x[i];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = tile[(tc * 16 + i) * WROW + cc];
+    phase_b<5, false>(x, tw, 1, tc, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) tile[(tc * 16 + i) * WROW + cc] = x[i];   // the positions this thread has just read
+  }
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = tile[r * WROW + i * 16 + t];
+  __syncwarp();                                                    // the row is in registers before its region turns into scratch
+  row_fwd_core(x, tile + r * WROW, t, tw, (1u << LN1) + r, q, q2);
+  __syncthreads();                                                 // the tile is free for the next operand
+}
+// registers (16 contiguous points of row r, [0, 2q)) -> g[N] (global), scaled by sc
+template <int LN1>
+__device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restrict__ g, uint32_t* tile, uint32_t tid,
+                                          const uint2* __restrict__ tw, const uint2 sc, uint32_t q, uint32_t q2) {
+  constexpr int TPC = (1 << LN1) / 16;
+  const uint32_t cc = tid & 255, tc = tid >> 8, r = tid >> 4, t = tid & 15;
+  row_inv_core(x, tile + r * WROW, t, tw, (1u << LN1) + r, q, q2);   // x[i] = point i * 16 + t of row r
+#pragma unroll
+  for (int i = 0; i < 16; ++i) tile[r * WROW + i * 16 + t] = x[i];
+  __syncthreads();
+  if constexpr (LN1 == 4) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = tile[i * WROW + cc];
+    phase_b<4, true>(x, tw, 1, 0, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) g[i * 256 + cc] = mul_shoup(x[i], sc.x, sc.y, q);
+  } else {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = tile[(tc * 16 + i) * WROW + cc];
+    phase_b<5, true>(x, tw, 1, tc, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) tile[(tc * 16 + i) * WROW + cc] = x[i];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = tile[(i * TPC + tc) * WROW + cc];
+    phase_a<true, 1>(x, tw, 1, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) g[(i * TPC + tc) * 256 + cc] = mul_shoup(x[i], sc.x, sc.y, q);
+  }
+  __syncthreads();                                                 // the tile is free for the next result
+}
+
+template <int PW, int LN1>
+__global__ void __launch_bounds__(16 << LN1, LN1 == 4 ? 2 : 1)
+ntt_whole_kernel(NttArgs a) {
+  pdl_sync();
+  extern __shared__ __align__(16) uint32_t tile[];                 // [N / 256][WROW]
+  const uint32_t tid = threadIdx.x;
+  const uint32_t item = blockIdx.x % a.nitems, j = blockIdx.x / a.nitems;   // the items of a prime side by side: its tables stay in L2
+  const size_t KN = (size_t)a.K * a.N, poff = (size_t)j * a.N;
+  const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
+  const uint2* twf = a.tw2 + (size_t)j * a.N;
+  const uint2* twi = a.tw + (size_t)j * a.N;
+  const uint2 sc = __ldg(a.scale + j);
+  if constexpr (PW == PW_POLYMUL) {
+    uint32_t* g = a.data + (size_t)item * KN + poff;
+    uint32_t x[16], y[16];
+    whole_load<LN1>(x, g, tid);
+    whole_load<LN1>(y, a.aux + (size_t)(item / a.aux_group) * KN + poff, tid);
+    whole_fwd<LN1>(x, tile, tid, twf, q, q2);
+    whole_fwd<LN1>(y, tile, tid, twf, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(canon4(x[i], q, q2), y[i], q, qn);
+    whole_inv<LN1>(x, g, tile, tid, twi, sc, q, q2);
+  } else if constexpr (PW == PW_TENSOR) {
+    uint32_t* g = a.data + (size_t)item * 4 * KN + poff;           // slots a0, a1, b0, b1 at g + slot * KN
+    uint32_t a0[16], a1[16], b0[16], b1[16], x[16];
+    whole_load<LN1>(a0, g, tid);
+    whole_load<LN1>(a1, g + KN, tid);
+    whole_load<LN1>(b0, g + 2 * KN, tid);
+    whole_load<LN1>(b1, g + 3 * KN, tid);
+    whole_fwd<LN1>(a0, tile, tid, twf, q, q2);
+    whole_fwd<LN1>(a1, tile, tid, twf, q, q2);
+    whole_fwd<LN1>(b0, tile, tid, twf, q, q2);
+    whole_fwd<LN1>(b1, tile, tid, twf, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { a0[i] = canon4(a0[i], q, q2); a1[i] = canon4(a1[i], q, q2); }
+    // every thread of the block has read all four operands (the barrier at the end of the last whole_fwd): slots 0..2 may go
+#pragma unroll 1
+    for (int op = 0; op < 3; ++op) {
+      if (op == 0) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = mm(a0[i], b0[i], q, qn);
+      } else if (op == 1) {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = mont_redc((uint64_t)a0[i] * b1[i] + (uint64_t)a1[i] * b0[i], q, qn);
+      } else {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
+      }
+      whole_inv<LN1>(x, g + (size_t)op * KN, tile, tid, twi, sc, q, q2);
+    }
+  } else {   // PW_RELIN: slot 0 = d2 residues; aux = the key, fully transformed and canonical (same point order as whole_fwd leaves)
+    static_assert(PW == PW_RELIN, "whole transform: unknown mode");
+    uint32_t* g = a.data + (size_t)item * 2 * KN + poff;
+    const uint32_t r = tid >> 4, t = tid & 15;
+    uint32_t d[16], e0[16], e1[16], x[16];
+    whole_load<LN1>(d, g, tid);
+    load16(e0, a.aux + poff + (size_t)r * 256 + t * 16);
+    load16(e1, a.aux + KN + poff + (size_t)r * 256 + t * 16);
+    whole_fwd<LN1>(d, tile, tid, twf, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) d[i] = canon4(d[i], q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e0[i], q, qn);
+    whole_inv<LN1>(x, g, tile, tid, twi, sc, q, q2);
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e1[i], q, qn);
+    whole_inv<LN1>(x, g + KN, tile, tid, twi, sc, q, q2);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
 // Calibration of the roofline the NTT kernels are held against ("calibrate the integer peak in the same
 // run with a register-only microbenchmark of the actual mix").  MODE 0: the forward butterfly itself (bf_fwd: one
 // IMAD.HI, two IMAD, three adds / min) on 16 registers per thread with register-resident twiddles, no memory traffic;
@@ -633,6 +784,24 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems; a.aux_group = aux_group ? aux_group : 1;
   const bool fin = c->logN == 8;
   cudaError_t e;
+  // the whole product in one launch (ntt_whole_kernel): measured 5-9 % faster than the three passes at N = 2^12, 8-13 % slower
+  // at N = 2^13 (512-thread blocks, one or two per SM: the block-wide barriers of the transpositions are not hidden), so
+  // N = 2^13 takes it only on request (fhe_debug_force_pipeline(ctx, 2))
+  if ((c->logN == 12 && c->force_pipe != 1) || (c->logN == 13 && c->force_pipe == 2)) {
+    a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = d_scale; a.U = Uout;
+    a.units = nitems * K;
+    const uint32_t threads = c->N / 16;
+    const size_t smem = (size_t)(c->N / 256) * WROW * sizeof(uint32_t);
+    LaunchTimer lt(c, KC_POINTWISE, s);
+#define WHOLE_CASE(PW)                                                                                      \
+  case PW:                                                                                                  \
+    e = c->logN == 12 ? launch_pdl(ntt_whole_kernel<PW, 4>, a.units, threads, smem, s, a)                   \
+                      : launch_pdl(ntt_whole_kernel<PW, 5>, a.units, threads, smem, s, a);                  \
+    break;
+    switch (pw_mode) { WHOLE_CASE(PW_POLYMUL) WHOLE_CASE(PW_TENSOR) WHOLE_CASE(PW_RELIN) default: e = cudaErrorInvalidValue; }
+#undef WHOLE_CASE
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
   if (!fin) {
     if ((e = launch_col<false>(c, a, nitems * Uin * K, s)) != cudaSuccess) return e;
     if (pw_mode == PW_POLYMUL) {

@@ -108,10 +108,10 @@ crt_small_kernel(uint32_t* __restrict__ out, size_t out_outer, size_t out_inner,
 }
 
 bool small_decompose_ok(const Context* c, uint32_t Lin_eff, uint32_t K) {
-  return !c->force_pipe && K <= 4 * SMALL_K && Lin_eff <= SMALL_LIMBS && K * Lin_eff <= SMALL_WORK && c->N >= SMALL_THREADS;
+  return c->force_pipe != 1 && K <= 4 * SMALL_K && Lin_eff <= SMALL_LIMBS && K * Lin_eff <= SMALL_WORK && c->N >= SMALL_THREADS;
 }
 bool small_crt_ok(const Context* c, const CrtTarget& tg, const PostParams& pp) {
-  return !c->force_pipe && pp.mode == POST_CKKS_MASK && tg.d_Wlimbs != nullptr && tg.K * tg.Lraw <= SMALL_WORK &&
+  return c->force_pipe != 1 && pp.mode == POST_CKKS_MASK && tg.d_Wlimbs != nullptr && tg.K * tg.Lraw <= SMALL_WORK &&
          c->N >= SMALL_THREADS && pp.L <= tg.Lraw;
 }
 

@@ -37,7 +37,7 @@ def _bitrev(i, bits):
                                              (512, 64, 2, 61), (2048, 256, 8, 250)])
 def test_decompose_matches_python_mod(N, logQ, Lin, mask, pipeline):
     """pipeline = False: small shapes convert on the CUDA cores (kernels_small.cu), the others on the tensor-core pipeline;
-    True: everything through the pipeline."""
+    True: everything through the pipeline (mode 1 of fhe_debug_force_pipeline)."""
     fhe = _lib()
     ctx = fhe.Context(N, logQ, logQ)
     ctx.fhe_debug_force_pipeline(pipeline)
@@ -106,7 +106,7 @@ def test_polymul_extremes_all_q_minus_1_and_zero():
     assert not out.any()
 
 
-@pytest.mark.parametrize("pipeline", [False, True])
+@pytest.mark.parametrize("pipeline", [0, 1, 2])
 def test_polymul_c2_shape(pipeline):
     """configs[1]: N = 2^13, 218-bit coefficients (7 limbs), a slice of the batch of 64 checked in full against the
     oracle's own NTT route, the rest on sampled coefficients from the definition."""
@@ -568,6 +568,42 @@ def test_exact_path_takes_every_flagged_coefficient_of_a_large_launch():
         for k in _structured_ks(N, b, B, 2, ctx.n_sm, per_item=16):
             want = _relin_coeff_ckks(prm, out3[b], evk, k, d2b)
             assert [coeff_from_limbs(out2[b, 0], k), coeff_from_limbs(out2[b, 1], k)] == want, (b, k)
+
+
+@pytest.mark.parametrize("N,logQ,logP,t", [(1 << 12, 128, 128, 0), (1 << 13, 100, 96, 0), (1 << 13, 150, 60, 0), (1 << 12, 120, 120, 257),
+                                            (1 << 13, 100, 130, 65537)])
+def test_whole_transform_sizes_full_pipeline(N, logQ, logP, t):
+    """N = 2^12 and (on request) 2^13 run every product (polymul, tensor, relin) through the single whole-transform kernel
+    (ntt_whole_kernel): every limb of he_mult, relinearize, rescale (CKKS) and polymul against the oracle's own NTT route."""
+    fhe = _lib()
+    prm = scheme.Params(N, logQ, logP, t)
+    ctx = fhe.Context(N, logQ, logP, t)
+    ctx.fhe_debug_force_pipeline(2)
+    g = synth.rng(N + logQ + t)
+    B = 2
+    bits = logQ                                                     # uniform below 2^logQ <= Q: canonical for both schemes
+    ct_np = synth.uniform_limbs(g, (2, B, 2), N, bits)
+    evk_np = synth.uniform_limbs(g, (2,), N, logQ + logP)           # below PQ for both
+    def pad(a, L):
+        return a if a.shape[-2] == L else np.concatenate([a, np.zeros(a.shape[:-2] + (L - a.shape[-2], N), np.uint32)], axis=-2)
+    ct_np, evk_np = pad(ct_np, ctx.L), pad(evk_np, ctx.L_PQ)
+    evk = tuple(from_limbs(evk_np[k]) for k in range(2))
+    ctx.fhe_set_evk(limbs_np_to_tensor(evk_np))
+    d1, d2 = limbs_np_to_tensor(ct_np[0]), limbs_np_to_tensor(ct_np[1])
+    t3 = ctx.fhe_he_mult(d1, d2)
+    t2 = ctx.fhe_relinearize(t3)
+    pm_out = ctx.fhe_polymul(d1[:, 0].contiguous(), d2[:, 1].contiguous())
+    got3, got2, gotpm = tensor_to_polys(t3), tensor_to_polys(t2), tensor_to_polys(pm_out)
+    for i in range(B):
+        c1 = tuple(from_limbs(ct_np[0, i, k]) for k in range(2))
+        c2 = tuple(from_limbs(ct_np[1, i, k]) for k in range(2))
+        want3 = scheme.he_mult(prm, c1, c2)
+        assert got3[i] == [list(p) for p in want3], i
+        want2 = scheme.relinearize(prm, want3, evk)
+        assert got2[i] == [list(p) for p in want2], i
+        assert gotpm[i] == ring.pm(c1[0], c2[1], prm.Q), i
+        if t == 0:
+            assert tensor_to_polys(ctx.fhe_mult_relin_rescale(d1, d2, 40)[i]) == [list(p) for p in scheme.rescale(prm, want2, 40)]
 
 
 # ---- NEXT-1 (SURVEY.md 8f): coefficient-wise operations, level drop, and a depth-2 circuit across two levels ----------------
