@@ -135,6 +135,9 @@ struct CrtParams {
   // (s1 + p = 32 ws + bs); roundings rbit1 at limb rb1 (divide by P; full form only), rbit2 at limb rb2 (rescale);
   // the result has Lr limbs, the top one masked with tm; lend = last limb of the total the stream must see
   uint32_t wd, bd, ws, bs, rb1, rbit1, rb2, rbit2, Lr, tm, tmq, lend;
+  // 2^8, 2^16, 2^24 as run-time values: with literal powers of two ptxas splits every mad.wide of the column sums into
+  // IMAD.SHL + IMAD.HI + carry adds (seven multiplier-pipe instructions per limb instead of one IMAD.WIDE per column)
+  uint32_t m8, m16, m24;
   PostParams pp;
 };
 
@@ -248,7 +251,7 @@ struct CrtEpi {
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     int g0 = 0;
     if (col0 == 0) {
-      uint64_t asum = madw(t[3], 1u << 24, madw(t[2], 1u << 16, madw(t[1], 256u, (uint64_t)t[0])));
+      uint64_t asum = madw(t[3], p.m24, madw(t[2], p.m16, madw(t[1], p.m8, (uint64_t)t[0])));
       asum += ((uint64_t)t[4] << 32) + ((uint64_t)t[5] << 40);
       alpha = (uint32_t)((asum + (1ull << (ALPHA_SHIFT - 1))) >> ALPHA_SHIFT);
       g0 = CRT_ALPHA_COLS / 4;
@@ -258,7 +261,7 @@ struct CrtEpi {
 #pragma unroll
     for (int g = 0; g < 8; ++g) {
       if (g < g0) { P[g] = 0; continue; }
-      P[g] = madw(alpha, negm[tb + g], madw(t[4 * g + 3], 1u << 24, madw(t[4 * g + 2], 1u << 16, madw(t[4 * g + 1], 256u, (uint64_t)t[4 * g]))));
+      P[g] = madw(alpha, negm[tb + g], madw(t[4 * g + 3], p.m24, madw(t[4 * g + 2], p.m16, madw(t[4 * g + 1], p.m8, (uint64_t)t[4 * g]))));
     }
     uint32_t l0 = tb;
     if constexpr (TOP) {
@@ -616,6 +619,7 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   ep.Lr = (nb + 31) / 32; ep.tm = top_mask(nb);
   ep.lend = ep.ws + pp.L;                                        // output limb m needs limbs ws + m and ws + m + 1 of the total
   ep.amb_bits = pp.amb_bits ? pp.amb_bits : TOP_AMB; ep.flags = d_flags;
+  ep.m8 = 1u << 8; ep.m16 = 1u << 16; ep.m24 = 1u << 24;
   cudaError_t e;
   {
     LaunchTimer lt(c, KC_CRT, s);
