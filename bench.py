@@ -550,6 +550,76 @@ def run_sweep(args):
     return 0
 
 
+# ---- profiles/: turn an exported ncu capture of this command into the committed summaries --------------------------------
+KERNEL_CLASS_PATTERNS = (   # substring of the kernel name -> bench.py's kernel class
+    ("DecEpi", "decompose"), ("decompose_small", "decompose"), ("CrtEpi", "crt"), ("crt_exact", "crt"), ("crt_small", "crt"),
+    ("ntt_row_fused", "pointwise"), ("ntt_whole", "pointwise"), ("rescale_kernel", "rescale"),
+)
+
+
+def kernel_class(name: str):
+    for pat, cls in KERNEL_CLASS_PATTERNS:
+        if pat in name:
+            return cls
+    if "ntt_col" in name or "ntt_row_fwd" in name or "ntt_row_inv" in name:
+        # ntt_col2_kernel<LN, INV> / ntt_col_kernel<LN, INV>: the second template argument is the direction
+        import re
+        m = re.search(r"<\s*\d+\s*,\s*(\w+)\s*>", name)
+        inv = "ntt_row_inv" in name or (m is not None and m.group(1) in ("1", "true"))
+        return "ntt_inv" if inv else "ntt_fwd"
+    return None
+
+
+def summarise_ncu(raw_csv: str, capture_name: str):
+    """raw_csv = `ncu -i <capture>.ncu-rep --page raw --csv` of `ncu --set full ... python bench.py ...` (one step's launches).
+    Writes profiles/dram_traffic.csv (read back by the roofline line) and prints a markdown table for profiles/*.md."""
+    import csv
+    with open(raw_csv) as f:
+        rows = list(csv.reader(f))
+    hdr, body = rows[0], rows[2:]
+    col = {h: i for i, h in enumerate(hdr)}
+    def num(r, key):
+        v = r[col[key]].replace(",", "") if key in col else ""
+        try:
+            return float(v)
+        except ValueError:
+            return 0.0
+    unit = {h: rows[1][i] for h, i in col.items()}
+    def to_bytes(v, u):
+        return v * {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(u, 1)
+    per = {}
+    lines = ["| # | kernel | class | us | DRAM read MB | DRAM write MB | dram % of peak | issue active % | tensor pipe % | regs |", "|---|---|---|---|---|---|---|---|---|---|"]
+    for n, r in enumerate(body):
+        name = r[col["Kernel Name"]]
+        cls = kernel_class(name)
+        rd = to_bytes(num(r, "dram__bytes_read.sum"), unit.get("dram__bytes_read.sum", "byte"))
+        wr = to_bytes(num(r, "dram__bytes_write.sum"), unit.get("dram__bytes_write.sum", "byte"))
+        us = num(r, "gpu__time_duration.sum") * {"ns": 1e-3, "us": 1.0, "ms": 1e3}.get(unit.get("gpu__time_duration.sum", "us"), 1.0)
+        dram_pct = num(r, "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed")
+        lines.append(f"| {n} | `{name[:60]}` | {cls} | {us:.1f} | {rd / 1e6:.1f} | {wr / 1e6:.1f} | {dram_pct:.1f} | "
+                     f"{num(r, 'smsp__issue_active.avg.pct_of_peak_sustained_active'):.1f} | "
+                     f"{num(r, 'sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active'):.1f} | {int(num(r, 'launch__registers_per_thread'))} |")
+        if cls:
+            d = per.setdefault(cls, [0, 0.0, 0.0])
+            d[0] += 1; d[1] += rd + wr; d[2] += us
+    head = kernel_source_hash()
+    with open(TRAFFIC_CSV, "w") as f:
+        f.write("# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) per launch and kernel class, one C5 step; written by\n"
+                "# `python bench.py --ncu-raw <csv> --capture-name <name>` from an `ncu --set full` capture of bench.py itself\n")
+        f.write("class,launches_per_step,dram_bytes_per_launch,kernel_source_sha256_16,capture\n")
+        for cls, (cnt, byts, us) in sorted(per.items()):
+            f.write(f"{cls},{cnt},{byts / cnt:.0f},{head},{capture_name}\n")
+    print("\n".join(lines))
+    print()
+    print("| class | launches | DRAM MB per step | us per step (serialised, cold cache) | share |")
+    print("|---|---|---|---|---|")
+    tot = sum(v[2] for v in per.values())
+    for cls, (cnt, byts, us) in sorted(per.items()):
+        print(f"| {cls} | {cnt} | {byts / 1e6:.1f} | {us:.1f} | {us / tot:.3f} |")
+    print(f"| total | {sum(v[0] for v in per.values())} | {sum(v[1] for v in per.values()) / 1e6:.1f} | {tot:.1f} | 1 |")
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -560,7 +630,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true",
                     help="standalone polymul sweep N = 2^12..2^16 x logQ in {64, 256, 620, 1240, 2480}: one JSON line per cell")
+    ap.add_argument("--ncu-raw", default=None, help="exported raw page (csv) of an ncu --set full capture of this command: "
+                                                    "write profiles/dram_traffic.csv and print the summary tables")
+    ap.add_argument("--capture-name", default="capture")
     args = ap.parse_args()
+    if args.ncu_raw:
+        return summarise_ncu(args.ncu_raw, args.capture_name)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not args.sweep:
         # plain `python bench.py --gpus N`: become the N-rank launch the contract describes (one process per GPU)
         port = os.environ.get("MASTER_PORT", "29511")
