@@ -528,7 +528,10 @@ def run_sweep(args):
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
             w = 4
-            alg = batch * N * w * (2 * L + 2 * K) + batch * N * w * (2 * 2 * K + 2 * K + K + 2 * K) + batch * N * w * (K + L)
+            # algorithmic bytes of the plan this cell runs: decompose a, b | transforms and products | CRT.  N = 2^12 runs the
+            # transforms in one kernel (operands in, product out: 3K words per point), the other N in three passes (9K)
+            ntt_words = 3 * K if N == (1 << 12) else (2 * 2 * K + 2 * K + K + 2 * K)
+            alg = batch * N * w * (2 * L + 2 * K) + batch * N * w * ntt_words + batch * N * w * (K + L)
             cpu = None
             if N <= (1 << 14) and not args.no_cpu_baseline:
                 # the oracle beside it: one pair per cell, cells with N <= 2^14 only, one host core
