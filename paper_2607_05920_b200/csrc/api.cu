@@ -41,9 +41,10 @@ fhe_status do_he_mult(Context* c, uint32_t* d_out3, const uint32_t* d_ct1, const
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   // slots (a0, a1, b0, b1) per batch item: ct1 polys go to slots 0,1 ; ct2 polys to slots 2,3
   CK(launch_decompose(c, ws, 4 * rp, rp, d_ct1, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct1");
-  CK(launch_decompose(c, ws + 2 * rp, 4 * rp, rp, d_ct2, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s), "decompose ct2");
+  // the second factor carries the final constant of the inverse transforms (scaled decompose image, fhe_internal.cuh)
+  CK(launch_decompose(c, ws + 2 * rp, 4 * rp, rp, d_ct2, (size_t)2 * L * N, (size_t)L * N, B, 2, L, K, mask, s, true, &c->tgt_tensor), "decompose ct2");
   // forward columns, fused rows (tensor product in registers), inverse columns: slots 0..2 <- INTT(d0^, d1^, d2^)
-  CK(launch_ntt_product(c, ws, nullptr, B, K, PW_TENSOR, c->tgt_tensor.d_scale, s), "ntt tensor");
+  CK(launch_ntt_product(c, ws, nullptr, B, K, PW_TENSOR, s), "ntt tensor");
   CK(launch_crt(c, c->tgt_tensor, c->post_tensor, d_out3, (size_t)3 * L * N, (size_t)L * N, ws, 4 * rp, rp, nullptr, 0, 0,
                 B, 3, s), "crt");
   return FHE_OK;
@@ -57,7 +58,7 @@ fhe_status do_relin(Context* c, uint32_t* d_out2, const uint32_t* d_in3, uint32_
   const size_t rp = (size_t)K * N;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ws, 2 * rp, 0, d_in3 + (size_t)2 * L * N, (size_t)3 * L * N, 0, B, 1, L, K, mask, s), "decompose d2");
-  CK(launch_ntt_product(c, ws, const_cast<uint32_t*>(d_key_hat), B, K, PW_RELIN, c->tgt_relin.d_scale, s), "ntt relin");
+  CK(launch_ntt_product(c, ws, const_cast<uint32_t*>(d_key_hat), B, K, PW_RELIN, s), "ntt relin");   // the key carries the final constant
   PostParams pp = c->post_relin;
   pp.rescale_bits = rescale_bits;
   pp.amb_bits = c->amb_bits;
@@ -101,6 +102,7 @@ static fhe_status install_key(Context* c, uint32_t** slot, const uint32_t* d_key
   const uint32_t mask = c->t == 0 ? c->logQ + c->logP : 0;
   CK(launch_decompose(c, *slot, 0, (size_t)c->K2 * c->N, d_key, 0, (size_t)c->L_PQ * c->N, 1, 2, c->L_PQ, c->K2, mask, s), "decompose key");
   CK(launch_ntt_fwd(c, *slot, 1, 2, 2, c->K2, s), "ntt key");
+  CK(launch_scale_rows(c, *slot, 2, c->K2, c->tgt_relin.d_scale, s), "scale key");   // the key carries the relin products' final constant
   return FHE_OK;
 }
 
@@ -159,8 +161,8 @@ static fhe_status do_polymul(Context* c, uint32_t* d_out, const uint32_t* d_a, c
   uint32_t* rb = ra + (size_t)npoly * rp;
   const uint32_t mask = c->t == 0 ? c->logQ : 0;
   CK(launch_decompose(c, ra, 0, rp, d_a, 0, (size_t)L * N, 1, npoly, L, K, mask, s), "decompose a");
-  CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, nb, L, K, mask, s), "decompose b");
-  CK(launch_ntt_product(c, ra, rb, npoly, K, PW_POLYMUL, c->tgt_pm.d_scale, s, group), "ntt polymul");
+  CK(launch_decompose(c, rb, 0, rp, d_b, 0, (size_t)L * N, 1, nb, L, K, mask, s, true, &c->tgt_pm), "decompose b");   // carries the final constant
+  CK(launch_ntt_product(c, ra, rb, npoly, K, PW_POLYMUL, s, group), "ntt polymul");
   CK(launch_crt(c, c->tgt_pm, c->post_pm, d_out, 0, (size_t)L * N, ra, 0, rp, nullptr, 0, 0, 1, npoly, s), "crt");
   return FHE_OK;
 }

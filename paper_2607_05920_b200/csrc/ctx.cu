@@ -103,8 +103,23 @@ static std::vector<uint8_t> bytes_of(const BigU& x, size_t n) {
 
 // CRT constants for the basis q_0..q_{K-1} and the target T (pow2: T = 2^(32 Lraw) with Lraw = ceil(width_bits/32);
 // else T = Tmod odd).  See fhe_internal.cuh (CrtTarget) and kernels_crt.cu for how the image is consumed.
+// decompose constant image [KBimg / 16][cols][16 bytes]: byte cc of (2^(8 kb) m_j) mod q_j at column 4 j + cc (m_j = 1: plain)
+static std::vector<uint8_t> dec_image(const Context* c, uint32_t K, const std::vector<uint2>* mult) {
+  std::vector<uint8_t> img((size_t)c->dec_KBimg * c->dec_cols, 0);
+  for (uint32_t j = 0; j < K; ++j) {
+    const uint32_t q = c->h_q[j];
+    uint32_t cur = mult ? (*mult)[j].x % q : 1u;
+    for (uint32_t kb = 0; kb < c->dec_KBimg; ++kb) {
+      for (uint32_t cc = 0; cc < 4; ++cc)
+        img[((size_t)(kb / 16) * c->dec_cols + 4 * j + cc) * 16 + kb % 16] = (uint8_t)(cur >> (8 * cc));
+      cur = mulmod(cur, 256u, q);
+    }
+  }
+  return img;
+}
+
 static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2, uint32_t width_bits,
-                                const BigU& Tmod, uint32_t post_limbs) {
+                                const BigU& Tmod, uint32_t post_limbs, bool scaled_image = false) {
   tg.K = K;
   tg.KB = (4 * K + 31) / 32 * 32;
   uint32_t clogK = 0;
@@ -151,6 +166,10 @@ static cudaError_t build_target(Context* c, CrtTarget& tg, uint32_t K, bool pow2
   cudaError_t e = upload(c, &tg.d_B, img);
   if (e != cudaSuccess) return e;
   if ((e = upload(c, &tg.d_negM, negM)) != cudaSuccess) return e;
+  if (scaled_image) {                                                   // the second factor's decompose carries the final constant
+    const std::vector<uint8_t> di = dec_image(c, K, &scale);
+    if ((e = upload(c, &tg.d_decB_scaled, di)) != cudaSuccess) return e;
+  }
   if (pow2 && K <= SMALL_K && tg.Lraw <= SMALL_LIMBS) {                 // limb form of the constants for the CUDA-core CRT
     std::vector<uint32_t> wl((size_t)(K + 1) * tg.Lraw, 0u);
     for (uint32_t i = 0; i < K; ++i) {
@@ -315,7 +334,6 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   // decompose constants: widest input is the evk (L_PQ limbs) or what fhe_debug_decompose may pass (MAX_LIMBS_IN)
   c->dec_KBimg = (4 * MAX_LIMBS_IN + 31) / 32 * 32;
   c->dec_cols = (Kmax + 15) / 16 * DEC_NC;               // image [dec_KBimg / 16][dec_cols][16 bytes] (pipe.cuh)
-  std::vector<uint8_t> decB((size_t)c->dec_KBimg * c->dec_cols, 0);
   c->h_psi.resize(Kmax);
   std::vector<uint2> twf((size_t)Kmax * N), twi((size_t)Kmax * N);
   std::vector<uint32_t> pw(N), ipw(N);
@@ -343,23 +361,18 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     }
     uint32_t ninv = powmod(N % q, q - 2, q);
     scale_plain[j] = make_uint2(ninv, shoup(ninv, q));
-    uint32_t cur = 1;                                  // 2^(8 kb) mod q, byte cc at column 4 j + cc
-    for (uint32_t kb = 0; kb < c->dec_KBimg; ++kb) {
-      for (uint32_t cc = 0; cc < 4; ++cc)
-        decB[((size_t)(kb / 16) * c->dec_cols + 4 * j + cc) * 16 + kb % 16] = (uint8_t)(cur >> (8 * cc));
-      cur = mulmod(cur, 256u, q);
-    }
   }
 #define UP(dst, vec)                                                                                   \
   if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
   UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_qsmall, qsmall) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
+  const std::vector<uint8_t> decB = dec_image(c, Kmax, nullptr);
   UP(d_scale_plain, scale_plain) UP(d_decB, decB)
 
   // ---- CRT targets -------------------------------------------------------------------------------------------------
   const bool ckks = (t == 0);
-  if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
-      (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q, c->L + 2)) != cudaSuccess ||
+  if ((e = build_target(c, c->tgt_pm, c->K_pm, ckks, logQ, Q, c->L + 2, true)) != cudaSuccess ||
+      (e = build_target(c, c->tgt_tensor, c->K1, ckks, logQ, Q, c->L + 2, true)) != cudaSuccess ||
       (e = (ckks && logP >= TOP_BITS) ? build_target_top(c, c->tgt_relin, c->K2, logP, logQ)
                                       : build_target(c, c->tgt_relin, c->K2, ckks, logQ + logP, PQ, c->L_PQ + 2)) != cudaSuccess) {
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "CRT table build failed: " + m);

@@ -27,6 +27,7 @@ struct CrtTarget {
   uint8_t* d_B = nullptr;      // [KB/16][64 nchunks][16]: the constant matrix as K-major 16-byte core-matrix rows (pipe.cuh)
   uint32_t* d_negM = nullptr;  // [Lraw]
   uint2* d_scale = nullptr;    // [K]: N^-1 * (M/q_i)^-1 * 2^32 mod q_i and its Shoup companion (folded into the iNTT)
+  uint8_t* d_decB_scaled = nullptr;   // decompose image whose constants carry d_scale: 2^(8 kb) s_j mod q_j (polymul / tensor targets)
   uint32_t* d_Wlimbs = nullptr; // small CKKS targets only (K <= SMALL_K, see kernels_small.cu): [K][Lraw] limbs of W_i, then [Lraw] negM
   // "Top" form of the CKKS relin target: the output needs floor((V mod 2^(logP+logQ) + 2^(logP-1)) >> logP)
   // mod 2^logQ only, i.e. the high logQ bits of W_i exactly and ONE carry out of the low logP bits.  That carry is taken
@@ -159,9 +160,10 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, s
 // Polynomials of a launch are indexed (o, i), o < nouter, i < ninner, and live at base + o * outer + i * inner (words).
 // decompose: limbs [Lin][N] -> residues [K][N] per polynomial; mask_bits > 0 reduces the input mod 2^mask_bits first;
 // lazy: residues in [0, 2q) instead of [0, q) (what the forward transforms accept)
+// tgt: the residues additionally carry that target's final constant (scaled constant image; nullptr: plain residues)
 cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                              size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin,
-                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy = true);
+                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy = true, const CrtTarget* tgt = nullptr);
 // Transforms live in an item-major residue buffer [nitems][S][K][N] (S slots per item); slots 0..U-1 of every item
 // are transformed in place.  Forward output is in bit-reversed order and canonical ([0, q)).
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s);
@@ -176,10 +178,14 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
 //   PW_POLYMUL S = 1: data <- INTT(NTT(data) * NTT(aux)), aux = [ceil(nitems / aux_group)][K][N], transformed in place too
 //   PW_TENSOR  S = 4: slots (a0, a1, b0, b1) -> slots 0..2 = INTT(a0^ b0^, a0^ b1^ + a1^ b0^, a1^ b1^)
 //   PW_RELIN   S = 2: slot 0 = d2 -> slots 0, 1 = INTT(d2^ * aux[0], d2^ * aux[1]), aux = a key already in the NTT domain [2][K][N]
-// (Montgomery products: each carries a factor 2^-32 that d_scale removes.)
+// (Montgomery products: each carries a factor 2^-32 that the folded constant removes.)
 // aux_group (PW_POLYMUL): item i multiplies aux polynomial i / aux_group, of which there are ceil(nitems / aux_group).
+// The final constant of the inverse (CrtTarget::d_scale) is NOT applied here: it rides on an operand -- the second factor is
+// decomposed with the target's scaled constant image (Context::d_decB_pm / d_decB_tensor), a key is multiplied by it when it
+// is installed (launch_scale_rows).
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
-                               const uint2* d_scale, cudaStream_t s, uint32_t aux_group = 1);
+                               cudaStream_t s, uint32_t aux_group = 1);
+cudaError_t launch_scale_rows(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, const uint2* d_scale, cudaStream_t s);
 // CRT + post: residues [K][N] -> limbs [L][N] per polynomial (o, i); d_add: for the relin modes, the polynomial added
 // at the end, else nullptr.  d_flags: top-form targets only, nouter * ninner * N / 32 words of workspace for the bitmap of the
 // coefficients the exact path recomputes (written in full by the launch: no initialisation needed)
@@ -190,7 +196,7 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
 bool small_decompose_ok(const Context* c, uint32_t Lin_eff, uint32_t K);
 cudaError_t launch_decompose_small(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                                    size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin_eff,
-                                   uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy);
+                                   uint32_t K, uint32_t mask_bits, cudaStream_t s, const uint2* d_scale);
 bool small_crt_ok(const Context* c, const CrtTarget& tg, const PostParams& pp);
 cudaError_t launch_crt_small(Context* c, const CrtTarget& tg, const PostParams& pp, uint32_t* d_out, size_t out_outer, size_t out_inner,
                              const uint32_t* d_res, size_t res_outer, size_t res_inner, uint32_t nouter, uint32_t ninner, cudaStream_t s);

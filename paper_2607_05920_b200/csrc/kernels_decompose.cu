@@ -85,20 +85,22 @@ struct DecEpi {
 
 cudaError_t launch_decompose(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                              size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin,
-                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy) {
+                             uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy, const CrtTarget* tgt) {
   if (nouter * ninner == 0) return cudaSuccess;
   uint32_t eff = Lin;
   if (mask_bits && (mask_bits + 31) / 32 < eff) eff = (mask_bits + 31) / 32;
   const uint32_t KB = (4 * eff + 31) / 32 * 32;
   if (KB > c->dec_KBimg || K > c->Kmax) return cudaErrorInvalidValue;
   if (small_decompose_ok(c, eff, K))                               // small shapes: one thread per coefficient (kernels_small.cu)
-    return launch_decompose_small(c, d_res, res_outer, res_inner, d_limbs, limb_outer, limb_inner, nouter, ninner, eff, K, mask_bits, s, lazy);
+    return launch_decompose_small(c, d_res, res_outer, res_inner, d_limbs, limb_outer, limb_inner, nouter, ninner, eff, K, mask_bits, s,
+                                  tgt ? tgt->d_scale : nullptr);
+  if (tgt && (!tgt->d_decB_scaled || K != tgt->K)) return cudaErrorInvalidValue;
   const pipe::Plan plan = pipe::make_plan(KB, (K + 15) / 16, (size_t)((K + 15) / 16) * 16 * sizeof(uint2), false);
   if (!plan.ok || plan.nA != 2) return cudaErrorInvalidConfiguration;
   pipe::PipeArgs a;
   a.src = d_limbs; a.src_outer = limb_outer; a.src_inner = limb_inner;
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = eff; a.mask_bits = mask_bits;
-  a.B = c->d_decB; a.b_cols = c->dec_cols;
+  a.B = tgt ? tgt->d_decB_scaled : c->d_decB; a.b_cols = c->dec_cols;
   pipe::fill_args(a, plan);
   DecParams ep;
   ep.res = d_res; ep.res_outer = res_outer; ep.res_inner = res_inner; ep.qmu = c->d_qmu; ep.K = K;

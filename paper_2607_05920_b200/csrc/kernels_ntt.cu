@@ -209,9 +209,14 @@ ntt_col_kernel(NttArgs a) {
 #pragma unroll
       for (int i = 0; i < 16; ++i) x[i] = sm[(i * TPC + t) * T + cc];
       phase_a<true, LN - 4>(x, tw, 1, q, q2);
-      const uint2 sc = __ldg(a.scale + j);
+      if (a.scale) {
+        const uint2 sc = __ldg(a.scale + j);
 #pragma unroll
-      for (int i = 0; i < 16; ++i) g[(size_t)(i * TPC + t) * 256] = mul_shoup(x[i], sc.x, sc.y, q);
+        for (int i = 0; i < 16; ++i) g[(size_t)(i * TPC + t) * 256] = mul_shoup(x[i], sc.x, sc.y, q);
+      } else {                                                     // the constant rides on an operand (fold_scale): canonicalise only
+#pragma unroll
+        for (int i = 0; i < 16; ++i) g[(size_t)(i * TPC + t) * 256] = csub(x[i], q);
+      }
     }
   } else {
 #pragma unroll
@@ -220,10 +225,13 @@ ntt_col_kernel(NttArgs a) {
     if (!INV) {
 #pragma unroll
       for (int i = 0; i < E; ++i) g[(size_t)i * 256] = x[i];
-    } else {
+    } else if (a.scale) {
       const uint2 sc = __ldg(a.scale + j);
 #pragma unroll
       for (int i = 0; i < E; ++i) g[(size_t)i * 256] = mul_shoup(x[i], sc.x, sc.y, q);
+    } else {
+#pragma unroll
+      for (int i = 0; i < E; ++i) g[(size_t)i * 256] = csub(x[i], q);
     }
   }
 }
@@ -273,10 +281,16 @@ ntt_col2_kernel(NttArgs a) {
 #pragma unroll
     for (int i = 0; i < 16; ++i) ld2(sm + (i * TPC + t) * W + 2 * cp, i);
     phase_a_multi<2, true, LN - 4>(x, tw, 1, q, q2);
-    const uint2 sc = __ldg(a.scale + j);
+    if (a.scale) {
+      const uint2 sc = __ldg(a.scale + j);
 #pragma unroll
-    for (int i = 0; i < 16; ++i)
-      *reinterpret_cast<uint2*>(g + (size_t)(i * TPC + t) * 256) = make_uint2(mul_shoup(x[0][i], sc.x, sc.y, q), mul_shoup(x[1][i], sc.x, sc.y, q));
+      for (int i = 0; i < 16; ++i)
+        *reinterpret_cast<uint2*>(g + (size_t)(i * TPC + t) * 256) = make_uint2(mul_shoup(x[0][i], sc.x, sc.y, q), mul_shoup(x[1][i], sc.x, sc.y, q));
+    } else {                                                       // the constant rides on an operand (fold_scale): canonicalise only
+#pragma unroll
+      for (int i = 0; i < 16; ++i)
+        *reinterpret_cast<uint2*>(g + (size_t)(i * TPC + t) * 256) = make_uint2(csub(x[0][i], q), csub(x[1][i], q));
+    }
   }
 }
 
@@ -417,10 +431,9 @@ ntt_row_fused_kernel(NttArgs a) {
   };
   auto finish = [&](uint32_t (&x)[16], uint32_t* g) {
     row_inv_core(x, srow, t, twi, base, q, q2);
-    if (FINAL) {
-      const uint2 sc = __ldg(a.scale + j);
+    if (FINAL) {                                                   // N = 256: no column pass; the constant rides on an operand
 #pragma unroll
-      for (int i = 0; i < 16; ++i) g[i * 16 + t] = mul_shoup(x[i], sc.x, sc.y, q);
+      for (int i = 0; i < 16; ++i) g[i * 16 + t] = csub(x[i], q);
     } else {
 #pragma unroll
       for (int i = 0; i < 16; ++i) g[i * 16 + t] = x[i];
@@ -531,10 +544,10 @@ __device__ __forceinline__ void whole_fwd(uint32_t (&x)[16], uint32_t* tile, uin
   row_fwd_core(x, tile + r * WROW, t, tw, (1u << LN1) + r, q, q2);
   __syncthreads();                                                 // the tile is free for the next operand
 }
-// registers (16 contiguous points of row r, [0, 2q)) -> g[N] (global), scaled by sc
+// registers (16 contiguous points of row r, [0, 2q)) -> g[N] (global), canonical (the final constant rides on an operand)
 template <int LN1>
 __device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restrict__ g, uint32_t* tile, uint32_t tid,
-                                          const uint2* __restrict__ tw, const uint2 sc, uint32_t q, uint32_t q2) {
+                                          const uint2* __restrict__ tw, uint32_t q, uint32_t q2) {
   constexpr int TPC = (1 << LN1) / 16;
   const uint32_t cc = tid & 255, tc = tid >> 8, r = tid >> 4, t = tid & 15;
   row_inv_core(x, tile + r * WROW, t, tw, (1u << LN1) + r, q, q2);   // x[i] = point i * 16 + t of row r
@@ -546,7 +559,7 @@ __device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restric
     for (int i = 0; i < 16; ++i) x[i] = tile[i * WROW + cc];
     phase_b<4, true>(x, tw, 1, 0, q, q2);
 #pragma unroll
-    for (int i = 0; i < 16; ++i) g[i * 256 + cc] = mul_shoup(x[i], sc.x, sc.y, q);
+    for (int i = 0; i < 16; ++i) g[i * 256 + cc] = csub(x[i], q);
   } else {
 #pragma unroll
     for (int i = 0; i < 16; ++i) x[i] = tile[(tc * 16 + i) * WROW + cc];
@@ -558,7 +571,7 @@ __device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restric
     for (int i = 0; i < 16; ++i) x[i] = tile[(i * TPC + tc) * WROW + cc];
     phase_a<true, 1>(x, tw, 1, q, q2);
 #pragma unroll
-    for (int i = 0; i < 16; ++i) g[(i * TPC + tc) * 256 + cc] = mul_shoup(x[i], sc.x, sc.y, q);
+    for (int i = 0; i < 16; ++i) g[(i * TPC + tc) * 256 + cc] = csub(x[i], q);
   }
   __syncthreads();                                                 // the tile is free for the next result
 }
@@ -574,7 +587,6 @@ ntt_whole_kernel(NttArgs a) {
   const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
   const uint2* twf = a.tw2 + (size_t)j * a.N;
   const uint2* twi = a.tw + (size_t)j * a.N;
-  const uint2 sc = __ldg(a.scale + j);
   if constexpr (PW == PW_POLYMUL) {
     uint32_t* g = a.data + (size_t)item * KN + poff;
     uint32_t x[16], y[16];
@@ -584,7 +596,7 @@ ntt_whole_kernel(NttArgs a) {
     whole_fwd<LN1>(y, tile, tid, twf, q, q2);
 #pragma unroll
     for (int i = 0; i < 16; ++i) x[i] = mm(canon4(x[i], q, q2), y[i], q, qn);
-    whole_inv<LN1>(x, g, tile, tid, twi, sc, q, q2);
+    whole_inv<LN1>(x, g, tile, tid, twi, q, q2);
   } else if constexpr (PW == PW_TENSOR) {
     uint32_t* g = a.data + (size_t)item * 4 * KN + poff;           // slots a0, a1, b0, b1 at g + slot * KN
     uint32_t a0[16], a1[16], b0[16], b1[16], x[16];
@@ -611,7 +623,7 @@ ntt_whole_kernel(NttArgs a) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) x[i] = mm(a1[i], b1[i], q, qn);
       }
-      whole_inv<LN1>(x, g + (size_t)op * KN, tile, tid, twi, sc, q, q2);
+      whole_inv<LN1>(x, g + (size_t)op * KN, tile, tid, twi, q, q2);
     }
   } else {   // PW_RELIN: slot 0 = d2 residues; aux = the key, fully transformed and canonical (same point order as whole_fwd leaves)
     static_assert(PW == PW_RELIN, "whole transform: unknown mode");
@@ -626,10 +638,10 @@ ntt_whole_kernel(NttArgs a) {
     for (int i = 0; i < 16; ++i) d[i] = canon4(d[i], q, q2);
 #pragma unroll
     for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e0[i], q, qn);
-    whole_inv<LN1>(x, g, tile, tid, twi, sc, q, q2);
+    whole_inv<LN1>(x, g, tile, tid, twi, q, q2);
 #pragma unroll
     for (int i = 0; i < 16; ++i) x[i] = mm(d[i], e1[i], q, qn);
-    whole_inv<LN1>(x, g + KN, tile, tid, twi, sc, q, q2);
+    whole_inv<LN1>(x, g + KN, tile, tid, twi, q, q2);
   }
 }
 
@@ -703,6 +715,25 @@ cudaError_t measure_int_peak(Context* c, int mode, double* per_s, cudaStream_t s
   return cudaSuccess;
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// The inverse transform of a product ends with a per-prime constant (N^-1 (M/q_j)^-1 2^32: the transform's own scale, the
+// CRT's y_i, the Montgomery factor of the pointwise product).  It is folded into an OPERAND instead (the transforms are
+// linear): the decompose of the second factor uses a constant image that carries it (ctx.cu), and a key (evk-hat, rotation
+// keys) is multiplied by it once, here, when it is installed.  The inverse column pass then only canonicalises.
+// ------------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+scale_rows_kernel(uint32_t* __restrict__ data, const uint2* __restrict__ scale, const uint32_t* __restrict__ qtab, uint32_t N, uint32_t K) {
+  const size_t idx = (size_t)blockIdx.x * 256 + threadIdx.x;      // over [npoly][K][N]
+  const uint32_t j = (uint32_t)((idx / N) % K);
+  const uint2 sc = __ldg(scale + j);
+  data[idx] = mul_shoup(data[idx], sc.x, sc.y, __ldg(qtab + j));
+}
+cudaError_t launch_scale_rows(Context* c, uint32_t* d_res, uint32_t npoly, uint32_t K, const uint2* d_scale, cudaStream_t s) {
+  LaunchTimer lt(c, KC_NTT_FWD, s);
+  scale_rows_kernel<<<(uint32_t)((size_t)npoly * K * c->N / 256), 256, 0, s>>>(d_res, d_scale, c->d_q, c->N, K);
+  return cudaGetLastError();
+}
+
 // ---- launchers ------------------------------------------------------------------------------------------------------
 template <bool INV>
 static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaStream_t s) {
@@ -770,7 +801,7 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
 // S2 + S3 + S4 of a product in three launches (four for PW_POLYMUL): forward column pass over the operand slots, the
 // fused row pass, inverse column pass over the result slots.
 cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uint32_t nitems, uint32_t K, int pw_mode,
-                               const uint2* d_scale, cudaStream_t s, uint32_t aux_group) {
+                               cudaStream_t s, uint32_t aux_group) {
   if (!nitems) return cudaSuccess;
   uint32_t S, Uin, Uout;
   switch (pw_mode) {
@@ -788,7 +819,7 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   // at N = 2^13 (512-thread blocks, one or two per SM: the block-wide barriers of the transpositions are not hidden), so
   // N = 2^13 takes it only on request (fhe_debug_force_pipeline(ctx, 2))
   if ((c->logN == 12 && c->force_pipe != 1) || (c->logN == 13 && c->force_pipe == 2)) {
-    a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = d_scale; a.U = Uout;
+    a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = nullptr; a.U = Uout;
     a.units = nitems * K;
     const uint32_t threads = c->N / 16;
     const size_t smem = (size_t)(c->N / 256) * WROW * sizeof(uint32_t);
@@ -810,7 +841,7 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
       a.data = d_res;
     }
   }
-  a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = d_scale; a.U = Uout;
+  a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = nullptr; a.U = Uout;
   a.units = nitems * K * a.N1;
   const uint32_t blocks = (a.units + FUSED_ROWS - 1) / FUSED_ROWS;
   {

@@ -33,7 +33,7 @@ template <int LMAX>
 __global__ void __launch_bounds__(SMALL_THREADS)
 decompose_small_kernel(uint32_t* __restrict__ res, size_t res_outer, size_t res_inner, const uint32_t* __restrict__ limbs,
                        size_t limb_outer, size_t limb_inner, uint32_t inner, uint32_t N, uint32_t Lin, uint32_t K,
-                       uint32_t mask_bits, const uint4* __restrict__ qsmall) {
+                       uint32_t mask_bits, const uint4* __restrict__ qsmall, const uint2* __restrict__ scale) {
   pdl_sync();
   __shared__ uint4 sq[SMALL_K * 4];
   for (uint32_t j = threadIdx.x; j < K; j += SMALL_THREADS) sq[j] = __ldg(qsmall + j);
@@ -57,6 +57,7 @@ decompose_small_kernel(uint32_t* __restrict__ res, size_t res_outer, size_t res_
     uint32_t r = 0;                                                // limbs >= Lin are zero: their Horner steps leave r = 0
 #pragma unroll
     for (int l = LMAX - 1; l >= 0; --l) r = (LMAX > 2 && (uint32_t)l >= Lin) ? r : horner_step(r, x[l], qc);
+    if (scale) { const uint2 sc = __ldg(scale + j); r = mul_shoup(r, sc.x, sc.y, qc.x); }   // the product's final constant rides here
     dst[(size_t)j * N] = r;                                        // canonical
   }
 }
@@ -117,13 +118,12 @@ bool small_crt_ok(const Context* c, const CrtTarget& tg, const PostParams& pp) {
 
 cudaError_t launch_decompose_small(Context* c, uint32_t* d_res, size_t res_outer, size_t res_inner, const uint32_t* d_limbs,
                                    size_t limb_outer, size_t limb_inner, uint32_t nouter, uint32_t ninner, uint32_t Lin_eff,
-                                   uint32_t K, uint32_t mask_bits, cudaStream_t s, bool lazy) {
-  (void)lazy;
+                                   uint32_t K, uint32_t mask_bits, cudaStream_t s, const uint2* d_scale) {
   LaunchTimer lt(c, KC_DECOMPOSE, s);
   const uint32_t grid = (c->N / SMALL_THREADS) * nouter * ninner;
   cudaError_t e;
 #define DEC_SMALL(LM) launch_pdl(decompose_small_kernel<LM>, grid, SMALL_THREADS, 0, s, d_res, res_outer, res_inner, d_limbs, \
-                                 limb_outer, limb_inner, ninner, c->N, Lin_eff, K, mask_bits, (const uint4*)c->d_qsmall)
+                                 limb_outer, limb_inner, ninner, c->N, Lin_eff, K, mask_bits, (const uint4*)c->d_qsmall, d_scale)
   if (Lin_eff <= 2) e = DEC_SMALL(2);
   else if (Lin_eff <= 4) e = DEC_SMALL(4);
   else if (Lin_eff <= 8) e = DEC_SMALL(8);
