@@ -152,6 +152,7 @@ struct CrtEpi {
   static constexpr int LOAD_WORDS = 64, MAX_REGS = 96;     // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K
   static constexpr uint32_t GROUPS = 2, LOAD_WARPS = 8;
   static constexpr bool LOAD_ALT = false;
+  static constexpr bool LOAD_TMA = true;                   // residues staged through shared memory by one tensor copy per tile
   static constexpr bool TILE_ALT = true;                   // two whole epilogues on alternate tiles: the epilogue bounds S5
   static constexpr bool CHUNK_ALT = false;
   static constexpr bool RELIN = MODE == POST_CKKS_RELIN || MODE == POST_BGV_RELIN;
@@ -595,15 +596,25 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   CrtParams ep;
   size_t epi_bytes;
   crt_scratch_layout(tg, pp, ep, epi_bytes);
-  const pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true, CrtEpiAny::TILE_ALT);
+  pipe::Plan plan = pipe::make_plan(tg.KB, tg.nchunks, epi_bytes, true, CrtEpiAny::TILE_ALT);
   if (!plan.ok) return cudaErrorInvalidConfiguration;
   const bool relin = pp.mode == POST_CKKS_RELIN || pp.mode == POST_BGV_RELIN;
   if (relin && !d_add) return cudaErrorInvalidValue;
+  // TMA staging of the residues: the source as a matrix [rows][N], polynomial (o, i) starting at row (o outer + i inner) / N
+  CUtensorMap tmap;
+  bool use_tma = false;
+  if (res_outer % c->N == 0 && res_inner % c->N == 0 && tg.K <= 256 && c->force_pipe != 2) {
+    pipe::add_ring(plan, tg.K);
+    const uint64_t rows = (uint64_t)(nouter - 1) * (res_outer / c->N) + (uint64_t)(ninner - 1) * (res_inner / c->N) + tg.K;
+    use_tma = plan.ring_slots > 0 && pipe::make_tensor_map(&tmap, d_res, rows, c->N, tg.K);
+  }
   pipe::PipeArgs a;
   a.src = d_res; a.src_outer = res_outer; a.src_inner = res_inner;
   a.inner = ninner; a.npoly = nouter * ninner; a.N = c->N; a.nwords = tg.K; a.mask_bits = 0;
   a.B = tg.d_B; a.b_cols = tg.nchunks * pipe::NC;
   pipe::fill_args(a, plan);
+  a.row_outer = (uint32_t)(res_outer / c->N); a.row_inner = (uint32_t)(res_inner / c->N);
+  const CUtensorMap* tm = use_tma ? &tmap : nullptr;
   ep.out = d_out; ep.out_outer = out_outer; ep.out_inner = out_inner;
   ep.add = relin ? d_add : nullptr; ep.add_outer = add_outer; ep.add_inner = add_inner;
   ep.negM = tg.d_negM; ep.Lraw = tg.Lraw; ep.Lx = tg.Lx; ep.pp = pp;
@@ -624,14 +635,14 @@ cudaError_t launch_crt(Context* c, const CrtTarget& tg, const PostParams& pp, ui
   {
     LaunchTimer lt(c, KC_CRT, s);
     switch (pp.mode) {
-      case POST_CKKS_MASK: e = pipe::launch_pipe<CrtEpi<POST_CKKS_MASK, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
-      case POST_BGV_MODQ: e = pipe::launch_pipe<CrtEpi<POST_BGV_MODQ, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
-      case POST_BGV_RELIN: e = pipe::launch_pipe<CrtEpi<POST_BGV_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s); break;
+      case POST_CKKS_MASK: e = pipe::launch_pipe<CrtEpi<POST_CKKS_MASK, false, false>>(a, ep, plan.smem, c->n_sm, s, tm); break;
+      case POST_BGV_MODQ: e = pipe::launch_pipe<CrtEpi<POST_BGV_MODQ, false, false>>(a, ep, plan.smem, c->n_sm, s, tm); break;
+      case POST_BGV_RELIN: e = pipe::launch_pipe<CrtEpi<POST_BGV_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s, tm); break;
       case POST_CKKS_RELIN:
-        if (tg.top) e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, true>>(a, ep, plan.smem, c->n_sm, s)
-                           : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, false>>(a, ep, plan.smem, c->n_sm, s);
-        else e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, true>>(a, ep, plan.smem, c->n_sm, s)
-                    : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s);
+        if (tg.top) e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, true>>(a, ep, plan.smem, c->n_sm, s, tm)
+                           : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, true, false>>(a, ep, plan.smem, c->n_sm, s, tm);
+        else e = pb ? pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, true>>(a, ep, plan.smem, c->n_sm, s, tm)
+                    : pipe::launch_pipe<CrtEpi<POST_CKKS_RELIN, false, false>>(a, ep, plan.smem, c->n_sm, s, tm);
         break;
       default: e = cudaErrorInvalidValue;
     }

@@ -32,6 +32,7 @@ struct DecEpi {
   static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
   static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
   static constexpr bool TILE_ALT = false, CHUNK_ALT = true;
+  static constexpr bool LOAD_TMA = false;
   static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: with four loader warps (one tile) the
                                                          // MMA thread waited 1400 cycles per tile for its A operand
   static constexpr int PPG = 8;                          // primes per consume call: half a chunk

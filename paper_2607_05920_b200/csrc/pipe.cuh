@@ -24,6 +24,8 @@
 // When the constant matrix has more columns than that (or than shared memory holds), the launch runs several passes over
 // its tiles, pass p with columns [p * cpp * 64, ...) of B resident in shared memory (loaded once per pass per CTA).
 #pragma once
+#include <cstring>
+#include <cuda.h>   // CUtensorMap (the type only; the encoder is fetched through the runtime, no libcuda link)
 #include "umma.cuh"
 
 namespace fhe {
@@ -42,6 +44,7 @@ struct Ctrl {
   uint64_t d_full[2][MAX_SPANS];              // [accumulator set] the span's accumulators finished (MMA commit)
   uint64_t d_free[2][MAX_CHUNKS];                // the chunk's accumulators are in registers (one arrival per epilogue warp)
   uint64_t g_full[MAX_SPANS][4];              // CHUNK_ALT: the span finished, barrier [wi mod 4] for work item wi
+  uint64_t r_full[2], r_free[2];              // TMA staging ring of the A source: slot landed (tx bytes) / read out by every loader warp
   uint64_t b_full, mma_done;                  // B of the pass landed (bulk copies) / every MMA of the pass finished
   uint32_t tmem_base;
 };
@@ -60,11 +63,15 @@ struct PipeArgs {
   uint32_t nA, nsets, tmem_cols;              // nsets: accumulator column sets (2: tiles alternate between them, TILE_ALT)
   uint32_t epi_stride;                        // TILE_ALT: bytes between the scratch regions of the two epilogue groups
   uint32_t epi_off, b_off;                    // byte offsets of the epilogue scratch and of B in dynamic smem
+  // TMA staging of the A source (Epi::LOAD_TMA): ring_slots tiles of [nwords][128] words at ring_off, filled by one 2-D
+  // tensor copy each from the matrix view [rows][N] of the source (row of word w of polynomial (o, i) = row_outer o + row_inner i + w)
+  uint32_t ring_slots, ring_off, row_outer, row_inner;
 };
 
 // ---- host-side plan -----------------------------------------------------------------------------------------------------
 struct Plan {
   uint32_t KB = 0, nchunks = 0, npass = 0, cpp = 0, nA = 0, nsets = 1, tmem_cols = 0, epi_off = 0, b_off = 0, epi_stride = 0;
+  uint32_t ring_slots = 0, ring_off = 0;      // TMA staging ring (add_ring)
   size_t smem = 0;
   bool ok = false;
 };
@@ -103,10 +110,23 @@ inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool sing
   p.ok = true;
   return p;
 }
+// Room behind B for TWO staged tiles of `nwords` source words ([nwords][128] uint32 each), or no ring at all.  The ring is
+// only taken while the CTA stays within RING_SMEM_CAP: the launches overlap their neighbours' tails (PDL), and a CTA that
+// fills the SM's shared memory cannot become resident beside the last CTAs of the transform before it -- measured at the
+// bench shape, a 204 KB relin CRT lost 0.075 ms of the step to that while its own time fell by 0.008 ms; one slot alone was
+// slower than register-landing loads.
+constexpr size_t RING_SMEM_CAP = 160 * 1024;
+inline void add_ring(Plan& p, uint32_t nwords) {
+  if (!p.ok || p.npass != 1) return;
+  const size_t off = (p.smem + 127) & ~(size_t)127, slot = (size_t)nwords * TILE_M * 4;
+  if (off + 2 * slot > RING_SMEM_CAP) return;
+  p.ring_slots = 2; p.ring_off = (uint32_t)off; p.smem = off + 2 * slot;
+}
 inline void fill_args(PipeArgs& a, const Plan& p) {
   a.KB = p.KB; a.nchunks = p.nchunks; a.npass = p.npass; a.cpp = p.cpp; a.nA = p.nA; a.nsets = p.nsets; a.tmem_cols = p.tmem_cols;
   a.epi_stride = p.epi_stride;
   a.epi_off = p.epi_off; a.b_off = p.b_off;
+  a.ring_slots = p.ring_slots; a.ring_off = p.ring_off; a.row_outer = a.row_inner = 0;
 }
 
 #ifdef __CUDACC__
@@ -142,6 +162,13 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// one 2-D tensor copy global -> shared (TMA): box [rows][128 words] at (column c0, row c1) of the tensor map, bytes counted on bar
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, uint32_t c0, uint32_t c1, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                   smem_u32(smem_dst)),
+               "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+               : "memory");
+}
 // streaming load: read once, no L1 line allocated for it
 __device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
   uint32_t v;
@@ -175,6 +202,8 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 //   static constexpr bool LOAD_ALT;                                   8 loader warps only.  false: the two warps of a lane quarter
 //                                                                     split the words of every tile; true: they take alternate
 //                                                                     tiles whole (two tiles' loads in flight; needs nA = 2)
+//   static constexpr bool LOAD_TMA;                                   the A source may be staged through shared memory by TMA
+//                                                                     (PipeArgs::ring_slots > 0; needs !LOAD_ALT and a single pass)
 //   static constexpr int LOAD_WORDS, MAX_REGS;                        words of its row a loader thread has in flight
 //                                                                     (multiple of 8); register cap of the kernel
 //   static constexpr uint32_t GROUPS;                                 1, 2 or 4 epilogue warp groups: group g takes columns
@@ -216,7 +245,8 @@ __device__ __forceinline__ void tmem_ld_cols(uint32_t taddr, uint32_t* r) {
 
 template <class Epi>
 __global__ void __maxnreg__(Epi::MAX_REGS)   // 64 K registers / (warps rounded up to a multiple of 4) / 32
-pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename Epi::Params ep) {
+pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename Epi::Params ep,
+            const __grid_constant__ CUtensorMap tmap) {
   constexpr uint32_t GROUPS = Epi::GROUPS, EPIW = 4 * GROUPS, LOAD_WARPS = Epi::LOAD_WARPS, HALVES = LOAD_WARPS / 4,
                      MMAW = EPIW + LOAD_WARPS, GC = NC / GROUPS;
   constexpr int LR = Epi::LOAD_WORDS;
@@ -246,6 +276,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
       mbar_init(&ctl->d_free[0][i], (Epi::TILE_ALT || Epi::CHUNK_ALT) ? 4 : EPIW);
       mbar_init(&ctl->d_free[1][i], (Epi::TILE_ALT || Epi::CHUNK_ALT) ? 4 : EPIW);
     }
+    for (uint32_t i = 0; i < 2; ++i) { mbar_init(&ctl->r_full[i], 1); mbar_init(&ctl->r_free[i], LOAD_WARPS); }
     mbar_init(&ctl->b_full, 1); mbar_init(&ctl->mma_done, 1);
     fence_barrier_init();
   }
@@ -319,6 +350,53 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
     // mask_bits != 0 reduces the row mod 2^mask_bits: its top word is cut (the words above are not loaded at all)
     const uint32_t mask_w = a.mask_bits >> 5, mask_m = (a.mask_bits & 31) ? (1u << (a.mask_bits & 31)) - 1u : 0u;
     uint32_t wi = 0;
+    if (Epi::LOAD_TMA && a.ring_slots) {
+      // TMA-staged source (single pass, loaders split the words of a tile): loader warp 0 keeps up to ring_slots tiles in
+      // flight as ONE 2-D tensor copy each into shared memory; every loader warp then moves its words shared -> registers ->
+      // TMEM.  The loads of the tiles ahead no longer wait for the registers of the tile being stored (with register-landing
+      // loads a tile's loads were issued only after the previous tile's tcgen05.st, and the MMA thread waited for its A
+      // operand 800-3300 cycles per tile), and 500 LDG.32 per tile leave the LSU.
+      const uint32_t nslots = a.ring_slots, slot_words = a.nwords * TILE_M;
+      uint32_t* ring = reinterpret_cast<uint32_t*>(smem + a.ring_off);
+      auto issue = [&](uint32_t k) {                               // lane 0 of loader warp 0
+        const uint32_t tile = blockIdx.x + k * gridDim.x, poly = tile / tpp, tin = tile % tpp;
+        const uint32_t row0 = (poly / a.inner) * a.row_outer + (poly % a.inner) * a.row_inner, slot = k % nslots;
+        mbar_expect_tx(&ctl->r_full[slot], slot_words * 4);
+        tma_load_2d(ring + (size_t)slot * slot_words, &tmap, tin * TILE_M, row0, &ctl->r_full[slot]);
+      };
+      if (lw == 0 && lane == 0)
+        for (uint32_t k = 0; k < nslots && k < mine; ++k) issue(k);
+      const uint32_t wph = ((a_cols + HALVES - 1) / HALVES + 7) / 8 * 8;
+      const uint32_t w_lo = half * wph, w_hi = w_lo + wph < a_cols ? w_lo + wph : a_cols;
+      const uint32_t lim = w_hi < a.nwords ? w_hi : a.nwords;
+      for (uint32_t k = 0; k < mine; ++k, ++wi) {
+        const uint32_t slot = k % nslots, ph = (k / nslots) & 1, abuf = wi & amask;
+        const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
+        const uint32_t* src = ring + (size_t)slot * slot_words + row;
+        mbar_wait(&ctl->r_full[slot], ph);
+        bool waited = false;
+        for (uint32_t w0 = w_lo; w0 < w_hi; w0 += LR) {
+          uint32_t w[LR];
+#pragma unroll
+          for (int i = 0; i < LR; ++i) w[i] = w0 + i < lim ? src[(w0 + i) * TILE_M] : 0u;   // warp-uniform predicate
+          if (!waited) {
+            mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
+            tc_fence_after();
+            waited = true;
+          }
+          store_batch<LR>(w, taddr, w0, w_hi);
+        }
+        if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
+        tmem_st_wait();                                            // the registers (hence the slot) have been read
+        tc_fence_before();
+        if (lane == 0) { mbar_arrive(&ctl->a_full[abuf]); mbar_arrive(&ctl->r_free[slot]); }
+        if (lw == 0 && lane == 0 && k + nslots < mine) {           // refill the slot once every loader warp is done with it
+          mbar_wait(&ctl->r_free[slot], ph);
+          issue(k + nslots);
+        }
+        __syncwarp();
+      }
+    } else
     for (uint32_t ps = 0; ps < a.npass; ++ps) {
       for (uint32_t k = 0; k < mine; ++k, ++wi) {
         if (ALT && (wi & 1) != half) continue;
@@ -468,8 +546,34 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   if (warp == MMAW) tmem_dealloc(tmem_a, a.tmem_cols);
 }
 
+// 2-D tensor map over a word-major source seen as a matrix [rows][N] of uint32, box [box_rows][128]: the driver's encoder,
+// fetched through the runtime (no link against libcuda).  false: no encoder / bad arguments -- the caller falls back to
+// register-landing loads.
+inline bool make_tensor_map(CUtensorMap* tm, const uint32_t* base, uint64_t rows, uint32_t N, uint32_t box_rows) {
+  typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                             const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Encode enc = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+      enc = (Encode)fn;
+    else
+      cudaGetLastError();
+  }
+  if (!enc || box_rows == 0 || box_rows > 256 || rows == 0) return false;
+  const cuuint64_t gdim[2] = {N, rows}, gstride[1] = {(cuuint64_t)N * 4};
+  const cuuint32_t box[2] = {(cuuint32_t)TILE_M, box_rows}, estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, (void*)base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <class Epi>
-inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params& ep, size_t smem, int n_sm, cudaStream_t s) {
+inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params& ep, size_t smem, int n_sm, cudaStream_t s,
+                               const CUtensorMap* tmap = nullptr) {
   // the attribute belongs to the (kernel, device) pair: one high-water mark per device
   constexpr int MAX_DEV = 64;
   static size_t configured[MAX_DEV] = {};
@@ -482,9 +586,11 @@ inline cudaError_t launch_pipe(const PipeArgs& a_in, const typename Epi::Params&
     if (dev >= 0 && dev < MAX_DEV) configured[dev] = smem;
   }
   PipeArgs a = a_in;
+  CUtensorMap tm;
+  if (tmap) tm = *tmap; else { memset(&tm, 0, sizeof(tm)); a.ring_slots = 0; }
   const uint32_t ntiles = a.npoly * (a.N / TILE_M);
   const uint32_t grid = ntiles < (uint32_t)n_sm ? ntiles : (uint32_t)n_sm;
-  const cudaError_t e = launch_pdl(pipe_kernel<Epi>, grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s, a, ep);
+  const cudaError_t e = launch_pdl(pipe_kernel<Epi>, grid, nthreads(Epi::GROUPS, Epi::LOAD_WARPS), smem, s, a, ep, tm);
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 #endif  // __CUDACC__
