@@ -229,6 +229,12 @@ __device__ __forceinline__ uint32_t mulhi32(uint32_t a, uint32_t b) { return __u
 
 // x in [0, 2q) -> [0, q)
 __device__ __forceinline__ uint32_t csub(uint32_t x, uint32_t q) { return min(x, x - q); }
+// a b + c with a 64-bit sum (IMAD.WIDE.U32): one instruction on the FMA pipe
+__device__ __forceinline__ uint64_t madw(uint32_t a, uint32_t b, uint64_t c) {
+  uint64_t d;
+  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
+  return d;
+}
 
 // Shoup multiplication by a constant w < q with companion w' = floor(w 2^32 / q): result in [0, 2q), any a < 2^32.
 __device__ __forceinline__ uint32_t mul_shoup_lazy(uint32_t a, uint32_t w, uint32_t wp, uint32_t q) {

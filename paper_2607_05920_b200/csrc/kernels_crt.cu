@@ -141,12 +141,6 @@ struct CrtParams {
   PostParams pp;
 };
 
-__device__ __forceinline__ uint64_t madw(uint32_t a, uint32_t b, uint64_t c) {
-  uint64_t d;
-  asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(d) : "r"(a), "r"(b), "l"(c));
-  return d;
-}
-
 template <int MODE, bool TOP, bool RESC>
 struct CrtEpi {
   static constexpr int LOAD_WORDS = 64, MAX_REGS = 96;     // 17 warps are allocated as 20: 20 x 32 x 96 <= 64 K

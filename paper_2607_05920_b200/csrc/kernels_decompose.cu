@@ -32,7 +32,8 @@ struct DecEpi {
   static constexpr int LOAD_WORDS = 40, MAX_REGS = 72;   // 25 warps are allocated as 28: 28 x 32 x 72 <= 64 K
   static constexpr uint32_t GROUPS = 4, LOAD_WARPS = 8;
   static constexpr bool TILE_ALT = false, CHUNK_ALT = true;
-  static constexpr bool LOAD_TMA = false;
+  static constexpr bool LOAD_TMA = false;                // staging the limbs through shared memory by TMA (as the CRT does) measured
+                                                         // 0.017 ms slower per step than two tiles of register-landing loads
   static constexpr bool LOAD_ALT = true;                 // the loads of two tiles in flight: with four loader warps (one tile) the
                                                          // MMA thread waited 1400 cycles per tile for its A operand
   static constexpr int PPG = 8;                          // primes per consume call: half a chunk
@@ -50,7 +51,10 @@ struct DecEpi {
   __device__ __forceinline__ void begin_tile(uint32_t o, uint32_t i, uint32_t n0) {
     out = p.res + (size_t)o * p.res_outer + (size_t)i * p.res_inner + n0 + etid;
   }
-  // qm = (2^32 - q, floor(2^53 / q)): with -q in the table the remainder is one multiply-add, lo + qh * (-q)
+  // qm = (2^32 - q, floor(2^53 / q)): with -q in the table the remainder is one multiply-add, lo + qh * (-q).  (Forming the
+  // 48-bit value with three 64-bit multiply-adds and one funnel shift -- 4 instructions for these 6 -- measured 0.025 ms
+  // SLOWER per step, and one multiply-add per store address 0.009 ms slower: IMAD.WIDE does not issue at the rate of the
+  // shifts and adds it replaces.)
   __device__ __forceinline__ uint32_t reduce(const uint32_t* t, const uint2 qm) const {
     const uint32_t lo = t[0] + (t[1] << 8) + (t[2] << 16) + (t[3] << 24);
     const uint32_t vh = (t[3] << 3) + (t[2] >> 5) + (t[1] >> 13);
@@ -58,17 +62,20 @@ struct DecEpi {
     const uint32_t r = lo + qh * qm.x;
     return LAZY ? r : csub(r, 0u - qm.x);
   }
-  // The constants are read and all residues of the call computed before the first store: a store through `out` may alias
-  // the table as far as the compiler knows, and interleaved they run one residue at a time (LDS -> chain -> STG: 65 cycles
-  // per residue measured) instead of PPG independent chains.
+  // The constants are read (two primes per 16-byte load) and all residues of the call computed before the first store: a
+  // store through `out` may alias the table as far as the compiler knows, and interleaved they run one residue at a time
+  // (LDS -> chain -> STG: 65 cycles per residue measured) instead of PPG independent chains.
   __device__ __forceinline__ void consume(uint32_t col0, const uint32_t* t) {
     const uint32_t j0 = col0 / 4;
-    uint2 qm[PPG];
+    uint4 qm2[PPG / 2];
 #pragma unroll
-    for (int e = 0; e < PPG; ++e) qm[e] = tab[j0 + e];
+    for (int e = 0; e < PPG / 2; ++e) qm2[e] = reinterpret_cast<const uint4*>(tab + j0)[e];
     uint32_t r[PPG];
 #pragma unroll
-    for (int e = 0; e < PPG; ++e) r[e] = reduce(t + 4 * e, qm[e]);
+    for (int e = 0; e < PPG; e += 2) {
+      r[e] = reduce(t + 4 * e, make_uint2(qm2[e / 2].x, qm2[e / 2].y));
+      r[e + 1] = reduce(t + 4 * e + 4, make_uint2(qm2[e / 2].z, qm2[e / 2].w));
+    }
     uint32_t* o = out + (size_t)j0 * N;
     if (j0 + PPG <= p.K) {
 #pragma unroll

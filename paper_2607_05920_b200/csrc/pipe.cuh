@@ -117,7 +117,7 @@ inline Plan make_plan(uint32_t KB, uint32_t nchunks, size_t epi_bytes, bool sing
 // slower than register-landing loads.
 constexpr size_t RING_SMEM_CAP = 160 * 1024;
 inline void add_ring(Plan& p, uint32_t nwords) {
-  if (!p.ok || p.npass != 1) return;
+  if (!p.ok) return;
   const size_t off = (p.smem + 127) & ~(size_t)127, slot = (size_t)nwords * TILE_M * 4;
   if (off + 2 * slot > RING_SMEM_CAP) return;
   p.ring_slots = 2; p.ring_off = (uint32_t)off; p.smem = off + 2 * slot;
@@ -203,7 +203,8 @@ __device__ __forceinline__ void store_batch(uint32_t (&w)[LR], uint32_t taddr_a,
 //                                                                     split the words of every tile; true: they take alternate
 //                                                                     tiles whole (two tiles' loads in flight; needs nA = 2)
 //   static constexpr bool LOAD_TMA;                                   the A source may be staged through shared memory by TMA
-//                                                                     (PipeArgs::ring_slots > 0; needs !LOAD_ALT and a single pass)
+//                                                                     (PipeArgs::ring_slots > 0; the loader warps of a lane quarter then
+//                                                                     split the words of every tile, whatever LOAD_ALT says)
 //   static constexpr int LOAD_WORDS, MAX_REGS;                        words of its row a loader thread has in flight
 //                                                                     (multiple of 8); register cap of the kernel
 //   static constexpr uint32_t GROUPS;                                 1, 2 or 4 epilogue warp groups: group g takes columns
@@ -265,7 +266,7 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   const uint32_t amask = a.nA - 1, ashift = a.nA - 1;              // nA in {1, 2}
 
   if (tid == 0) {
-    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], ALT ? 4 : LOAD_WARPS); mbar_init(&ctl->a_free[i], 1); }
+    for (uint32_t i = 0; i < MAX_A; ++i) { mbar_init(&ctl->a_full[i], (ALT && !(Epi::LOAD_TMA && a.ring_slots)) ? 4 : LOAD_WARPS); mbar_init(&ctl->a_free[i], 1); }
     for (uint32_t i = 0; i < MAX_SPANS; ++i) {
       mbar_init(&ctl->d_full[0][i], 1); mbar_init(&ctl->d_full[1][i], 1);
       for (uint32_t g = 0; g < 4; ++g) mbar_init(&ctl->g_full[i][g], 1);
@@ -351,26 +352,27 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
     const uint32_t mask_w = a.mask_bits >> 5, mask_m = (a.mask_bits & 31) ? (1u << (a.mask_bits & 31)) - 1u : 0u;
     uint32_t wi = 0;
     if (Epi::LOAD_TMA && a.ring_slots) {
-      // TMA-staged source (single pass, loaders split the words of a tile): loader warp 0 keeps up to ring_slots tiles in
+      // TMA-staged source (the loader warps of a lane quarter split the words of a tile): loader warp 0 keeps up to ring_slots tiles in
       // flight as ONE 2-D tensor copy each into shared memory; every loader warp then moves its words shared -> registers ->
       // TMEM.  The loads of the tiles ahead no longer wait for the registers of the tile being stored (with register-landing
       // loads a tile's loads were issued only after the previous tile's tcgen05.st, and the MMA thread waited for its A
       // operand 800-3300 cycles per tile), and 500 LDG.32 per tile leave the LSU.
       const uint32_t nslots = a.ring_slots, slot_words = a.nwords * TILE_M;
       uint32_t* ring = reinterpret_cast<uint32_t*>(smem + a.ring_off);
-      auto issue = [&](uint32_t k) {                               // lane 0 of loader warp 0
-        const uint32_t tile = blockIdx.x + k * gridDim.x, poly = tile / tpp, tin = tile % tpp;
-        const uint32_t row0 = (poly / a.inner) * a.row_outer + (poly % a.inner) * a.row_inner, slot = k % nslots;
+      const uint32_t total = a.npass * mine;                       // every pass stages the tiles again
+      auto issue = [&](uint32_t it) {                              // lane 0 of loader warp 0
+        const uint32_t tile = blockIdx.x + (it % mine) * gridDim.x, poly = tile / tpp, tin = tile % tpp;
+        const uint32_t row0 = (poly / a.inner) * a.row_outer + (poly % a.inner) * a.row_inner, slot = it % nslots;
         mbar_expect_tx(&ctl->r_full[slot], slot_words * 4);
         tma_load_2d(ring + (size_t)slot * slot_words, &tmap, tin * TILE_M, row0, &ctl->r_full[slot]);
       };
       if (lw == 0 && lane == 0)
-        for (uint32_t k = 0; k < nslots && k < mine; ++k) issue(k);
+        for (uint32_t it = 0; it < nslots && it < total; ++it) issue(it);
       const uint32_t wph = ((a_cols + HALVES - 1) / HALVES + 7) / 8 * 8;
       const uint32_t w_lo = half * wph, w_hi = w_lo + wph < a_cols ? w_lo + wph : a_cols;
       const uint32_t lim = w_hi < a.nwords ? w_hi : a.nwords;
-      for (uint32_t k = 0; k < mine; ++k, ++wi) {
-        const uint32_t slot = k % nslots, ph = (k / nslots) & 1, abuf = wi & amask;
+      for (; wi < total; ++wi) {
+        const uint32_t slot = wi % nslots, ph = (wi / nslots) & 1, abuf = wi & amask;
         const uint32_t taddr = tmem_a + abuf * a_cols + ((quarter * 32u) << 16);
         const uint32_t* src = ring + (size_t)slot * slot_words + row;
         mbar_wait(&ctl->r_full[slot], ph);
@@ -384,15 +386,20 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
             tc_fence_after();
             waited = true;
           }
+          if (mask_m && mask_w - w0 < (uint32_t)LR) {              // the batch holding the top word of a masked input
+#pragma unroll
+            for (int i = 0; i < LR; ++i)
+              if (w0 + i == mask_w) w[i] &= mask_m;
+          }
           store_batch<LR>(w, taddr, w0, w_hi);
         }
         if (!waited) mbar_wait(&ctl->a_free[abuf], ((wi >> ashift) & 1) ^ 1);
         tmem_st_wait();                                            // the registers (hence the slot) have been read
         tc_fence_before();
         if (lane == 0) { mbar_arrive(&ctl->a_full[abuf]); mbar_arrive(&ctl->r_free[slot]); }
-        if (lw == 0 && lane == 0 && k + nslots < mine) {           // refill the slot once every loader warp is done with it
+        if (lw == 0 && lane == 0 && wi + nslots < total) {         // refill the slot once every loader warp is done with it
           mbar_wait(&ctl->r_free[slot], ph);
-          issue(k + nslots);
+          issue(wi + nslots);
         }
         __syncwarp();
       }
