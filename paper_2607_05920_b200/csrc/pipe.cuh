@@ -25,7 +25,6 @@
 // its tiles, pass p with columns [p * cpp * 64, ...) of B resident in shared memory (loaded once per pass per CTA).
 #pragma once
 #include <cstring>
-#include <cuda.h>   // CUtensorMap (the type only; the encoder is fetched through the runtime, no libcuda link)
 #include "umma.cuh"
 
 namespace fhe {
@@ -162,13 +161,6 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
-// one 2-D tensor copy global -> shared (TMA): box [rows][128 words] at (column c0, row c1) of the tensor map, bytes counted on bar
-__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, uint32_t c0, uint32_t c1, uint64_t* bar) {
-  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
-                   smem_u32(smem_dst)),
-               "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-               : "memory");
-}
 // streaming load: read once, no L1 line allocated for it
 __device__ __forceinline__ uint32_t ld_stream(const uint32_t* p) {
   uint32_t v;
@@ -551,31 +543,6 @@ pipe_kernel(const __grid_constant__ PipeArgs a, const __grid_constant__ typename
   tc_fence_before();
   __syncthreads();
   if (warp == MMAW) tmem_dealloc(tmem_a, a.tmem_cols);
-}
-
-// 2-D tensor map over a word-major source seen as a matrix [rows][N] of uint32, box [box_rows][128]: the driver's encoder,
-// fetched through the runtime (no link against libcuda).  false: no encoder / bad arguments -- the caller falls back to
-// register-landing loads.
-inline bool make_tensor_map(CUtensorMap* tm, const uint32_t* base, uint64_t rows, uint32_t N, uint32_t box_rows) {
-  typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                             const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  static Encode enc = nullptr;
-  static bool tried = false;
-  if (!tried) {
-    tried = true;
-    void* fn = nullptr;
-    cudaDriverEntryPointQueryResult qr;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
-      enc = (Encode)fn;
-    else
-      cudaGetLastError();
-  }
-  if (!enc || box_rows == 0 || box_rows > 256 || rows == 0) return false;
-  const cuuint64_t gdim[2] = {N, rows}, gstride[1] = {(cuuint64_t)N * 4};
-  const cuuint32_t box[2] = {(cuuint32_t)TILE_M, box_rows}, estr[2] = {1, 1};
-  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, (void*)base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 template <class Epi>

@@ -9,6 +9,7 @@
 // matrices), accumulators in TMEM, read back with tcgen05.ld.  The pipeline built from these pieces is pipe.cuh.
 // Everything here is inline PTX; there is no library dependency.
 #pragma once
+#include <cuda.h>   // CUtensorMap (the type only; the encoder is fetched through the runtime, no libcuda link)
 #include <cuda_runtime.h>
 #include <cstdint>
 
@@ -17,6 +18,32 @@ namespace umma {
 
 constexpr int TILE_M = 128;          // rows (coefficients) per CTA = TMEM lanes = threads
 constexpr int KSTEP = 32;            // bytes of the contraction dimension one kind::i8 instruction consumes
+
+// 2-D tensor map over a word matrix [rows][cols] of uint32 (row-major, dense), box [box_rows][box_cols]: the driver's
+// encoder, fetched through the runtime (no link against libcuda).  false: no encoder / bad arguments -- callers fall back
+// to loads that land in registers.
+inline bool make_tensor_map(CUtensorMap* tm, const uint32_t* base, uint64_t rows, uint32_t cols, uint32_t box_rows,
+                            uint32_t box_cols = TILE_M) {
+  typedef CUresult (*Encode)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                             const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                             CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static Encode enc = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+      enc = (Encode)fn;
+    else
+      cudaGetLastError();
+  }
+  if (!enc || box_rows == 0 || box_rows > 256 || box_cols == 0 || box_cols > 256 || rows == 0) return false;
+  const cuuint64_t gdim[2] = {cols, rows}, gstride[1] = {(cuuint64_t)cols * 4};
+  const cuuint32_t box[2] = {box_cols, box_rows}, estr[2] = {1, 1};
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, (void*)base, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -60,6 +87,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   }
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// one 2-D tensor copy global -> shared (TMA): the map's box at (column c0, row c1) of the tensor map, bytes counted on bar
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, uint32_t c0, uint32_t c1, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                   smem_u32(smem_dst)),
+               "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+               : "memory");
+}
+// orders this thread's earlier generic-proxy accesses to shared memory before later async-proxy (TMA) ones
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 // ---- bulk copy global -> shared (1-D TMA), completion counted in bytes on an mbarrier -------------------------------------
 __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
