@@ -335,8 +335,8 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   c->dec_KBimg = (4 * MAX_LIMBS_IN + 31) / 32 * 32;
   c->dec_cols = (Kmax + 15) / 16 * DEC_NC;               // image [dec_KBimg / 16][dec_cols][16 bytes] (pipe.cuh)
   c->h_psi.resize(Kmax);
-  std::vector<uint2> twf((size_t)Kmax * N), twi((size_t)Kmax * N);
-  std::vector<uint32_t> pw(N), ipw(N);
+  std::vector<uint2> twf((size_t)Kmax * N);             // the one twiddle table: the inverse stages read it mirrored (kernels_ntt.cu, bf_inv)
+  std::vector<uint32_t> pw(N);
   for (uint32_t j = 0; j < Kmax; ++j) {
     const uint32_t q = c->h_q[j];
     uint32_t inv = 1;                                  // q^-1 mod 2^32 by Newton iteration
@@ -351,13 +351,11 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     }
     if (!psi) { destroy(c); return fail(nullptr, FHE_ERR_UNSUPPORTED, "no primitive root found"); }
     c->h_psi[j] = psi;
-    const uint32_t ipsi = powmod(psi, q - 2, q);
-    pw[0] = ipw[0] = 1;
-    for (uint32_t k = 1; k < N; ++k) { pw[k] = mulmod(pw[k - 1], psi, q); ipw[k] = mulmod(ipw[k - 1], ipsi, q); }
+    pw[0] = 1;
+    for (uint32_t k = 1; k < N; ++k) pw[k] = mulmod(pw[k - 1], psi, q);
     for (uint32_t k = 0; k < N; ++k) {
       uint32_t r = bitrev(k, c->logN);
       twf[(size_t)j * N + k] = make_uint2(pw[r], shoup(pw[r], q));
-      twi[(size_t)j * N + k] = make_uint2(ipw[r], shoup(ipw[r], q));
     }
     uint32_t ninv = powmod(N % q, q - 2, q);
     scale_plain[j] = make_uint2(ninv, shoup(ninv, q));
@@ -365,7 +363,7 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
 #define UP(dst, vec)                                                                                   \
   if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
-  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_qsmall, qsmall) UP(d_tw_fwd, twf) UP(d_tw_inv, twi)
+  UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_qsmall, qsmall) UP(d_tw_fwd, twf)
   const std::vector<uint8_t> decB = dec_image(c, Kmax, nullptr);
   UP(d_scale_plain, scale_plain) UP(d_decB, decB)
 

@@ -83,8 +83,7 @@ struct Context {
   uint32_t* d_qinv_neg = nullptr; // [Kmax] -q^-1 mod 2^32 (Montgomery)
   uint2* d_qmu = nullptr;         // [Kmax] (q, floor(2^53 / q)): one-word Barrett pair of the decompose epilogue
   uint4* d_qsmall = nullptr;      // [Kmax] (q, 2^32 mod q, floor(2^61 / q), floor(2^48 / q)): the CUDA-core conversions
-  uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion
-  uint2* d_tw_inv = nullptr;      // [Kmax][N]: psi^-bitrev(k) and Shoup companion
+  uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion; the inverse transforms read it mirrored (bf_inv)
   uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
   uint8_t* d_decB = nullptr;      // [dec_KBimg/16][dec_cols][16]: byte c of 2^(8 kb) mod q_j at column 4 j + c
   uint32_t dec_cols = 0;          // columns of the decompose image: 64 ceil(Kmax / 16)

@@ -2,8 +2,8 @@
 // Eq. 7), formed in registers between the last forward and the first inverse pass (ntt_row_fused_kernel).
 //
 // Formulation: merged-psi Cooley-Tukey forward / Gentleman-Sande inverse; the psi^j "twist" of
-// PAPER.md:346-350 lives in the butterfly twiddles, so there is no separate twist pass.  tw_fwd[k] = psi^bitrev(k),
-// tw_inv[k] = psi^-bitrev(k).  A forward stage with m groups pairs j and j + N/(2m) with twiddle index m + group;
+// PAPER.md:346-350 lives in the butterfly twiddles, so there is no separate twist pass.  tw[k] = psi^bitrev(k); the
+// inverse needs psi^-bitrev(k) = -tw[3m - 1 - k] (m = the level of k) and reads the same table (bf_inv).  A forward stage with m groups pairs j and j + N/(2m) with twiddle index m + group;
 // the forward output is in bit-reversed order, the pointwise products do not care and the inverse undoes it.
 //
 // Split (the paper's two-pass / four-step idea): N = N1 * 256.  The first log2 N1 stages act on
@@ -28,13 +28,20 @@ __device__ __forceinline__ void bf_fwd(uint32_t& X, uint32_t& Y, const uint2 w, 
   X = x + t;
   Y = x - t + q2;
 }
-// inverse: X, Y in [0, 2q) -> X + Y, w (X - Y) in [0, 2q)
+// inverse: X, Y in [0, 2q) -> X + Y, w^-1 (X - Y) in [0, 2q).  There is no inverse table: with k = m + i, 0 <= i < m,
+// psi^-bitrev(k) = -psi^bitrev(3m - 1 - k) (psi^N = -1, and the bit reversal of the complement of i is the complement of its
+// bit reversal), so the inverse stages read the FORWARD table mirrored inside each level -- w below is tw_fwd[3m - 1 - k] --
+// and the sign goes into the difference: w^-1 (X - Y) = w (Y - X).  Same instructions as with a table of its own; half the
+// twiddle bytes, and in the fused row pass both directions hit the same L1 lines.
 __device__ __forceinline__ void bf_inv(uint32_t& X, uint32_t& Y, const uint2 w, const uint32_t q, const uint32_t q2) {
   const uint32_t s = X + Y;
-  const uint32_t d = X - Y + q2;
+  const uint32_t d = Y - X + q2;
   X = min(s, s - q2);
   Y = mul_shoup_lazy(d, w.x, w.y, q);
 }
+// mirror of a base inside its level: a local transform with base b in [m0, 2 m0) uses twiddle indices (b << s) + i at its
+// stage s; mirrored, (mir_base(b, m0) << s) + (2^s - 1 - i)
+__device__ __forceinline__ uint32_t mir_base(uint32_t base, uint32_t m0) { return 3 * m0 - 1 - base; }
 
 template <int NG>
 __device__ __forceinline__ void load_tw(const uint2* __restrict__ p, uint2 (&w)[8]) {
@@ -63,7 +70,7 @@ __device__ __forceinline__ void reg_stage(uint32_t (&x)[16], const uint2* __rest
     for (int k = 0; k < H; ++k) {
       const int i0 = g * 2 * H + k;
       if (!INV) bf_fwd(x[i0], x[i0 + H], w[g], q, q2);
-      else bf_inv(x[i0], x[i0 + H], w[g], q, q2);
+      else bf_inv(x[i0], x[i0 + H], w[NG - 1 - g], q, q2);           // mirrored table: `tw` points at the mirrored block
     }
 }
 
@@ -89,6 +96,7 @@ __device__ __forceinline__ void phase_a(uint32_t (&x)[16], const uint2* __restri
 template <int LN, bool INV>
 __device__ __forceinline__ void phase_b(uint32_t (&x)[16], const uint2* __restrict__ tw, uint32_t base, uint32_t tb, uint32_t q, uint32_t q2) {
   constexpr int LE = LN < 4 ? LN : 4, E = 1 << LE, S0 = LN - LE;
+  if (INV) tb = (1u << S0) - 1 - tb;                               // inverse: `base` is the mirrored base, and the thread's block mirrors too
 #define STG(S) reg_stage<E, S, INV>(x, tw + (base << (S0 + S)) + (tb << S), q, q2)
   if (!INV) {
     if constexpr (LE > 0) STG(0);
@@ -119,7 +127,7 @@ __device__ __forceinline__ void reg_stage_multi(uint32_t (&x)[NOPS][16], const u
       for (int k = 0; k < H; ++k) {
         const int i0 = g * 2 * H + k;
         if (!INV) bf_fwd(x[o][i0], x[o][i0 + H], w[g], q, q2);
-        else bf_inv(x[o][i0], x[o][i0 + H], w[g], q, q2);
+        else bf_inv(x[o][i0], x[o][i0 + H], w[NG - 1 - g], q, q2);
       }
 }
 template <int NOPS, bool INV, int NS>
@@ -139,6 +147,7 @@ __device__ __forceinline__ void phase_a_multi(uint32_t (&x)[NOPS][16], const uin
 template <int NOPS, int LN, bool INV>
 __device__ __forceinline__ void phase_b_multi(uint32_t (&x)[NOPS][16], const uint2* __restrict__ tw, uint32_t base, uint32_t tb, uint32_t q, uint32_t q2) {
   constexpr int S0 = LN - 4;
+  if (INV) tb = (1u << S0) - 1 - tb;
 #define STGM(S) reg_stage_multi<NOPS, 16, S, INV>(x, tw + (base << (S0 + S)) + (tb << S), q, q2)
   if (!INV) { STGM(0); STGM(1); STGM(2); STGM(3); }
   else { STGM(3); STGM(2); STGM(1); STGM(0); }
@@ -155,8 +164,7 @@ __device__ __forceinline__ uint32_t mm(uint32_t a, uint32_t b, uint32_t q, uint3
 struct NttArgs {
   uint32_t* data;            // transforms: item-major [nitems][S][K][N]; slots 0..U-1 of every item are transformed
   const uint32_t* aux;       // PW_POLYMUL: b [nitems][K][N]; PW_RELIN: evk-hat [2][K][N]
-  const uint2* tw;           // [Kmax][N] twiddles of the direction (fused row pass: inverse)
-  const uint2* tw2;          // fused row pass only: forward twiddles
+  const uint2* tw;           // [Kmax][N] psi^bitrev(k) with Shoup companions: the one table of both directions (bf_inv)
   const uint32_t* q;         // [Kmax]
   const uint32_t* qn;        // [Kmax] -q^-1 mod 2^32
   const uint2* scale;        // [K] final constant of the inverse (with Shoup companion)
@@ -318,7 +326,8 @@ __device__ __forceinline__ void row_fwd_core(uint32_t (&x)[16], uint32_t* srow, 
   __syncwarp();
   phase_b<8, false>(x, tw, base, t, q, q2);
 }
-// in: x = the thread's 16 contiguous points (values in [0, 2q)); out: x[i] = point i * 16 + t
+// in: x = the thread's 16 contiguous points (values in [0, 2q)); out: x[i] = point i * 16 + t.  tw = the FORWARD table,
+// base = the row's mirrored base (mir_base)
 __device__ __forceinline__ void row_inv_core(uint32_t (&x)[16], uint32_t* srow, uint32_t t, const uint2* tw, uint32_t base,
                                              uint32_t q, uint32_t q2) {
   phase_b<8, true>(x, tw, base, t, q, q2);
@@ -377,7 +386,7 @@ ntt_row_inv_kernel(NttArgs a) {
   uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + (size_t)r * 256;
   uint32_t x[16];
   load16(x, g + t * 16);
-  row_inv_core(x, sm + rl * ROW_SM, t, tw, a.N1 + r, q, q2);
+  row_inv_core(x, sm + rl * ROW_SM, t, tw, mir_base(a.N1 + r, a.N1), q, q2);
   if (FINAL) {
     const uint2 sc = __ldg(a.scale + j);
 #pragma unroll
@@ -418,8 +427,7 @@ ntt_row_fused_kernel(NttArgs a) {
   uint32_t* srow = sm + rl * ROW_SM;
   const size_t KN = (size_t)a.K * a.N;
   const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
-  const uint2* twf = a.tw2 + (size_t)j * a.N;
-  const uint2* twi = a.tw + (size_t)j * a.N;
+  const uint2* twf = a.tw + (size_t)j * a.N;                       // both directions read the forward table (bf_inv)
   const uint32_t base = a.N1 + r;
   const size_t poff = (size_t)j * a.N + (size_t)r * 256;
 
@@ -430,7 +438,7 @@ ntt_row_fused_kernel(NttArgs a) {
     for (int i = 0; i < 16; ++i) x[i] = canon4(x[i], q, q2);
   };
   auto finish = [&](uint32_t (&x)[16], uint32_t* g) {
-    row_inv_core(x, srow, t, twi, base, q, q2);
+    row_inv_core(x, srow, t, twf, mir_base(base, a.N1), q, q2);
     if (FINAL) {                                                   // N = 256: no column pass; the constant rides on an operand
 #pragma unroll
       for (int i = 0; i < 16; ++i) g[i * 16 + t] = csub(x[i], q);
@@ -550,7 +558,7 @@ __device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restric
                                           const uint2* __restrict__ tw, uint32_t q, uint32_t q2) {
   constexpr int TPC = (1 << LN1) / 16;
   const uint32_t cc = tid & 255, tc = tid >> 8, r = tid >> 4, t = tid & 15;
-  row_inv_core(x, tile + r * WROW, t, tw, (1u << LN1) + r, q, q2);   // x[i] = point i * 16 + t of row r
+  row_inv_core(x, tile + r * WROW, t, tw, mir_base((1u << LN1) + r, 1u << LN1), q, q2);   // x[i] = point i * 16 + t of row r
 #pragma unroll
   for (int i = 0; i < 16; ++i) tile[r * WROW + i * 16 + t] = x[i];
   __syncthreads();
@@ -585,8 +593,8 @@ ntt_whole_kernel(NttArgs a) {
   const uint32_t item = blockIdx.x % a.nitems, j = blockIdx.x / a.nitems;   // the items of a prime side by side: its tables stay in L2
   const size_t KN = (size_t)a.K * a.N, poff = (size_t)j * a.N;
   const uint32_t q = __ldg(a.q + j), q2 = 2 * q, qn = __ldg(a.qn + j);
-  const uint2* twf = a.tw2 + (size_t)j * a.N;
-  const uint2* twi = a.tw + (size_t)j * a.N;
+  const uint2* twf = a.tw + (size_t)j * a.N;
+  const uint2* twi = twf;                                         // both directions read the forward table (bf_inv)
   if constexpr (PW == PW_POLYMUL) {
     uint32_t* g = a.data + (size_t)item * KN + poff;
     uint32_t x[16], y[16];
@@ -764,7 +772,7 @@ static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaSt
 cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_t S, uint32_t U, uint32_t K, cudaStream_t s) {
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
-  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
   const uint32_t ntr = nitems * U * K;
   a.units = ntr * a.N1;
@@ -781,7 +789,7 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
                            const uint2* d_scale, cudaStream_t s) {
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
-  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_inv; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
   const bool fin = c->logN == 8;
   a.units = nitems * U * K * a.N1;
@@ -811,7 +819,7 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
     default: return cudaErrorInvalidValue;
   }
   NttArgs a;
-  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.tw2 = nullptr; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
+  a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems; a.aux_group = aux_group ? aux_group : 1;
   const bool fin = c->logN == 8;
   cudaError_t e;
@@ -819,7 +827,7 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   // at N = 2^13 (512-thread blocks, one or two per SM: the block-wide barriers of the transpositions are not hidden), so
   // N = 2^13 takes it only on request (fhe_debug_force_pipeline(ctx, 2))
   if ((c->logN == 12 && c->force_pipe != 1) || (c->logN == 13 && c->force_pipe == 2)) {
-    a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = nullptr; a.U = Uout;
+    a.aux = d_aux; a.scale = nullptr; a.U = Uout;
     a.units = nitems * K;
     const uint32_t threads = c->N / 16;
     const size_t smem = (size_t)(c->N / 256) * WROW * sizeof(uint32_t);
@@ -841,7 +849,7 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
       a.data = d_res;
     }
   }
-  a.aux = d_aux; a.tw = c->d_tw_inv; a.tw2 = c->d_tw_fwd; a.scale = nullptr; a.U = Uout;
+  a.aux = d_aux; a.scale = nullptr; a.U = Uout;
   a.units = nitems * K * a.N1;
   const uint32_t blocks = (a.units + FUSED_ROWS - 1) / FUSED_ROWS;
   {
