@@ -334,6 +334,84 @@ def test_ckks_full_size_every_limb_of_one_pair_and_structured_samples(N, logQ, l
             assert np.array_equal(diff & ((1 << 62) - 1), expect & ((1 << 62) - 1))
 
 
+# ---- the paper's own workload shape: cnum = 4, logN = 16, logQ = 1024, logp = 60 ----------------------
+def test_paper_table1_shape_structured_samples_incl_rotation_and_plaintext_product():
+    """The shape bench.py --table1 times: N = 2^16, Q = 2^1024 (32 whole limbs: logQ a multiple of 32 at full size), keys
+    mod 2^2048, rescale by 2^60.  Uniform ciphertexts and keys (parity needs no decryption); every call the table times
+    that runs the multiplication pipeline -- he_mult, relinearize, rescale, rotate (X -> X^5), conjugate (X -> X^(2N-1)),
+    mult_plain -- is compared on positions chosen by the kernels' structure, from the definition Eq. 5-6 one coefficient
+    at a time; the streaming operations are compared on every limb (plain multi-word arithmetic on Python integers)."""
+    fhe = _lib()
+    N, logQ, logP, B, p = 1 << 16, 1024, 1024, 4, 60
+    prm = scheme.Params(N, logQ, logP, 0)
+    Q, PQ = prm.Q, prm.PQ
+    ctx = fhe.Context(N, logQ, logP)
+    assert ctx.L == 32 and ctx.L_PQ == 64
+    g = synth.rng(1024)
+    ct1 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    ct2 = synth.uniform_limbs(g, (B, 2), N, logQ)
+    pt = synth.uniform_limbs(g, (B,), N, logQ)
+    keys = {name: synth.uniform_limbs(g, (2,), N, logQ + logP) for name in ("evk", "rot5", "conj")}
+    kp = {name: [from_limbs(v[0]), from_limbs(v[1])] for name, v in keys.items()}
+    ctx.fhe_set_evk(limbs_np_to_tensor(keys["evk"]))
+    ctx.fhe_set_rotation_key(0, 5, limbs_np_to_tensor(keys["rot5"]))
+    ctx.fhe_set_rotation_key(1, 2 * N - 1, limbs_np_to_tensor(keys["conj"]))
+    d1, d2, dpt = limbs_np_to_tensor(ct1), limbs_np_to_tensor(ct2), limbs_np_to_tensor(pt)
+    t3 = ctx.fhe_he_mult(d1, d2)
+    t2 = ctx.fhe_relinearize(t3)
+    tr = ctx.fhe_rescale(t2, p)
+    assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, p), tr)
+    out3, out2, outr = tensor_to_np(t3), tensor_to_np(t2), tensor_to_np(tr)
+    rot = {0: tensor_to_np(ctx.fhe_rotate(d1, 0)), 1: tensor_to_np(ctx.fhe_rotate(d1, 1))}
+    mp = tensor_to_np(ctx.fhe_mult_plain(d1, dpt, 1))
+    checked = 0
+    for b in (0, B - 1):
+        c = [from_limbs(ct1[b, 0]), from_limbs(ct1[b, 1])]
+        e = [from_limbs(ct2[b, 0]), from_limbs(ct2[b, 1])]
+        ks = _structured_ks(N, b, B, 3, ctx.n_sm, per_item=24)
+        for n, k in enumerate(ks):
+            which = (n + b) % 3
+            if which == 0:
+                want = ring.pm_coeff(c[0], e[0], k, Q)
+            elif which == 1:
+                want = (ring.pm_coeff(c[0], e[1], k, Q) + ring.pm_coeff(c[1], e[0], k, Q)) % Q
+            else:
+                want = ring.pm_coeff(c[1], e[1], k, Q)
+            assert coeff_from_limbs(out3[b, which], k) == want, ("he_mult", b, which, k)
+        d2b = from_limbs(out3[b, 2])
+        for n, k in enumerate(_structured_ks(N, b, B, 2, ctx.n_sm, per_item=24)):
+            comp = (n + b) % 2
+            want = (coeff_from_limbs(out3[b, comp], k) + scheme.round_shift(ring.pm_coeff(d2b, kp["evk"][comp], k, PQ), logP)) % Q
+            assert coeff_from_limbs(out2[b, comp], k) == want, ("relin", b, comp, k)
+            assert coeff_from_limbs(outr[b, comp], k) == scheme.round_shift(want, p) % (1 << (logQ - p)), ("rescale", b, comp, k)
+        for slot, kgal, name in ((0, 5, "rot5"), (1, 2 * N - 1, "conj")):
+            s0, s1 = scheme.automorphism(c[0], kgal, Q), scheme.automorphism(c[1], kgal, Q)
+            for n, k in enumerate(_structured_ks(N, b, B, 2, ctx.n_sm, per_item=16)):
+                comp = (n + b + slot) % 2
+                want = ((s0[k] if comp == 0 else 0) + scheme.round_shift(ring.pm_coeff(s1, kp[name][comp], k, PQ), logP)) % Q
+                assert coeff_from_limbs(rot[slot][b, comp], k) == want, (name, b, comp, k)
+                checked += 1
+        m = from_limbs(pt[b])
+        for n, k in enumerate(_structured_ks(N, b, B, 2, ctx.n_sm, per_item=12)):
+            comp = (n + b) % 2
+            assert coeff_from_limbs(mp[b, comp], k) == ring.pm_coeff(c[comp], m, k, Q), ("mult_plain", b, comp, k)
+        checked += len(ks)
+    assert checked >= 200
+    # the streaming rows of the table, every limb: whole-limb Q makes them plain multi-word arithmetic
+    a64 = [from_limbs(ct1[1, i]) for i in range(2)]
+    b64 = [from_limbs(ct2[1, i]) for i in range(2)]
+    one = slice(1, 2)
+    assert tensor_to_polys(ctx.fhe_add(d1[one], d2[one]))[0] == [[(x + y) % Q for x, y in zip(a64[i], b64[i])] for i in range(2)]
+    assert tensor_to_polys(ctx.fhe_sub(d1[one], d2[one]))[0] == [[(x - y) % Q for x, y in zip(a64[i], b64[i])] for i in range(2)]
+    assert tensor_to_polys(ctx.fhe_negate(d1[one]))[0] == [[(-x) % Q for x in a64[i]] for i in range(2)]
+    assert tensor_to_polys(ctx.fhe_moddown(d1[one], logQ - p))[0] == [[x % (1 << (logQ - p)) for x in a64[i]] for i in range(2)]
+    h = N // 2                                       # X^(N/2) a: coefficient i moves to i + N/2, negated when it wraps (pin P3)
+    assert tensor_to_polys(ctx.fhe_mul_monomial(d1[one], h))[0] == [[(-x) % Q for x in a64[i][h:]] + a64[i][:h] for i in range(2)]
+    assert tensor_to_polys(ctx.fhe_mult_scalar(d1[one], 123456789))[0] == [[(x * 123456789) % Q for x in a64[i]] for i in range(2)]
+    m1 = from_limbs(pt[1])
+    assert tensor_to_polys(ctx.fhe_add_plain(d1[one], dpt[one], 1))[0] == [[(x + y) % Q for x, y in zip(a64[0], m1)], a64[1]]
+
+
 # ---- configs[3]: non-RNS BGV ---------------------------------------------------------------------------------------------
 def _bgv_setup(N, logQ, logP, t, B, seed):
     prm = scheme.Params(N, logQ, logP, t)
