@@ -101,6 +101,23 @@ fhe_status fhe_set_evk(fhe_ctx* ctx, const uint32_t* d_evk, void* d_ws, size_t w
 fhe_status fhe_polymul(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,
                        void* d_ws, size_t ws_bytes, void* stream);
 
+/* fhe_polymul for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same ring product with the intermediate residue matrix in a
+ * 32 MiB device array that is part of the library image -- every GPU that loads the library holds it until the process
+ * exits -- instead of a caller workspace.  d_out, d_a, d_b: [batch][L][N], caller-owned, as for fhe_polymul; enqueued on
+ * `stream`; no cudaMalloc / cudaFree / allocating routine is called.  A batch whose fhe_workspace_bytes(FHE_OP_POLYMUL)
+ * exceeds fhe_static_scratch_bytes() is rejected with FHE_ERR_NOMEM (text in fhe_last_error): use fhe_polymul then.
+ * All calls on a device SHARE the array and find the previous call's contents in it (nothing in it needs clearing: the
+ * decompose writes every word the later kernels read); calls that overlap on the GPU -- other streams, concurrent graph
+ * launches -- race on it and must be ordered by the caller.
+ * fhe_polymul_static_init looks up the array's device address (cudaGetSymbolAddress, once per device, with the context's
+ * device current); fhe_polymul_static does the same on its first call, so calling init first is only needed to keep that
+ * lookup out of a graph capture. */
+size_t fhe_static_scratch_bytes(void);
+fhe_status fhe_polymul_static_init(fhe_ctx* ctx);
+fhe_status fhe_polymul_static(fhe_ctx* ctx, uint32_t* d_out, const uint32_t* d_a, const uint32_t* d_b, uint32_t batch,
+                              void* stream);
+
 /* Tensor product (north_star item 4): d0 = c0 c0', d1 = c0 c1' + c1 c0', d2 = c1 c1' (mod Q).
  * d_out3: [batch][3][L][N]; d_ct1, d_ct2: [batch][2][L][N]. */
 fhe_status fhe_he_mult(fhe_ctx* ctx, uint32_t* d_out3, const uint32_t* d_ct1, const uint32_t* d_ct2,

@@ -26,6 +26,7 @@ EXPORTS = [
     "fhe_debug_launch_count", "fhe_debug_timing", "fhe_debug_timing_read", "fhe_debug_int_peak", "fhe_debug_crt_ambiguity",
     "fhe_add", "fhe_sub", "fhe_negate", "fhe_moddown", "fhe_mul_monomial", "fhe_set_rotation_key", "fhe_rotate", "fhe_mult_plain",
     "fhe_add_plain", "fhe_mult_scalar", "fhe_modswitch", "fhe_debug_force_pipeline",
+    "fhe_static_scratch_bytes", "fhe_polymul_static_init", "fhe_polymul_static",
 ]
 
 
@@ -70,6 +71,12 @@ def load_library() -> ctypes.CDLL:
     lib.fhe_set_evk.restype = c_int
     lib.fhe_polymul.argtypes = [vp, vp, vp, vp, c_uint32, vp, c_size_t, vp]
     lib.fhe_polymul.restype = c_int
+    lib.fhe_static_scratch_bytes.argtypes = []
+    lib.fhe_static_scratch_bytes.restype = c_size_t
+    lib.fhe_polymul_static_init.argtypes = [vp]
+    lib.fhe_polymul_static_init.restype = c_int
+    lib.fhe_polymul_static.argtypes = [vp, vp, vp, vp, c_uint32, vp]
+    lib.fhe_polymul_static.restype = c_int
     lib.fhe_he_mult.argtypes = [vp, vp, vp, vp, c_uint32, vp, c_size_t, vp]
     lib.fhe_he_mult.restype = c_int
     lib.fhe_relinearize.argtypes = [vp, vp, vp, c_uint32, vp, c_size_t, vp]
@@ -253,6 +260,21 @@ class Context:
         ws = self._workspace(nb)
         self._check(self._lib.fhe_polymul(self._h, _dev_ptr(out, n, "out"), _dev_ptr(a, n, "a"), _dev_ptr(b, n, "b"),
                                           batch, ws.data_ptr(), nb, self._stream(stream)))
+        return out
+
+    def fhe_static_scratch_bytes(self) -> int:
+        return int(self._lib.fhe_static_scratch_bytes())
+
+    def fhe_polymul_static_init(self):
+        self._check(self._lib.fhe_polymul_static_init(self._h))
+
+    def fhe_polymul_static(self, a, b, out, stream=None):
+        """fhe_polymul with the library's static scratch instead of a workspace: `out` is required (the caller owns every
+        buffer; nothing is allocated here or in the library)."""
+        batch = a.shape[0]
+        n = batch * self.L * self.N
+        self._check(self._lib.fhe_polymul_static(self._h, _dev_ptr(out, n, "out"), _dev_ptr(a, n, "a"), _dev_ptr(b, n, "b"),
+                                                 batch, self._stream(stream)))
         return out
 
     def fhe_he_mult(self, ct1, ct2, out=None, stream=None):

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfhe_b200.so")
-SOURCES = ["ctx.cu", "api.cu", "kernels_decompose.cu", "kernels_ntt.cu", "kernels_crt.cu", "kernels_elem.cu", "kernels_small.cu"]
+SOURCES = ["ctx.cu", "api.cu", "api_static.cu", "kernels_decompose.cu", "kernels_ntt.cu", "kernels_crt.cu", "kernels_elem.cu", "kernels_small.cu"]
 HEADERS = ["fhe_internal.cuh", "umma.cuh", "pipe.cuh", "bigu.hpp", os.path.join("..", "..", "include", "fhe.h")]
 
 
