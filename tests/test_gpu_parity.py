@@ -412,6 +412,45 @@ def test_paper_table1_shape_structured_samples_incl_rotation_and_plaintext_produ
     assert tensor_to_polys(ctx.fhe_add_plain(d1[one], dpt[one], 1))[0] == [[(x + y) % Q for x, y in zip(a64[0], m1)], a64[1]]
 
 
+# ---- CUDA graph capture: the hot-path calls allocate nothing, synchronise nothing and stay on the caller's stream ---------
+def test_hot_path_is_cuda_graph_capturable_and_replays_bit_identically():
+    """include/fhe.h, "Ownership": hot-path calls enqueue on the caller's stream, allocate nothing and never synchronise.
+    A CUDA graph capture fails on any of those, so: capture fhe_mult_relin_rescale (12 launches, programmatic dependent
+    launch attributes included) and fhe_polymul_static once, replay them on new inputs written into the captured buffers,
+    and compare every limb with the direct calls."""
+    fhe = _lib()
+    N, logQ, logP, B, p = 1 << 10, 128, 128, 2, 40
+    ctx = fhe.Context(N, logQ, logP)
+    g = synth.rng(31337)
+    ctx.fhe_set_evk(limbs_np_to_tensor(synth.uniform_limbs(g, (2,), N, logQ + logP)))
+    def fresh():
+        return (limbs_np_to_tensor(synth.uniform_limbs(g, (B, 2), N, logQ)), limbs_np_to_tensor(synth.uniform_limbs(g, (B, 2), N, logQ)))
+    x, y = fresh()
+    out = torch.empty_like(x)
+    pm = torch.empty((B, ctx.L, N), dtype=torch.int32, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):                    # warm-up on the capture stream: workspace of the binding, kernel attributes
+        ctx.fhe_mult_relin_rescale(x, y, p, out=out, stream=side)
+        ctx.fhe_polymul_static(x[:, 0].contiguous(), y[:, 0].contiguous(), pm, stream=side)
+    side.synchronize()
+    xa, ya = x[:, 0].contiguous(), y[:, 0].contiguous()
+    graph = torch.cuda.CUDAGraph()
+    l0 = ctx.launch_count()
+    with torch.cuda.graph(graph, stream=side):
+        ctx.fhe_mult_relin_rescale(x, y, p, out=out, stream=torch.cuda.current_stream())
+        ctx.fhe_polymul_static(xa, ya, pm, stream=torch.cuda.current_stream())
+    assert ctx.launch_count() - l0 >= 12
+    for _ in range(2):
+        nx, ny = fresh()
+        x.copy_(nx); y.copy_(ny); xa.copy_(nx[:, 0]); ya.copy_(ny[:, 0])
+        out.fill_(-1); pm.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ctx.fhe_mult_relin_rescale(nx, ny, p))
+        assert torch.equal(pm, ctx.fhe_polymul(nx[:, 0].contiguous(), ny[:, 0].contiguous()))
+
+
 # ---- configs[3]: non-RNS BGV ---------------------------------------------------------------------------------------------
 def _bgv_setup(N, logQ, logP, t, B, seed):
     prm = scheme.Params(N, logQ, logP, t)
