@@ -364,6 +364,16 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
   if ((e = upload(c, &c->dst, vec)) != cudaSuccess) {                                                  \
     std::string m = cudaGetErrorString(e); destroy(c); return fail(nullptr, FHE_ERR_CUDA, "upload failed: " + m); }
   UP(d_q, c->h_q) UP(d_qinv_neg, qn) UP(d_qmu, qmu) UP(d_qsmall, qsmall) UP(d_tw_fwd, twf)
+  {
+    const uint32_t kd = Kmax < SMALL_DEC_K ? Kmax : SMALL_DEC_K;
+    std::vector<uint32_t> pw32((size_t)kd * SMALL_LIMBS);
+    for (uint32_t j = 0; j < kd; ++j) {
+      const uint32_t q = c->h_q[j], c32 = (uint32_t)((1ull << 32) % q);
+      uint32_t v = 1;
+      for (uint32_t l = 0; l < SMALL_LIMBS; ++l) { pw32[(size_t)j * SMALL_LIMBS + l] = v; v = mulmod(v, c32, q); }
+    }
+    UP(d_pow32q, pw32)
+  }
   const std::vector<uint8_t> decB = dec_image(c, Kmax, nullptr);
   UP(d_scale_plain, scale_plain) UP(d_decB, decB)
 

@@ -43,7 +43,11 @@ struct CrtTarget {
 constexpr uint32_t TOP_BITS = 96, TOP_LIMBS = 6, TOP_AMB = 58;
 // Shapes below these bounds convert on the CUDA cores (kernels_small.cu): a 128-coefficient tile of the tensor-core pipeline
 // costs a few thousand cycles whatever its size, which two-limb coefficients cannot amortise.
-constexpr uint32_t SMALL_K = 32, SMALL_LIMBS = 16, SMALL_WORK = 48;   // K, limbs, K x limbs
+#ifndef FHE_SMALL_WORK
+#define FHE_SMALL_WORK 192
+#endif
+constexpr uint32_t SMALL_K = 32, SMALL_LIMBS = 16, SMALL_WORK = FHE_SMALL_WORK;   // K, limbs, K x limbs
+constexpr uint32_t SMALL_DEC_K = 128;          // primes the CUDA-core decompose has constants for
 
 enum PostMode : int {
   POST_CKKS_MASK = 0,    // out = X mod 2^logQ
@@ -83,6 +87,7 @@ struct Context {
   uint32_t* d_qinv_neg = nullptr; // [Kmax] -q^-1 mod 2^32 (Montgomery)
   uint2* d_qmu = nullptr;         // [Kmax] (q, floor(2^53 / q)): one-word Barrett pair of the decompose epilogue
   uint4* d_qsmall = nullptr;      // [Kmax] (q, 2^32 mod q, floor(2^61 / q), floor(2^48 / q)): the CUDA-core conversions
+  uint32_t* d_pow32q = nullptr;   // [min(Kmax, SMALL_DEC_K)][SMALL_LIMBS]: 2^(32 l) mod q_j, the CUDA-core decompose
   uint2* d_tw_fwd = nullptr;      // [Kmax][N]: psi^bitrev(k) and Shoup companion; the inverse transforms read it mirrored (bf_inv)
   uint2* d_scale_plain = nullptr; // [Kmax]: N^-1 (debug inverse transform)
   uint8_t* d_decB = nullptr;      // [dec_KBimg/16][dec_cols][16]: byte c of 2^(8 kb) mod q_j at column 4 j + c

@@ -55,6 +55,34 @@ def test_decompose_matches_python_mod(N, logQ, Lin, mask, pipeline):
             assert np.array_equal(res[p, j], want), (p, j)
 
 
+@pytest.mark.parametrize("Lin,mask", [(12, 0), (16, 0), (16, 500), (9, 0), (3, 70)])
+def test_small_decompose_limb_bounds_and_largest_lazy_sums(Lin, mask):
+    """The CUDA-core decompose keeps sum_l x_l (2^(32 l) mod q) lazily in 64 bits (kernels_small.cu): every limb bound it
+    is instantiated for (2, 4, 8, 12, 16), with coefficients whose limbs are all 2^32 - 1 (the largest sums the folds
+    must hold), all zero, and random, on every prime -- against Python's %."""
+    fhe = _lib()
+    N = 512
+    ctx = fhe.Context(N, 96, 96)
+    K = ctx.K2
+    assert K * Lin <= 192                             # the small path takes it (fhe_internal.cuh: SMALL_WORK)
+    g = synth.rng(100 + Lin)
+    limbs = synth.uniform_limbs(g, (2,), N, 32 * Lin)
+    limbs[0, :, :8] = 0xFFFFFFFF
+    limbs[0, :, 8:12] = 0
+    limbs[1, ::2, 16:24] = 0xFFFFFFFF                 # alternating all-ones / zero limbs
+    limbs[1, 1::2, 16:24] = 0
+    q, _ = ctx.primes(K)
+    res = tensor_to_np(ctx.fhe_debug_decompose(limbs_np_to_tensor(limbs), K, mask))
+    ctx.fhe_debug_force_pipeline(1)
+    assert np.array_equal(res, tensor_to_np(ctx.fhe_debug_decompose(limbs_np_to_tensor(limbs), K, mask)))   # the tensor-core route agrees
+    for p in range(2):
+        vals = from_limbs(limbs[p])
+        if mask:
+            vals = [v % (1 << mask) for v in vals]
+        for j in range(K):
+            assert np.array_equal(res[p, j], np.array([v % q[j] for v in vals], dtype=np.uint32)), (p, j)
+
+
 # ---- S2 / S4: NTT against the oracle's Eq. 8 with the library's own (q, psi) -----------------------------------
 @pytest.mark.parametrize("N", [256, 1024, 8192, 16384, 65536])
 def test_ntt_forward_is_eq8_bitreversed_and_inverse_roundtrips(N):
