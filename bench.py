@@ -675,9 +675,9 @@ def kernel_class(name: str):
         if pat in name:
             return cls
     if "ntt_col" in name or "ntt_row_fwd" in name or "ntt_row_inv" in name:
-        # ntt_col2_kernel<LN, INV> / ntt_col_kernel<LN, INV>: the second template argument is the direction
+        # ntt_col2_kernel<LN, INV, PM> / ntt_col_kernel<LN, INV>: the second template argument is the direction
         import re
-        m = re.search(r"<\s*\d+\s*,\s*(\w+)\s*>", name)
+        m = re.search(r"<\s*\d+\s*,\s*(\w+)\s*[,>]", name)
         inv = "ntt_row_inv" in name or (m is not None and m.group(1) in ("1", "true"))
         return "ntt_inv" if inv else "ntt_fwd"
     return None

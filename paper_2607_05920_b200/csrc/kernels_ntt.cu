@@ -170,7 +170,14 @@ struct NttArgs {
   const uint2* scale;        // [K] final constant of the inverse (with Shoup companion)
   uint32_t N, K, N1, S, U, units, nitems;
   uint32_t aux_group;        // PW_POLYMUL: item i multiplies aux polynomial i / aux_group (1: pairwise; > 1: shared operand)
+  // Traversal order, so that a pass STARTS on what the pass before it wrote LAST (the tail of a 260-350 MB output is still in
+  // the L2 when the next kernel begins).  Column pass: 0 = transforms in memory order (item, slot, prime); 1 = prime-major,
+  // ascending.  Fused row pass: 1 = units in descending order.
+  uint32_t order;
 };
+#ifndef NTT_L2_ORDER
+#define NTT_L2_ORDER 1
+#endif
 
 // ------------------------------------------------------------------------------------------------------------------
 // Column pass: 2^LN-point transforms over elements e * 256 + c (c = column), in place.  A block owns T adjacent
@@ -249,7 +256,7 @@ ntt_col_kernel(NttArgs a) {
 // points as 8-byte pairs, so that a warp access is two full 128-byte lines of two rows instead of two half lines, and the
 // two columns share the twiddles of every stage.  A block owns 2 T2 adjacent columns of one (polynomial, prime).
 // ------------------------------------------------------------------------------------------------------------------
-template <int LN, bool INV>
+template <int LN, bool INV, bool PM>
 __global__ void __launch_bounds__(256, 4)
 ntt_col2_kernel(NttArgs a) {
   pdl_sync();
@@ -261,7 +268,10 @@ ntt_col2_kernel(NttArgs a) {
   const uint32_t tid = threadIdx.x, cp = tid % T2, t = tid / T2;
   constexpr uint32_t tiles = 256 / W;
   const uint32_t tr = blockIdx.x / tiles, c0 = (blockIdx.x % tiles) * W;
-  const uint32_t item = tr / (a.U * a.K), rem = tr % (a.U * a.K), slot = rem / a.K, j = rem % a.K;
+  // PM: prime-major traversal (the transforms of a prime side by side, primes ascending) instead of memory order (item, slot, prime)
+  const uint32_t d1 = PM ? a.nitems * a.U : a.U * a.K, d2 = PM ? a.U : a.K;
+  const uint32_t hi = tr / d1, rem = tr % d1, mid = rem / d2, lo = rem % d2;
+  const uint32_t item = PM ? mid : hi, slot = PM ? lo : mid, j = PM ? hi : lo;
   const uint32_t q = __ldg(a.q + j), q2 = 2 * q;
   const uint2* tw = a.tw + (size_t)j * a.N;
   uint32_t* g = a.data + ((size_t)(item * a.S + slot) * a.K + j) * a.N + c0 + 2 * cp;
@@ -420,8 +430,9 @@ ntt_row_fused_kernel(NttArgs a) {
   const uint32_t tid = threadIdx.x, t = tid & 15, rl = tid >> 4;
   // unit = (j * N1 + r) * nitems + item: the half-warps of a block that share (j, r) share every twiddle of both
   // directions (2 KB per row and direction, twice the row itself), so the tables cross L2 -> SM once per (j, r)
-  const uint32_t unit = blockIdx.x * FUSED_ROWS + rl;
+  uint32_t unit = blockIdx.x * FUSED_ROWS + rl;
   if (unit >= a.units) return;
+  if (a.order) unit = a.units - 1 - unit;                          // start on the primes the forward column pass wrote last
   const uint32_t item = unit % a.nitems, jr = unit / a.nitems;
   const uint32_t r = jr % a.N1, j = jr / a.N1;
   uint32_t* srow = sm + rl * ROW_SM;
@@ -585,7 +596,12 @@ __device__ __forceinline__ void whole_inv(uint32_t (&x)[16], uint32_t* __restric
 }
 
 template <int PW, int LN1>
-__global__ void __launch_bounds__(16 << LN1, LN1 == 4 ? 2 : 1)
+// blocks per SM at N = 2^12: two with four operand arrays in registers; the plain product (two arrays) takes three -- measured
+// 3.39 -> 3.30 ms per call at logQ = 1240 with 68 bytes of spills, four blocks (64 registers, 190 bytes of spills) 3.56 ms
+#ifndef WHOLE_PM_MINB
+#define WHOLE_PM_MINB 3
+#endif
+__global__ void __launch_bounds__(16 << LN1, LN1 == 4 ? (PW == PW_POLYMUL ? WHOLE_PM_MINB : 2) : 1)
 ntt_whole_kernel(NttArgs a) {
   pdl_sync();
   extern __shared__ __align__(16) uint32_t tile[];                 // [N / 256][WROW]
@@ -757,7 +773,8 @@ static cudaError_t launch_col(Context* c, const NttArgs& a, uint32_t ntr, cudaSt
 #define COL2_CASE(LN)                                                                          \
   case LN: {                                                                                   \
     constexpr int TPC = (1 << LN) / 16;                                                        \
-    e = launch_pdl(ntt_col2_kernel<LN, INV>, ntr * (256 / (2 * (256 / TPC))), 256, 0, s, a);   \
+    e = a.order ? launch_pdl(ntt_col2_kernel<LN, INV, true>, ntr * (256 / (2 * (256 / TPC))), 256, 0, s, a)    \
+                : launch_pdl(ntt_col2_kernel<LN, INV, false>, ntr * (256 / (2 * (256 / TPC))), 256, 0, s, a);  \
     break;                                                                                     \
   }
   switch (ln1) {   // blocks per transform = 256 / T = TPC (single columns) or TPC / 2 (column pairs)
@@ -773,7 +790,7 @@ cudaError_t launch_ntt_fwd(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
   a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1; a.order = 0;
   const uint32_t ntr = nitems * U * K;
   a.units = ntr * a.N1;
   if (c->logN > 8) {
@@ -790,7 +807,7 @@ cudaError_t launch_ntt_inv(Context* c, uint32_t* d_res, uint32_t nitems, uint32_
   if (!nitems || !U) return cudaSuccess;
   NttArgs a;
   a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = d_scale;
-  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1;
+  a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = U; a.nitems = nitems; a.aux_group = 1; a.order = 0;
   const bool fin = c->logN == 8;
   a.units = nitems * U * K * a.N1;
   const uint32_t blocks = (a.units + 15) / 16;
@@ -821,6 +838,10 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   NttArgs a;
   a.data = d_res; a.aux = nullptr; a.tw = c->d_tw_fwd; a.q = c->d_q; a.qn = c->d_qinv_neg; a.scale = nullptr;
   a.N = c->N; a.K = K; a.N1 = c->N / 256; a.S = S; a.U = Uin; a.units = 0; a.nitems = nitems; a.aux_group = aux_group ? aux_group : 1;
+  // product path: forward columns prime-major ascending, fused rows descending, inverse columns prime-major ascending (the
+  // fused rows then finish on prime 0) -- each pass starts on the tail of the previous one's output
+  const uint32_t l2o = NTT_L2_ORDER;
+  a.order = l2o ? 1 : 0;
   const bool fin = c->logN == 8;
   cudaError_t e;
   // the whole product in one launch (ntt_whole_kernel): measured 5-9 % faster than the three passes at N = 2^12, 8-13 % slower
@@ -844,9 +865,9 @@ cudaError_t launch_ntt_product(Context* c, uint32_t* d_res, uint32_t* d_aux, uin
   if (!fin) {
     if ((e = launch_col<false>(c, a, nitems * Uin * K, s)) != cudaSuccess) return e;
     if (pw_mode == PW_POLYMUL) {
-      a.data = d_aux;
-      if ((e = launch_col<false>(c, a, ((nitems + a.aux_group - 1) / a.aux_group) * K, s)) != cudaSuccess) return e;
-      a.data = d_res;
+      a.data = d_aux; a.nitems = (nitems + a.aux_group - 1) / a.aux_group;   // the shared operands: their own item count
+      if ((e = launch_col<false>(c, a, a.nitems * K, s)) != cudaSuccess) return e;
+      a.data = d_res; a.nitems = nitems;
     }
   }
   a.aux = d_aux; a.scale = nullptr; a.U = Uout;
