@@ -411,6 +411,18 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
     UP(d_pow32_t, p32)
     pp.d_Q = c->d_Qlimbs; pp.d_P = c->d_Plimbs; pp.d_PQ = c->d_PQlimbs; pp.d_muP = c->d_muP; pp.d_pow32_t = c->d_pow32_t;
     pp.mu1_Q = mu1_of(Q); pp.mu1_PQ = mu1_of(PQ);
+    {
+      const uint64_t eP = modulus_offset(logP, t);
+      uint32_t be = 0;
+      while (be < 64 && (eP >> be)) ++be;
+      pp.eP = (uint32_t)eP;
+      pp.fold_div = (eP >> 32) == 0 && logP >= 96 && be + pp.bitsQ + 1 <= logP + 60 ? 1u : 0u;
+      if (pp.scratch_limbs < c->L_PQ - (logP >> 5) + 2) pp.scratch_limbs = c->L_PQ - (logP >> 5) + 2;
+      pp.mu_t = tt < (1u << 31) ? ~0ull / tt : 0ull;
+      const uint64_t eQ = modulus_offset(logQ, t);
+      pp.eQ = (uint32_t)eQ;
+      pp.fold_modq = eQ < (1ull << 22) && logQ >= 64 ? 1u : 0u;
+    }
     pp.t = tt; pp.Pinv_t = powmod(P.mod_small(tt), (uint64_t)tt - 2, tt);
     // t need not be prime: fall back to a search-free extended Euclid if Fermat fails
     if (mulmod(pp.Pinv_t, P.mod_small(tt), tt) != 1 % tt) {

@@ -69,6 +69,13 @@ struct PostParams {
   uint32_t L_P, muP_limbs, g_limbs, scratch_limbs;
   uint64_t mu1_Q, mu1_PQ;      // floor(2^(bits+62) / Q), floor(2^(bitsPQ+62) / PQ): one-word Barrett quotient estimates
   uint32_t t, Pinv_t;          // plaintext modulus and P^-1 mod t
+  // P = 2^logP + eP (the least odd integer above 2^logP that is 1 mod t).  fold_div: the divide-by-P of the BGV relinearisation
+  // goes through that shape -- xc = A 2^logP + B = A P + (B - A eP), and when that is negative one more fold of the same kind
+  // (kernels_crt.cu) -- instead of a general multi-limb Barrett division; set when logP >= 96 and the second fold's quotient
+  // fits 60 bits (bits(eP) + bitsQ + 1 <= logP + 60: every shape with logQ <= logP + 38 or so)
+  uint32_t eP, fold_div;
+  uint32_t eQ, fold_modq;      // Q = 2^logQ + eQ; fold_modq: V mod Q as (V mod 2^logQ) - (V >> logQ) eQ (+ Q), set when eQ < 2^22 and logQ >= 64
+  uint64_t mu_t;               // floor((2^64 - 1) / t) when t < 2^31 (word-sized Barrett steps mod t), else 0
   const uint32_t* d_pow32_t;   // [L_P+1]: 2^(32 i) mod t
 };
 
@@ -253,6 +260,14 @@ __device__ __forceinline__ uint32_t mont_redc(uint64_t t, uint32_t q, uint32_t q
   uint32_t m = (uint32_t)t * qn;
   uint64_t u = t + (uint64_t)m * q;   // < 2^64: t < 2^63, m q < 2^63
   return csub((uint32_t)(u >> 32), q);
+}
+// acc * 2^32 + limb  mod t   (acc < t < 2^31; mu = floor(2^64 / t) or one less)
+__device__ __forceinline__ uint32_t horner_mod(uint32_t acc, uint32_t limb, uint32_t t, uint64_t mu) {
+  const uint64_t v = ((uint64_t)acc << 32) | limb;
+  uint64_t r = v - __umul64hi(v, mu) * t;                           // quotient estimate at most 2 short: r in [0, 3 t)
+  if (r >= t) r -= t;
+  if (r >= t) r -= t;
+  return (uint32_t)r;
 }
 // v < 2^49 -> v mod q with mu = floor(2^53 / q): the quotient estimate mulhi(v >> 21, mu) is floor(v/q) or one less
 // (v >> 21 < 2^28 and mu < 2^24 lose < 2^-4 + 2^-8 of a unit), so the 32-bit remainder lies in [0, 2q).

@@ -105,6 +105,33 @@ __device__ __forceinline__ void col_barrett1(Col x, uint32_t nx, const uint32_t*
   }
 }
 
+// V (nx limbs, V < 2^(k + 40)) -> V mod M in place, M = 2^k + e with e < 2^22 (the BGV moduli: the least odd integer above the
+// power of two that is 1 mod t): V = A 2^k + B is congruent to B - A e, and A e < 2^63 is a two-word number, so the reduction is
+// one masked copy, one subtraction and at most one addition of M instead of a Barrett step with the limbs of M.
+__device__ __forceinline__ void col_fold_mod(Col x, uint32_t nx, uint32_t k, uint32_t e) {
+  const uint32_t wq = k >> 5, bq = k & 31, nm = wq + 1;
+  const uint32_t a0 = x.get(wq), a1 = wq + 1 < nx ? x.get(wq + 1) : 0u, a2 = wq + 2 < nx ? x.get(wq + 2) : 0u;
+  const uint64_t A = bq ? ((uint64_t)(a0 >> bq) | ((uint64_t)a1 << (32 - bq)) | ((uint64_t)a2 << (64 - bq))) : ((uint64_t)a0 | ((uint64_t)a1 << 32));
+  x.set(wq, bq ? a0 & ((1u << bq) - 1u) : 0u);
+  for (uint32_t l = nm; l < nx; ++l) x.set(l, 0u);
+  const uint64_t s = A * e;
+  uint32_t borrow = 0;
+  for (uint32_t l = 0; l < nm; ++l) {
+    const uint32_t sub = l == 0 ? (uint32_t)s : l == 1 ? (uint32_t)(s >> 32) : 0u, v = x.get(l), d = v - sub, d2 = d - borrow;
+    borrow = (v < sub) | (d < borrow);
+    x.set(l, d2);
+    if (l >= 1 && !borrow) break;                                  // nothing left to propagate
+  }
+  if (borrow) {                                                    // negative: + M once (A e < 2^63 < M)
+    uint32_t carry = 0;
+    for (uint32_t l = 0; l < nm; ++l) {
+      const uint64_t sum = (uint64_t)x.get(l) + ((l == 0 ? e : 0u) + (l == wq ? 1u << bq : 0u)) + carry;
+      x.set(l, (uint32_t)sum);
+      carry = (uint32_t)(sum >> 32);
+    }
+  }
+}
+
 // ------------------------------------------------------------------------------------------------------------------
 // CRT epilogue of the conversion pipeline (pipe.cuh).  The loaders stage the residues y[i][n] as the A operand (word i =
 // column i), the tensor cores contract them with the constant image B: column 8 + e receives
@@ -367,7 +394,8 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
   Col ad{adds + etid};
   const uint32_t L = pp.L;
   if constexpr (MODE == POST_BGV_MODQ) {
-    col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
+    if (pp.fold_modq) col_fold_mod(x, Lx, pp.logQ, pp.eQ);
+    else col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
     for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     return;
   }
@@ -375,9 +403,72 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
   if constexpr (MODE == POST_BGV_RELIN) {
     const uint32_t LP = pp.L_P, LPQ = pp.L_PQ, g = pp.g_limbs;   // g = LPQ - LP
     col_barrett1(x, Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);     // x[0..LPQ) = xc
+    Col sc{scratch + etid};
+    Col q3{sc.p};                                    // the quotient's limbs (nq of them)
+    uint32_t nq, qinc = 0;
+    if (pp.fold_div) {
+      // P = 2^kP + eP: xc = A 2^kP + B = A P + z, z = B - A eP (signed, |z| < 2^(bitsQ + 1 + bits(eP))).  When z < 0, y = -z =
+      // j 2^kP + yl = j P + w, w = yl - j eP with j < 2^60 and j eP < 2^92 < 2^kP (ctx.cu: fold_div), so
+      //   w > 0:  xc = (A - j - 1) P + (P - w);     w <= 0:  xc = (A - j) P + (-w)
+      // -- quotient and remainder in O(L) word operations instead of the two multi-limb products of a Barrett division.
+      const uint32_t kP = pp.logP, wq = kP >> 5, bq = kP & 31, eP = pp.eP;      // LP == wq + 1
+      const uint32_t nA = LPQ - wq;                                              // limbs of A = xc >> kP
+      for (uint32_t i = 0; i < nA; ++i) {
+        const uint32_t lo = x.get(wq + i), hi = wq + i + 1 < LPQ ? x.get(wq + i + 1) : 0u;
+        sc.set(i, bq ? (lo >> bq) | (hi << (32 - bq)) : lo);
+      }
+      sc.set(nA, 0u);
+      x.set(wq, bq ? x.get(wq) & ((1u << bq) - 1u) : 0u);                       // B = xc mod 2^kP in x[0 .. LP)
+      const uint32_t nz = (LP > nA + 1 ? LP : nA + 1) + 1;                      // limbs of z
+      for (uint32_t l = LP; l < nz; ++l) x.set(l, 0u);
+      uint32_t borrow = 0, mc = 0;
+      for (uint32_t l = 0; l < nz; ++l) {
+        const uint64_t pr = (l < nA ? (uint64_t)sc.get(l) * eP : 0ull) + mc;
+        const uint32_t sub = (uint32_t)pr, v = x.get(l), d = v - sub, d2 = d - borrow;
+        mc = (uint32_t)(pr >> 32);
+        borrow = (v < sub) | (d < borrow);
+        x.set(l, d2);
+      }
+      uint64_t hdec = 0;                                                         // what comes off A
+      if (borrow) {
+        uint32_t c1 = 1;                                                         // y = -z
+        for (uint32_t l = 0; l < nz; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c1; x.set(l, (uint32_t)sm); c1 = (uint32_t)(sm >> 32); }
+        const uint32_t j0 = x.get(wq), j1 = wq + 1 < nz ? x.get(wq + 1) : 0u, j2 = wq + 2 < nz ? x.get(wq + 2) : 0u;
+        const uint64_t j = bq ? ((uint64_t)(j0 >> bq) | ((uint64_t)j1 << (32 - bq)) | ((uint64_t)j2 << (64 - bq))) : ((uint64_t)j0 | ((uint64_t)j1 << 32));
+        x.set(wq, bq ? j0 & ((1u << bq) - 1u) : 0u);                            // yl
+        for (uint32_t l = LP; l < nz; ++l) x.set(l, 0u);
+        const uint64_t p0 = (uint64_t)(uint32_t)j * eP, p1 = (j >> 32) * eP + (p0 >> 32);
+        const uint32_t je[3] = {(uint32_t)p0, (uint32_t)p1, (uint32_t)(p1 >> 32)};
+        uint32_t bw = 0, any = 0;
+        for (uint32_t l = 0; l <= LP; ++l) {                                     // w = yl - j eP
+          const uint32_t sub = l < 3 ? je[l] : 0u, v = x.get(l), d = v - sub, d2 = d - bw;
+          bw = (v < sub) | (d < bw);
+          x.set(l, d2); any |= d2;
+        }
+        if (!bw && any) {                                                        // w > 0: one more multiple, remainder P - w
+          hdec = j + 1;
+          uint32_t b2 = 0;
+          for (uint32_t l = 0; l <= LP; ++l) {
+            const uint32_t pl = (l == 0 ? eP : 0u) + (l == wq ? 1u << bq : 0u), v = x.get(l), d = pl - v, d2 = d - b2;
+            b2 = (pl < v) | (d < b2);
+            x.set(l, d2);
+          }
+        } else {                                                                 // w <= 0: remainder -w
+          hdec = j;
+          uint32_t c2 = 1;
+          for (uint32_t l = 0; l <= LP; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c2; x.set(l, (uint32_t)sm); c2 = (uint32_t)(sm >> 32); }
+        }
+      }
+      nq = nA + 1;
+      uint32_t bw = 0;                                                           // quotient = A - hdec (>= 0)
+      for (uint32_t l = 0; l < nq; ++l) {
+        const uint32_t sub = l == 0 ? (uint32_t)hdec : l == 1 ? (uint32_t)(hdec >> 32) : 0u, v = sc.get(l), d = v - sub, d2 = d - bw;
+        bw = (v < sub) | (d < bw);
+        sc.set(l, d2);
+      }
+    } else {
     // Barrett quotient estimate (HAC 14.42 generalised): q1 = xc >> 32(LP-1)  (g+1 limbs),
     // q3 = (q1 * mu) >> 32(g+1), mu = floor(2^(32 LPQ) / P)  (muP_limbs limbs); true quotient - q3 in {0,1,2}.
-    Col sc{scratch + etid};
     const uint32_t n1 = g + 1, nmu = pp.muP_limbs;
     {
       uint64_t acc_lo = 0; uint32_t acc_hi = 0;
@@ -393,8 +484,8 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       }
     }
     // q3 = sc[g+1 .. g+1+n1]; rem = xc - q3 * P over LP+1 limbs
-    Col q3{sc.p + (size_t)(g + 1) * TC};
-    const uint32_t nq = n1;                          // limbs of q3 kept (q3 <= Q < 2^(32 (g+1)))
+    q3 = Col{sc.p + (size_t)(g + 1) * TC};
+    nq = n1;                                         // limbs of q3 kept (q3 <= Q < 2^(32 (g+1)))
     {
       uint64_t acc_lo = 0; uint32_t acc_hi = 0; uint32_t borrow = 0;
       for (uint32_t r = 0; r <= LP; ++r) {
@@ -414,9 +505,9 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       }
     }
     // corrections: rem in [0, 3P)
-    uint32_t qinc = 0;
     for (int it = 0; it < 2; ++it) {
       if (x.get(LP) != 0 || col_ge(x, pp.d_P, LP)) { col_sub(x, pp.d_P, LP + 1); ++qinc; }
+    }
     }
     // centre: rem > (P-1)/2  <=>  2 rem > P - 1  <=> 2 rem >= P + 1 <=> 2 rem > P (P odd)
     bool neg;
@@ -434,7 +525,13 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
     if (neg) ++qinc;                                 // hi = q + 1, r = rem - P
     // r mod t
     uint64_t rt = 0;
-    for (uint32_t k = 0; k < LP; ++k) rt = (rt + (uint64_t)x.get(k) * __ldg(pp.d_pow32_t + k)) % pp.t;
+    if (pp.mu_t) {                                   // word-sized Barrett steps from the top limb down
+      uint32_t acc = 0;
+      for (uint32_t k = LP; k-- > 0;) acc = horner_mod(acc, x.get(k), pp.t, pp.mu_t);
+      rt = acc;
+    } else {
+      for (uint32_t k = 0; k < LP; ++k) rt = (rt + (uint64_t)x.get(k) * __ldg(pp.d_pow32_t + k)) % pp.t;
+    }
     if (neg) { uint64_t Pt = __ldg(pp.d_pow32_t + LP); rt = (rt + pp.t - Pt) % pp.t; }   // d_pow32_t[LP] holds P mod t
     uint64_t kk = ((pp.t - rt) % pp.t) * pp.Pinv_t % pp.t;     // (-r P^-1) mod t in [0, t)
     const bool kneg = kk > pp.t / 2;                            // centred: kk - t

@@ -312,14 +312,6 @@ mult_scalar_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, 
 // ------------------------------------------------------------------------------------------------------------------
 constexpr uint32_t MS_H = ELEM_MAX_LIMBS + 2, MS_X = 2 * ELEM_MAX_LIMBS + 6;
 
-// acc * 2^32 + limb  mod t   (acc < t < 2^31; mu = floor(2^64 / t))
-__device__ __forceinline__ uint32_t horner_mod(uint32_t acc, uint32_t limb, uint32_t t, uint64_t mu) {
-  const uint64_t v = ((uint64_t)acc << 32) | limb;
-  uint64_t r = v - __umul64hi(v, mu) * t;                           // quotient estimate at most 1 short: r in [0, 2 t)
-  if (r >= t) r -= t;
-  return (uint32_t)r;
-}
-
 __global__ void __launch_bounds__(128)
 modswitch_bgv_kernel(uint32_t* __restrict__ out, const uint32_t* __restrict__ in, uint32_t N, uint32_t L, uint32_t logQ,
                      uint32_t e, uint32_t b, uint32_t e2, uint32_t t, uint64_t mu_t) {
