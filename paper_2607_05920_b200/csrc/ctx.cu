@@ -417,11 +417,19 @@ static fhe_status create(Context** out, uint32_t N, uint32_t logQ, uint32_t logP
       while (be < 64 && (eP >> be)) ++be;
       pp.eP = (uint32_t)eP;
       pp.fold_div = (eP >> 32) == 0 && logP >= 96 && be + pp.bitsQ + 1 <= logP + 60 ? 1u : 0u;
-      if (pp.scratch_limbs < c->L_PQ - (logP >> 5) + 2) pp.scratch_limbs = c->L_PQ - (logP >> 5) + 2;
+      if (pp.scratch_limbs < c->L_PQ + 4 - (logP >> 5) + 2) pp.scratch_limbs = c->L_PQ + 4 - (logP >> 5) + 2;   // A of V itself: Lx - wq limbs, Lx <= L_PQ + 4
       pp.mu_t = tt < (1u << 31) ? ~0ull / tt : 0ull;
       const uint64_t eQ = modulus_offset(logQ, t);
       pp.eQ = (uint32_t)eQ;
       pp.fold_modq = eQ < (1ull << 22) && logQ >= 64 ? 1u : 0u;
+      {
+        // V < 2^(bitsPQ + 40): A = V >> logP has at most ba bits, the second fold's quotient j at most bj, the quotient's own
+        // excess over 2^logQ at most bx
+        uint32_t bq2 = 0;
+        while (bq2 < 64 && (eQ >> bq2)) ++bq2;
+        const int ba = (int)pp.bitsPQ + 40 - (int)logP, bj = ba + (int)be - (int)logP, bx = ba - (int)logQ;
+        pp.fold_full = pp.fold_div && pp.fold_modq && bj <= 95 && (bj <= 0 || bj + (int)be < (int)logP) && bx + (int)bq2 <= 63 ? 1u : 0u;
+      }
     }
     pp.t = tt; pp.Pinv_t = powmod(P.mod_small(tt), (uint64_t)tt - 2, tt);
     // t need not be prime: fall back to a search-free extended Euclid if Fermat fails

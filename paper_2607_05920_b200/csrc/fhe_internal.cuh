@@ -74,6 +74,8 @@ struct PostParams {
   // (kernels_crt.cu) -- instead of a general multi-limb Barrett division; set when logP >= 96 and the second fold's quotient
   // fits 60 bits (bits(eP) + bitsQ + 1 <= logP + 60: every shape with logQ <= logP + 38 or so)
   uint32_t eP, fold_div;
+  uint32_t fold_full;          // fold_div on V itself, without reducing it mod PQ first (floor(V / P) mod Q and V mod P do not change
+                               // with multiples of PQ): set when the second fold's quotient fits 95 bits and the quotient's fold mod Q 63
   uint32_t eQ, fold_modq;      // Q = 2^logQ + eQ; fold_modq: V mod Q as (V mod 2^logQ) - (V >> logQ) eQ (+ Q), set when eQ < 2^22 and logQ >= 64
   uint64_t mu_t;               // floor((2^64 - 1) / t) when t < 2^31 (word-sized Barrett steps mod t), else 0
   const uint32_t* d_pow32_t;   // [L_P+1]: 2^(32 i) mod t

@@ -402,7 +402,8 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
   // POST_BGV_RELIN: V -> xc = V mod PQ -> (q3, rem) = divmod(xc, P) -> centred r, kk -> (hi - kk + d) mod Q
   if constexpr (MODE == POST_BGV_RELIN) {
     const uint32_t LP = pp.L_P, LPQ = pp.L_PQ, g = pp.g_limbs;   // g = LPQ - LP
-    col_barrett1(x, Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);     // x[0..LPQ) = xc
+    if (!pp.fold_full) col_barrett1(x, Lx, pp.d_PQ, LPQ, pp.bitsPQ, pp.mu1_PQ);     // x[0..LPQ) = xc = V mod PQ
+    const uint32_t NXX = pp.fold_full ? Lx : LPQ;              // fold_full: the division runs on V itself (see PostParams)
     Col sc{scratch + etid};
     Col q3{sc.p};                                    // the quotient's limbs (nq of them)
     uint32_t nq, qinc = 0;
@@ -412,9 +413,9 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       //   w > 0:  xc = (A - j - 1) P + (P - w);     w <= 0:  xc = (A - j) P + (-w)
       // -- quotient and remainder in O(L) word operations instead of the two multi-limb products of a Barrett division.
       const uint32_t kP = pp.logP, wq = kP >> 5, bq = kP & 31, eP = pp.eP;      // LP == wq + 1
-      const uint32_t nA = LPQ - wq;                                              // limbs of A = xc >> kP
+      const uint32_t nA = NXX - wq;                                              // limbs of A = xc >> kP
       for (uint32_t i = 0; i < nA; ++i) {
-        const uint32_t lo = x.get(wq + i), hi = wq + i + 1 < LPQ ? x.get(wq + i + 1) : 0u;
+        const uint32_t lo = x.get(wq + i), hi = wq + i + 1 < NXX ? x.get(wq + i + 1) : 0u;
         sc.set(i, bq ? (lo >> bq) | (hi << (32 - bq)) : lo);
       }
       sc.set(nA, 0u);
@@ -429,24 +430,28 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
         borrow = (v < sub) | (d < borrow);
         x.set(l, d2);
       }
-      uint64_t hdec = 0;                                                         // what comes off A
+      uint32_t hd[4] = {0u, 0u, 0u, 0u};                                         // what comes off A: j or j + 1, j < 2^95
       if (borrow) {
         uint32_t c1 = 1;                                                         // y = -z
         for (uint32_t l = 0; l < nz; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c1; x.set(l, (uint32_t)sm); c1 = (uint32_t)(sm >> 32); }
-        const uint32_t j0 = x.get(wq), j1 = wq + 1 < nz ? x.get(wq + 1) : 0u, j2 = wq + 2 < nz ? x.get(wq + 2) : 0u;
-        const uint64_t j = bq ? ((uint64_t)(j0 >> bq) | ((uint64_t)j1 << (32 - bq)) | ((uint64_t)j2 << (64 - bq))) : ((uint64_t)j0 | ((uint64_t)j1 << 32));
-        x.set(wq, bq ? j0 & ((1u << bq) - 1u) : 0u);                            // yl
+        uint32_t jw[3];                                                          // j = y >> kP
+        for (uint32_t i = 0; i < 3; ++i) {
+          const uint32_t lo = wq + i < nz ? x.get(wq + i) : 0u, hi = wq + i + 1 < nz ? x.get(wq + i + 1) : 0u;
+          jw[i] = bq ? (lo >> bq) | (hi << (32 - bq)) : lo;
+        }
+        x.set(wq, bq ? x.get(wq) & ((1u << bq) - 1u) : 0u);                     // yl
         for (uint32_t l = LP; l < nz; ++l) x.set(l, 0u);
-        const uint64_t p0 = (uint64_t)(uint32_t)j * eP, p1 = (j >> 32) * eP + (p0 >> 32);
-        const uint32_t je[3] = {(uint32_t)p0, (uint32_t)p1, (uint32_t)(p1 >> 32)};
+        const uint64_t p0 = (uint64_t)jw[0] * eP, p1 = (uint64_t)jw[1] * eP + (p0 >> 32), p2 = (uint64_t)jw[2] * eP + (p1 >> 32);
+        const uint32_t je[4] = {(uint32_t)p0, (uint32_t)p1, (uint32_t)p2, (uint32_t)(p2 >> 32)};
         uint32_t bw = 0, any = 0;
         for (uint32_t l = 0; l <= LP; ++l) {                                     // w = yl - j eP
-          const uint32_t sub = l < 3 ? je[l] : 0u, v = x.get(l), d = v - sub, d2 = d - bw;
+          const uint32_t sub = l == 0 ? je[0] : l == 1 ? je[1] : l == 2 ? je[2] : l == 3 ? je[3] : 0u, v = x.get(l), d = v - sub, d2 = d - bw;
           bw = (v < sub) | (d < bw);
           x.set(l, d2); any |= d2;
         }
+        uint32_t inc;
         if (!bw && any) {                                                        // w > 0: one more multiple, remainder P - w
-          hdec = j + 1;
+          inc = 1;
           uint32_t b2 = 0;
           for (uint32_t l = 0; l <= LP; ++l) {
             const uint32_t pl = (l == 0 ? eP : 0u) + (l == wq ? 1u << bq : 0u), v = x.get(l), d = pl - v, d2 = d - b2;
@@ -454,17 +459,24 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
             x.set(l, d2);
           }
         } else {                                                                 // w <= 0: remainder -w
-          hdec = j;
+          inc = 0;
           uint32_t c2 = 1;
           for (uint32_t l = 0; l <= LP; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c2; x.set(l, (uint32_t)sm); c2 = (uint32_t)(sm >> 32); }
         }
+        uint32_t cy = inc;
+        for (uint32_t i = 0; i < 3; ++i) { const uint64_t sm = (uint64_t)jw[i] + cy; hd[i] = (uint32_t)sm; cy = (uint32_t)(sm >> 32); }
+        hd[3] = cy;
       }
       nq = nA + 1;
       uint32_t bw = 0;                                                           // quotient = A - hdec (>= 0)
       for (uint32_t l = 0; l < nq; ++l) {
-        const uint32_t sub = l == 0 ? (uint32_t)hdec : l == 1 ? (uint32_t)(hdec >> 32) : 0u, v = sc.get(l), d = v - sub, d2 = d - bw;
+        const uint32_t sub = l == 0 ? hd[0] : l == 1 ? hd[1] : l == 2 ? hd[2] : l == 3 ? hd[3] : 0u, v = sc.get(l), d = v - sub, d2 = d - bw;
         bw = (v < sub) | (d < bw);
         sc.set(l, d2);
+      }
+      if (pp.fold_full) {                                                        // floor(V / P) -> mod Q (it is below 2^(logQ + 42))
+        col_fold_mod(sc, nq, pp.logQ, pp.eQ);
+        nq = L;
       }
     } else {
     // Barrett quotient estimate (HAC 14.42 generalised): q1 = xc >> 32(LP-1)  (g+1 limbs),
