@@ -494,9 +494,11 @@ def _bgv_setup(N, logQ, logP, t, B, seed):
     return prm, s, evk, cts1, cts2, ms
 
 
-# (256, 220, 120, 257): logQ far above logP -- the divide-by-P takes the general Barrett route instead of the fold through P = 2^logP + e
-@pytest.mark.parametrize("N,logQ,logP,t", [(256, 100, 100, 257), (1024, 437, 437, 65537), (512, 150, 220, 65537), (256, 220, 120, 257),
-                                          (256, 136, 96, 786433)])
+# The divide-by-P of the BGV relinearisation has three routes (kernels_crt.cu, PostParams::fold_*): the fold through P = 2^logP + e on
+# V itself (the first three shapes), the fold after a Barrett reduction mod PQ ((256, 174, 128, 257): the second fold's quotient
+# needs 96 bits), and the general Barrett division ((256, 220, 120, 257), (256, 136, 96, 786433): logQ too far above logP)
+@pytest.mark.parametrize("N,logQ,logP,t", [(256, 100, 100, 257), (1024, 437, 437, 65537), (512, 150, 220, 65537), (256, 174, 128, 257),
+                                          (256, 220, 120, 257), (256, 136, 96, 786433)])
 def test_bgv_small_full(N, logQ, logP, t):
     fhe = _lib()
     prm, s, evk, cts1, cts2, ms = _bgv_setup(N, logQ, logP, t, 2, seed=N + t)
