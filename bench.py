@@ -11,7 +11,8 @@ Multi-GPU: the batch dimension shards with no data-path collective (SURVEY.md 8e
 workload's shape per step, mod Q and mod PQ in the 4 : 2 mix of an op) on the host cores.
 `python bench.py --gpus N` without a launcher re-executes itself under torch.distributed.run with N ranks.
 `--sweep`: the standalone polymul sweep; `--table1`: the operations of the paper's Table 1 at the paper's own shape
-(cnum = 4, N = 2^16, logQ = 1024), one JSON line each with the paper's T4 latency beside it (context, not a target).
+(cnum = 4, N = 2^16, logQ = 1024), one JSON line each with the paper's T4 latency beside it (context, not a target);
+`--configs`: the call of each of the five BASELINE.json configs, one JSON line each.
 """
 from __future__ import annotations
 
@@ -663,6 +664,65 @@ def run_table1(args):
                           "dtype": "u32 (exact integer)", "data": "synthetic", "reps": reps}), flush=True)
     return 0
 
+# ---- all five BASELINE.json configs, one JSON line each (context for the parity cases; the metric is quoted on C5) --------
+def run_configs(args):
+    import numpy as np
+    import torch
+    import synth
+    import paper_2607_05920_b200 as fhe
+
+    rank, local_rank, world = dist_env()
+    if rank != 0:
+        return 0
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    stream = torch.cuda.current_stream(dev)
+    cfgs = (   # name, N, logQ, logP, t, batch, call
+        ("c1", 1 << 10, 128, 128, 0, 1, "mult_relin_rescale"),
+        ("c2", 1 << 13, 218, 32, 0, 64, "polymul"),
+        ("c3", 1 << 15, 620, 620, 0, 8, "mult_relin_rescale"),
+        ("c4", 1 << 14, 437, 437, 65537, 16, "mult_relin"),
+        ("c5", 1 << 16, 1240, 1240, 0, 4, "mult_relin_rescale"),
+    )
+    for name, N, logQ, logP, t, B, call in cfgs:
+        ctx = fhe.Context(N, logQ, logP, t)
+        g = synth.rng(77)
+
+        def limbs(lead, bits):
+            return torch.from_numpy(synth.uniform_limbs(g, lead, N, bits).view(np.int32)).to(dev)   # < 2^bits <= the modulus
+
+        if call == "polymul":
+            a, b = limbs((B,), logQ), limbs((B,), logQ)
+            out = torch.empty_like(a)
+            fn = lambda: ctx.fhe_polymul(a, b, out=out, stream=stream)
+            unit = "polymuls/s"
+        else:
+            a, b = limbs((B, 2), logQ), limbs((B, 2), logQ)
+            ctx.fhe_set_evk(limbs((2,), logQ + logP))
+            out = torch.empty_like(a)
+            fn = lambda: ctx.fhe_mult_relin_rescale(a, b, 40 if t == 0 else 0, out=out, stream=stream)
+            unit = "ops/s"
+        for _ in range(max(args.warmup, 3)):
+            fn()
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        reps = max(args.steps, 10)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / reps
+        print(json.dumps({"configs": True, "config": {"workload": name, "N": N, "logQ": logQ, "logP": logP, "t": t, "batch": B, "call": call},
+                          "metric": unit, "value": B / (ms / 1e3), "unit": unit, "ms_per_step": ms, "us_per_item": ms * 1e3 / B,
+                          "launches_per_step": (ctx.launch_count() - l0) // reps, "L": ctx.L, "K": ctx.K_pm if call == "polymul" else [ctx.K1, ctx.K2],
+                          "dtype": "u32 (exact integer)", "data": "synthetic"}), flush=True)
+        del ctx, a, b, out
+        torch.cuda.empty_cache()
+    return 0
+
+
 # ---- profiles/: turn an exported ncu capture of this command into the committed summaries --------------------------------
 KERNEL_CLASS_PATTERNS = (   # substring of the kernel name -> bench.py's kernel class
     ("DecEpi", "decompose"), ("decompose_small", "decompose"), ("CrtEpi", "crt"), ("crt_exact", "crt"), ("crt_small", "crt"),
@@ -745,13 +805,14 @@ def main():
                     help="standalone polymul sweep N = 2^12..2^16 x logQ in {64, 256, 620, 1240, 2480}: one JSON line per cell")
     ap.add_argument("--table1", action="store_true",
                     help="the operations of the paper's Table 1 at the paper's shape (cnum = 4, N = 2^16, logQ = 1024): one JSON line each")
+    ap.add_argument("--configs", action="store_true", help="time the call of each of the five BASELINE.json configs: one JSON line each")
     ap.add_argument("--ncu-raw", default=None, help="exported raw page (csv) of an ncu --set full capture of this command: "
                                                     "write profiles/dram_traffic.csv and print the summary tables")
     ap.add_argument("--capture-name", default="capture")
     args = ap.parse_args()
     if args.ncu_raw:
         return summarise_ncu(args.ncu_raw, args.capture_name)
-    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not args.sweep and not args.table1:
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and not args.sweep and not args.table1 and not args.configs:
         # plain `python bench.py --gpus N`: become the N-rank launch the contract describes (one process per GPU)
         port = os.environ.get("MASTER_PORT", "29511")
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
@@ -763,6 +824,8 @@ def main():
         return run_sweep(args)
     if args.table1:
         return run_table1(args)
+    if args.configs:
+        return run_configs(args)
     return run_ours(args)
 
 
