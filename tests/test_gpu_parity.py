@@ -479,6 +479,60 @@ def test_hot_path_is_cuda_graph_capturable_and_replays_bit_identically():
         assert torch.equal(pm, ctx.fhe_polymul(nx[:, 0].contiguous(), ny[:, 0].contiguous()))
 
 
+# ---- a grid of small shapes: every path selection that depends on (logQ, logP, t) ------------------------------------------
+_GRID = [(lq, lp, 0) for lq in (33, 64, 96, 127, 160, 200, 256, 300) for lp in (32, 95, 96, 128, 250)] + \
+        [(lq, lp, t) for t in (3, 257, 65537) for lq, lp in ((64, 96), (96, 96), (100, 160), (128, 100), (150, 96), (200, 200), (250, 130))]
+
+
+@pytest.mark.parametrize("logQ,logP,t", _GRID)
+def test_grid_of_small_shapes_full_pipeline(logQ, logP, t):
+    """N = 256, two uniform pairs (parity needs no encryption) with one all-(Q - 1) polynomial, through polymul, he_mult,
+    relinearize and (CKKS) rescale by 1, 17 and logQ - 1 against the oracle, in the default path selection and with everything
+    forced through the tensor-core pipeline.  The grid crosses the bounds that select a path: CUDA-core vs pipeline conversions
+    (K x limbs <= 192), top-form vs full CKKS relin target (logP >= 96), the three BGV divide-by-P routes, logQ and logP
+    multiples of 32 and not."""
+    fhe = _lib()
+    N, B = 256, 2
+    prm = scheme.Params(N, logQ, logP, t)
+    try:
+        ctx = fhe.Context(N, logQ, logP, t)
+    except fhe.FheError as ex:
+        pytest.skip(f"shape not supported: {ex}")
+    Q, PQ = prm.Q, prm.PQ
+    rnd = np.random.default_rng(logQ * 1000 + logP + t)
+    def poly(M):
+        return [int.from_bytes(rnd.bytes((M.bit_length() + 7) // 8 + 1), "little") % M for _ in range(N)]
+    ct1 = [[poly(Q), poly(Q)] for _ in range(B)]
+    ct2 = [[poly(Q), poly(Q)] for _ in range(B)]
+    ct1[1][0] = [Q - 1] * N
+    ct2[1][1] = [Q - 1] * N
+    evk = (poly(PQ), poly(PQ))
+    d1, d2 = polys_to_tensor(ct1, ctx.L), polys_to_tensor(ct2, ctx.L)
+    ctx.fhe_set_evk(polys_to_tensor(list(evk), ctx.L_PQ))
+    want_pm = [ring.pm(ct1[i][0], ct2[i][1], Q) for i in range(B)]
+    want3 = [scheme.he_mult(prm, tuple(ct1[i]), tuple(ct2[i])) for i in range(B)]
+    want2 = [scheme.relinearize(prm, want3[i], evk) for i in range(B)]
+    for mode in (0, 1):
+        ctx.fhe_debug_force_pipeline(mode)
+        assert tensor_to_polys(ctx.fhe_polymul(d1[:, 0].contiguous(), d2[:, 1].contiguous())) == [list(p) for p in want_pm], mode
+        try:
+            t3 = ctx.fhe_he_mult(d1, d2)
+            t2 = ctx.fhe_relinearize(t3)
+        except fhe.FheError as ex:
+            if "too large" in str(ex):
+                continue                                   # a CRT target the pipeline cannot hold: the calls say so
+            raise
+        assert tensor_to_polys(t3) == [[list(p) for p in w] for w in want3], mode
+        assert tensor_to_polys(t2) == [[list(p) for p in w] for w in want2], mode
+        if t == 0:
+            for pb in (1, 17, logQ - 1):
+                wantr = [scheme.rescale(prm, want2[i], pb) for i in range(B)]
+                assert tensor_to_polys(ctx.fhe_rescale(t2, pb)) == [[list(p) for p in w] for w in wantr], (mode, pb)
+                assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, pb), ctx.fhe_rescale(t2, pb)), (mode, pb)
+        else:
+            assert torch.equal(ctx.fhe_mult_relin_rescale(d1, d2, 0), t2), mode
+
+
 # ---- configs[3]: non-RNS BGV ---------------------------------------------------------------------------------------------
 def _bgv_setup(N, logQ, logP, t, B, seed):
     prm = scheme.Params(N, logQ, logP, t)
