@@ -228,8 +228,8 @@ fhe_status fhe_debug_ntt(fhe_ctx* ctx, uint32_t* d_res, uint32_t npoly, uint32_t
  * and maximum 58: the truncation error is below 2^-58, so nothing else can be wrong).  A smaller value
  * only sends more coefficients down the exact path -- results are identical -- which is how the tests reach it. */
 fhe_status fhe_debug_crt_ambiguity(fhe_ctx* ctx, uint32_t bits);
-/* Path selection by shape.  Small conversions (K <= 32 primes, <= 16 limbs, K x limbs <= 48) run on the CUDA cores, one
- * thread per coefficient, because a tile of the tensor-core pipeline costs more than it moves there; N = 2^12 runs every
+/* Path selection by shape.  Small conversions (K <= 32 primes, <= 16 limbs, K x limbs <= 192) run on the CUDA cores, one
+ * thread per pair of coefficients, because a tile of the tensor-core pipeline costs more than it moves there; N = 2^12 runs every
  * product's transforms in ONE kernel (whole prime-polynomial in shared memory), larger N in three passes.  mode 0: that
  * choice (by measurement); 1: the large-shape paths everywhere (tensor-core conversions, three-pass NTT); 2: the small-shape
  * paths wherever they exist (the whole-transform NTT also at N = 2^13, where the three passes measure 8-13 % faster).
