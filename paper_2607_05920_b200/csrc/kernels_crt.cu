@@ -414,18 +414,20 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       // -- quotient and remainder in O(L) word operations instead of the two multi-limb products of a Barrett division.
       const uint32_t kP = pp.logP, wq = kP >> 5, bq = kP & 31, eP = pp.eP;      // LP == wq + 1
       const uint32_t nA = NXX - wq;                                              // limbs of A = xc >> kP
-      for (uint32_t i = 0; i < nA; ++i) {
-        const uint32_t lo = x.get(wq + i), hi = wq + i + 1 < NXX ? x.get(wq + i + 1) : 0u;
-        sc.set(i, bq ? (lo >> bq) | (hi << (32 - bq)) : lo);
-      }
-      sc.set(nA, 0u);
-      x.set(wq, bq ? x.get(wq) & ((1u << bq) - 1u) : 0u);                       // B = xc mod 2^kP in x[0 .. LP)
-      const uint32_t nz = (LP > nA + 1 ? LP : nA + 1) + 1;                      // limbs of z
-      for (uint32_t l = LP; l < nz; ++l) x.set(l, 0u);
+      // one pass: limb l of A (a funnel shift of limbs wq + l, wq + l + 1, which this pass has not overwritten yet) goes to the
+      // scratch column and, times eP, off limb l of B = xc mod 2^kP
+      const uint32_t nz = (LP > nA + 1 ? LP : nA + 1) + 1;                      // limbs of z = B - A eP (signed)
+      const uint32_t bmask = bq ? (1u << bq) - 1u : 0u;
       uint32_t borrow = 0, mc = 0;
       for (uint32_t l = 0; l < nz; ++l) {
-        const uint64_t pr = (l < nA ? (uint64_t)sc.get(l) * eP : 0ull) + mc;
-        const uint32_t sub = (uint32_t)pr, v = x.get(l), d = v - sub, d2 = d - borrow;
+        uint32_t al = 0;
+        if (l < nA) {
+          const uint32_t lo = x.get(wq + l), hi = wq + l + 1 < NXX ? x.get(wq + l + 1) : 0u;
+          al = bq ? (lo >> bq) | (hi << (32 - bq)) : lo;
+        }
+        if (l <= nA) sc.set(l, al);
+        const uint64_t pr = (uint64_t)al * eP + mc;
+        const uint32_t sub = (uint32_t)pr, v = l < wq ? x.get(l) : l == wq ? x.get(l) & bmask : 0u, d = v - sub, d2 = d - borrow;
         mc = (uint32_t)(pr >> 32);
         borrow = (v < sub) | (d < borrow);
         x.set(l, d2);
@@ -548,27 +550,21 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
     uint64_t kk = ((pp.t - rt) % pp.t) * pp.Pinv_t % pp.t;     // (-r P^-1) mod t in [0, t)
     const bool kneg = kk > pp.t / 2;                            // centred: kk - t
     const uint32_t kmag = kneg ? (uint32_t)(pp.t - kk) : (uint32_t)kk;
-    // res = q3 + qinc - kk_centred, as an (L+1)-limb value in x[0..L], then mod Q, then + d mod Q
+    // res = q3 + qinc - kk_centred + d as an (L+1)-limb value in x[0 .. L] (between -t/2 and 2 Q + t), then mod Q: one addition of
+    // Q or at most two subtractions -- the same residue as reducing before and after the addition of d
     {
-      int64_t adj = (int64_t)qinc + (kneg ? (int64_t)kmag : -(int64_t)kmag);
-      int64_t cc = adj;
+      int64_t cc = (int64_t)qinc + (kneg ? (int64_t)kmag : -(int64_t)kmag);
       for (uint32_t k = 0; k <= L; ++k) {
-        int64_t v = (int64_t)(k < nq ? q3.get(k) : 0u) + cc;
+        const int64_t v = (int64_t)(k < nq ? q3.get(k) : 0u) + (int64_t)(k < L ? ad.get(k) : 0u) + cc;
         x.set(k, (uint32_t)v);
         cc = v >> 32;
       }
-      // cc == -1 here means the value is negative (only possible when q3 + qinc < kk): add Q
-      if (cc < 0) { col_add(x, pp.d_Q, L + 1); }
-      else if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
-      // + d
-      uint32_t cy = 0;
-      for (uint32_t k = 0; k < L; ++k) {
-        uint64_t s = (uint64_t)x.get(k) + ad.get(k) + cy;
-        x.set(k, (uint32_t)s);
-        cy = (uint32_t)(s >> 32);
+      if (cc < 0) {
+        col_add(x, pp.d_Q, L + 1);
+      } else {
+        for (int it = 0; it < 2; ++it)
+          if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
       }
-      x.set(L, cy);
-      if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
       for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     }
   }
