@@ -55,6 +55,7 @@ __device__ __forceinline__ bool col_ge(Col x, const uint32_t* __restrict__ m, ui
 // x -= m over nl limbs (wraps)
 __device__ __forceinline__ void col_sub(Col x, const uint32_t* __restrict__ m, uint32_t nl) {
   uint32_t borrow = 0;
+  _Pragma("unroll 4")
   for (uint32_t l = 0; l < nl; ++l) {
     uint32_t a = x.get(l), b = __ldg(m + l);
     uint32_t d = a - b, d2 = d - borrow;
@@ -65,6 +66,7 @@ __device__ __forceinline__ void col_sub(Col x, const uint32_t* __restrict__ m, u
 // x += m over nl limbs (wraps)
 __device__ __forceinline__ void col_add(Col x, const uint32_t* __restrict__ m, uint32_t nl) {
   uint32_t carry = 0;
+  _Pragma("unroll 4")
   for (uint32_t l = 0; l < nl; ++l) {
     uint64_t s = (uint64_t)x.get(l) + __ldg(m + l) + carry;
     x.set(l, (uint32_t)s);
@@ -77,6 +79,7 @@ __device__ __forceinline__ void col_submul64(Col x, const uint32_t* __restrict__
   // product limbs p_l = sum k0*m[l] + k1*m[l-1], streamed with a 96-bit carry
   uint64_t acc_lo = 0; uint32_t acc_hi = 0;  // acc = acc_hi * 2^64 + acc_lo
   uint32_t borrow = 0;
+  _Pragma("unroll 4")
   for (uint32_t l = 0; l < nx; ++l) {
     uint64_t t0 = (l < nm) ? (uint64_t)k0 * __ldg(m + l) : 0ull;
     uint64_t t1 = (l >= 1 && l - 1 < nm) ? (uint64_t)k1 * __ldg(m + l - 1) : 0ull;
@@ -116,6 +119,7 @@ __device__ __forceinline__ void col_fold_mod(Col x, uint32_t nx, uint32_t k, uin
   for (uint32_t l = nm; l < nx; ++l) x.set(l, 0u);
   const uint64_t s = A * e;
   uint32_t borrow = 0;
+  _Pragma("unroll 4")
   for (uint32_t l = 0; l < nm; ++l) {
     const uint32_t sub = l == 0 ? (uint32_t)s : l == 1 ? (uint32_t)(s >> 32) : 0u, v = x.get(l), d = v - sub, d2 = d - borrow;
     borrow = (v < sub) | (d < borrow);
@@ -124,6 +128,7 @@ __device__ __forceinline__ void col_fold_mod(Col x, uint32_t nx, uint32_t k, uin
   }
   if (borrow) {                                                    // negative: + M once (A e < 2^63 < M)
     uint32_t carry = 0;
+    _Pragma("unroll 4")
     for (uint32_t l = 0; l < nm; ++l) {
       const uint64_t sum = (uint64_t)x.get(l) + ((l == 0 ? e : 0u) + (l == wq ? 1u << bq : 0u)) + carry;
       x.set(l, (uint32_t)sum);
@@ -396,6 +401,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
   if constexpr (MODE == POST_BGV_MODQ) {
     if (pp.fold_modq) col_fold_mod(x, Lx, pp.logQ, pp.eQ);
     else col_barrett1(x, Lx, pp.d_Q, L, pp.bitsQ, pp.mu1_Q);
+    _Pragma("unroll 4")
     for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     return;
   }
@@ -419,6 +425,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       const uint32_t nz = (LP > nA + 1 ? LP : nA + 1) + 1;                      // limbs of z = B - A eP (signed)
       const uint32_t bmask = bq ? (1u << bq) - 1u : 0u;
       uint32_t borrow = 0, mc = 0;
+      _Pragma("unroll 4")
       for (uint32_t l = 0; l < nz; ++l) {
         uint32_t al = 0;
         if (l < nA) {
@@ -435,6 +442,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       uint32_t hd[4] = {0u, 0u, 0u, 0u};                                         // what comes off A: j or j + 1, j < 2^95
       if (borrow) {
         uint32_t c1 = 1;                                                         // y = -z
+        _Pragma("unroll 4")
         for (uint32_t l = 0; l < nz; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c1; x.set(l, (uint32_t)sm); c1 = (uint32_t)(sm >> 32); }
         uint32_t jw[3];                                                          // j = y >> kP
         for (uint32_t i = 0; i < 3; ++i) {
@@ -446,6 +454,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
         const uint64_t p0 = (uint64_t)jw[0] * eP, p1 = (uint64_t)jw[1] * eP + (p0 >> 32), p2 = (uint64_t)jw[2] * eP + (p1 >> 32);
         const uint32_t je[4] = {(uint32_t)p0, (uint32_t)p1, (uint32_t)p2, (uint32_t)(p2 >> 32)};
         uint32_t bw = 0, any = 0;
+        _Pragma("unroll 4")
         for (uint32_t l = 0; l <= LP; ++l) {                                     // w = yl - j eP
           const uint32_t sub = l == 0 ? je[0] : l == 1 ? je[1] : l == 2 ? je[2] : l == 3 ? je[3] : 0u, v = x.get(l), d = v - sub, d2 = d - bw;
           bw = (v < sub) | (d < bw);
@@ -455,6 +464,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
         if (!bw && any) {                                                        // w > 0: one more multiple, remainder P - w
           inc = 1;
           uint32_t b2 = 0;
+          _Pragma("unroll 4")
           for (uint32_t l = 0; l <= LP; ++l) {
             const uint32_t pl = (l == 0 ? eP : 0u) + (l == wq ? 1u << bq : 0u), v = x.get(l), d = pl - v, d2 = d - b2;
             b2 = (pl < v) | (d < b2);
@@ -463,6 +473,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
         } else {                                                                 // w <= 0: remainder -w
           inc = 0;
           uint32_t c2 = 1;
+          _Pragma("unroll 4")
           for (uint32_t l = 0; l <= LP; ++l) { const uint64_t sm = (uint64_t)(~x.get(l)) + c2; x.set(l, (uint32_t)sm); c2 = (uint32_t)(sm >> 32); }
         }
         uint32_t cy = inc;
@@ -471,6 +482,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       }
       nq = nA + 1;
       uint32_t bw = 0;                                                           // quotient = A - hdec (>= 0)
+      _Pragma("unroll 4")
       for (uint32_t l = 0; l < nq; ++l) {
         const uint32_t sub = l == 0 ? hd[0] : l == 1 ? hd[1] : l == 2 ? hd[2] : l == 3 ? hd[3] : 0u, v = sc.get(l), d = v - sub, d2 = d - bw;
         bw = (v < sub) | (d < bw);
@@ -544,6 +556,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
       for (uint32_t k = LP; k-- > 0;) acc = horner_mod(acc, x.get(k), pp.t, pp.mu_t);
       rt = acc;
     } else {
+      _Pragma("unroll 4")
       for (uint32_t k = 0; k < LP; ++k) rt = (rt + (uint64_t)x.get(k) * __ldg(pp.d_pow32_t + k)) % pp.t;
     }
     if (neg) { uint64_t Pt = __ldg(pp.d_pow32_t + LP); rt = (rt + pp.t - Pt) % pp.t; }   // d_pow32_t[LP] holds P mod t
@@ -554,6 +567,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
     // Q or at most two subtractions -- the same residue as reducing before and after the addition of d
     {
       int64_t cc = (int64_t)qinc + (kneg ? (int64_t)kmag : -(int64_t)kmag);
+      _Pragma("unroll 4")
       for (uint32_t k = 0; k <= L; ++k) {
         const int64_t v = (int64_t)(k < nq ? q3.get(k) : 0u) + (int64_t)(k < L ? ad.get(k) : 0u) + cc;
         x.set(k, (uint32_t)v);
@@ -565,6 +579,7 @@ __device__ void CrtEpi<MODE, TOP, RESC>::post() {
         for (int it = 0; it < 2; ++it)
           if (x.get(L) != 0 || col_ge(x, pp.d_Q, L)) col_sub(x, pp.d_Q, L + 1);
       }
+      _Pragma("unroll 4")
       for (uint32_t k = 0; k < L; ++k) out[(size_t)k * N] = x.get(k);
     }
   }
