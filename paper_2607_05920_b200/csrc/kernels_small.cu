@@ -7,8 +7,8 @@
 // (logQ = 256) 13 KB.  Below K <= 32, limbs <= 16, K x limbs <= SMALL_WORK the arithmetic is small enough for the CUDA cores,
 // one thread per PAIR of adjacent coefficients (8-byte accesses: twice the bytes in flight per thread):
 //   decompose   r_j = sum_l x_l (2^(32 l) mod q_j) mod q_j -- the paper's own formulation -- with the
-//               sum kept lazily in 64 bits: one multiply-add per limb and prime, a "fold" (v -> hi32(v) (2^32 mod q) + lo32(v),
-//               the same residue below 2^62 + 2^32) after the first four terms and after every three more, one word-sized
+//               sum kept lazily in 64 bits: one multiply-add per limb above the first and prime, a "fold" (v -> hi32(v) (2^32 mod q)
+//               + lo32(v), the same residue below 2^62 + 2^32) after limb 4 and after every three more, one word-sized
 //               Barrett step at the end
 //   CRT         V = sum_i y_i W_i + alpha negM mod 2^(32 Lraw) limb by limb: 64-bit sums of four products each, added into a
 //               96-bit accumulator, alpha as in kernels_crt.cu; CKKS mask mode (the product is reduced mod 2^logQ)
@@ -36,9 +36,9 @@ __device__ __forceinline__ uint32_t barrett60(uint64_t v, uint32_t q, uint32_t m
 
 // LMAX: compile-time bound of the limb count (2, 4, 8, 12, 16): the loops over the limbs are unrolled over registers; limbs
 // between Lin and LMAX are zero and cost their multiply-adds.
-// Bounds of the lazy sum: a term is below (2^32 - 1)(2^30 - 1) < 2^62 - 2^32, so four terms stay below 2^64, and so does a
-// folded value (< 2^62 + 2^32) plus three terms.  Two folds bring any 64-bit value below 2^60 + 2^32 (the second one multiplies
-// at most 2^30 by c32 < 2^30), which barrett60 accepts.
+// Bounds of the lazy sum: a product is below (2^32 - 1)(2^30 - 1) < 2^62 - 2^32, so limb 0 (taken as it is) plus four products
+// stay below 2^64, and so does a folded value (< 2^62 + 2^32) plus three products.  Two folds bring any 64-bit value below
+// 2^60 + 2^32 (the second one multiplies at most 2^30 by c32 < 2^30), which barrett60 accepts.
 template <int LMAX>
 __global__ void __launch_bounds__(SMALL_THREADS)
 decompose_small_kernel(uint32_t* __restrict__ res, size_t res_outer, size_t res_inner, const uint32_t* __restrict__ limbs,
@@ -80,18 +80,23 @@ decompose_small_kernel(uint32_t* __restrict__ res, size_t res_outer, size_t res_
       const uint4 v = *reinterpret_cast<const uint4*>(sp + j * LP + l);
       cw[l] = v.x; cw[l + 1] = v.y; cw[l + 2] = v.z; cw[l + 3] = v.w;
     }
-    uint64_t acc0 = 0, acc1 = 0;
+    uint64_t acc0 = x0[0], acc1 = x1[0];                           // limb 0's constant is 2^0 mod q = 1: no multiplication
 #pragma unroll
-    for (int l = 0; l < LMAX; ++l) {
+    for (int l = 1; l < LMAX; ++l) {
       acc0 = madw(x0[l], cw[l], acc0);
       acc1 = madw(x1[l], cw[l], acc1);
-      if (l >= 3 && (l - 3) % 3 == 0 && l + 1 < LMAX) {           // after terms 4, 7, 10, 13
+      if (l >= 4 && (l - 4) % 3 == 0 && l + 1 < LMAX) {           // after limbs 4, 7, 10, 13
         acc0 = fold32(acc0, qc.y);
         acc1 = fold32(acc1, qc.y);
       }
     }
-    uint32_t r0 = barrett60(fold32(fold32(acc0, qc.y), qc.y), qc.x, qc.z);
-    uint32_t r1 = barrett60(fold32(fold32(acc1, qc.y), qc.y), qc.x, qc.z);
+    acc0 = fold32(acc0, qc.y);
+    acc1 = fold32(acc1, qc.y);
+    if constexpr (LMAX > 2) {                                      // two limbs: x0 + x1 c < 2^62 + 2^32 already, one fold is enough
+      acc0 = fold32(acc0, qc.y);
+      acc1 = fold32(acc1, qc.y);
+    }
+    uint32_t r0 = barrett60(acc0, qc.x, qc.z), r1 = barrett60(acc1, qc.x, qc.z);
     if (scale) {                                                   // the product's final constant rides here
       const uint2 sc = __ldg(scale + j);
       r0 = mul_shoup(r0, sc.x, sc.y, qc.x); r1 = mul_shoup(r1, sc.x, sc.y, qc.x);
